@@ -1,0 +1,176 @@
+/* tt.h - C ABI of libtt: the block lower-triangular Toeplitz parameter-to-observable
+ * map F of a linear autonomous dynamical system, its transpose F^T and the normal
+ * operator F^T F, applied by FFT on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed (PAPER.md = /root/reference/PAPER.md, arxiv 2501.14911):
+ *
+ *   The discrete p2o map is block lower-triangular Toeplitz (eq 2.4-2.6),
+ *   zero-based in time:
+ *
+ *        d_i = sum_{j=0..i} F_{i-j} m_j ,   i = 0..N_t-1 ,   F_k := B A^k C  (N_d x N_m)   (eq 2.5)
+ *
+ *   and is fully defined by its first block column F_0..F_{N_t-1}.  It is applied by
+ *   embedding it in a block circulant of length L = 2 N_t that the DFT block-diagonalises
+ *   (PAPER.md:263-269): zero-pad the time axis, FFT along time, one N_d x N_m complex
+ *   matvec per frequency against the spectrum Fhat (computed ONCE per matrix), inverse
+ *   FFT, keep the first N_t steps.  The adjoint applies the conjugate-transposed Fourier
+ *   blocks of the same Fhat and is the plain Euclidean transpose
+ *   (reading R2):
+ *
+ *        m'_j = sum_{i=j..N_t-1} F_{i-j}^T d_i ,   j = 0..N_t-1 .
+ *
+ *   tt_normal applies F^T F, the data-misfit Hessian of eq (2.12) with identity noise
+ *   covariance.  The k-RHS calls do the same for k vectors at once
+ *   (the many-matvec workloads of PAPER.md:296, 407, 421-423).
+ *
+ * Conventions
+ *   - Every call returns TT_OK (0) or a negative tt_status; nothing throws, aborts or
+ *     prints.  tt_status_string() names a code; tt_plan_last_cuda_error() returns the
+ *     cudaError_t behind the last TT_ERR_CUDA / TT_ERR_OOM of a plan.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Apply calls only ENQUEUE work on it: no host synchronisation, no allocation
+ *     (except the *_host convenience calls, see below).  A kernel fault therefore
+ *     surfaces at the caller's next synchronisation.
+ *   - A plan owns Fhat and its scratch buffers; the caller owns every vector and the
+ *     block column (read-only, not retained).  A plan is immutable after creation but
+ *     its scratch is shared: calls on one plan must be serialised (one stream, or
+ *     externally ordered).
+ *   - dtype TT_F32: real vectors are float, Fhat is complex64 (computed in fp64 and
+ *     rounded once).  dtype TT_F64: double / complex128.
+ *   - Layout TT_TIME_MAJOR is the paper's stacking:
+ *        m[j*N_m + p], d[i*N_d + s], block column F[(k*N_d + s)*N_m + p];
+ *     k-RHS vectors put the right-hand-side index fastest: M[(j*N_m + p)*k + r],
+ *     D[(i*N_d + s)*k + r].  TT_SPACE_MAJOR (time contiguous: m[p*N_t + j], d[s*N_t + i];
+ *     k-RHS M[(r*N_m + p)*N_t + j]) only changes the vectors, never the block column.
+ *   - N_t must factor into {2,3,5,7} and fit the shared-memory FFT (see
+ *     TT_ERR_UNSUPPORTED_NT); there is no CPU fallback of any kind.
+ */
+#ifndef TT_H_
+#define TT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tt_plan tt_plan;
+
+typedef enum tt_dtype { TT_F32 = 0, TT_F64 = 1 } tt_dtype;
+typedef enum tt_layout { TT_TIME_MAJOR = 0, TT_SPACE_MAJOR = 1 } tt_layout;
+
+typedef enum tt_status {
+    TT_OK = 0,
+    TT_ERR_NULL = -1,           /* a required pointer is NULL */
+    TT_ERR_SHAPE = -2,          /* a dimension < 1, or a size overflows 63 bits */
+    TT_ERR_DTYPE = -3,
+    TT_ERR_LAYOUT = -4,
+    TT_ERR_UNSUPPORTED_NT = -5, /* N_t has a prime factor outside {2,3,5,7}, or one series
+                                   of N_t complex values does not fit 227 KB of shared memory
+                                   at 8 series per CTA (N_t > 3632 for TT_F32, > 1816 for TT_F64) */
+    TT_ERR_K = -6,              /* k < 1 or k > k_max */
+    TT_ERR_ALIAS = -7,          /* out aliases in (tt_normal) */
+    TT_ERR_OOM = -8,            /* cudaMalloc failed */
+    TT_ERR_CUDA = -9,           /* any other CUDA runtime error (see tt_plan_last_cuda_error) */
+    TT_ERR_NO_DEVICE = -10      /* no CUDA device / wrong architecture: there is no CPU path */
+} tt_status;
+
+/* Library version, major*10000 + minor*100 + patch. */
+int tt_version(void);
+
+/* Static, NUL-terminated name of a status code. */
+const char* tt_status_string(int status);
+
+/* P0 - plan creation and the one-time DFT of the matrix ("The DFT only
+ * needs to be done once for each matrix").
+ *
+ * For every (s,p) the series F_k[s,p], k < N_t, is zero-padded to L = 2 N_t and
+ * transformed, Fhat_w[s,p] = sum_k F_k[s,p] exp(-2 pi i w k / L), keeping w = 0..N_t
+ * (real input: the other half is the conjugate).  Unnormalised forward transform; the
+ * 1/L sits in the inverse.
+ *
+ *   out                 receives the plan (set to NULL on failure)
+ *   N_d, N_m, N_t       sensors, spatial parameters, time steps (all >= 1)
+ *   dtype, layout       see above
+ *   k_max               largest k the k-RHS calls will be given (>= 1); sizes the scratch
+ *   first_block_column  [N_t][N_d][N_m] reals of `dtype`, p fastest; HOST or DEVICE pointer
+ *                       (detected); read during the call, not retained
+ *   stream              work is enqueued here and the call returns after it has completed
+ */
+int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dtype, int layout,
+                   int k_max, const void* first_block_column, void* stream);
+
+/* Frees Fhat and all scratch.  NULL-safe.  The caller must have synchronised any stream
+ * that still runs work of this plan. */
+void tt_plan_destroy(tt_plan* plan);
+
+/* Bytes of device memory the plan holds (Fhat + tables + scratch). */
+size_t tt_plan_device_bytes(const tt_plan* plan);
+
+/* cudaError_t (as int) recorded by the last failing CUDA call made for this plan; 0 if none. */
+int tt_plan_last_cuda_error(const tt_plan* plan);
+
+/* Test hook: copies Fhat, unpadded, to dst_device as [N_t+1][N_d][N_m] interleaved complex
+ * (complex64 for TT_F32, complex128 for TT_F64), on `stream`. */
+int tt_plan_get_spectrum(const tt_plan* plan, void* dst_device, void* stream);
+
+/* d = F m  (eq 2.5; FFT algorithm of).
+ *   m  DEVICE, N_t*N_m reals, read-only;   d  DEVICE, N_t*N_d reals, overwritten. */
+int tt_matvec(const tt_plan* plan, const void* m, void* d, void* stream);
+
+/* m = F^T d  (transpose of eq 2.5; "conjugate-transposed diagonal blocks").
+ *   d  DEVICE, N_t*N_d reals, read-only;   m  DEVICE, N_t*N_m reals, overwritten. */
+int tt_rmatvec(const tt_plan* plan, const void* d, void* m, void* stream);
+
+/* out = F^T (F m)  (eq 2.12 with Gamma_noise = I).  The intermediate
+ * data vector lives in plan scratch on the device.  Between F and F^T it IS inverse
+ * transformed, truncated to N_t steps, re-padded and transformed again: the truncation
+ * is a projection in time that is not diagonal in frequency (reading R6).
+ *   m, out  DEVICE, N_t*N_m reals; out == m returns TT_ERR_ALIAS. */
+int tt_normal(const tt_plan* plan, const void* m, void* out, void* stream);
+
+/* k-RHS variants, 1 <= k <= k_max: column r of the result equals the single-vector result
+ * on column r.  The per-frequency products are complex GEMMs (N_d x N_m)(N_m x k) and
+ * (N_m x N_d)(N_d x k).
+ *   M  DEVICE, N_t*N_m*k reals;   D  DEVICE, N_t*N_d*k reals (layouts above). */
+int tt_matvec_batched(const tt_plan* plan, int k, const void* M, void* D, void* stream);
+int tt_rmatvec_batched(const tt_plan* plan, int k, const void* D, void* M, void* stream);
+
+/* Convenience calls with HOST vectors (pinned memory recommended): copy the input to a
+ * device staging buffer on `stream`, apply, copy the result back; all asynchronous on
+ * `stream` when the host memory is pinned.  The staging buffers are allocated on first
+ * use (the only apply-time allocation in the library) and freed with the plan. */
+int tt_matvec_host(const tt_plan* plan, const void* m_host, void* d_host, void* stream);
+int tt_rmatvec_host(const tt_plan* plan, const void* d_host, void* m_host, void* stream);
+int tt_normal_host(const tt_plan* plan, const void* m_host, void* out_host, void* stream);
+
+/* Measurement hooks (bench.py's roofline object).
+ *
+ * tt_plan_set_profiling(plan, 1) makes every apply call record CUDA events, on the stream
+ * it launches on, around each of its kernels; tt_plan_stage_ms() then returns, after the
+ * caller has synchronised that stream, the device time of the stages of the LAST apply
+ * call: ms[0] forward FFT of the input, ms[1] per-frequency matvec / matmul (the kernel
+ * that streams Fhat), ms[2] inverse FFT (+ partial reduce).  tt_normal reports the sum of
+ * its two halves.  n = number of floats ms can hold (>= 3).
+ */
+int tt_plan_set_profiling(tt_plan* plan, int enabled);
+int tt_plan_stage_ms(const tt_plan* plan, float* ms, int n);
+
+/* Read-only streaming probe: sums `bytes` (multiple of 16) of device memory at `src` with
+ * 128-bit loads and writes one 16-byte result per CTA to `sink` (>= 16*4096 bytes).  Used
+ * by bench.py to measure the read-only HBM bandwidth next to the copy figure. */
+int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream);
+
+/* Test hook for the planner's host logic (needs no GPU): the FFT plan of an N_t-point series.
+ *   n_stages  receives the number of decimation-in-frequency stages
+ *   radix     int[16], receives their radices (product = N_t)
+ *   pos       unsigned short[N_t], pos[k] = slot of the in-place DIF output holding bin k
+ *   tw        double[4*N_t], interleaved (re, im) of exp(-2 pi i k / (2 N_t)), k < 2 N_t
+ * Returns TT_ERR_UNSUPPORTED_NT if N_t does not factor into {2,3,5,7} or exceeds 65535. */
+int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* pos, double* tw);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TT_H_ */

@@ -1,0 +1,268 @@
+"""Thin Python binding of libtt (include/tt.h): argument marshalling only.
+
+Every function has the name and the argument order of the C call it wraps; tensors are
+passed as raw pointers (`tensor.data_ptr()`), streams as `torch.cuda.Stream.cuda_stream`.
+PyTorch is used for device memory and streams only; every step of the path runs in the
+library's own CUDA kernels.  If libtt.so cannot be built or loaded this module raises:
+there is no CPU or PyTorch fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+TT_F32, TT_F64 = 0, 1
+TT_TIME_MAJOR, TT_SPACE_MAJOR = 0, 1
+TT_OK = 0
+
+_lib = None
+
+
+class TTError(RuntimeError):
+    def __init__(self, call: str, status: int, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        name = lib().tt_status_string(status).decode()
+        extra = f" (cudaError {cuda_error})" if cuda_error else ""
+        super().__init__(f"{call} failed: {name} [{status}]{extra}")
+
+
+def lib() -> ctypes.CDLL:
+    """Loads (building first if needed) paper_2501_14911_b200/libtt.so."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or os.environ.get("TT_REBUILD") == "1":
+        path = _build.build()
+    else:
+        try:
+            path = _build.build()  # no-op when the source hash matches
+        except RuntimeError:
+            pass  # no nvcc on this box: use the library that travelled with the repo
+    L = ctypes.CDLL(path)
+    vp, i64, ci, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_size_t
+    pp = ctypes.POINTER(vp)
+    sigs = {
+        "tt_version": (ci, []),
+        "tt_status_string": (ctypes.c_char_p, [ci]),
+        "tt_plan_create": (ci, [pp, i64, i64, i64, ci, ci, ci, vp, vp]),
+        "tt_plan_destroy": (None, [vp]),
+        "tt_plan_device_bytes": (sz, [vp]),
+        "tt_plan_last_cuda_error": (ci, [vp]),
+        "tt_plan_get_spectrum": (ci, [vp, vp, vp]),
+        "tt_matvec": (ci, [vp, vp, vp, vp]),
+        "tt_rmatvec": (ci, [vp, vp, vp, vp]),
+        "tt_normal": (ci, [vp, vp, vp, vp]),
+        "tt_matvec_batched": (ci, [vp, ci, vp, vp, vp]),
+        "tt_rmatvec_batched": (ci, [vp, ci, vp, vp, vp]),
+        "tt_matvec_host": (ci, [vp, vp, vp, vp]),
+        "tt_rmatvec_host": (ci, [vp, vp, vp, vp]),
+        "tt_normal_host": (ci, [vp, vp, vp, vp]),
+        "tt_plan_set_profiling": (ci, [vp, ci]),
+        "tt_plan_stage_ms": (ci, [vp, ctypes.POINTER(ctypes.c_float), ci]),
+        "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
+        "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
+                                     ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
+    }
+    for name, (res, args) in sigs.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy", "tt_plan_device_bytes",
+           "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
+           "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
+           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_debug_fft_tables"]
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _check(call: str, status: int, plan: int | None = None):
+    if status != TT_OK:
+        ce = lib().tt_plan_last_cuda_error(plan) if plan else 0
+        raise TTError(call, status, ce)
+
+
+def tt_version() -> int:
+    return lib().tt_version()
+
+
+def tt_status_string(status: int) -> str:
+    return lib().tt_status_string(status).decode()
+
+
+def tt_plan_create(N_d: int, N_m: int, N_t: int, dtype: int, layout: int, k_max: int,
+                   first_block_column, stream=None) -> int:
+    """Returns the plan handle (an integer address).  first_block_column: tensor (cpu or cuda) or raw pointer."""
+    ptr = first_block_column if isinstance(first_block_column, int) else first_block_column.data_ptr()
+    out = ctypes.c_void_p()
+    st = lib().tt_plan_create(ctypes.byref(out), N_d, N_m, N_t, dtype, layout, k_max, ptr, _stream(stream))
+    _check("tt_plan_create", st)
+    return out.value
+
+
+def tt_plan_destroy(plan: int) -> None:
+    lib().tt_plan_destroy(plan)
+
+
+def tt_plan_device_bytes(plan: int) -> int:
+    return lib().tt_plan_device_bytes(plan)
+
+
+def tt_plan_last_cuda_error(plan: int) -> int:
+    return lib().tt_plan_last_cuda_error(plan)
+
+
+def tt_plan_get_spectrum(plan: int, dst: torch.Tensor, stream=None) -> None:
+    _check("tt_plan_get_spectrum", lib().tt_plan_get_spectrum(plan, dst.data_ptr(), _stream(stream)), plan)
+
+
+def _ptr(x) -> int:
+    return x if isinstance(x, int) else x.data_ptr()
+
+
+def tt_matvec(plan: int, m, d, stream=None) -> None:
+    _check("tt_matvec", lib().tt_matvec(plan, _ptr(m), _ptr(d), _stream(stream)), plan)
+
+
+def tt_rmatvec(plan: int, d, m, stream=None) -> None:
+    _check("tt_rmatvec", lib().tt_rmatvec(plan, _ptr(d), _ptr(m), _stream(stream)), plan)
+
+
+def tt_normal(plan: int, m, out, stream=None) -> None:
+    _check("tt_normal", lib().tt_normal(plan, _ptr(m), _ptr(out), _stream(stream)), plan)
+
+
+def tt_matvec_batched(plan: int, k: int, M, D, stream=None) -> None:
+    _check("tt_matvec_batched", lib().tt_matvec_batched(plan, k, _ptr(M), _ptr(D), _stream(stream)), plan)
+
+
+def tt_rmatvec_batched(plan: int, k: int, D, M, stream=None) -> None:
+    _check("tt_rmatvec_batched", lib().tt_rmatvec_batched(plan, k, _ptr(D), _ptr(M), _stream(stream)), plan)
+
+
+def tt_matvec_host(plan: int, m_host, d_host, stream=None) -> None:
+    _check("tt_matvec_host", lib().tt_matvec_host(plan, _ptr(m_host), _ptr(d_host), _stream(stream)), plan)
+
+
+def tt_rmatvec_host(plan: int, d_host, m_host, stream=None) -> None:
+    _check("tt_rmatvec_host", lib().tt_rmatvec_host(plan, _ptr(d_host), _ptr(m_host), _stream(stream)), plan)
+
+
+def tt_normal_host(plan: int, m_host, out_host, stream=None) -> None:
+    _check("tt_normal_host", lib().tt_normal_host(plan, _ptr(m_host), _ptr(out_host), _stream(stream)), plan)
+
+
+def tt_plan_set_profiling(plan: int, enabled: bool) -> None:
+    _check("tt_plan_set_profiling", lib().tt_plan_set_profiling(plan, int(bool(enabled))), plan)
+
+
+def tt_plan_stage_ms(plan: int) -> tuple[float, float, float]:
+    buf = (ctypes.c_float * 3)()
+    _check("tt_plan_stage_ms", lib().tt_plan_stage_ms(plan, buf, 3), plan)
+    return float(buf[0]), float(buf[1]), float(buf[2])
+
+
+def tt_probe_stream_read(src, nbytes: int, sink, stream=None) -> None:
+    _check("tt_probe_stream_read", lib().tt_probe_stream_read(_ptr(src), nbytes, _ptr(sink), _stream(stream)))
+
+
+def tt_debug_fft_tables(N_t: int):
+    """(radices, pos, tw) of the planner's FFT plan for an N_t-point series; runs without a GPU."""
+    import numpy as np
+    n = ctypes.c_int()
+    radix = (ctypes.c_int * 16)()
+    pos = (ctypes.c_ushort * max(1, N_t))()
+    tw = (ctypes.c_double * (4 * max(1, N_t)))()
+    st = lib().tt_debug_fft_tables(N_t, ctypes.byref(n), radix, pos, tw)
+    _check("tt_debug_fft_tables", st)
+    return (list(radix[: n.value]), np.array(pos[:N_t], dtype=np.int64),
+            np.array(tw[: 4 * N_t]).reshape(2 * N_t, 2) @ np.array([1.0, 1.0j]))
+
+
+_DT = {torch.float32: TT_F32, torch.float64: TT_F64}
+
+
+class Plan:
+    """RAII convenience over the calls above (tests and bench.py use it).
+
+    Vectors are torch CUDA tensors in the plan's dtype and layout (time-major [N_t, N_m] /
+    [N_t, N_d], or [N_t, N_*, k] for the k-RHS calls); outputs are allocated with torch.
+    """
+
+    def __init__(self, first_block_column: torch.Tensor, layout: int = TT_TIME_MAJOR, k_max: int = 1,
+                 stream=None):
+        assert first_block_column.dim() == 3 and first_block_column.is_contiguous()
+        self.N_t, self.N_d, self.N_m = first_block_column.shape
+        self.dtype = first_block_column.dtype
+        self.layout, self.k_max = layout, k_max
+        self.handle = tt_plan_create(self.N_d, self.N_m, self.N_t, _DT[self.dtype], layout, k_max,
+                                     first_block_column, stream)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            torch.cuda.synchronize()
+            tt_plan_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def _shape(self, n_space: int, k: int | None):
+        base = (self.N_t, n_space) if self.layout == TT_TIME_MAJOR else (n_space, self.N_t)
+        if k is None:
+            return base
+        return base + (k,) if self.layout == TT_TIME_MAJOR else (k,) + base
+
+    def _out(self, n_space: int, k: int | None = None):
+        return torch.empty(self._shape(n_space, k), dtype=self.dtype, device="cuda")
+
+    def matvec(self, m, out=None, stream=None):
+        out = self._out(self.N_d) if out is None else out
+        tt_matvec(self.handle, m, out, stream)
+        return out
+
+    def rmatvec(self, d, out=None, stream=None):
+        out = self._out(self.N_m) if out is None else out
+        tt_rmatvec(self.handle, d, out, stream)
+        return out
+
+    def normal(self, m, out=None, stream=None):
+        out = self._out(self.N_m) if out is None else out
+        tt_normal(self.handle, m, out, stream)
+        return out
+
+    def matvec_batched(self, M, out=None, stream=None):
+        k = M.shape[-1] if self.layout == TT_TIME_MAJOR else M.shape[0]
+        out = self._out(self.N_d, k) if out is None else out
+        tt_matvec_batched(self.handle, k, M, out, stream)
+        return out
+
+    def rmatvec_batched(self, D, out=None, stream=None):
+        k = D.shape[-1] if self.layout == TT_TIME_MAJOR else D.shape[0]
+        out = self._out(self.N_m, k) if out is None else out
+        tt_rmatvec_batched(self.handle, k, D, out, stream)
+        return out
+
+    def spectrum(self):
+        cdt = torch.complex64 if self.dtype == torch.float32 else torch.complex128
+        out = torch.empty((self.N_t + 1, self.N_d, self.N_m), dtype=cdt, device="cuda")
+        tt_plan_get_spectrum(self.handle, out)
+        return out
+
+    @property
+    def device_bytes(self) -> int:
+        return tt_plan_device_bytes(self.handle)

@@ -1,0 +1,572 @@
+// tt_api.cu - the C ABI of libtt (include/tt.h): validation, the planner (FFT factorisation,
+// tables, tile sizes, scratch), the one-time DFT of the block column (P0) and the kernel
+// sequences of the apply calls.  Every step of the path runs in this library's own kernels;
+// there is no CPU fallback and no library FFT/BLAS call.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/tt.h"
+#include "tt_internal.h"
+
+using namespace tt;
+
+namespace {
+
+constexpr int kVersion = 100;  // 0.1.0
+constexpr int kNumEvents = 8;
+
+inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
+
+}  // namespace
+
+struct tt_plan {
+    long long N_d = 0, N_m = 0, N_t = 0;
+    int dtype = 0, layout = 0, k_max = 1;
+    int n_f = 0;
+    long long ldp = 0;  // padded N_m: row pitch of Fhat and of the single-vector spectrum
+    int n_stages = 0;
+    int radix[kMaxStages] = {};
+    void* tw_d = nullptr;  // c128[2N]
+    void* tw_f = nullptr;  // c64[2N] (TT_F32 only)
+    unsigned short* pos = nullptr;
+    void* Fhat = nullptr;
+    void* xhat = nullptr;     // [n_f][ldp] complex
+    void* dhat = nullptr;     // [n_f][N_d] complex
+    void* partial = nullptr;  // [n_f][n_chunks][N_d] complex
+    void* dwork = nullptr;    // [N_t][N_d] reals (tt_normal)
+    void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
+    void* d_stage = nullptr;
+    void* m_stage2 = nullptr;
+    int chunk = 0, n_chunks = 0;
+    size_t bytes = 0;
+    mutable int last_cuda = 0;
+    bool prof = false;
+    cudaEvent_t ev[kNumEvents] = {};
+    mutable int ev_used = 0;
+};
+
+namespace {
+
+int fail_cuda(const tt_plan* p, cudaError_t e) {
+    if (p) p->last_cuda = (int)e;
+    (void)cudaGetLastError();  // clear the non-sticky error state
+    return e == cudaErrorMemoryAllocation ? TT_ERR_OOM : TT_ERR_CUDA;
+}
+
+#define TT_CUDA(plan, call)                                  \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) return fail_cuda(plan, e__); \
+    } while (0)
+
+int dev_alloc(tt_plan* p, void** ptr, size_t bytes) {
+    *ptr = nullptr;
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(ptr, bytes);
+    if (e != cudaSuccess) { *ptr = nullptr; return fail_cuda(p, e); }
+    p->bytes += bytes;
+    return TT_OK;
+}
+
+// Radices of the N-point complex FFT: 4s first (fewest passes over shared memory), then what is left.
+bool factorise(long long N, int* radix, int* n_stages) {
+    int n = 0;
+    long long r = N;
+    const int cand[5] = {4, 2, 3, 5, 7};
+    for (int c = 0; c < 5; ++c)
+        while (r % cand[c] == 0 && r > 1) {
+            if (n >= kMaxStages) return false;
+            radix[n++] = cand[c];
+            r /= cand[c];
+        }
+    if (r != 1) return false;
+    if (n == 0) radix[n++] = 1;  // N == 1: handled as zero stages below
+    *n_stages = (N == 1) ? 0 : n;
+    return true;
+}
+
+// pos[k] = slot of the in-place decimation-in-frequency output that holds bin k:
+// slot = q1*(N/r1) + q2*(N/(r1 r2)) + ... holds bin k = q1 + r1*(q2 + r2*(q3 + ...)).
+void build_pos(int N, const int* radix, int n_stages, std::vector<unsigned short>& pos) {
+    pos.assign(N, 0);
+    for (int slot = 0; slot < N; ++slot) {
+        int rem = slot, span = N, k = 0, mul = 1;
+        for (int st = 0; st < n_stages; ++st) {
+            span /= radix[st];
+            const int q = rem / span;
+            rem -= q * span;
+            k += q * mul;
+            mul *= radix[st];
+        }
+        pos[k] = (unsigned short)slot;
+    }
+}
+
+// tw[k] = exp(-2 pi i k / L), k < L, exact on the axes and symmetric by construction.
+void build_twiddles(int L, std::vector<double>& tw) {
+    tw.assign(2 * (size_t)L, 0.0);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int k = 0; k < L; ++k) {
+        double c, s;
+        if ((4LL * k) % L == 0) {
+            const int q = (int)((4LL * k) / L);  // quarter turns
+            c = q == 0 ? 1.0 : q == 2 ? -1.0 : 0.0;
+            s = q == 1 ? 1.0 : q == 3 ? -1.0 : 0.0;
+        } else {
+            const long double a = two_pi * (long double)k / (long double)L;
+            c = (double)cosl(a);
+            s = (double)sinl(a);
+        }
+        tw[2 * (size_t)k] = c;
+        tw[2 * (size_t)k + 1] = -s;
+    }
+}
+
+void fill_fft_common(const tt_plan* p, FftParams& P, bool fp32_tables) {
+    std::memset(&P, 0, sizeof(P));
+    P.N = (int)p->N_t;
+    P.n_stages = p->n_stages;
+    for (int i = 0; i < p->n_stages; ++i) P.radix[i] = p->radix[i];
+    P.tw = fp32_tables ? p->tw_f : p->tw_d;
+    P.pos = p->pos;
+    P.n_part = 1;
+    P.scale = 1.0 / (2.0 * (double)p->N_t);
+}
+
+// Where column r of a (k-RHS) vector lives: element (b, j) is base[b*bs + j*ts] (in elements).
+struct VecView {
+    long long off, bs, ts;
+};
+VecView view(const tt_plan* p, long long n_space, int k, int r) {
+    if (p->layout == TT_SPACE_MAJOR) return VecView{(long long)r * n_space * p->N_t, p->N_t, 1};
+    return VecView{(long long)r, (long long)k, n_space * k};
+}
+inline const void* at(const void* base, long long off, size_t es) { return static_cast<const char*>(base) + (size_t)off * es; }
+inline void* at(void* base, long long off, size_t es) { return static_cast<char*>(base) + (size_t)off * es; }
+
+struct Prof {
+    const tt_plan* p;
+    cudaStream_t s;
+    int base;
+    void mark(int i) const {
+        if (p->prof) cudaEventRecord(p->ev[base + i], s);
+    }
+};
+
+// d = F m on device buffers (steps A1, A2, A3).
+int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_base, int k = 1, int r = 0) {
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
+    const size_t es = esize(p->dtype);
+    const VecView vm = view(p, p->N_m, k, r), vd = view(p, p->N_d, k, r);
+    Prof pr{p, s, ev_base};
+    pr.mark(0);
+    FftParams P;
+    fill_fft_common(p, P, f32);
+    P.B = p->N_m; P.B_store = p->ldp;
+    P.r_ys = 0; P.r_bs = vm.bs; P.r_ts = vm.ts;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
+    TT_CUDA(p, fft_r2c_launch(t, t, t, at(m, vm.off, es), p->xhat, P, 1, s));
+    pr.mark(1);
+    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks};
+    TT_CUDA(p, gemv_fwd_launch(t, p->Fhat, p->xhat, p->partial, g, s));
+    pr.mark(2);
+    fill_fft_common(p, P, f32);
+    P.B = p->N_d; P.B_store = p->N_d;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = (long long)p->n_chunks * p->N_d;
+    P.n_part = p->n_chunks; P.c_ps = p->N_d;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts;
+    TT_CUDA(p, fft_c2r_launch(t, p->partial, at(d, vd.off, es), P, 1, s));
+    pr.mark(3);
+    return TT_OK;
+}
+
+// m = F^T d on device buffers (steps B1, B2, B3).
+int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev_base, int k = 1, int r = 0) {
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
+    const size_t es = esize(p->dtype);
+    const VecView vm = view(p, p->N_m, k, r), vd = view(p, p->N_d, k, r);
+    Prof pr{p, s, ev_base};
+    pr.mark(0);
+    FftParams P;
+    fill_fft_common(p, P, f32);
+    P.B = p->N_d; P.B_store = p->N_d;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
+    TT_CUDA(p, fft_r2c_launch(t, t, t, at(d, vd.off, es), p->dhat, P, 1, s));
+    pr.mark(1);
+    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks};
+    TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
+    pr.mark(2);
+    fill_fft_common(p, P, f32);
+    P.B = p->N_m; P.B_store = p->N_m;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
+    P.r_ys = 0; P.r_bs = vm.bs; P.r_ts = vm.ts;
+    TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
+    pr.mark(3);
+    return TT_OK;
+}
+
+// P0: Fhat from one slab of sensors [s0, s0+ns) of the block column, device resident as
+// col[(k*ns_pitch + s)*N_m + p].
+int run_plan_fft(tt_plan* p, const void* col, long long s0, long long ns, long long ns_pitch, cudaStream_t s) {
+    const bool f32 = p->dtype == TT_F32;
+    FftParams P;
+    fill_fft_common(p, P, /*fp32_tables=*/false);  // the matrix is always transformed in fp64
+    P.B = p->N_m; P.B_store = p->ldp;
+    P.r_ys = p->N_m; P.r_bs = 1; P.r_ts = ns_pitch * p->N_m;
+    P.c_ys = p->ldp; P.c_bs = 1; P.c_fs = p->N_d * p->ldp;
+    char* out = static_cast<char*>(p->Fhat) + (size_t)s0 * p->ldp * 2 * esize(p->dtype);
+    for (long long y0 = 0; y0 < ns; y0 += 32768) {  // gridDim.y limit
+        const long long ny = ns - y0 < 32768 ? ns - y0 : 32768;
+        const char* in = static_cast<const char*>(col) + (size_t)y0 * p->N_m * esize(p->dtype);
+        char* o = out + (size_t)y0 * p->ldp * 2 * esize(p->dtype);
+        TT_CUDA(p, fft_r2c_launch(f32 ? 0 : 1, 1, f32 ? 0 : 1, in, o, P, (int)ny, s));
+    }
+    return TT_OK;
+}
+
+int check_apply(const tt_plan* p, const void* a, const void* b) {
+    if (!p || !a || !b) return TT_ERR_NULL;
+    return TT_OK;
+}
+
+int ensure_staging(const tt_plan* cp) {
+    tt_plan* p = const_cast<tt_plan*>(cp);
+    const size_t es = esize(p->dtype);
+    if (!p->m_stage) {
+        int r = dev_alloc(p, &p->m_stage, (size_t)p->N_t * p->N_m * es);
+        if (r) return r;
+    }
+    if (!p->m_stage2) {
+        int r = dev_alloc(p, &p->m_stage2, (size_t)p->N_t * p->N_m * es);
+        if (r) return r;
+    }
+    if (!p->d_stage) {
+        int r = dev_alloc(p, &p->d_stage, (size_t)p->N_t * p->N_d * es);
+        if (r) return r;
+    }
+    return TT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tt_version(void) { return kVersion; }
+
+const char* tt_status_string(int status) {
+    switch (status) {
+        case TT_OK: return "TT_OK";
+        case TT_ERR_NULL: return "TT_ERR_NULL";
+        case TT_ERR_SHAPE: return "TT_ERR_SHAPE";
+        case TT_ERR_DTYPE: return "TT_ERR_DTYPE";
+        case TT_ERR_LAYOUT: return "TT_ERR_LAYOUT";
+        case TT_ERR_UNSUPPORTED_NT: return "TT_ERR_UNSUPPORTED_NT";
+        case TT_ERR_K: return "TT_ERR_K";
+        case TT_ERR_ALIAS: return "TT_ERR_ALIAS";
+        case TT_ERR_OOM: return "TT_ERR_OOM";
+        case TT_ERR_CUDA: return "TT_ERR_CUDA";
+        case TT_ERR_NO_DEVICE: return "TT_ERR_NO_DEVICE";
+        default: return "TT_ERR_UNKNOWN";
+    }
+}
+
+void tt_plan_destroy(tt_plan* p) {
+    if (!p) return;
+    void* bufs[] = {p->tw_d, p->tw_f, p->pos, p->Fhat, p->xhat, p->dhat, p->partial,
+                    p->dwork, p->m_stage, p->m_stage2, p->d_stage};
+    for (void* b : bufs)
+        if (b) cudaFree(b);
+    for (int i = 0; i < kNumEvents; ++i)
+        if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    delete p;
+}
+
+int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dtype, int layout, int k_max,
+                   const void* first_block_column, void* stream) {
+    if (!out) return TT_ERR_NULL;
+    *out = nullptr;
+    if (!first_block_column) return TT_ERR_NULL;
+    if (N_d < 1 || N_m < 1 || N_t < 1) return TT_ERR_SHAPE;
+    if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
+    if (layout != TT_TIME_MAJOR && layout != TT_SPACE_MAJOR) return TT_ERR_LAYOUT;
+    if (k_max < 1) return TT_ERR_K;
+    // sizes: every element count must stay below 2^62 and N_d, N_t within int range
+    const long double lim = 4.0e18L;
+    if (N_d > 0x7fffffffLL || N_t > 0x3fffffffLL) return TT_ERR_SHAPE;
+    if ((long double)N_d * (long double)(N_m + 16) * (long double)(N_t + 1) * 16.0L > lim) return TT_ERR_SHAPE;
+    if ((long double)(N_m + 16) * (long double)(N_t + 1) * (long double)k_max * 16.0L > lim) return TT_ERR_SHAPE;
+
+    int radix[kMaxStages] = {};
+    int n_stages = 0;
+    if (N_t > 65535 || !factorise(N_t, radix, &n_stages)) return TT_ERR_UNSUPPORTED_NT;
+    const FftChoice cd = fft_choose((int)N_t, 16);  // the fp64 transform of the matrix is the largest user
+    if (cd.T == 0) return TT_ERR_UNSUPPORTED_NT;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return TT_ERR_NO_DEVICE; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return TT_ERR_NO_DEVICE;
+    }
+    if (prop.major != 10) return TT_ERR_NO_DEVICE;  // built for sm_100a only
+
+    tt_plan* p = new (std::nothrow) tt_plan();
+    if (!p) return TT_ERR_OOM;
+    p->N_d = N_d; p->N_m = N_m; p->N_t = N_t;
+    p->dtype = dtype; p->layout = layout; p->k_max = k_max;
+    p->n_f = (int)N_t + 1;
+    p->ldp = (N_m + 15) / 16 * 16;
+    p->n_stages = n_stages;
+    for (int i = 0; i < n_stages; ++i) p->radix[i] = radix[i];
+    p->chunk = 2048;
+    p->n_chunks = (int)((p->ldp + p->chunk - 1) / p->chunk);
+
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t es = esize(dtype), cs = 2 * es;
+    const int L = 2 * (int)N_t;
+    int rc = TT_OK;
+
+#define TT_TRY(expr)                                  \
+    do {                                              \
+        rc = (expr);                                  \
+        if (rc != TT_OK) { tt_plan_destroy(p); return rc; } \
+    } while (0)
+#define TT_TRYC(call)                                                              \
+    do {                                                                           \
+        cudaError_t e__ = (call);                                                  \
+        if (e__ != cudaSuccess) { rc = fail_cuda(p, e__); tt_plan_destroy(p); return rc; } \
+    } while (0)
+
+    // tables
+    {
+        std::vector<double> tw;
+        build_twiddles(L, tw);
+        std::vector<unsigned short> pos;
+        build_pos((int)N_t, radix, n_stages, pos);
+        TT_TRY(dev_alloc(p, &p->tw_d, tw.size() * sizeof(double)));
+        TT_TRYC(cudaMemcpyAsync(p->tw_d, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+        std::vector<float> twf(tw.size());
+        for (size_t i = 0; i < tw.size(); ++i) twf[i] = (float)tw[i];
+        if (dtype == TT_F32) {
+            TT_TRY(dev_alloc(p, &p->tw_f, twf.size() * sizeof(float)));
+            TT_TRYC(cudaMemcpyAsync(p->tw_f, twf.data(), twf.size() * sizeof(float), cudaMemcpyHostToDevice, s));
+        }
+        TT_TRY(dev_alloc(p, reinterpret_cast<void**>(&p->pos), pos.size() * sizeof(unsigned short)));
+        TT_TRYC(cudaMemcpyAsync(p->pos, pos.data(), pos.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, s));
+        TT_TRYC(cudaStreamSynchronize(s));  // the host vectors die at the end of this scope
+    }
+
+    // spectrum and scratch
+    const size_t fhat_elems = (size_t)p->n_f * (size_t)N_d * (size_t)p->ldp;
+    TT_TRY(dev_alloc(p, &p->Fhat, fhat_elems * cs));
+    const size_t ldx = ((size_t)N_m * k_max + 15) / 16 * 16;
+    const size_t xhat_elems = (size_t)p->n_f * (k_max == 1 ? (size_t)p->ldp : ldx);
+    TT_TRY(dev_alloc(p, &p->xhat, xhat_elems * cs));
+    TT_TRY(dev_alloc(p, &p->dhat, (size_t)p->n_f * N_d * k_max * cs));
+    TT_TRY(dev_alloc(p, &p->partial, (size_t)p->n_f * p->n_chunks * N_d * k_max * cs));
+    TT_TRY(dev_alloc(p, &p->dwork, (size_t)N_t * N_d * k_max * es));
+    for (int i = 0; i < kNumEvents; ++i) TT_TRYC(cudaEventCreate(&p->ev[i]));
+
+    // P0: transform the block column (device pointer: in place; host pointer: by sensor slabs)
+    cudaPointerAttributes attr;
+    cudaError_t ea = cudaPointerGetAttributes(&attr, first_block_column);
+    bool on_device = false;
+    if (ea == cudaSuccess) on_device = (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged);
+    else (void)cudaGetLastError();
+    if (on_device) {
+        TT_TRY(run_plan_fft(p, first_block_column, 0, N_d, N_d, s));
+        TT_TRYC(cudaStreamSynchronize(s));
+    } else {
+        const size_t plane = (size_t)N_t * (size_t)N_m * es;  // bytes of one sensor's series
+        long long ds = (long long)((size_t(1) << 30) / (plane ? plane : 1));
+        if (ds < 1) ds = 1;
+        if (ds > N_d) ds = N_d;
+        void* slab = nullptr;
+        cudaError_t e = cudaMalloc(&slab, plane * (size_t)ds);
+        if (e != cudaSuccess) { rc = fail_cuda(p, e); tt_plan_destroy(p); return rc; }
+        for (long long s0 = 0; s0 < N_d; s0 += ds) {
+            const long long ns = N_d - s0 < ds ? N_d - s0 : ds;
+            const char* src = static_cast<const char*>(first_block_column) + (size_t)s0 * N_m * es;
+            e = cudaMemcpy2DAsync(slab, (size_t)ns * N_m * es, src, (size_t)N_d * N_m * es, (size_t)ns * N_m * es,
+                                  (size_t)N_t, cudaMemcpyHostToDevice, s);
+            if (e == cudaSuccess) {
+                rc = run_plan_fft(p, slab, s0, ns, ns, s);
+                if (rc == TT_OK) e = cudaStreamSynchronize(s);
+            }
+            if (e != cudaSuccess || rc != TT_OK) {
+                if (e != cudaSuccess) rc = fail_cuda(p, e);
+                cudaFree(slab);
+                tt_plan_destroy(p);
+                return rc;
+            }
+        }
+        cudaFree(slab);
+    }
+#undef TT_TRY
+#undef TT_TRYC
+    *out = p;
+    return TT_OK;
+}
+
+size_t tt_plan_device_bytes(const tt_plan* p) { return p ? p->bytes : 0; }
+
+int tt_plan_last_cuda_error(const tt_plan* p) { return p ? p->last_cuda : 0; }
+
+int tt_plan_get_spectrum(const tt_plan* p, void* dst, void* stream) {
+    if (!p || !dst) return TT_ERR_NULL;
+    const size_t cs = 2 * esize(p->dtype);
+    TT_CUDA(p, cudaMemcpy2DAsync(dst, (size_t)p->N_m * cs, p->Fhat, (size_t)p->ldp * cs, (size_t)p->N_m * cs,
+                                 (size_t)p->n_f * (size_t)p->N_d, cudaMemcpyDeviceToDevice,
+                                 static_cast<cudaStream_t>(stream)));
+    return TT_OK;
+}
+
+int tt_matvec(const tt_plan* p, const void* m, void* d, void* stream) {
+    int r = check_apply(p, m, d);
+    if (r) return r;
+    p->ev_used = 4;
+    return run_matvec(p, m, d, static_cast<cudaStream_t>(stream), 0);
+}
+
+int tt_rmatvec(const tt_plan* p, const void* d, void* m, void* stream) {
+    int r = check_apply(p, d, m);
+    if (r) return r;
+    p->ev_used = 4;
+    return run_rmatvec(p, d, m, static_cast<cudaStream_t>(stream), 0);
+}
+
+int tt_normal(const tt_plan* p, const void* m, void* out, void* stream) {
+    int r = check_apply(p, m, out);
+    if (r) return r;
+    if (m == out) return TT_ERR_ALIAS;
+    p->ev_used = 8;
+    r = run_matvec(p, m, p->dwork, static_cast<cudaStream_t>(stream), 0);
+    if (r) return r;
+    return run_rmatvec(p, p->dwork, out, static_cast<cudaStream_t>(stream), 4);
+}
+
+// Interim k-RHS path: one pass of the single-vector kernels per right-hand side, addressing
+// column r through the strides of the fused FFT load/store.  (Replaced by the DMMA GEMM path.)
+int tt_matvec_batched(const tt_plan* p, int k, const void* M, void* D, void* stream) {
+    int r = check_apply(p, M, D);
+    if (r) return r;
+    if (k < 1 || k > p->k_max) return TT_ERR_K;
+    p->ev_used = 4;
+    for (int c = 0; c < k; ++c) {
+        r = run_matvec(p, M, D, static_cast<cudaStream_t>(stream), 0, k, c);
+        if (r) return r;
+    }
+    return TT_OK;
+}
+
+int tt_rmatvec_batched(const tt_plan* p, int k, const void* D, void* M, void* stream) {
+    int r = check_apply(p, D, M);
+    if (r) return r;
+    if (k < 1 || k > p->k_max) return TT_ERR_K;
+    p->ev_used = 4;
+    for (int c = 0; c < k; ++c) {
+        r = run_rmatvec(p, D, M, static_cast<cudaStream_t>(stream), 0, k, c);
+        if (r) return r;
+    }
+    return TT_OK;
+}
+
+int tt_matvec_host(const tt_plan* p, const void* m_host, void* d_host, void* stream) {
+    int r = check_apply(p, m_host, d_host);
+    if (r) return r;
+    r = ensure_staging(p);
+    if (r) return r;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t es = esize(p->dtype);
+    TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
+    p->ev_used = 4;
+    r = run_matvec(p, p->m_stage, p->d_stage, s, 0);
+    if (r) return r;
+    TT_CUDA(p, cudaMemcpyAsync(d_host, p->d_stage, (size_t)p->N_t * p->N_d * es, cudaMemcpyDeviceToHost, s));
+    return TT_OK;
+}
+
+int tt_rmatvec_host(const tt_plan* p, const void* d_host, void* m_host, void* stream) {
+    int r = check_apply(p, d_host, m_host);
+    if (r) return r;
+    r = ensure_staging(p);
+    if (r) return r;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t es = esize(p->dtype);
+    TT_CUDA(p, cudaMemcpyAsync(p->d_stage, d_host, (size_t)p->N_t * p->N_d * es, cudaMemcpyHostToDevice, s));
+    p->ev_used = 4;
+    r = run_rmatvec(p, p->d_stage, p->m_stage, s, 0);
+    if (r) return r;
+    TT_CUDA(p, cudaMemcpyAsync(m_host, p->m_stage, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
+    return TT_OK;
+}
+
+int tt_normal_host(const tt_plan* p, const void* m_host, void* out_host, void* stream) {
+    int r = check_apply(p, m_host, out_host);
+    if (r) return r;
+    r = ensure_staging(p);
+    if (r) return r;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t es = esize(p->dtype);
+    TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
+    p->ev_used = 8;
+    r = run_matvec(p, p->m_stage, p->dwork, s, 0);
+    if (r) return r;
+    r = run_rmatvec(p, p->dwork, p->m_stage2, s, 4);
+    if (r) return r;
+    TT_CUDA(p, cudaMemcpyAsync(out_host, p->m_stage2, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
+    return TT_OK;
+}
+
+int tt_plan_set_profiling(tt_plan* p, int enabled) {
+    if (!p) return TT_ERR_NULL;
+    p->prof = enabled != 0;
+    return TT_OK;
+}
+
+int tt_plan_stage_ms(const tt_plan* p, float* ms, int n) {
+    if (!p || !ms) return TT_ERR_NULL;
+    if (n < 3) return TT_ERR_SHAPE;
+    ms[0] = ms[1] = ms[2] = 0.f;
+    if (!p->prof) return TT_OK;
+    for (int base = 0; base + 4 <= p->ev_used; base += 4)
+        for (int i = 0; i < 3; ++i) {
+            float t = 0.f;
+            TT_CUDA(p, cudaEventElapsedTime(&t, p->ev[base + i], p->ev[base + i + 1]));
+            ms[i] += t;
+        }
+    return TT_OK;
+}
+
+int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* pos, double* tw) {
+    if (!n_stages || !radix || !pos || !tw) return TT_ERR_NULL;
+    if (N_t < 1) return TT_ERR_SHAPE;
+    int rx[kMaxStages] = {};
+    if (N_t > 65535 || !factorise(N_t, rx, n_stages)) return TT_ERR_UNSUPPORTED_NT;
+    for (int i = 0; i < kMaxStages; ++i) radix[i] = i < *n_stages ? rx[i] : 0;
+    std::vector<unsigned short> pv;
+    build_pos((int)N_t, rx, *n_stages, pv);
+    std::memcpy(pos, pv.data(), pv.size() * sizeof(unsigned short));
+    std::vector<double> tv;
+    build_twiddles(2 * (int)N_t, tv);
+    std::memcpy(tw, tv.data(), tv.size() * sizeof(double));
+    return TT_OK;
+}
+
+int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream) {
+    if (!src || !sink) return TT_ERR_NULL;
+    if (bytes % 16) return TT_ERR_SHAPE;
+    cudaError_t e = probe_stream_read_launch(src, bytes, sink, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
+    return TT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,79 @@
+// tt_internal.h - host-side declarations shared by the libtt translation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace tt {
+
+constexpr int kMaxStages = 16;
+constexpr int kMaxSmem = 232448;  // 227 KB: largest dynamic shared memory per CTA on sm_100
+
+// Geometry of one batched 1-D FFT launch along time.  A "series" is one time series of
+// N_t reals; the transforms use the packed real-FFT trick, i.e. one N-point complex FFT
+// (N = N_t) of z_n = x_{2n} + i x_{2n+1} stands for the L = 2N-point real FFT of the
+// zero-padded series.
+//
+// Element addresses (in elements of the respective type), series b in [0,B), y = blockIdx.y:
+//   real side    : real[y*r_ys + b*r_bs + j*r_ts]              j = 0..N-1   (time step)
+//   complex side : cplx[y*c_ys + b*c_bs + w*c_fs (+ c*c_ps)]    w = 0..N     (frequency)
+struct FftParams {
+    int N;                  // complex FFT length = N_t
+    int n_stages;
+    int radix[kMaxStages];  // product = N, applied in order as decimation-in-frequency stages
+    const void* tw;         // Cx<Tc>[2N]: tw[k] = exp(-2 pi i k / (2N))
+    const unsigned short* pos;  // pos[k] = slot of the in-place DIF output that holds bin k
+    long long B;            // series per y-row
+    long long B_store;      // forward only: series in [B, B_store) are stored as zeros (row padding)
+    long long r_ys, r_bs, r_ts;
+    long long c_ys, c_bs, c_fs;
+    int n_part;             // inverse only: the input is the sum of n_part partial spectra ...
+    long long c_ps;         // ... c_ps elements apart
+    double scale;           // inverse only: factor applied to the real output (1/L)
+};
+
+struct FftChoice {
+    int T;        // series per CTA
+    int threads;  // threads per CTA
+    size_t smem;  // dynamic shared memory bytes
+};
+// elem = sizeof(Cx<Tc>); returns T = 0 if even T = 8 does not fit.
+FftChoice fft_choose(int N, size_t elem);
+
+// tin/tc/tout: 0 = float, 1 = double.  ny = gridDim.y.
+cudaError_t fft_r2c_launch(int tin, int tc, int tout, const void* real_in, void* cplx_out,
+                           const FftParams& P, int ny, cudaStream_t s);
+cudaError_t fft_c2r_launch(int tc, const void* cplx_in, void* real_out, const FftParams& P, int ny,
+                           cudaStream_t s);
+
+// Per-frequency matvecs.  Fhat[(w*N_d + s)*ldp + p], xhat[w*ldp + p], dhat[w*N_d + s];
+// partial[(w*n_chunks + c)*N_d + s] = sum over chunk c of Fhat_w[s,:] xhat_w[:].
+struct GemvGeom {
+    int n_f;        // N_t + 1 frequencies
+    int N_d;
+    long long ldp;  // padded N_m (multiple of 16 elements)
+    int chunk;      // forward: elements of p per CTA (multiple of 64)
+    int n_chunks;
+};
+cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,
+                            cudaStream_t s);
+cudaError_t gemv_adj_launch(int dt, const void* Fhat, const void* dhat, void* xhat_out, const GemvGeom& g,
+                            cudaStream_t s);
+
+// k-RHS per-frequency complex GEMMs on the FP64 tensor pipe (DMMA) / fp32 FMA.
+//   Xhat[(w*N_m_pad... see tt_gemm.cu
+struct GemmGeom {
+    int n_f, N_d, k;
+    long long N_m, ldp;     // Fhat row pitch
+    long long ldx;          // Xhat pitch per frequency: Xhat[w*ldx + p*k + r]
+    int split;              // forward: number of p-splits (partials)
+    long long p_per_split;
+};
+cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g,
+                            cudaStream_t s);
+cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
+                            cudaStream_t s);
+
+cudaError_t probe_stream_read_launch(const void* src, size_t bytes, void* sink, cudaStream_t s);
+
+}  // namespace tt

@@ -1,0 +1,298 @@
+"""GPU parity: the CUDA path, called through the C ABI (libtt.so via the ctypes binding),
+against the CPU oracle (oracle/), element by element on the same seeded inputs.
+
+Bar (BASELINE.json north_star): relative L2 error over the whole output vector
+  <= 1e-12 for fp64/complex128,  <= 1e-5 for fp32/complex64.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import toeplitz_blocked as ob
+from oracle import toeplitz_plain as op
+from paper_2501_14911_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float64: 1e-12, torch.float32: 1e-5}
+
+
+@pytest.fixture(scope="module")
+def tt():
+    from paper_2501_14911_b200 import binding
+    binding.lib()
+    return binding
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
+
+
+def workload(base, N_d, N_m, N_t, dtype=None):
+    w = synth.CONFIGS[base].scaled(N_d=N_d, N_m=N_m, N_t=N_t)
+    if dtype is not None:
+        w = w.scaled(dtype=dtype)
+    return w
+
+
+def inputs(w):
+    F = synth.block_column(w)
+    m = synth.vector_m(w, k_rhs=1)
+    d = synth.vector_d(w, k_rhs=1)
+    return F, m, d
+
+
+# (base recipe, N_d, N_m, N_t): C1 as given; shrunken copies of C2..C5 that still span several
+# FFT tiles (32 series), several GEMV chunks (2048) and ragged tails; odd / prime-factor N_t.
+SHAPES = [
+    ("C1", 4, 64, 32),
+    ("C1", 3, 5, 7),
+    ("C1", 1, 1, 1),
+    ("C1", 2, 3, 1),
+    ("C1", 1, 4, 6),
+    ("C1", 4, 1, 5),
+    ("C1", 5, 100, 15),
+    ("C1", 3, 70, 35),
+    ("C1", 2, 33, 21),
+    ("C1", 2, 40, 49),
+    ("C2", 7, 1000, 50),
+    ("C2", 64, 4099, 64),
+    ("C2", 16, 6000, 256),
+    ("C3", 10, 5000, 400),
+    ("C3", 100, 2500, 100),
+    ("C4", 8, 4500, 512),
+    ("C5", 20, 3000, 400),
+    ("C5", 3, 2049, 500),
+    ("C2", 2, 17, 900),
+]
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("base,N_d,N_m,N_t", SHAPES)
+def test_matvec_rmatvec_normal_vs_oracle(tt, base, N_d, N_m, N_t, dtype):
+    w = workload(base, N_d, N_m, N_t, dtype)
+    F, m, d = inputs(w)
+    plan = tt.Plan(F.cuda())
+    try:
+        got_d = plan.matvec(m.cuda()).cpu().numpy()
+        got_m = plan.rmatvec(d.cuda()).cpu().numpy()
+        got_n = plan.normal(m.cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    orc = op if N_t * N_t * N_d * N_m < 2e6 else ob
+    ref_d = orc.matvec(F.numpy(), m.numpy())
+    ref_m = orc.rmatvec(F.numpy(), d.numpy())
+    ref_n = orc.rmatvec(F.numpy().astype(np.float64), ref_d)
+    tol = TOL[dtype]
+    assert rel(got_d, ref_d) <= tol
+    assert rel(got_m, ref_m) <= tol
+    assert rel(got_n, ref_n) <= tol
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_host_block_column_equals_device_block_column(tt, dtype):
+    w = workload("C2", 9, 700, 48, dtype)
+    F, m, _ = inputs(w)
+    p1, p2 = tt.Plan(F.cuda()), tt.Plan(F)  # device pointer / pageable host pointer
+    try:
+        assert torch.equal(p1.spectrum(), p2.spectrum())
+        assert torch.equal(p1.matvec(m.cuda()), p2.matvec(m.cuda()))
+    finally:
+        p1.close(); p2.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_spectrum_pins(tt, dtype):
+    """Fhat against what the mathematics fixes: DC and Nyquist bins, Parseval, a naive O(L^2) DFT."""
+    w = workload("C2", 3, 37, 20, dtype)
+    F = synth.block_column(w)
+    plan = tt.Plan(F.cuda())
+    try:
+        S = plan.spectrum().cpu().numpy().astype(np.complex128)
+    finally:
+        plan.close()
+    Fn = F.numpy().astype(np.float64)
+    N_t = w.N_t
+    L = 2 * N_t
+    tol = 1e-13 if dtype == torch.float64 else 2e-7
+    scale = np.abs(Fn).sum(axis=0).max()
+    assert np.abs(S[0] - Fn.sum(axis=0)).max() <= tol * scale
+    sign = (-1.0) ** np.arange(N_t)
+    assert np.abs(S[N_t] - np.tensordot(sign, Fn, axes=(0, 0))).max() <= tol * scale
+    assert np.abs(S[0].imag).max() == 0.0 and np.abs(S[N_t].imag).max() == 0.0
+    wts = np.full(N_t + 1, 2.0); wts[0] = wts[-1] = 1.0
+    lhs = np.tensordot(wts, np.abs(S) ** 2, axes=(0, 0))
+    rhs = L * (Fn ** 2).sum(axis=0)
+    assert np.abs(lhs - rhs).max() <= 50 * tol * rhs.max()
+    k = np.arange(N_t)
+    for (s, p) in [(0, 0), (2, 36), (1, 17)]:
+        for om in [1, 7, N_t - 1]:
+            naive = np.sum(Fn[:, s, p] * np.exp(-2j * np.pi * om * k / L))
+            assert abs(S[om, s, p] - naive) <= tol * scale
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_impulse_returns_block_column(tt, dtype):
+    """m = e_(j0,p0) => d_i = F_{i-j0}[:,p0] for i >= j0, ~0 before (causality); adjoint with the
+    impulse at the LAST step returns F_{N_t-1-j}[s0,:] (catches keeping the wrong half)."""
+    w = workload("C1", 4, 64, 32, dtype)
+    F = synth.block_column(w)
+    Fn = F.numpy().astype(np.float64)
+    N_t, N_d, N_m = F.shape
+    tol = TOL[dtype]
+    plan = tt.Plan(F.cuda())
+    try:
+        j0, p0 = 5, 17
+        m = torch.zeros((N_t, N_m), dtype=dtype); m[j0, p0] = 1.0
+        d = plan.matvec(m.cuda()).cpu().numpy().astype(np.float64)
+        expect = np.zeros((N_t, N_d)); expect[j0:] = Fn[: N_t - j0, :, p0]
+        assert np.linalg.norm(d - expect) <= tol * np.linalg.norm(expect)
+        assert np.abs(d[:j0]).max() <= tol * np.abs(Fn).max()
+        i0, s0 = N_t - 1, 2
+        dd = torch.zeros((N_t, N_d), dtype=dtype); dd[i0, s0] = 1.0
+        mm = plan.rmatvec(dd.cuda()).cpu().numpy().astype(np.float64)
+        expect = Fn[::-1][:, s0, :]  # m'_j = F_{i0-j}[s0,:]
+        assert np.linalg.norm(mm - expect) <= tol * np.linalg.norm(expect)
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_adjoint_identity_linearity_shift_on_gpu(tt, dtype):
+    w = workload("C5", 6, 777, 60, dtype)
+    F, m, d = inputs(w)
+    tol = TOL[dtype]
+    plan = tt.Plan(F.cuda())
+    try:
+        mc, dc = m.cuda(), d.cuda()
+        Fm = plan.matvec(mc).double()
+        Ftd = plan.rmatvec(dc).double()
+        lhs = float((Fm * dc.double()).sum()); rhs = float((mc.double() * Ftd).sum())
+        assert abs(lhs - rhs) <= 10 * tol * float(Fm.norm() * dc.double().norm())
+        # linearity
+        m2 = synth.vector_m(w.scaled(seed=w.seed + 100), k_rhs=1).cuda()
+        comb = plan.matvec((2.0 * mc - 3.0 * m2)).double()
+        sep = 2.0 * Fm - 3.0 * plan.matvec(m2).double()
+        assert float((comb - sep).norm()) <= 10 * tol * float(sep.norm())
+        # shift equivariance (block Toeplitz): delaying m by tau delays d by tau
+        tau = 7
+        ms = torch.zeros_like(mc); ms[tau:] = mc[:-tau]
+        ds = plan.matvec(ms).double()
+        assert float((ds[tau:] - Fm[:-tau]).norm()) <= 10 * tol * float(Fm.norm())
+        assert float(ds[:tau].abs().max()) <= 10 * tol * float(Fm.abs().max())
+        # normal operator: <m, F^T F m> = |F m|^2
+        n = plan.normal(mc).double()
+        assert abs(float((mc.double() * n).sum()) - float(Fm.norm() ** 2)) <= 10 * tol * float(Fm.norm() ** 2)
+    finally:
+        plan.close()
+
+
+def test_exact_integer_case(tt):
+    """Small-integer F and m: every sum is exact in fp64, so the fp64 GPU result rounds to the exact integers."""
+    rng = np.random.default_rng(5)
+    F = torch.from_numpy(rng.integers(-3, 4, size=(16, 3, 50)).astype(np.float64))
+    m = torch.from_numpy(rng.integers(-3, 4, size=(16, 50)).astype(np.float64))
+    plan = tt.Plan(F.cuda())
+    try:
+        d = plan.matvec(m.cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    ref = op.matvec(F.numpy(), m.numpy())
+    assert np.array_equal(np.rint(d), ref)
+    assert np.abs(d - ref).max() < 1e-9
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("k", [1, 3, 8, 32])
+def test_batched_columns_equal_oracle(tt, dtype, k):
+    w = workload("C4", 6, 300, 32, dtype)
+    F = synth.block_column(w)
+    M = synth.vector_m(w, k_rhs=k).reshape(w.N_t, w.N_m, k)
+    D = synth.vector_d(w, k_rhs=k).reshape(w.N_t, w.N_d, k)
+    plan = tt.Plan(F.cuda(), k_max=32)
+    try:
+        gd = plan.matvec_batched(M.cuda()).cpu().numpy()
+        gm = plan.rmatvec_batched(D.cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    rd = op.matvec(F.numpy(), M.numpy())
+    rm = op.rmatvec(F.numpy(), D.numpy())
+    tol = TOL[dtype]
+    for r in range(k):
+        assert rel(gd[..., r], rd[..., r]) <= tol
+        assert rel(gm[..., r], rm[..., r]) <= tol
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_space_major_layout(tt, dtype):
+    """TT_SPACE_MAJOR (time contiguous, the 'm (64x32)' shapes of BASELINE.json) gives the same numbers."""
+    w = workload("C1", 4, 64, 32, dtype)
+    F, m, d = inputs(w)
+    plan = tt.Plan(F.cuda(), layout=tt.TT_SPACE_MAJOR, k_max=2)
+    try:
+        gd = plan.matvec(m.t().contiguous().cuda()).cpu().numpy().T
+        gm = plan.rmatvec(d.t().contiguous().cuda()).cpu().numpy().T
+        M = synth.vector_m(w, k_rhs=2)                      # [N_t, N_m, 2]
+        gD = plan.matvec_batched(M.permute(2, 1, 0).contiguous().cuda()).cpu().numpy()  # [2, N_d, N_t]
+    finally:
+        plan.close()
+    tol = TOL[dtype]
+    assert rel(gd, op.matvec(F.numpy(), m.numpy())) <= tol
+    assert rel(gm, op.rmatvec(F.numpy(), d.numpy())) <= tol
+    rD = op.matvec(F.numpy(), M.numpy())
+    assert rel(np.transpose(gD, (2, 1, 0)), rD) <= tol
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+def test_host_vector_calls(tt, dtype):
+    w = workload("C3", 5, 1200, 40, dtype)
+    F, m, d = inputs(w)
+    plan = tt.Plan(F.cuda())
+    try:
+        mh, dh = m.pin_memory(), d.pin_memory()
+        d_out = torch.empty_like(d).pin_memory()
+        m_out = torch.empty_like(m).pin_memory()
+        n_out = torch.empty_like(m).pin_memory()
+        tt.tt_matvec_host(plan.handle, mh, d_out)
+        tt.tt_rmatvec_host(plan.handle, dh, m_out)
+        tt.tt_normal_host(plan.handle, mh, n_out)
+        torch.cuda.synchronize()
+        assert torch.equal(d_out, plan.matvec(m.cuda()).cpu())
+        assert torch.equal(m_out, plan.rmatvec(d.cuda()).cpu())
+        assert torch.equal(n_out, plan.normal(m.cuda()).cpu())
+    finally:
+        plan.close()
+
+
+def test_error_codes(tt):
+    import ctypes
+    L = tt.lib()
+    F = torch.zeros((11, 2, 3), dtype=torch.float64, device="cuda")
+    out = ctypes.c_void_p()
+    st = torch.cuda.current_stream().cuda_stream
+
+    def create(N_d, N_m, N_t, dtype=tt.TT_F64, layout=0, k=1, ptr=F.data_ptr()):
+        return L.tt_plan_create(ctypes.byref(out), N_d, N_m, N_t, dtype, layout, k, ptr, st)
+
+    assert tt.tt_status_string(create(2, 3, 11)) == "TT_ERR_UNSUPPORTED_NT"
+    assert tt.tt_status_string(create(2, 3, 4000)) == "TT_ERR_UNSUPPORTED_NT"
+    assert tt.tt_status_string(create(0, 3, 8)) == "TT_ERR_SHAPE"
+    assert tt.tt_status_string(create(2, -1, 8)) == "TT_ERR_SHAPE"
+    assert tt.tt_status_string(create(2, 3, 8, dtype=7)) == "TT_ERR_DTYPE"
+    assert tt.tt_status_string(create(2, 3, 8, layout=9)) == "TT_ERR_LAYOUT"
+    assert tt.tt_status_string(create(2, 3, 8, k=0)) == "TT_ERR_K"
+    assert tt.tt_status_string(create(2, 3, 8, ptr=None)) == "TT_ERR_NULL"
+    assert out.value is None
+    plan = tt.Plan(F[:10].contiguous(), k_max=2)
+    try:
+        v = torch.zeros((10, 3), dtype=torch.float64, device="cuda")
+        assert tt.tt_status_string(L.tt_normal(plan.handle, v.data_ptr(), v.data_ptr(), st)) == "TT_ERR_ALIAS"
+        assert tt.tt_status_string(L.tt_matvec(plan.handle, None, v.data_ptr(), st)) == "TT_ERR_NULL"
+        assert tt.tt_status_string(L.tt_matvec_batched(plan.handle, 3, v.data_ptr(), v.data_ptr(), st)) == "TT_ERR_K"
+        assert plan.device_bytes > 0
+    finally:
+        plan.close()
+    L.tt_plan_destroy(None)  # NULL-safe
