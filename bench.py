@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py - ms per F.m and F^T.d at ~1e8 parameters, and achieved HBM GB/s vs the B200 peak.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: d = F m (kernels A1, A2, A3) followed by
+m' = F^T d (B1, B2, B3) on the BASELINE.json configs[2] workload (C3: N_d=100, N_m=250000,
+N_t=400, fp32 vectors, complex64 spectrum of 80.2 GB), synthetic seeded inputs resident in HBM.
+The JSON line carries
+  value      ms per step (one F.m plus one F^T.d), device time, max over ranks, / n_gpus
+  e2e        the same through tt_matvec_host / tt_rmatvec_host with pinned HOST vectors
+             (H2D of the input and D2H of the result inside the timed region)
+  roofline   the dominant kernel (the per-frequency matvec that streams Fhat): algorithmic
+             bytes per launch / its mean launch duration, measured live with CUDA events
+             recorded by the library on the launching stream, vs MEASURED_PEAKS.json
+  cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a
+             bounded sample of the same workload, extrapolated by the MAC count
+Multi-GPU: the north star is a one-GPU path (no sharding, no collectives): --gpus N runs N
+independent replicas ("replicas only"), timed as the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2501_14911_b200 import synth  # noqa: E402
+
+METRIC = "ms per F·m and F^T·d at ~1e8 params; achieved HBM GB/s vs B200 peak"
+NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0    # B200_PROFILING.md fallback
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return json.load(f), "measured"
+    except OSError:
+        return {"hbm_gbs": FALLBACK_HBM_GBS}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+            time.sleep(0.3)
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(w, F_s, m_s, d_s):
+    """Times the CPU oracle (blocked C build) on a sample; returns (seconds matvec, seconds rmatvec, threads)."""
+    from oracle import toeplitz_blocked as ob
+    ob.build()
+    t0 = time.perf_counter(); ob.matvec(F_s, m_s); t1 = time.perf_counter()
+    ob.rmatvec(F_s, d_s); t2 = time.perf_counter()
+    return t1 - t0, t2 - t1, ob.num_threads()
+
+
+def cpu_baseline(w, draw, target_s=15.0):
+    """draw(ns, npar) -> (F_s [N_t,ns,npar], m_s [N_t,npar], d_s [N_t,ns]) numpy.  Extrapolates by MAC count."""
+    npar = min(w.N_m, 25000)
+    ns = min(w.N_d, 2)
+    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # calibration (also warms the library)
+    per_sensor = max(1e-3, (ta + tb) / ns)
+    ns2 = int(max(ns, min(w.N_d, 40, round(target_s / per_sensor))))
+    ta, tb, thr = oracle_sample(w, *draw(ns2, npar))
+    scale = (w.N_d * w.N_m) / float(ns2 * npar)
+    return {
+        "value": (ta + tb) * scale * 1e3, "unit": "ms", "cores": thr, "kind": "oracle",
+        "sample": (f"oracle/toeplitz_blocked.c (direct O(N_t^2) block convolution, fp64) timed on sensors 0..{ns2 - 1} x "
+                   f"parameters 0..{npar - 1} x all {w.N_t} steps of the same workload ({ta + tb:.2f} s for F.m + F^T.d), "
+                   f"scaled by N_d*N_m/(sample) = {scale:.1f} to the full matvec pair"),
+        "matvec_ms": ta * scale * 1e3, "rmatvec_ms": tb * scale * 1e3,
+    }
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on the host cores, each step one bounded sample, same metric."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    npar, ns = min(w.N_m, 25000), min(w.N_d, 4)
+    F_s = synth.block_column(w, s_range=(0, ns), p_range=(0, npar)).numpy()
+    m_s = synth.vector_m(w.scaled(N_m=npar), k_rhs=1).numpy()
+    d_s = synth.vector_d(w.scaled(N_d=ns), k_rhs=1).numpy()
+    thr = 0
+    for _ in range(args.warmup):
+        _, _, thr = oracle_sample(w, F_s, m_s, d_s)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, _, thr = oracle_sample(w, F_s, m_s, d_s)
+    dt = (time.perf_counter() - t0) / args.steps
+    scale = (w.N_d * w.N_m) / float(ns * npar)
+    ms = dt * scale * 1e3
+    sample = (f"each step = oracle F.m + F^T.d on sensors 0..{ns - 1} x parameters 0..{npar - 1} x all {w.N_t} steps "
+              f"({dt:.2f} s), scaled by {scale:.1f} to the full workload")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": config_dict(w, args),
+        "cpu_baseline": {"value": ms, "unit": "ms", "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+    return 0
+
+
+def config_dict(w, args):
+    return {"workload": f"{w.name}: N_d={w.N_d}, N_m={w.N_m}, N_t={w.N_t} ({w.n_params:.3g} parameters), "
+                        f"{'fp32 vectors / complex64 spectrum' if w.dtype == torch.float32 else 'fp64 / complex128'}",
+            "baseline_config": args.config, "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)",
+            "layout": "time-major", "parallelism": "replicas only" if args.gpus > 1 else "single GPU",
+            "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = synth.CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libtt has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_2501_14911_b200 import binding as tt
+    tt.lib()
+    dev = torch.device("cuda", local_rank)
+    es = 4 if w.dtype == torch.float32 else 8
+
+    # ---- inputs, resident in HBM ----------------------------------------------------------
+    t0 = time.perf_counter()
+    F = synth.block_column(w, device=dev)
+    m = synth.vector_m(w, device=dev, k_rhs=1)
+    d = synth.vector_d(w, device=dev, k_rhs=1)
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t0
+
+    def draw(ns, npar):  # the CPU baseline's sample: the same bytes, copied from the device
+        return (F[:, :ns, :npar].contiguous().cpu().numpy(), m[:, :npar].contiguous().cpu().numpy(),
+                d[:, :ns].contiguous().cpu().numpy())
+
+    samples = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        # fetch the largest sample cpu_baseline() may ask for before the column is freed
+        samples = draw(min(w.N_d, 40), min(w.N_m, 25000))
+
+    t0 = time.perf_counter()
+    plan = tt.Plan(F)
+    torch.cuda.synchronize()
+    t_plan = time.perf_counter() - t0
+    del F
+    torch.cuda.empty_cache()
+
+    stream = torch.cuda.Stream(device=dev)
+    d_out = torch.empty_like(d)
+    m_out = torch.empty_like(m)
+    h = plan.handle
+
+    def step():
+        tt.tt_matvec(h, m, d_out, stream)
+        tt.tt_rmatvec(h, d, m_out, stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            step()
+    barrier()
+
+    # ---- timed region: device-resident ------------------------------------------------------
+    tt.tt_plan_set_profiling(h, True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev0.record(stream)
+        for _ in range(args.steps):
+            step()
+        ev1.record(stream)
+        barrier()
+    ms_step = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
+    fwd = tt.tt_plan_stage_ms(h, tt.TT_OP_MATVEC)
+    adj = tt.tt_plan_stage_ms(h, tt.TT_OP_RMATVEC)
+    tt.tt_plan_set_profiling(h, False)
+
+    # ---- separate ms per F.m and per F^T.d (same launch configuration) -----------------------
+    def time_op(fn, n):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(stream)
+        for _ in range(n):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    ms_fwd = max_over_ranks(time_op(lambda: tt.tt_matvec(h, m, d_out, stream), args.steps))
+    ms_adj = max_over_ranks(time_op(lambda: tt.tt_rmatvec(h, d, m_out, stream), args.steps))
+
+    # ---- end to end through the C ABI with HOST vectors -------------------------------------
+    m_h, d_h = m.cpu().pin_memory(), d.cpu().pin_memory()
+    d_oh, m_oh = torch.empty_like(d_h).pin_memory(), torch.empty_like(m_h).pin_memory()
+
+    def step_host():
+        tt.tt_matvec_host(h, m_h, d_oh, stream)
+        tt.tt_rmatvec_host(h, d_h, m_oh, stream)
+
+    step_host()
+    torch.cuda.synchronize()
+    n_e2e = max(2, min(args.steps, 5))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        step_host()
+    stream.synchronize()
+    ms_e2e = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e)
+    h2d = (m_h.numel() + d_h.numel()) * es
+    d2h = (d_oh.numel() + m_oh.numel()) * es
+
+    # ---- roofline of the dominant kernel ---------------------------------------------------
+    peaks, peak_kind = measured_peaks()
+    peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
+    n_f, ldp = w.N_t + 1, (w.N_m + 15) // 16 * 16
+    fhat_bytes = n_f * w.N_d * ldp * 2 * es
+    xhat_bytes = n_f * ldp * 2 * es
+    dhat_bytes = n_f * w.N_d * 2 * es
+    n_chunks = (ldp + 2047) // 2048
+    part_bytes = n_f * n_chunks * w.N_d * 2 * es
+    bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
+    bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written
+    vec_bytes = (w.N_t * w.N_m + w.N_t * w.N_d) * es
+    bytes_op = fhat_bytes + vec_bytes                           # north_star: |Fhat| plus the vectors
+    ach_fwd = bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0
+    ach_adj = bytes_adj_kernel / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
+    roofline = {
+        "bound": "hbm", "kernel": "gemv_fwd_kernel (A2, per-frequency matvec streaming Fhat)",
+        "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak, "traffic": None,
+        "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
+                     else "fallback 6.65 TB/s (B200_PROFILING.md)",
+        "algorithmic_bytes_per_launch": bytes_fwd_kernel, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
+        "frac_of_nominal_8TBs": ach_fwd / NOMINAL_HBM_GBS,
+        "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
+                           "algorithmic_bytes_per_launch": bytes_adj_kernel, "ms_per_launch": adj[1],
+                           "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
+    }
+
+    # ---- bandwidth probes in the same run (copy and read-only stream) -------------------------
+    probe = {}
+    try:
+        nb = 8 << 30
+        a = torch.empty(nb, dtype=torch.uint8, device=dev); a.zero_()
+        b = torch.empty(nb, dtype=torch.uint8, device=dev)
+        sink = torch.empty(1 << 16, dtype=torch.uint8, device=dev)
+        with torch.cuda.stream(stream):
+            probe["read_only_gbs"] = nb / (min(time_op(lambda: tt.tt_probe_stream_read(a, nb, sink, stream), 5)
+                                               for _ in range(3)) * 1e-3) / 1e9
+            probe["copy_gbs"] = 2 * nb / (min(time_op(lambda: b.copy_(a), 5) for _ in range(3)) * 1e-3) / 1e9
+        del a, b
+    except RuntimeError as e:  # pragma: no cover
+        probe["error"] = str(e)
+
+    out = {
+        "metric": METRIC, "value": ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if w.dtype == torch.float32 else "f64", "data": "synthetic",
+        "config": config_dict(w, args),
+        "e2e": {"value": ms_e2e / args.gpus, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": n_e2e, "api": "tt_matvec_host + tt_rmatvec_host, pinned host vectors"},
+        "gpu_launches": 6 * args.steps,
+        "clocks": clocks.summary(),
+        "roofline": roofline,
+        "ops": {
+            "matvec_ms": ms_fwd, "rmatvec_ms": ms_adj,
+            "matvec_GBs": bytes_op / (ms_fwd * 1e-3) / 1e9, "rmatvec_GBs": bytes_op / (ms_adj * 1e-3) / 1e9,
+            "roofline_bytes_per_op": bytes_op,
+            "matvec_frac_of_8TBs": bytes_op / (ms_fwd * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "rmatvec_frac_of_8TBs": bytes_op / (ms_adj * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "matvec_frac_of_measured_copy": bytes_op / (ms_fwd * 1e-3) / 1e9 / peak,
+            "rmatvec_frac_of_measured_copy": bytes_op / (ms_adj * 1e-3) / 1e9 / peak,
+            "stages_matvec_ms": {"A1_fft": fwd[0], "A2_gemv": fwd[1], "A3_reduce_ifft": fwd[2]},
+            "stages_rmatvec_ms": {"B1_fft": adj[0], "B2_gemv": adj[1], "B3_ifft": adj[2]},
+        },
+        "probe": probe,
+        "plan": {"create_s": t_plan, "device_bytes": plan.device_bytes, "input_generation_s": t_gen},
+    }
+
+    # ---- CPU baseline: the oracle on this box's host cores, bounded sample -------------------
+    if samples is not None:
+        Fs, ms_, ds_ = samples
+
+        def draw_cached(ns, npar):
+            return (Fs[:, :ns, :npar].copy(), ms_[:, :npar].copy(), ds_[:, :ns].copy())
+
+        out["cpu_baseline"] = cpu_baseline(w, draw_cached)
+        out["cpu_baseline"]["note"] = "reported baseline, not the optimisation target"
+
+    plan.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -148,14 +148,19 @@ int tt_normal_host(const tt_plan* plan, const void* m_host, void* out_host, void
 /* Measurement hooks (bench.py's roofline object).
  *
  * tt_plan_set_profiling(plan, 1) makes every apply call record CUDA events, on the stream
- * it launches on, around each of its kernels; tt_plan_stage_ms() then returns, after the
- * caller has synchronised that stream, the device time of the stages of the LAST apply
- * call: ms[0] forward FFT of the input, ms[1] per-frequency matvec / matmul (the kernel
- * that streams Fhat), ms[2] inverse FFT (+ partial reduce).  tt_normal reports the sum of
- * its two halves.  n = number of floats ms can hold (>= 3).
+ * it launches on, around each of its kernels, and forgets earlier records; the last 64
+ * profiled calls are kept.  After the caller has synchronised that stream,
+ * tt_plan_stage_ms(plan, op, ms, n) returns the device time per call, averaged over the
+ * recorded calls of kind `op` (a tt_op): ms[0] forward FFT of the input, ms[1] the kernel that
+ * streams Fhat (per-frequency matvec / matmul), ms[2] inverse FFT (+ partial reduce),
+ * ms[3] = number of calls averaged (0: nothing recorded).  TT_OP_NORMAL reports the sum of
+ * its two halves.  n = number of floats ms can hold (>= 4).
  */
+typedef enum tt_op {
+    TT_OP_MATVEC = 0, TT_OP_RMATVEC = 1, TT_OP_NORMAL = 2, TT_OP_MATVEC_BATCHED = 3, TT_OP_RMATVEC_BATCHED = 4
+} tt_op;
 int tt_plan_set_profiling(tt_plan* plan, int enabled);
-int tt_plan_stage_ms(const tt_plan* plan, float* ms, int n);
+int tt_plan_stage_ms(const tt_plan* plan, int op, float* ms, int n);
 
 /* Read-only streaming probe: sums `bytes` (multiple of 16) of device memory at `src` with
  * 128-bit loads and writes one 16-byte result per CTA to `sink` (>= 16*4096 bytes).  Used

@@ -18,6 +18,7 @@ from . import build as _build
 TT_F32, TT_F64 = 0, 1
 TT_TIME_MAJOR, TT_SPACE_MAJOR = 0, 1
 TT_OK = 0
+TT_OP_MATVEC, TT_OP_RMATVEC, TT_OP_NORMAL, TT_OP_MATVEC_BATCHED, TT_OP_RMATVEC_BATCHED = range(5)
 
 _lib = None
 
@@ -64,7 +65,7 @@ def lib() -> ctypes.CDLL:
         "tt_rmatvec_host": (ci, [vp, vp, vp, vp]),
         "tt_normal_host": (ci, [vp, vp, vp, vp]),
         "tt_plan_set_profiling": (ci, [vp, ci]),
-        "tt_plan_stage_ms": (ci, [vp, ctypes.POINTER(ctypes.c_float), ci]),
+        "tt_plan_stage_ms": (ci, [vp, ci, ctypes.POINTER(ctypes.c_float), ci]),
         "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
         "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
@@ -171,10 +172,11 @@ def tt_plan_set_profiling(plan: int, enabled: bool) -> None:
     _check("tt_plan_set_profiling", lib().tt_plan_set_profiling(plan, int(bool(enabled))), plan)
 
 
-def tt_plan_stage_ms(plan: int) -> tuple[float, float, float]:
-    buf = (ctypes.c_float * 3)()
-    _check("tt_plan_stage_ms", lib().tt_plan_stage_ms(plan, buf, 3), plan)
-    return float(buf[0]), float(buf[1]), float(buf[2])
+def tt_plan_stage_ms(plan: int, op: int) -> tuple[float, float, float, int]:
+    """(fft_ms, stream_kernel_ms, ifft_ms, n_calls) averaged over the recorded calls of kind `op`."""
+    buf = (ctypes.c_float * 4)()
+    _check("tt_plan_stage_ms", lib().tt_plan_stage_ms(plan, op, buf, 4), plan)
+    return float(buf[0]), float(buf[1]), float(buf[2]), int(buf[3])
 
 
 def tt_probe_stream_read(src, nbytes: int, sink, stream=None) -> None:

@@ -16,7 +16,8 @@ using namespace tt;
 namespace {
 
 constexpr int kVersion = 100;  // 0.1.0
-constexpr int kNumEvents = 8;
+constexpr int kRing = 64;       // profiled apply calls remembered
+constexpr int kSlotEvents = 8;  // two kernel triples (tt_normal) x 4 marks
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
 
@@ -44,8 +45,10 @@ struct tt_plan {
     size_t bytes = 0;
     mutable int last_cuda = 0;
     bool prof = false;
-    cudaEvent_t ev[kNumEvents] = {};
-    mutable int ev_used = 0;
+    cudaEvent_t* ev = nullptr;  // kRing * kSlotEvents, created by tt_plan_set_profiling
+    mutable int slot_op[kRing];
+    mutable int slot_sets[kRing];
+    mutable long long n_calls = 0;  // profiled apply calls so far
 };
 
 namespace {
@@ -155,6 +158,16 @@ struct Prof {
         if (p->prof) cudaEventRecord(p->ev[base + i], s);
     }
 };
+
+// Claims the next ring slot for a profiled apply call; returns its first event index.
+int begin_call(const tt_plan* p, int op, int sets) {
+    if (!p->prof) return 0;
+    const int slot = (int)(p->n_calls % kRing);
+    p->slot_op[slot] = op;
+    p->slot_sets[slot] = sets;
+    ++p->n_calls;
+    return slot * kSlotEvents;
+}
 
 // d = F m on device buffers (steps A1, A2, A3).
 int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_base, int k = 1, int r = 0) {
@@ -282,8 +295,11 @@ void tt_plan_destroy(tt_plan* p) {
                     p->dwork, p->m_stage, p->m_stage2, p->d_stage};
     for (void* b : bufs)
         if (b) cudaFree(b);
-    for (int i = 0; i < kNumEvents; ++i)
-        if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    if (p->ev) {
+        for (int i = 0; i < kRing * kSlotEvents; ++i)
+            if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+        delete[] p->ev;
+    }
     delete p;
 }
 
@@ -373,7 +389,6 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     TT_TRY(dev_alloc(p, &p->dhat, (size_t)p->n_f * N_d * k_max * cs));
     TT_TRY(dev_alloc(p, &p->partial, (size_t)p->n_f * p->n_chunks * N_d * k_max * cs));
     TT_TRY(dev_alloc(p, &p->dwork, (size_t)N_t * N_d * k_max * es));
-    for (int i = 0; i < kNumEvents; ++i) TT_TRYC(cudaEventCreate(&p->ev[i]));
 
     // P0: transform the block column (device pointer: in place; host pointer: by sensor slabs)
     cudaPointerAttributes attr;
@@ -432,25 +447,23 @@ int tt_plan_get_spectrum(const tt_plan* p, void* dst, void* stream) {
 int tt_matvec(const tt_plan* p, const void* m, void* d, void* stream) {
     int r = check_apply(p, m, d);
     if (r) return r;
-    p->ev_used = 4;
-    return run_matvec(p, m, d, static_cast<cudaStream_t>(stream), 0);
+    return run_matvec(p, m, d, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC, 1));
 }
 
 int tt_rmatvec(const tt_plan* p, const void* d, void* m, void* stream) {
     int r = check_apply(p, d, m);
     if (r) return r;
-    p->ev_used = 4;
-    return run_rmatvec(p, d, m, static_cast<cudaStream_t>(stream), 0);
+    return run_rmatvec(p, d, m, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC, 1));
 }
 
 int tt_normal(const tt_plan* p, const void* m, void* out, void* stream) {
     int r = check_apply(p, m, out);
     if (r) return r;
     if (m == out) return TT_ERR_ALIAS;
-    p->ev_used = 8;
-    r = run_matvec(p, m, p->dwork, static_cast<cudaStream_t>(stream), 0);
+    const int e0 = begin_call(p, TT_OP_NORMAL, 2);
+    r = run_matvec(p, m, p->dwork, static_cast<cudaStream_t>(stream), e0);
     if (r) return r;
-    return run_rmatvec(p, p->dwork, out, static_cast<cudaStream_t>(stream), 4);
+    return run_rmatvec(p, p->dwork, out, static_cast<cudaStream_t>(stream), e0 + 4);
 }
 
 // Interim k-RHS path: one pass of the single-vector kernels per right-hand side, addressing
@@ -459,9 +472,8 @@ int tt_matvec_batched(const tt_plan* p, int k, const void* M, void* D, void* str
     int r = check_apply(p, M, D);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
-    p->ev_used = 4;
     for (int c = 0; c < k; ++c) {
-        r = run_matvec(p, M, D, static_cast<cudaStream_t>(stream), 0, k, c);
+        r = run_matvec(p, M, D, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC_BATCHED, 1), k, c);
         if (r) return r;
     }
     return TT_OK;
@@ -471,9 +483,8 @@ int tt_rmatvec_batched(const tt_plan* p, int k, const void* D, void* M, void* st
     int r = check_apply(p, D, M);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
-    p->ev_used = 4;
     for (int c = 0; c < k; ++c) {
-        r = run_rmatvec(p, D, M, static_cast<cudaStream_t>(stream), 0, k, c);
+        r = run_rmatvec(p, D, M, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC_BATCHED, 1), k, c);
         if (r) return r;
     }
     return TT_OK;
@@ -487,8 +498,7 @@ int tt_matvec_host(const tt_plan* p, const void* m_host, void* d_host, void* str
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
     TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
-    p->ev_used = 4;
-    r = run_matvec(p, p->m_stage, p->d_stage, s, 0);
+    r = run_matvec(p, p->m_stage, p->d_stage, s, begin_call(p, TT_OP_MATVEC, 1));
     if (r) return r;
     TT_CUDA(p, cudaMemcpyAsync(d_host, p->d_stage, (size_t)p->N_t * p->N_d * es, cudaMemcpyDeviceToHost, s));
     return TT_OK;
@@ -502,8 +512,7 @@ int tt_rmatvec_host(const tt_plan* p, const void* d_host, void* m_host, void* st
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
     TT_CUDA(p, cudaMemcpyAsync(p->d_stage, d_host, (size_t)p->N_t * p->N_d * es, cudaMemcpyHostToDevice, s));
-    p->ev_used = 4;
-    r = run_rmatvec(p, p->d_stage, p->m_stage, s, 0);
+    r = run_rmatvec(p, p->d_stage, p->m_stage, s, begin_call(p, TT_OP_RMATVEC, 1));
     if (r) return r;
     TT_CUDA(p, cudaMemcpyAsync(m_host, p->m_stage, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
     return TT_OK;
@@ -517,10 +526,10 @@ int tt_normal_host(const tt_plan* p, const void* m_host, void* out_host, void* s
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
     TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
-    p->ev_used = 8;
-    r = run_matvec(p, p->m_stage, p->dwork, s, 0);
+    const int e0 = begin_call(p, TT_OP_NORMAL, 2);
+    r = run_matvec(p, p->m_stage, p->dwork, s, e0);
     if (r) return r;
-    r = run_rmatvec(p, p->dwork, p->m_stage2, s, 4);
+    r = run_rmatvec(p, p->dwork, p->m_stage2, s, e0 + 4);
     if (r) return r;
     TT_CUDA(p, cudaMemcpyAsync(out_host, p->m_stage2, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
     return TT_OK;
@@ -528,21 +537,37 @@ int tt_normal_host(const tt_plan* p, const void* m_host, void* out_host, void* s
 
 int tt_plan_set_profiling(tt_plan* p, int enabled) {
     if (!p) return TT_ERR_NULL;
+    if (enabled && !p->ev) {
+        p->ev = new (std::nothrow) cudaEvent_t[kRing * kSlotEvents]();
+        if (!p->ev) return TT_ERR_OOM;
+        for (int i = 0; i < kRing * kSlotEvents; ++i) TT_CUDA(p, cudaEventCreate(&p->ev[i]));
+    }
     p->prof = enabled != 0;
+    p->n_calls = 0;
     return TT_OK;
 }
 
-int tt_plan_stage_ms(const tt_plan* p, float* ms, int n) {
+int tt_plan_stage_ms(const tt_plan* p, int op, float* ms, int n) {
     if (!p || !ms) return TT_ERR_NULL;
-    if (n < 3) return TT_ERR_SHAPE;
-    ms[0] = ms[1] = ms[2] = 0.f;
-    if (!p->prof) return TT_OK;
-    for (int base = 0; base + 4 <= p->ev_used; base += 4)
-        for (int i = 0; i < 3; ++i) {
-            float t = 0.f;
-            TT_CUDA(p, cudaEventElapsedTime(&t, p->ev[base + i], p->ev[base + i + 1]));
-            ms[i] += t;
-        }
+    if (n < 4) return TT_ERR_SHAPE;
+    ms[0] = ms[1] = ms[2] = ms[3] = 0.f;
+    if (!p->ev) return TT_OK;
+    const int have = p->n_calls < kRing ? (int)p->n_calls : kRing;
+    double acc[3] = {0, 0, 0};
+    int count = 0;
+    for (int slot = 0; slot < have; ++slot) {
+        if (p->slot_op[slot] != op) continue;
+        for (int set = 0; set < p->slot_sets[slot]; ++set)
+            for (int i = 0; i < 3; ++i) {
+                float t = 0.f;
+                const int e = slot * kSlotEvents + set * 4 + i;
+                TT_CUDA(p, cudaEventElapsedTime(&t, p->ev[e], p->ev[e + 1]));
+                acc[i] += t;
+            }
+        ++count;
+    }
+    if (count) for (int i = 0; i < 3; ++i) ms[i] = (float)(acc[i] / count);
+    ms[3] = (float)count;
     return TT_OK;
 }
 
