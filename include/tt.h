@@ -172,8 +172,19 @@ int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream
  *   radix     int[16], receives their radices (product = N_t)
  *   pos       unsigned short[N_t], pos[k] = slot of the in-place DIF output holding bin k
  *   tw        double[4*N_t], interleaved (re, im) of exp(-2 pi i k / (2 N_t)), k < 2 N_t
- * Returns TT_ERR_UNSUPPORTED_NT if N_t does not factor into {2,3,5,7} or exceeds 65535. */
+ * Returns TT_ERR_UNSUPPORTED_NT if N_t does not factor into {2,3,5,7} or exceeds 65535.
+ * The radices are taken from {25,20,16,8,7,5,4,3,2}, largest first. */
 int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* pos, double* tw);
+
+/* Test hook (no GPU): the compile-time trigonometry the register butterflies use for their
+ * internal twiddles, evaluated on the host: *c = cos(2 pi k / n), *s = sin(2 pi k / n). */
+int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
+
+/* Tuning hook for experiments (process-wide, affects plans created / calls made afterwards):
+ * "fft_T" = series per CTA of the FFT kernels (8, 16, 32; 0 = planner's choice),
+ * "gemv_chunk" = parameters per CTA of the forward matvec (multiple of 64; 0 = planner's choice).
+ * Returns TT_ERR_SHAPE for an unknown key. */
+int tt_debug_set(const char* key, int value);
 
 #ifdef __cplusplus
 }

@@ -69,6 +69,8 @@ def lib() -> ctypes.CDLL:
         "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
         "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
+        "tt_debug_trig": (ci, [i64, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
+        "tt_debug_set": (ci, [ctypes.c_char_p, ci]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(L, name)
@@ -81,7 +83,8 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
-           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_debug_fft_tables"]
+           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_debug_fft_tables",
+           "tt_debug_trig", "tt_debug_set"]
 
 
 def _stream(stream) -> int:
@@ -194,6 +197,16 @@ def tt_debug_fft_tables(N_t: int):
     _check("tt_debug_fft_tables", st)
     return (list(radix[: n.value]), np.array(pos[:N_t], dtype=np.int64),
             np.array(tw[: 4 * N_t]).reshape(2 * N_t, 2) @ np.array([1.0, 1.0j]))
+
+
+def tt_debug_trig(k: int, n: int) -> tuple[float, float]:
+    c, s = ctypes.c_double(), ctypes.c_double()
+    _check("tt_debug_trig", lib().tt_debug_trig(k, n, ctypes.byref(c), ctypes.byref(s)))
+    return c.value, s.value
+
+
+def tt_debug_set(key: str, value: int) -> None:
+    _check("tt_debug_set", lib().tt_debug_set(key.encode(), value))
 
 
 _DT = {torch.float32: TT_F32, torch.float64: TT_F64}

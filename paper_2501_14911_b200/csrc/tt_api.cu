@@ -20,6 +20,7 @@ constexpr int kRing = 64;       // profiled apply calls remembered
 constexpr int kSlotEvents = 8;  // two kernel triples (tt_normal) x 4 marks
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
+int g_gemv_chunk = 0;  // tt_debug_set("gemv_chunk"): 0 = planner's choice
 
 }  // namespace
 
@@ -74,12 +75,13 @@ int dev_alloc(tt_plan* p, void** ptr, size_t bytes) {
     return TT_OK;
 }
 
-// Radices of the N-point complex FFT: 4s first (fewest passes over shared memory), then what is left.
+// Radices of the N-point complex FFT, largest register butterflies first (fewest passes over
+// shared memory): N = 400 -> 25*16, 500 -> 25*20, 256 -> 16*16, 512 -> 16*16*2.
 bool factorise(long long N, int* radix, int* n_stages) {
     int n = 0;
     long long r = N;
-    const int cand[5] = {4, 2, 3, 5, 7};
-    for (int c = 0; c < 5; ++c)
+    const int cand[9] = {25, 20, 16, 8, 7, 5, 4, 3, 2};
+    for (int c = 0; c < 9; ++c)
         while (r % cand[c] == 0 && r > 1) {
             if (n >= kMaxStages) return false;
             radix[n++] = cand[c];
@@ -132,10 +134,14 @@ void fill_fft_common(const tt_plan* p, FftParams& P, bool fp32_tables) {
     std::memset(&P, 0, sizeof(P));
     P.N = (int)p->N_t;
     P.n_stages = p->n_stages;
-    for (int i = 0; i < p->n_stages; ++i) P.radix[i] = p->radix[i];
+    int Ns = P.N;
+    for (int i = 0; i < p->n_stages; ++i) {
+        P.radix[i] = p->radix[i];
+        Ns /= p->radix[i];
+        P.magic[i] = Ns > 1 ? (unsigned)((0x100000000ULL + (unsigned long long)Ns - 1) / (unsigned long long)Ns) : 0u;
+    }
     P.tw = fp32_tables ? p->tw_f : p->tw_d;
     P.pos = p->pos;
-    P.n_part = 1;
     P.scale = 1.0 / (2.0 * (double)p->N_t);
 }
 
@@ -187,12 +193,12 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
     GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks};
     TT_CUDA(p, gemv_fwd_launch(t, p->Fhat, p->xhat, p->partial, g, s));
     pr.mark(2);
+    TT_CUDA(p, reduce_partials_launch(t, p->partial, p->dhat, p->n_f, p->n_chunks, (int)p->N_d, s));
     fill_fft_common(p, P, f32);
     P.B = p->N_d; P.B_store = p->N_d;
-    P.c_ys = 0; P.c_bs = 1; P.c_fs = (long long)p->n_chunks * p->N_d;
-    P.n_part = p->n_chunks; P.c_ps = p->N_d;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
     P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts;
-    TT_CUDA(p, fft_c2r_launch(t, p->partial, at(d, vd.off, es), P, 1, s));
+    TT_CUDA(p, fft_c2r_launch(t, p->dhat, at(d, vd.off, es), P, 1, s));
     pr.mark(3);
     return TT_OK;
 }
@@ -342,7 +348,8 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     p->ldp = (N_m + 15) / 16 * 16;
     p->n_stages = n_stages;
     for (int i = 0; i < n_stages; ++i) p->radix[i] = radix[i];
-    p->chunk = 2048;
+    p->chunk = g_gemv_chunk > 0 ? g_gemv_chunk / 64 * 64 : 2048;
+    if (p->chunk < 64) p->chunk = 64;
     p->n_chunks = (int)((p->ldp + p->chunk - 1) / p->chunk);
 
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -584,6 +591,21 @@ int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* 
     build_twiddles(2 * (int)N_t, tv);
     std::memcpy(tw, tv.data(), tv.size() * sizeof(double));
     return TT_OK;
+}
+
+int tt_debug_trig(int64_t k, int64_t n, double* c, double* s) {
+    if (!c || !s) return TT_ERR_NULL;
+    if (n < 1) return TT_ERR_SHAPE;
+    *c = debug_cos2pi(k, n);
+    *s = debug_sin2pi(k, n);
+    return TT_OK;
+}
+
+int tt_debug_set(const char* key, int value) {
+    if (!key) return TT_ERR_NULL;
+    if (!std::strcmp(key, "fft_T")) { fft_debug_force_T(value); return TT_OK; }
+    if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
+    return TT_ERR_SHAPE;
 }
 
 int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream) {

@@ -6,91 +6,162 @@
 // fastest), so that the T lanes working on the same butterfly of T different series touch
 // consecutive shared-memory words (no bank conflicts) and consecutive global addresses
 // (time-major vectors have the space index fastest), and every twiddle factor is uniform over
-// those lanes.  The N-point complex FFT is an in-place decimation-in-frequency Cooley-Tukey
-// with radices from {2,3,4,5,7}; its digit-reversed output order is undone for free by the
-// gather of the following step through the plan's `pos` table.
+// those lanes.  The N-point complex FFT is an in-place decimation-in-frequency Cooley-Tukey.
+// A pass is a radix-R butterfly done entirely in registers, R from {2,3,4,5,7} or a composite
+// {8,16,20,25} built from those at compile time (so N = 400 = 16*25 is two passes over shared
+// memory, 512 = 16*8*4 three); the digit-reversed output order of the passes is undone for
+// free by the gather of the following step through the plan's `pos` table.
 //
 // Real-input trick: the L = 2N-point DFT X of the zero-padded real series x is obtained from
 // the N-point DFT Z of z_n = x_{2n} + i x_{2n+1}:
 //     X_k = (Z_k + conj Z_{N-k})/2  -  i w^k (Z_k - conj Z_{N-k})/2 ,   w = exp(-2 pi i / L),
 // k = 0..N (Z_N := Z_0), and inverted the same way for the real inverse transform.
+#include <type_traits>
+
 #include "tt_common.cuh"
 #include "tt_internal.h"
 
 namespace tt {
 
 // ---------------------------------------------------------------------------------------
-// radix butterflies (forward sign, exp(-2 pi i a q / R))
+// compile-time trigonometry: cos/sin(2 pi k / n), exact on the axes
 // ---------------------------------------------------------------------------------------
-__host__ __device__ constexpr double tw_cos(int rad, int k) {
-    return rad == 3 ? (k == 0 ? 1.0 : -0.5)
-         : rad == 5 ? (k == 0 ? 1.0 : (k == 1 || k == 4) ? 0.30901699437494742410 : -0.80901699437494742410)
-         : /*7*/      (k == 0 ? 1.0 : (k == 1 || k == 6) ? 0.62348980185873353053
-                                    : (k == 2 || k == 5) ? -0.22252093395631440429 : -0.90096886790241912624);
+__host__ __device__ constexpr double sin_small(double x) {  // |x| <= pi/4
+    const double x2 = x * x;
+    return x * (1 - x2 / 6 * (1 - x2 / 20 * (1 - x2 / 42 * (1 - x2 / 72 * (1 - x2 / 110 * (1 - x2 / 156 *
+               (1 - x2 / 210 * (1 - x2 / 272))))))));
 }
-__host__ __device__ constexpr double tw_sin(int rad, int k) {  // sin(2 pi k / rad)
-    return rad == 3 ? (k == 0 ? 0.0 : k == 1 ? 0.86602540378443864676 : -0.86602540378443864676)
-         : rad == 5 ? (k == 0 ? 0.0 : k == 1 ? 0.95105651629515357212 : k == 2 ? 0.58778525229247312917
-                                    : k == 3 ? -0.58778525229247312917 : -0.95105651629515357212)
-         : /*7*/      (k == 0 ? 0.0 : k == 1 ? 0.78183148246802980871 : k == 2 ? 0.97492791218182360702
-                                    : k == 3 ? 0.43388373911755812048 : k == 4 ? -0.43388373911755812048
-                                    : k == 5 ? -0.97492791218182360702 : -0.78183148246802980871);
+__host__ __device__ constexpr double cos_small(double x) {  // |x| <= pi/4
+    const double x2 = x * x;
+    return 1 - x2 / 2 * (1 - x2 / 12 * (1 - x2 / 30 * (1 - x2 / 56 * (1 - x2 / 90 * (1 - x2 / 132 *
+               (1 - x2 / 182 * (1 - x2 / 240 * (1 - x2 / 306))))))));
+}
+// cos(2 pi t8 / (8 n)): the angle in eighths of 1/n of a turn, reduced to the first octant in integers
+__host__ __device__ constexpr double cos_units(long long t8, long long n) {
+    const long long full = 8 * n;
+    t8 %= full;
+    if (t8 < 0) t8 += full;
+    if (t8 > 4 * n) t8 = full - t8;
+    bool neg = false;
+    if (t8 > 2 * n) { neg = true; t8 = 4 * n - t8; }
+    const double two_pi = 6.283185307179586476925286766559;
+    const double v = t8 > n ? sin_small(two_pi * (double)(2 * n - t8) / (double)full)
+                            : cos_small(two_pi * (double)t8 / (double)full);
+    return neg ? -v : v;
+}
+__host__ __device__ constexpr double cos2pi(long long k, long long n) { return cos_units(8 * k, n); }
+__host__ __device__ constexpr double sin2pi(long long k, long long n) { return cos_units(8 * k - 2 * n, n); }
+
+double debug_cos2pi(long long k, long long n) { return cos2pi(k, n); }
+double debug_sin2pi(long long k, long long n) { return sin2pi(k, n); }
+
+template <int I, int N, typename F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+
+// a * exp(-2 pi i K / N) with compile-time K, N
+template <typename R, int K, int N>
+__device__ __forceinline__ Cx<R> mul_w(Cx<R> a) {
+    constexpr double c = cos2pi(K, N), s = sin2pi(K, N);
+    if constexpr (c == 1.0 && s == 0.0) return a;
+    else if constexpr (c == 0.0 && s == 1.0) return mul_mi(a);
+    else if constexpr (c == -1.0 && s == 0.0) return mk<R>(-a.re, -a.im);
+    else if constexpr (c == 0.0 && s == -1.0) return mul_pi(a);
+    else return mk<R>(fma(a.im, R(s), a.re * R(c)), fma(-a.re, R(s), a.im * R(c)));
+}
+
+// ---------------------------------------------------------------------------------------
+// radix butterflies in registers (forward sign, exp(-2 pi i a q / R)), natural order in and out
+// ---------------------------------------------------------------------------------------
+constexpr int first_factor(int r) {
+    return (r % 4 == 0 && r > 4) ? 4 : (r % 5 == 0 && r > 5) ? 5 : (r % 2 == 0 && r > 2) ? 2
+         : (r % 3 == 0 && r > 3) ? 3 : (r % 7 == 0 && r > 7) ? 7 : r;
 }
 
 template <typename R, int RAD>
 __device__ __forceinline__ void butterfly(Cx<R> (&x)[RAD]) {
     if constexpr (RAD == 2) {
-        Cx<R> a = x[0], b = x[1];
+        const Cx<R> a = x[0], b = x[1];
         x[0] = a + b; x[1] = a - b;
     } else if constexpr (RAD == 4) {
-        Cx<R> t0 = x[0] + x[2], t1 = x[0] - x[2], t2 = x[1] + x[3], t3 = mul_mi(x[1] - x[3]);
+        const Cx<R> t0 = x[0] + x[2], t1 = x[0] - x[2], t2 = x[1] + x[3], t3 = mul_mi(x[1] - x[3]);
         x[0] = t0 + t2; x[1] = t1 + t3; x[2] = t0 - t2; x[3] = t1 - t3;
-    } else {
+    } else if constexpr (first_factor(RAD) == RAD) {
+        // odd prime: pair a with RAD-a;  y_q = A_q - i B_q,  y_{RAD-q} = A_q + i B_q
         constexpr int H = (RAD - 1) / 2;
         Cx<R> t[H + 1], u[H + 1], y[RAD];
-#pragma unroll
-        for (int a = 1; a <= H; ++a) { t[a] = x[a] + x[RAD - a]; u[a] = x[a] - x[RAD - a]; }
+        static_for<1, H + 1>([&](auto a_) {
+            constexpr int a = a_;
+            t[a] = x[a] + x[RAD - a]; u[a] = x[a] - x[RAD - a];
+        });
         y[0] = x[0];
-#pragma unroll
-        for (int a = 1; a <= H; ++a) y[0] = y[0] + t[a];
-#pragma unroll
-        for (int q = 1; q <= H; ++q) {
+        static_for<1, H + 1>([&](auto a_) { constexpr int a = a_; y[0] = y[0] + t[a]; });
+        static_for<1, H + 1>([&](auto q_) {
+            constexpr int q = q_;
             Cx<R> A = x[0], Bv = mk<R>(R(0), R(0));
-#pragma unroll
-            for (int a = 1; a <= H; ++a) {
-                const R c = R(tw_cos(RAD, (a * q) % RAD)), s = R(tw_sin(RAD, (a * q) % RAD));
-                A.re = fma(c, t[a].re, A.re); A.im = fma(c, t[a].im, A.im);
-                Bv.re = fma(s, u[a].re, Bv.re); Bv.im = fma(s, u[a].im, Bv.im);
-            }
-            y[q] = A + mul_mi(Bv);        // A - i B
-            y[RAD - q] = A + mul_pi(Bv);  // A + i B
-        }
-#pragma unroll
-        for (int q = 0; q < RAD; ++q) x[q] = y[q];
+            static_for<1, H + 1>([&](auto a_) {
+                constexpr int a = a_;
+                constexpr double c = cos2pi(a * q, RAD), s = sin2pi(a * q, RAD);
+                A.re = fma(R(c), t[a].re, A.re); A.im = fma(R(c), t[a].im, A.im);
+                Bv.re = fma(R(s), u[a].re, Bv.re); Bv.im = fma(R(s), u[a].im, Bv.im);
+            });
+            y[q] = A + mul_mi(Bv);
+            y[RAD - q] = A + mul_pi(Bv);
+        });
+        static_for<0, RAD>([&](auto q_) { constexpr int q = q_; x[q] = y[q]; });
+    } else {
+        // composite RAD = R1*R2: radix-R1 over stride R2, twiddle exp(-2 pi i a2 q1 / RAD), radix-R2 on
+        // each block; slot q1*R2 + q2 then holds bin q1 + R1*q2 - undone by register renaming.
+        constexpr int R1 = first_factor(RAD), R2 = RAD / R1;
+        static_for<0, R2>([&](auto a2_) {
+            constexpr int a2 = a2_;
+            Cx<R> t[R1];
+            static_for<0, R1>([&](auto a1_) { constexpr int a1 = a1_; t[a1] = x[a2 + R2 * a1]; });
+            butterfly<R, R1>(t);
+            static_for<0, R1>([&](auto q1_) {
+                constexpr int q1 = q1_;
+                x[a2 + R2 * q1] = mul_w<R, a2 * q1, RAD>(t[q1]);
+            });
+        });
+        Cx<R> y[RAD];
+        static_for<0, R1>([&](auto q1_) {
+            constexpr int q1 = q1_;
+            Cx<R> t[R2];
+            static_for<0, R2>([&](auto a2_) { constexpr int a2 = a2_; t[a2] = x[q1 * R2 + a2]; });
+            butterfly<R, R2>(t);
+            static_for<0, R2>([&](auto q2_) { constexpr int q2 = q2_; y[q1 + R1 * q2] = t[q2]; });
+        });
+        static_for<0, RAD>([&](auto q_) { constexpr int q = q_; x[q] = y[q]; });
     }
 }
 
-// One decimation-in-frequency stage on every length-Ns block of the N-point array:
+// One decimation-in-frequency pass on every length-Ns block of the N-point array:
 //   y_q[j] = w_Ns^{j q} * sum_a x[j + a M] w_R^{a q},  M = Ns/R,  stored in place at j + q M.
 template <typename R, int T, int RAD>
 __device__ __forceinline__ void fft_stage(Cx<R>* __restrict__ sm, const Cx<R>* __restrict__ tw, int N, int Ns,
-                                          int lane_s, int g, int G) {
-    const int M = Ns / RAD;
+                                          int M, unsigned magic, int lane_s, int g, int G) {
     const int nb = N / RAD;
     const int tws = (N / Ns) * 2;  // w_Ns = w_L^(2N/Ns)
+    const int MT = M * T;
     for (int u = g; u < nb; u += G) {
-        const int blk = u / M, j = u - blk * M;
-        Cx<R>* p = sm + (size_t)(blk * Ns + j) * T + lane_s;
+        const int blk = M == 1 ? u : (int)__umulhi((unsigned)u, magic);  // u / M
+        const int j = u - blk * M;
+        Cx<R>* p = sm + (blk * Ns + j) * T + lane_s;
         Cx<R> x[RAD];
 #pragma unroll
-        for (int a = 0; a < RAD; ++a) x[a] = p[(size_t)a * M * T];
+        for (int a = 0; a < RAD; ++a) x[a] = p[a * MT];
         butterfly<R, RAD>(x);
         if (M > 1) {
+            const Cx<R>* w = tw + j * tws;
 #pragma unroll
-            for (int q = 1; q < RAD; ++q) x[q] = x[q] * tw[j * q * tws];
+            for (int q = 1; q < RAD; ++q) x[q] = x[q] * w[(q - 1) * j * tws];
         }
 #pragma unroll
-        for (int q = 0; q < RAD; ++q) p[(size_t)q * M * T] = x[q];
+        for (int q = 0; q < RAD; ++q) p[q * MT] = x[q];
     }
 }
 
@@ -101,14 +172,20 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
     for (int st = 0; st < P.n_stages; ++st) {
         __syncthreads();
         const int r = P.radix[st];
+        const int M = Ns / r;
+        const unsigned mg = P.magic[st];
         switch (r) {
-            case 2: fft_stage<R, T, 2>(sm, tw, P.N, Ns, lane_s, g, G); break;
-            case 3: fft_stage<R, T, 3>(sm, tw, P.N, Ns, lane_s, g, G); break;
-            case 4: fft_stage<R, T, 4>(sm, tw, P.N, Ns, lane_s, g, G); break;
-            case 5: fft_stage<R, T, 5>(sm, tw, P.N, Ns, lane_s, g, G); break;
-            default: fft_stage<R, T, 7>(sm, tw, P.N, Ns, lane_s, g, G); break;
+            case 2: fft_stage<R, T, 2>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 3: fft_stage<R, T, 3>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 4: fft_stage<R, T, 4>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 5: fft_stage<R, T, 5>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 7: fft_stage<R, T, 7>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 8: fft_stage<R, T, 8>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 16: fft_stage<R, T, 16>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 20: fft_stage<R, T, 20>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            default: fft_stage<R, T, 25>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
         }
-        Ns /= r;
+        Ns = M;
     }
     __syncthreads();
 }
@@ -116,12 +193,13 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
 // ---------------------------------------------------------------------------------------
 // forward: zero-pad + real-to-complex FFT + frequency-major store          (P0, A1, B1)
 // ---------------------------------------------------------------------------------------
-template <typename Tin, typename Tc, typename Tout, int T>
-__global__ void fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out,
-                               const __grid_constant__ FftParams P) {
+template <typename Tin, typename Tc, typename Tout, int T, int NT>
+__global__ void __launch_bounds__(NT)
+fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
-    const int lane_s = threadIdx.x % T, g = threadIdx.x / T, G = blockDim.x / T;
+    constexpr int G = NT / T;
+    const int lane_s = threadIdx.x % T, g = threadIdx.x / T;
     const long long b = (long long)blockIdx.x * T + lane_s;
     const bool live = b < P.B;
     const int N = P.N;
@@ -135,7 +213,7 @@ __global__ void fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict_
             re = Tc(src[(long long)j0 * P.r_ts]);
             if (j0 + 1 < N) im = Tc(src[(long long)(j0 + 1) * P.r_ts]);
         }
-        sm[(size_t)n * T + lane_s] = mk<Tc>(re, im);
+        sm[n * T + lane_s] = mk<Tc>(re, im);
     }
     fft_inplace<Tc, T>(sm, P, lane_s, g, G);
 
@@ -145,8 +223,8 @@ __global__ void fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict_
         for (int k = g; k <= N; k += G) {
             const int ka = (k == N) ? 0 : k;
             const int kb = (k == 0 || k == N) ? 0 : N - k;
-            const Cx<Tc> Zk = sm[(size_t)P.pos[ka] * T + lane_s];
-            const Cx<Tc> Zn = conj(sm[(size_t)P.pos[kb] * T + lane_s]);
+            const Cx<Tc> Zk = sm[(int)P.pos[ka] * T + lane_s];
+            const Cx<Tc> Zn = conj(sm[(int)P.pos[kb] * T + lane_s]);
             Cx<Tc> E = Zk + Zn, O = mul_mi(Zk - Zn);
             E.re *= Tc(0.5); E.im *= Tc(0.5); O.re *= Tc(0.5); O.im *= Tc(0.5);
             Cx<Tc> X = E + tw[k] * O;
@@ -157,36 +235,24 @@ __global__ void fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict_
 }
 
 // ---------------------------------------------------------------------------------------
-// inverse: (sum of partial spectra) + complex-to-real inverse FFT + truncate + scale   (A3, B3)
+// inverse: complex-to-real inverse FFT + truncate + scale                               (A3, B3)
 // ---------------------------------------------------------------------------------------
-template <typename Tc, int T>
-__global__ void fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out,
-                               const __grid_constant__ FftParams P) {
+template <typename Tc, int T, int NT>
+__global__ void __launch_bounds__(NT)
+fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
-    const int lane_s = threadIdx.x % T, g = threadIdx.x / T, G = blockDim.x / T;
+    constexpr int G = NT / T;
+    const int lane_s = threadIdx.x % T, g = threadIdx.x / T;
     const long long b = (long long)blockIdx.x * T + lane_s;
     const bool live = b < P.B;
     const int N = P.N;
     const Cx<Tc>* src = in + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
 
-    // X_k, k = 0..N, summed over the partial spectra in fixed order (fp64 accumulator)
     for (int k = g; k <= N; k += G) {
         Cx<Tc> v = mk<Tc>(Tc(0), Tc(0));
-        if (live) {
-            const Cx<Tc>* q = src + (long long)k * P.c_fs;
-            if (P.n_part == 1) {
-                v = q[0];
-            } else {
-                double ar = 0.0, ai = 0.0;
-                for (int c = 0; c < P.n_part; ++c) {
-                    const Cx<Tc> t = q[(long long)c * P.c_ps];
-                    ar += double(t.re); ai += double(t.im);
-                }
-                v = mk<Tc>(Tc(ar), Tc(ai));
-            }
-        }
-        sm[(size_t)k * T + lane_s] = v;
+        if (live) v = src[(long long)k * P.c_fs];
+        sm[k * T + lane_s] = v;
     }
     __syncthreads();
 
@@ -195,17 +261,17 @@ __global__ void fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ o
     const Cx<Tc>* tw = reinterpret_cast<const Cx<Tc>*>(P.tw);
     for (int k = g; k <= N / 2; k += G) {
         if (k == 0) {
-            const Tc x0 = sm[lane_s].re, xn = sm[(size_t)N * T + lane_s].re;  // DC, Nyquist: real parts only
+            const Tc x0 = sm[lane_s].re, xn = sm[N * T + lane_s].re;  // DC, Nyquist: real parts only
             sm[lane_s] = mk<Tc>(x0 + xn, -(x0 - xn));
         } else {
             const int kk = N - k;
-            const Cx<Tc> Xk = sm[(size_t)k * T + lane_s], Xn = sm[(size_t)kk * T + lane_s];
+            const Cx<Tc> Xk = sm[k * T + lane_s], Xn = sm[kk * T + lane_s];
             const Cx<Tc> Zk = (Xk + conj(Xn)) + mul_pi((Xk - conj(Xn)) * conj(tw[k]));
             if (kk != k) {
                 const Cx<Tc> Zkk = (Xn + conj(Xk)) + mul_pi((Xn - conj(Xk)) * conj(tw[kk]));
-                sm[(size_t)kk * T + lane_s] = conj(Zkk);
+                sm[kk * T + lane_s] = conj(Zkk);
             }
-            sm[(size_t)k * T + lane_s] = conj(Zk);
+            sm[k * T + lane_s] = conj(Zk);
         }
     }
     fft_inplace<Tc, T>(sm, P, lane_s, g, G);
@@ -215,7 +281,7 @@ __global__ void fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ o
         Tc* dst = out + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
         const Tc sc = Tc(P.scale);
         for (int n = g; 2 * n < N; n += G) {
-            const Cx<Tc> v = sm[(size_t)P.pos[n] * T + lane_s];
+            const Cx<Tc> v = sm[(int)P.pos[n] * T + lane_s];
             dst[(long long)(2 * n) * P.r_ts] = v.re * sc;
             if (2 * n + 1 < N) dst[(long long)(2 * n + 1) * P.r_ts] = -v.im * sc;
         }
@@ -223,11 +289,56 @@ __global__ void fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ o
 }
 
 // ---------------------------------------------------------------------------------------
+// A3 helper: dhat[w][s] = sum_c partial[w][c][s], fixed order, fp64 accumulator
+// ---------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(256)
+reduce_partials_kernel(const Cx<R>* __restrict__ partial, Cx<R>* __restrict__ dhat, int n_f, int n_chunks, int N_d) {
+    const int w = blockIdx.y;
+    const int s = blockIdx.x * 256 + threadIdx.x;
+    if (s >= N_d) return;
+    const Cx<R>* q = partial + (long long)w * n_chunks * N_d + s;
+    double ar = 0.0, ai = 0.0;
+    int c = 0;
+    for (; c + 8 <= n_chunks; c += 8) {
+        Cx<R> t[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) t[u] = q[(long long)(c + u) * N_d];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { ar += double(t[u].re); ai += double(t[u].im); }
+    }
+    for (; c < n_chunks; ++c) {
+        const Cx<R> t = q[(long long)c * N_d];
+        ar += double(t.re); ai += double(t.im);
+    }
+    dhat[(long long)w * N_d + s] = mk<R>(R(ar), R(ai));
+}
+
+cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int n_f, int n_chunks, int N_d,
+                                   cudaStream_t s) {
+    dim3 grid((unsigned)((N_d + 255) / 256), (unsigned)n_f);
+    if (dt == 0)
+        reduce_partials_kernel<float><<<grid, 256, 0, s>>>(static_cast<const c64*>(partial), static_cast<c64*>(dhat),
+                                                           n_f, n_chunks, N_d);
+    else
+        reduce_partials_kernel<double><<<grid, 256, 0, s>>>(static_cast<const c128*>(partial),
+                                                            static_cast<c128*>(dhat), n_f, n_chunks, N_d);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
+static int g_force_T = 0;
+void fft_debug_force_T(int T) { g_force_T = T; }
+
 FftChoice fft_choose(int N, size_t elem) {
     const int Ts[3] = {32, 16, 8};
-    FftChoice c{0, 256, 0};
+    FftChoice c{0, elem == 8 ? 512 : 256, 0};
+    if (g_force_T) {
+        const size_t bytes = size_t(N + 1) * g_force_T * elem;
+        if (bytes <= size_t(kMaxSmem)) { c.T = g_force_T; c.smem = bytes; return c; }
+    }
     for (int pass = 0; pass < 2; ++pass) {
         const size_t limit = pass == 0 ? size_t(113) * 1024 : size_t(kMaxSmem);
         for (int i = 0; i < 3; ++i) {
@@ -242,14 +353,15 @@ template <typename Tin, typename Tc, typename Tout>
 static cudaError_t r2c_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
     if (c.T == 0) return cudaErrorInvalidValue;
+    constexpr int NT = sizeof(Tc) == 4 ? 512 : 256;
     const long long nb = (P.B_store > P.B ? P.B_store : P.B);
     dim3 grid((unsigned)((nb + c.T - 1) / c.T), (unsigned)ny);
 #define TT_R2C(TT)                                                                                           \
     {                                                                                                        \
-        auto k = fft_r2c_kernel<Tin, Tc, Tout, TT>;                                                          \
+        auto k = fft_r2c_kernel<Tin, Tc, Tout, TT, NT>;                                                      \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
-        k<<<grid, c.threads, c.smem, s>>>(static_cast<const Tin*>(in), static_cast<Cx<Tout>*>(out), P);      \
+        k<<<grid, NT, c.smem, s>>>(static_cast<const Tin*>(in), static_cast<Cx<Tout>*>(out), P);             \
     }
     if (c.T == 32) TT_R2C(32) else if (c.T == 16) TT_R2C(16) else TT_R2C(8)
 #undef TT_R2C
@@ -268,13 +380,14 @@ template <typename Tc>
 static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
     if (c.T == 0) return cudaErrorInvalidValue;
+    constexpr int NT = sizeof(Tc) == 4 ? 512 : 256;
     dim3 grid((unsigned)((P.B + c.T - 1) / c.T), (unsigned)ny);
 #define TT_C2R(TT)                                                                                           \
     {                                                                                                        \
-        auto k = fft_c2r_kernel<Tc, TT>;                                                                     \
+        auto k = fft_c2r_kernel<Tc, TT, NT>;                                                                 \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
-        k<<<grid, c.threads, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P);         \
+        k<<<grid, NT, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P);                \
     }
     if (c.T == 32) TT_C2R(32) else if (c.T == 16) TT_C2R(16) else TT_C2R(8)
 #undef TT_C2R

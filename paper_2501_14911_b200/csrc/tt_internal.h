@@ -20,15 +20,15 @@ constexpr int kMaxSmem = 232448;  // 227 KB: largest dynamic shared memory per C
 struct FftParams {
     int N;                  // complex FFT length = N_t
     int n_stages;
-    int radix[kMaxStages];  // product = N, applied in order as decimation-in-frequency stages
+    int radix[kMaxStages];  // product = N, applied in order as decimation-in-frequency passes;
+                            // each from {2,3,4,5,7,8,16,20,25}
+    unsigned magic[kMaxStages];  // ceil(2^32 / M_st), M_st = block length after pass st (exact u / M_st for u < 2^16)
     const void* tw;         // Cx<Tc>[2N]: tw[k] = exp(-2 pi i k / (2N))
     const unsigned short* pos;  // pos[k] = slot of the in-place DIF output that holds bin k
     long long B;            // series per y-row
     long long B_store;      // forward only: series in [B, B_store) are stored as zeros (row padding)
     long long r_ys, r_bs, r_ts;
     long long c_ys, c_bs, c_fs;
-    int n_part;             // inverse only: the input is the sum of n_part partial spectra ...
-    long long c_ps;         // ... c_ps elements apart
     double scale;           // inverse only: factor applied to the real output (1/L)
 };
 
@@ -45,6 +45,12 @@ cudaError_t fft_r2c_launch(int tin, int tc, int tout, const void* real_in, void*
                            const FftParams& P, int ny, cudaStream_t s);
 cudaError_t fft_c2r_launch(int tc, const void* cplx_in, void* real_out, const FftParams& P, int ny,
                            cudaStream_t s);
+// dhat[w*N_d + s] = sum_c partial[(w*n_chunks + c)*N_d + s] (fixed order, fp64 accumulator)
+cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int n_f, int n_chunks, int N_d,
+                                   cudaStream_t s);
+void fft_debug_force_T(int T);  // 0 = planner's choice
+double debug_cos2pi(long long k, long long n);
+double debug_sin2pi(long long k, long long n);
 
 // Per-frequency matvecs.  Fhat[(w*N_d + s)*ldp + p], xhat[w*ldp + p], dhat[w*N_d + s];
 // partial[(w*n_chunks + c)*N_d + s] = sum over chunk c of Fhat_w[s,:] xhat_w[:].

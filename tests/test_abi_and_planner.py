@@ -78,7 +78,7 @@ def replay_dif(z, radices, tw):
 def test_fft_plan_tables_reproduce_numpy_fft(tt, N_t):
     radices, pos, tw = tt.tt_debug_fft_tables(N_t)
     assert int(np.prod(radices)) == N_t if radices else N_t == 1
-    assert all(r in (2, 3, 4, 5, 7) for r in radices)
+    assert all(r in (2, 3, 4, 5, 7, 8, 16, 20, 25) for r in radices)
     assert sorted(pos.tolist()) == list(range(N_t))                     # a permutation
     L = 2 * N_t
     k = np.arange(L)
@@ -96,6 +96,20 @@ def test_fft_plan_tables_reproduce_numpy_fft(tt, N_t):
     X = 0.5 * (Zk + Zn) + tw[kk] * (-0.5j) * (Zk - Zn)
     ref = np.fft.rfft(np.concatenate([x, np.zeros(N_t)]))
     assert np.abs(X - ref).max() < 1e-11 * max(1.0, np.abs(ref).max())
+
+
+def test_compile_time_trig_matches_libm(tt):
+    """cos/sin(2 pi k/n) used for the butterflies' internal twiddles: exact on the axes, <= 2 ulp elsewhere."""
+    two_pi = 2 * np.longdouble("3.14159265358979323846264338327950288")    # 80-bit reference
+    for n in (3, 5, 7, 8, 16, 20, 25):
+        for k in range(-n, 2 * n + 1):
+            c, s = tt.tt_debug_trig(k, n)
+            a = two_pi * np.longdouble(k % n) / np.longdouble(n)
+            assert abs(np.longdouble(c) - np.cos(a)) < 2.3e-16 and abs(np.longdouble(s) - np.sin(a)) < 2.3e-16
+    assert tt.tt_debug_trig(0, 16) == (1.0, 0.0) and tt.tt_debug_trig(4, 16) == (0.0, 1.0)
+    assert tt.tt_debug_trig(8, 16) == (-1.0, 0.0) and tt.tt_debug_trig(12, 16) == (0.0, -1.0)
+    c, s = tt.tt_debug_trig(2, 16)
+    assert c == s                                                       # (1 - i)/sqrt(2) symmetric
 
 
 @pytest.mark.parametrize("N_t", [11, 13, 22, 65536 * 2])
