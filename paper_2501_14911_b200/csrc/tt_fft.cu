@@ -205,31 +205,45 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
     const int N = P.N;
     const Tin* src = in + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
 
-    // z_n = x_{2n} + i x_{2n+1}; x_j = 0 for j >= N_t = N (the zero padding)
-    for (int n = g; n < N; n += G) {
-        Tc re = Tc(0), im = Tc(0);
-        const int j0 = 2 * n;
-        if (live && j0 < N) {
-            re = Tc(src[(long long)j0 * P.r_ts]);
-            if (j0 + 1 < N) im = Tc(src[(long long)(j0 + 1) * P.r_ts]);
+    // z_n = x_{2n} + i x_{2n+1}; x_j = 0 for j >= N_t = N (the zero padding).  The global loads are
+    // issued in batches of 2*UB independent requests per thread before any of them is consumed.
+    constexpr int UB = 8;
+    const int nh = (N + 1) / 2;  // slots n >= nh are pure padding
+    for (int n0 = g; n0 < nh; n0 += G * UB) {
+        Tin v0[UB], v1[UB];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int n = n0 + u * G;
+            v0[u] = Tin(0); v1[u] = Tin(0);
+            if (live && n < nh) {
+                v0[u] = src[(long long)(2 * n) * P.r_ts];
+                if (2 * n + 1 < N) v1[u] = src[(long long)(2 * n + 1) * P.r_ts];
+            }
         }
-        sm[n * T + lane_s] = mk<Tc>(re, im);
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int n = n0 + u * G;
+            if (n < nh) sm[n * T + lane_s] = mk<Tc>(Tc(v0[u]), Tc(v1[u]));
+        }
     }
+    for (int n = nh + g; n < N; n += G) sm[n * T + lane_s] = mk<Tc>(Tc(0), Tc(0));
     fft_inplace<Tc, T>(sm, P, lane_s, g, G);
 
     const Cx<Tc>* tw = reinterpret_cast<const Cx<Tc>*>(P.tw);
     Cx<Tout>* dst = out + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
     if (b < P.B_store) {
-        for (int k = g; k <= N; k += G) {
-            const int ka = (k == N) ? 0 : k;
-            const int kb = (k == 0 || k == N) ? 0 : N - k;
-            const Cx<Tc> Zk = sm[(int)P.pos[ka] * T + lane_s];
-            const Cx<Tc> Zn = conj(sm[(int)P.pos[kb] * T + lane_s]);
+        // bins k and N-k share their inputs:  X_k = E + w^k O,  X_{N-k} = conj(E - w^k O)
+        for (int k = g; k <= N / 2; k += G) {
+            const int kk = N - k;
+            const Cx<Tc> Zk = sm[(int)P.pos[k] * T + lane_s];
+            const Cx<Tc> Zn = conj(sm[(int)P.pos[k == 0 ? 0 : kk] * T + lane_s]);
             Cx<Tc> E = Zk + Zn, O = mul_mi(Zk - Zn);
             E.re *= Tc(0.5); E.im *= Tc(0.5); O.re *= Tc(0.5); O.im *= Tc(0.5);
-            Cx<Tc> X = E + tw[k] * O;
-            if (!live) X = mk<Tc>(Tc(0), Tc(0));
-            dst[(long long)k * P.c_fs] = mk<Tout>(Tout(X.re), Tout(X.im));
+            const Cx<Tc> wO = tw[k] * O;
+            Cx<Tc> Xa = E + wO, Xb = conj(E - wO);
+            if (!live) { Xa = mk<Tc>(Tc(0), Tc(0)); Xb = Xa; }
+            dst[(long long)k * P.c_fs] = mk<Tout>(Tout(Xa.re), Tout(Xa.im));
+            if (kk != k) dst[(long long)kk * P.c_fs] = mk<Tout>(Tout(Xb.re), Tout(Xb.im));
         }
     }
 }
@@ -249,10 +263,20 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
     const int N = P.N;
     const Cx<Tc>* src = in + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
 
-    for (int k = g; k <= N; k += G) {
-        Cx<Tc> v = mk<Tc>(Tc(0), Tc(0));
-        if (live) v = src[(long long)k * P.c_fs];
-        sm[k * T + lane_s] = v;
+    constexpr int UB = 8;
+    for (int k0 = g; k0 <= N; k0 += G * UB) {
+        Cx<Tc> v[UB];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int k = k0 + u * G;
+            v[u] = mk<Tc>(Tc(0), Tc(0));
+            if (live && k <= N) v[u] = src[(long long)k * P.c_fs];
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int k = k0 + u * G;
+            if (k <= N) sm[k * T + lane_s] = v[u];
+        }
     }
     __syncthreads();
 
