@@ -112,17 +112,18 @@ def oracle_sample(w, F_s, m_s, d_s):
 def cpu_baseline(w, draw, target_s=15.0):
     """draw(ns, npar) -> (F_s [N_t,ns,npar], m_s [N_t,npar], d_s [N_t,ns]) numpy.  Extrapolates by MAC count."""
     npar = min(w.N_m, 25000)
-    ns = min(w.N_d, 2)
-    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # calibration (also warms the library)
+    ns = min(w.N_d, 8)
+    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # warms the library and the caches
+    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # calibration
     per_sensor = max(1e-3, (ta + tb) / ns)
     ns2 = int(max(ns, min(w.N_d, 40, round(target_s / per_sensor))))
     ta, tb, thr = oracle_sample(w, *draw(ns2, npar))
-    scale = (w.N_d * w.N_m) / float(ns2 * npar)
+    scale = (w.N_d * w.N_m) / float(ns2 * npar) * w.k_rhs   # k-RHS: the oracle does the columns one by one
     return {
         "value": (ta + tb) * scale * 1e3, "unit": "ms", "cores": thr, "kind": "oracle",
         "sample": (f"oracle/toeplitz_blocked.c (direct O(N_t^2) block convolution, fp64) timed on sensors 0..{ns2 - 1} x "
                    f"parameters 0..{npar - 1} x all {w.N_t} steps of the same workload ({ta + tb:.2f} s for F.m + F^T.d), "
-                   f"scaled by N_d*N_m/(sample) = {scale:.1f} to the full matvec pair"),
+                   f"scaled by N_d*N_m/(sample){' * k' if w.k_rhs > 1 else ''} = {scale:.1f} to the full step"),
         "matvec_ms": ta * scale * 1e3, "rmatvec_ms": tb * scale * 1e3,
     }
 
@@ -143,7 +144,7 @@ def run_reference(args, w):
     for _ in range(args.steps):
         _, _, thr = oracle_sample(w, F_s, m_s, d_s)
     dt = (time.perf_counter() - t0) / args.steps
-    scale = (w.N_d * w.N_m) / float(ns * npar)
+    scale = (w.N_d * w.N_m) / float(ns * npar) * w.k_rhs
     ms = dt * scale * 1e3
     sample = (f"each step = oracle F.m + F^T.d on sensors 0..{ns - 1} x parameters 0..{npar - 1} x all {w.N_t} steps "
               f"({dt:.2f} s), scaled by {scale:.1f} to the full workload")
@@ -160,8 +161,11 @@ def run_reference(args, w):
 
 def config_dict(w, args):
     return {"workload": f"{w.name}: N_d={w.N_d}, N_m={w.N_m}, N_t={w.N_t} ({w.n_params:.3g} parameters), "
-                        f"{'fp32 vectors / complex64 spectrum' if w.dtype == torch.float32 else 'fp64 / complex128'}",
-            "baseline_config": args.config, "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)",
+                        f"{'fp32 vectors / complex64 spectrum' if w.dtype == torch.float32 else 'fp64 / complex128'}"
+                        + (f", k={w.k_rhs} right-hand sides" if w.k_rhs > 1 else ""),
+            "baseline_config": args.config,
+            "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)" if w.k_rhs == 1
+                    else f"one batched F.M + one batched F^T.D, k={w.k_rhs} (batched FFTs + per-frequency DMMA GEMMs)",
             "layout": "time-major", "parallelism": "replicas only" if args.gpus > 1 else "single GPU",
             "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
 
@@ -199,14 +203,17 @@ def main() -> int:
     # ---- inputs, resident in HBM ----------------------------------------------------------
     t0 = time.perf_counter()
     F = synth.block_column(w, device=dev)
-    m = synth.vector_m(w, device=dev, k_rhs=1)
-    d = synth.vector_d(w, device=dev, k_rhs=1)
+    K = w.k_rhs                                   # > 1: the k-RHS batched calls (C4)
+    m = synth.vector_m(w, device=dev)             # [N_t, N_m] or [N_t, N_m, K]
+    d = synth.vector_d(w, device=dev)
     torch.cuda.synchronize()
     t_gen = time.perf_counter() - t0
 
-    def draw(ns, npar):  # the CPU baseline's sample: the same bytes, copied from the device
-        return (F[:, :ns, :npar].contiguous().cpu().numpy(), m[:, :npar].contiguous().cpu().numpy(),
-                d[:, :ns].contiguous().cpu().numpy())
+    def draw(ns, npar):  # the CPU baseline's sample: the same bytes, copied from the device (column 0 if k-RHS)
+        m1 = m if K == 1 else m[..., 0]
+        d1 = d if K == 1 else d[..., 0]
+        return (F[:, :ns, :npar].contiguous().cpu().numpy(), m1[:, :npar].contiguous().cpu().numpy(),
+                d1[:, :ns].contiguous().cpu().numpy())
 
     samples = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -214,7 +221,7 @@ def main() -> int:
         samples = draw(min(w.N_d, 40), min(w.N_m, 25000))
 
     t0 = time.perf_counter()
-    plan = tt.Plan(F)
+    plan = tt.Plan(F, k_max=K)
     torch.cuda.synchronize()
     t_plan = time.perf_counter() - t0
     del F
@@ -225,9 +232,18 @@ def main() -> int:
     m_out = torch.empty_like(m)
     h = plan.handle
 
+    if K == 1:
+        op_fwd = lambda: tt.tt_matvec(h, m, d_out, stream)
+        op_adj = lambda: tt.tt_rmatvec(h, d, m_out, stream)
+        tag_fwd, tag_adj = tt.TT_OP_MATVEC, tt.TT_OP_RMATVEC
+    else:
+        op_fwd = lambda: tt.tt_matvec_batched(h, K, m, d_out, stream)
+        op_adj = lambda: tt.tt_rmatvec_batched(h, K, d, m_out, stream)
+        tag_fwd, tag_adj = tt.TT_OP_MATVEC_BATCHED, tt.TT_OP_RMATVEC_BATCHED
+
     def step():
-        tt.tt_matvec(h, m, d_out, stream)
-        tt.tt_rmatvec(h, d, m_out, stream)
+        op_fwd()
+        op_adj()
 
     def barrier():
         if dist is not None:
@@ -257,8 +273,8 @@ def main() -> int:
         ev1.record(stream)
         barrier()
     ms_step = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
-    fwd = tt.tt_plan_stage_ms(h, tt.TT_OP_MATVEC)
-    adj = tt.tt_plan_stage_ms(h, tt.TT_OP_RMATVEC)
+    fwd = tt.tt_plan_stage_ms(h, tag_fwd)
+    adj = tt.tt_plan_stage_ms(h, tag_adj)
     tt.tt_plan_set_profiling(h, False)
 
     # ---- separate ms per F.m and per F^T.d (same launch configuration) -----------------------
@@ -272,20 +288,37 @@ def main() -> int:
         torch.cuda.synchronize()
         return a.elapsed_time(b) / n
 
-    ms_fwd = max_over_ranks(time_op(lambda: tt.tt_matvec(h, m, d_out, stream), args.steps))
-    ms_adj = max_over_ranks(time_op(lambda: tt.tt_rmatvec(h, d, m_out, stream), args.steps))
+    ms_fwd = max_over_ranks(time_op(op_fwd, args.steps))
+    ms_adj = max_over_ranks(time_op(op_adj, args.steps))
+    ms_normal = None
+    if K == 1:  # F^T F m (one solver iteration, configs[4]); the intermediate d never leaves the device
+        n_out = torch.empty_like(m)
+        ms_normal = max_over_ranks(time_op(lambda: tt.tt_normal(h, m, n_out, stream), args.steps))
+        del n_out
 
     # ---- end to end through the C ABI with HOST vectors -------------------------------------
     m_h, d_h = m.cpu().pin_memory(), d.cpu().pin_memory()
     d_oh, m_oh = torch.empty_like(d_h).pin_memory(), torch.empty_like(m_h).pin_memory()
 
-    def step_host():
-        tt.tt_matvec_host(h, m_h, d_oh, stream)
-        tt.tt_rmatvec_host(h, d_h, m_oh, stream)
+    if K == 1:
+        def step_host():
+            tt.tt_matvec_host(h, m_h, d_oh, stream)
+            tt.tt_rmatvec_host(h, d_h, m_oh, stream)
+        e2e_api = "tt_matvec_host + tt_rmatvec_host, pinned host vectors"
+    else:
+        def step_host():  # no *_host variant of the k-RHS calls: explicit copies on the same stream
+            with torch.cuda.stream(stream):
+                m.copy_(m_h, non_blocking=True)
+                tt.tt_matvec_batched(h, K, m, d_out, stream)
+                d_oh.copy_(d_out, non_blocking=True)
+                d.copy_(d_h, non_blocking=True)
+                tt.tt_rmatvec_batched(h, K, d, m_out, stream)
+                m_oh.copy_(m_out, non_blocking=True)
+        e2e_api = "pinned host -> device copies + tt_matvec_batched / tt_rmatvec_batched + device -> host copies"
 
     step_host()
     torch.cuda.synchronize()
-    n_e2e = max(2, min(args.steps, 5))
+    n_e2e = max(2, min(args.steps, 5 if K == 1 else 2))
     barrier()
     t0 = time.perf_counter()
     for _ in range(n_e2e):
@@ -300,27 +333,50 @@ def main() -> int:
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
     n_f, ldp = w.N_t + 1, (w.N_m + 15) // 16 * 16
     fhat_bytes = n_f * w.N_d * ldp * 2 * es
-    xhat_bytes = n_f * ldp * 2 * es
-    dhat_bytes = n_f * w.N_d * 2 * es
-    n_chunks = (ldp + 2047) // 2048
-    part_bytes = n_f * n_chunks * w.N_d * 2 * es
-    bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
-    bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written
-    vec_bytes = (w.N_t * w.N_m + w.N_t * w.N_d) * es
+    vec_bytes = (w.N_t * w.N_m + w.N_t * w.N_d) * es * K
     bytes_op = fhat_bytes + vec_bytes                           # north_star: |Fhat| plus the vectors
-    ach_fwd = bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0
-    ach_adj = bytes_adj_kernel / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
-    roofline = {
-        "bound": "hbm", "kernel": "gemv_fwd_kernel (A2, per-frequency matvec streaming Fhat)",
-        "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak, "traffic": None,
-        "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
-                     else "fallback 6.65 TB/s (B200_PROFILING.md)",
-        "algorithmic_bytes_per_launch": bytes_fwd_kernel, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
-        "frac_of_nominal_8TBs": ach_fwd / NOMINAL_HBM_GBS,
-        "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
-                           "algorithmic_bytes_per_launch": bytes_adj_kernel, "ms_per_launch": adj[1],
-                           "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
-    }
+    if K == 1:
+        xhat_bytes = n_f * ldp * 2 * es
+        dhat_bytes = n_f * w.N_d * 2 * es
+        n_chunks = (ldp + 2047) // 2048
+        part_bytes = n_f * n_chunks * w.N_d * 2 * es
+        bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
+        bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written
+        ach_fwd = bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0
+        ach_adj = bytes_adj_kernel / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
+        roofline = {
+            "bound": "hbm", "kernel": "gemv_fwd_kernel (A2, per-frequency matvec streaming Fhat)",
+            "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak, "traffic": None,
+            "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
+                         else "fallback 6.65 TB/s (B200_PROFILING.md)",
+            "algorithmic_bytes_per_launch": bytes_fwd_kernel, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
+            "frac_of_nominal_8TBs": ach_fwd / NOMINAL_HBM_GBS,
+            "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
+                               "algorithmic_bytes_per_launch": bytes_adj_kernel, "ms_per_launch": adj[1],
+                               "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
+        }
+    else:
+        # the k-RHS per-frequency GEMMs are a dense contraction on the FP64 tensor pipe (DMMA); its peak is
+        # measured in this run by the library's DMMA probe (there is no FP64 figure in MEASURED_PEAKS.json)
+        sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device=dev)
+        best = 0.0
+        for _ in range(3):
+            fl = [0.0]
+            t = time_op(lambda: fl.__setitem__(0, tt.tt_probe_dmma(4000, sink, stream)), 3)
+            best = max(best, fl[0] / (t * 1e-3) / 1e12)
+        flops = 8.0 * n_f * w.N_d * w.N_m * K                  # 4 real MACs per complex MAC
+        ach_fwd = flops / (fwd[1] * 1e-3) / 1e12 if fwd[1] > 0 else 0.0
+        ach_adj = flops / (adj[1] * 1e-3) / 1e12 if adj[1] > 0 else 0.0
+        roofline = {
+            "bound": "tensor", "kernel": "gemm_fwd_kernel (k-RHS A2: per-frequency complex GEMM, mma.sync m8n8k4 f64)",
+            "achieved": ach_fwd, "peak": best, "unit": "TFLOP/s", "frac": ach_fwd / best if best else None,
+            "traffic": None, "peak_kind": "FP64 DMMA peak measured in this run by tt_probe_dmma "
+                                          "(bf16 measured 1620 TF/s x nominal fp64/bf16 ratio 40/2250 = 28.8 TF/s for comparison)",
+            "algorithmic_flops_per_launch": flops, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
+            "hbm_bytes_per_launch": fhat_bytes + n_f * w.N_m * K * 16,
+            "adjoint_kernel": {"kernel": "gemm_adj_kernel (k-RHS B2)", "achieved": ach_adj,
+                               "frac": ach_adj / best if best else None, "ms_per_launch": adj[1]},
+        }
 
     # ---- bandwidth probes in the same run (copy and read-only stream) -------------------------
     probe = {}
@@ -343,12 +399,13 @@ def main() -> int:
         "vs_baseline": None, "dtype": "f32" if w.dtype == torch.float32 else "f64", "data": "synthetic",
         "config": config_dict(w, args),
         "e2e": {"value": ms_e2e / args.gpus, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "api": "tt_matvec_host + tt_rmatvec_host, pinned host vectors"},
-        "gpu_launches": 6 * args.steps,
+                "steps": n_e2e, "api": e2e_api},
+        "gpu_launches": (6 if K == 1 else 7) * args.steps,
         "clocks": clocks.summary(),
         "roofline": roofline,
         "ops": {
-            "matvec_ms": ms_fwd, "rmatvec_ms": ms_adj,
+            "matvec_ms": ms_fwd, "rmatvec_ms": ms_adj, "normal_ms": ms_normal, "k_rhs": K,
+            "normal_GBs": (2 * fhat_bytes + 2 * w.N_t * w.N_m * es) / (ms_normal * 1e-3) / 1e9 if ms_normal else None,
             "matvec_GBs": bytes_op / (ms_fwd * 1e-3) / 1e9, "rmatvec_GBs": bytes_op / (ms_adj * 1e-3) / 1e9,
             "roofline_bytes_per_op": bytes_op,
             "matvec_frac_of_8TBs": bytes_op / (ms_fwd * 1e-3) / 1e9 / NOMINAL_HBM_GBS,

@@ -167,6 +167,11 @@ int tt_plan_stage_ms(const tt_plan* plan, int op, float* ms, int n);
  * by bench.py to measure the read-only HBM bandwidth next to the copy figure. */
 int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream);
 
+/* FP64 tensor-pipe probe: every warp of 148*8 CTAs x 256 threads issues iters x 16 independent
+ * mma.sync m8n8k4 f64 (DMMA); *flops (host, may be NULL) receives the flop count of the launch.
+ * sink: DEVICE, >= 148*8*256 doubles.  bench.py times it for the measured DMMA peak. */
+int tt_probe_dmma(int iters, void* sink, double* flops, void* stream);
+
 /* Test hook for the planner's host logic (needs no GPU): the FFT plan of an N_t-point series.
  *   n_stages  receives the number of decimation-in-frequency stages
  *   radix     int[16], receives their radices (product = N_t)

@@ -69,6 +69,7 @@ def lib() -> ctypes.CDLL:
         "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
         "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
+        "tt_probe_dmma": (ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]),
         "tt_debug_trig": (ci, [i64, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_set": (ci, [ctypes.c_char_p, ci]),
     }
@@ -83,7 +84,7 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
-           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_debug_fft_tables",
+           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set"]
 
 
@@ -184,6 +185,13 @@ def tt_plan_stage_ms(plan: int, op: int) -> tuple[float, float, float, int]:
 
 def tt_probe_stream_read(src, nbytes: int, sink, stream=None) -> None:
     _check("tt_probe_stream_read", lib().tt_probe_stream_read(_ptr(src), nbytes, _ptr(sink), _stream(stream)))
+
+
+def tt_probe_dmma(iters: int, sink, stream=None) -> float:
+    """Enqueues the DMMA probe; returns the flop count of the launch."""
+    fl = ctypes.c_double()
+    _check("tt_probe_dmma", lib().tt_probe_dmma(iters, _ptr(sink), ctypes.byref(fl), _stream(stream)))
+    return fl.value
 
 
 def tt_debug_fft_tables(N_t: int):

@@ -230,6 +230,80 @@ int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev
     return TT_OK;
 }
 
+// k-RHS on the FP64 tensor pipe (step D): batched FFTs with the RHS index fastest, one complex
+// GEMM per frequency.  TT_F64 only; TT_F32 plans take the per-column path in the callers.
+GemmGeom gemm_geom(const tt_plan* p, int k) {
+    GemmGeom g;
+    g.n_f = p->n_f; g.N_d = (int)p->N_d; g.k = k;
+    g.N_m = p->N_m; g.ldp = p->ldp;
+    g.ldx = ((long long)p->N_m * k + 15) / 16 * 16;
+    // p-splits of the forward reduction: enough CTAs for ~8 waves of 2 CTAs/SM, never more than n_chunks
+    const long long mblocks = (p->N_d + 63) / 64;
+    long long want = (148LL * 2 * 8 + p->n_f * mblocks - 1) / (p->n_f * mblocks);
+    if (want < 1) want = 1;
+    if (want > p->n_chunks) want = p->n_chunks;
+    long long pps = (p->N_m + want - 1) / want;
+    pps = (pps + 31) / 32 * 32;
+    g.p_per_split = pps;
+    g.split = (int)((p->N_m + pps - 1) / pps);
+    return g;
+}
+
+void batched_views(const tt_plan* p, FftParams& P, long long n_space, int k, long long c_pitch, int* ny) {
+    // series b = x*k + r (x = space index): time-major vectors have it contiguous; space-major ones
+    // are [r][x][j], addressed with one grid row per r.
+    if (p->layout == TT_SPACE_MAJOR) {
+        P.B = n_space; P.B_store = n_space;
+        P.r_ys = n_space * p->N_t; P.r_bs = p->N_t; P.r_ts = 1;
+        P.c_ys = 1; P.c_bs = k; P.c_fs = c_pitch;
+        *ny = k;
+    } else {
+        P.B = n_space * k; P.B_store = n_space * k;
+        P.r_ys = 0; P.r_bs = 1; P.r_ts = n_space * k;
+        P.c_ys = 0; P.c_bs = 1; P.c_fs = c_pitch;
+        *ny = 1;
+    }
+}
+
+int run_matvec_gemm(const tt_plan* p, int k, const void* M, void* D, cudaStream_t s, int ev_base) {
+    Prof pr{p, s, ev_base};
+    const GemmGeom g = gemm_geom(p, k);
+    int ny = 1;
+    pr.mark(0);
+    FftParams P;
+    fill_fft_common(p, P, false);
+    batched_views(p, P, p->N_m, k, g.ldx, &ny);
+    TT_CUDA(p, fft_r2c_launch(1, 1, 1, M, p->xhat, P, ny, s));
+    pr.mark(1);
+    TT_CUDA(p, gemm_fwd_launch(1, p->Fhat, p->xhat, p->partial, g, s));
+    pr.mark(2);
+    TT_CUDA(p, reduce_partials_launch(1, p->partial, p->dhat, p->n_f, g.split, (int)(p->N_d * k), s));
+    fill_fft_common(p, P, false);
+    batched_views(p, P, p->N_d, k, p->N_d * k, &ny);
+    TT_CUDA(p, fft_c2r_launch(1, p->dhat, D, P, ny, s));
+    pr.mark(3);
+    return TT_OK;
+}
+
+int run_rmatvec_gemm(const tt_plan* p, int k, const void* D, void* M, cudaStream_t s, int ev_base) {
+    Prof pr{p, s, ev_base};
+    const GemmGeom g = gemm_geom(p, k);
+    int ny = 1;
+    pr.mark(0);
+    FftParams P;
+    fill_fft_common(p, P, false);
+    batched_views(p, P, p->N_d, k, p->N_d * k, &ny);
+    TT_CUDA(p, fft_r2c_launch(1, 1, 1, D, p->dhat, P, ny, s));
+    pr.mark(1);
+    TT_CUDA(p, gemm_adj_launch(1, p->Fhat, p->dhat, p->xhat, g, s));
+    pr.mark(2);
+    fill_fft_common(p, P, false);
+    batched_views(p, P, p->N_m, k, g.ldx, &ny);
+    TT_CUDA(p, fft_c2r_launch(1, p->xhat, M, P, ny, s));
+    pr.mark(3);
+    return TT_OK;
+}
+
 // P0: Fhat from one slab of sensors [s0, s0+ns) of the block column, device resident as
 // col[(k*ns_pitch + s)*N_m + p].
 int run_plan_fft(tt_plan* p, const void* col, long long s0, long long ns, long long ns_pitch, cudaStream_t s) {
@@ -473,12 +547,15 @@ int tt_normal(const tt_plan* p, const void* m, void* out, void* stream) {
     return run_rmatvec(p, p->dwork, out, static_cast<cudaStream_t>(stream), e0 + 4);
 }
 
-// Interim k-RHS path: one pass of the single-vector kernels per right-hand side, addressing
-// column r through the strides of the fused FFT load/store.  (Replaced by the DMMA GEMM path.)
+// k-RHS: TT_F64 plans run batched FFTs + one FP64 DMMA complex GEMM per frequency (tt_gemm.cu);
+// TT_F32 plans (and k = 1) run the single-vector kernels once per right-hand side, addressing
+// column r through the strides of the fused FFT load/store.
 int tt_matvec_batched(const tt_plan* p, int k, const void* M, void* D, void* stream) {
     int r = check_apply(p, M, D);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
+    if (p->dtype == TT_F64 && k > 1)
+        return run_matvec_gemm(p, k, M, D, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC_BATCHED, 1));
     for (int c = 0; c < k; ++c) {
         r = run_matvec(p, M, D, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC_BATCHED, 1), k, c);
         if (r) return r;
@@ -490,6 +567,8 @@ int tt_rmatvec_batched(const tt_plan* p, int k, const void* D, void* M, void* st
     int r = check_apply(p, D, M);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
+    if (p->dtype == TT_F64 && k > 1)
+        return run_rmatvec_gemm(p, k, D, M, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC_BATCHED, 1));
     for (int c = 0; c < k; ++c) {
         r = run_rmatvec(p, D, M, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC_BATCHED, 1), k, c);
         if (r) return r;
@@ -590,6 +669,14 @@ int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* 
     std::vector<double> tv;
     build_twiddles(2 * (int)N_t, tv);
     std::memcpy(tw, tv.data(), tv.size() * sizeof(double));
+    return TT_OK;
+}
+
+int tt_probe_dmma(int iters, void* sink, double* flops, void* stream) {
+    if (!sink) return TT_ERR_NULL;
+    if (iters < 1) return TT_ERR_SHAPE;
+    cudaError_t e = probe_dmma_launch(iters, sink, flops, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
     return TT_OK;
 }
 

@@ -80,6 +80,8 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s);
 
+// sink: >= 148*8*256 doubles
+cudaError_t probe_dmma_launch(int iters, void* sink, double* flops, cudaStream_t s);
 cudaError_t probe_stream_read_launch(const void* src, size_t bytes, void* sink, cudaStream_t s);
 
 }  // namespace tt

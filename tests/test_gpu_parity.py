@@ -226,6 +226,31 @@ def test_batched_columns_equal_oracle(tt, dtype, k):
         assert rel(gm[..., r], rm[..., r]) <= tol
 
 
+@pytest.mark.parametrize("N_d,N_m,N_t,k", [(70, 5000, 16, 5), (130, 4500, 12, 33), (64, 8192, 64, 32),
+                                            (9, 257, 20, 17), (3, 31, 6, 40)])
+def test_dmma_gemm_path_shapes(tt, N_d, N_m, N_t, k):
+    """fp64 k-RHS path (batched FFTs + per-frequency DMMA GEMMs): ragged sensor blocks (N_d not a multiple
+    of 64, > 64), several p-splits, N_m not a multiple of 256, k not a multiple of 8 and k > 32."""
+    w = workload("C4", N_d, N_m, N_t, torch.float64)
+    F = synth.block_column(w)
+    M = synth.vector_m(w, k_rhs=k)
+    D = synth.vector_d(w, k_rhs=k)
+    plan = tt.Plan(F.cuda(), k_max=k)
+    try:
+        gd = plan.matvec_batched(M.cuda()).cpu().numpy()
+        gm = plan.rmatvec_batched(D.cuda()).cpu().numpy()
+        one_d = plan.matvec(M[..., 1].contiguous().cuda()).cpu().numpy()
+        one_m = plan.rmatvec(D[..., 1].contiguous().cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    cols = sorted({0, 1, k // 2, k - 1})
+    for r in cols:
+        assert rel(gd[..., r], ob.matvec(F.numpy(), M[..., r].contiguous().numpy())) <= 1e-12
+        assert rel(gm[..., r], ob.rmatvec(F.numpy(), D[..., r].contiguous().numpy())) <= 1e-12
+    # column r of the batched result equals the single-vector result on column r (include/tt.h)
+    assert rel(gd[..., 1], one_d) <= 1e-13 and rel(gm[..., 1], one_m) <= 1e-13
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
 def test_space_major_layout(tt, dtype):
     """TT_SPACE_MAJOR (time contiguous, the 'm (64x32)' shapes of BASELINE.json) gives the same numbers."""
