@@ -103,3 +103,38 @@ def test_paper_scale_slices_and_properties(tt, cfg):
     q = float((m.double() * FtFm.double()).sum())
     n2 = float(Fm.double().norm() ** 2)
     assert abs(q - n2) <= 10 * tol * n2                        # <m, F^T F m> = |F m|^2
+
+
+def test_c4_krhs_slices(tt):
+    """configs[3]: fp64, k = 32 right-hand sides through the DMMA GEMM path, at full size (34 GB spectrum).
+    Whole time series of sampled (sensor, column) and (parameter range, column) pairs against the oracle."""
+    w = synth.CONFIGS["C4"]
+    need_memory(110)
+    k = w.k_rhs
+    F = synth.block_column(w, device="cuda")
+    M, D = synth.vector_m(w, device="cuda"), synth.vector_d(w, device="cuda")   # [N_t, N_m, k], [N_t, N_d, k]
+    sensors, cols = [0, w.N_d - 1], [0, 13, k - 1]
+    p_ranges = [(0, 40), (w.N_m - 24, w.N_m)]
+    F_rows = {s: F[:, s:s + 1, :].contiguous().cpu().numpy() for s in sensors}
+    F_cols = {pr: F[:, :, pr[0]:pr[1]].contiguous().cpu().numpy() for pr in p_ranges}
+    plan = tt.Plan(F, k_max=k)
+    del F
+    torch.cuda.empty_cache()
+    try:
+        FM = plan.matvec_batched(M)
+        FtD = plan.rmatvec_batched(D)
+        torch.cuda.synchronize()
+    finally:
+        plan.close()
+    for r in cols:
+        m_r = M[..., r].contiguous().cpu().numpy()
+        d_r = D[..., r].contiguous().cpu().numpy()
+        for s in sensors:
+            ref = ob.matvec(F_rows[s], m_r)[:, 0]
+            assert rel(FM[:, s, r].cpu().numpy(), ref) <= 1e-12, f"F M, sensor {s}, column {r}"
+        for pr in p_ranges:
+            ref = ob.rmatvec(F_cols[pr], d_r)
+            assert rel(FtD[:, pr[0]:pr[1], r].cpu().numpy(), ref) <= 1e-12, f"F^T D, parameters {pr}, column {r}"
+    # adjoint identity over all columns at once: <F M, D> = <M, F^T D>
+    lhs, rhs = float((FM * D).sum()), float((M * FtD).sum())
+    assert abs(lhs - rhs) <= 1e-12 * float(FM.norm() * D.norm())
