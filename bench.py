@@ -178,6 +178,7 @@ def main() -> int:
     ap.add_argument("--config", default="C3", choices=sorted(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-library-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = synth.CONFIGS[args.config]
@@ -393,6 +394,37 @@ def main() -> int:
     except RuntimeError as e:  # pragma: no cover
         probe["error"] = str(e)
 
+    # ---- comparison row: the same operation with library FFTs and batched library matmuls ------
+    # (torch.fft = cuFFT, torch.bmm = cuBLAS; timed on the plan's own spectrum, never linked into libtt)
+    libs = None
+    if K == 1 and not args.no_library_baseline:
+        try:
+            Fv = tt.tt_debug_spectrum_view(h, w.N_t, w.N_d, w.dtype)[:, :, :w.N_m]
+            L2 = 2 * w.N_t
+
+            def lib_fwd():
+                mh_ = torch.fft.rfft(m, n=L2, dim=0)                       # [n_f, N_m]
+                dh_ = torch.bmm(Fv, mh_.unsqueeze(2)).squeeze(2)           # [n_f, N_d]
+                return torch.fft.irfft(dh_, n=L2, dim=0)[:w.N_t]
+
+            def lib_adj():
+                dh_ = torch.fft.rfft(d, n=L2, dim=0)                       # [n_f, N_d]
+                mh_ = torch.bmm(Fv.conj().transpose(1, 2), dh_.unsqueeze(2)).squeeze(2)
+                return torch.fft.irfft(mh_, n=L2, dim=0)[:w.N_t]
+
+            with torch.cuda.stream(stream):
+                r1, r2 = lib_fwd(), lib_adj()
+                e1 = float((r1 - d_out).norm() / d_out.norm()); e2 = float((r2 - m_out).norm() / m_out.norm())
+                del r1, r2
+                t_lf = time_op(lib_fwd, max(2, args.steps // 2))
+                t_la = time_op(lib_adj, max(2, args.steps // 2))
+            libs = {"what": "torch.fft.rfft/irfft (cuFFT) + torch.bmm over frequencies (cuBLAS) on the same spectrum",
+                    "matvec_ms": t_lf, "rmatvec_ms": t_la, "rel_diff_vs_libtt": [e1, e2]}
+            del Fv
+        except Exception as e:  # e.g. out of memory for the library temporaries
+            libs = {"error": str(e)[:200]}
+            torch.cuda.empty_cache()
+
     out = {
         "metric": METRIC, "value": ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
@@ -416,6 +448,7 @@ def main() -> int:
             "stages_rmatvec_ms": {"B1_fft": adj[0], "B2_gemv": adj[1], "B3_ifft": adj[2]},
         },
         "probe": probe,
+        "library_baseline": libs,
         "plan": {"create_s": t_plan, "device_bytes": plan.device_bytes, "input_generation_s": t_gen},
     }
 

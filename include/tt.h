@@ -167,6 +167,12 @@ int tt_plan_stage_ms(const tt_plan* plan, int op, float* ms, int n);
  * by bench.py to measure the read-only HBM bandwidth next to the copy figure. */
 int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream);
 
+/* Comparison hook (bench.py's cuFFT/cuBLAS baseline reads the plan's spectrum in place instead of
+ * holding a second 80 GB copy): *ptr = DEVICE address of Fhat[(w*N_d + s)*row_pitch + p], interleaved
+ * complex of the plan's dtype; *row_pitch in complex elements (N_m rounded up to 16).  Read-only; valid
+ * until tt_plan_destroy. */
+int tt_debug_spectrum_view(const tt_plan* plan, void** ptr, int64_t* row_pitch);
+
 /* FP64 tensor-pipe probe: every warp of 148*8 CTAs x 256 threads issues iters x 16 independent
  * mma.sync m8n8k4 f64 (DMMA); *flops (host, may be NULL) receives the flop count of the launch.
  * sink: DEVICE, >= 148*8*256 doubles.  bench.py times it for the measured DMMA peak. */

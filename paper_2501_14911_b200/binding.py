@@ -69,6 +69,7 @@ def lib() -> ctypes.CDLL:
         "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
         "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
+        "tt_debug_spectrum_view": (ci, [vp, pp, ctypes.POINTER(i64)]),
         "tt_probe_dmma": (ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]),
         "tt_debug_trig": (ci, [i64, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_set": (ci, [ctypes.c_char_p, ci]),
@@ -84,7 +85,7 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
-           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_fft_tables",
+           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set"]
 
 
@@ -185,6 +186,22 @@ def tt_plan_stage_ms(plan: int, op: int) -> tuple[float, float, float, int]:
 
 def tt_probe_stream_read(src, nbytes: int, sink, stream=None) -> None:
     _check("tt_probe_stream_read", lib().tt_probe_stream_read(_ptr(src), nbytes, _ptr(sink), _stream(stream)))
+
+
+class _CudaView:
+    """Minimal __cuda_array_interface__ carrier so that torch can wrap plan-owned device memory."""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (ptr, False),
+                                         "version": 3, "strides": None}
+
+
+def tt_debug_spectrum_view(plan: int, N_t: int, N_d: int, dtype) -> torch.Tensor:
+    """Read-only torch view [N_t+1, N_d, row_pitch] (complex) of the plan's spectrum, no copy."""
+    ptr, pitch = ctypes.c_void_p(), ctypes.c_int64()
+    _check("tt_debug_spectrum_view", lib().tt_debug_spectrum_view(plan, ctypes.byref(ptr), ctypes.byref(pitch)), plan)
+    ts = "<c8" if dtype == torch.float32 else "<c16"
+    return torch.as_tensor(_CudaView(ptr.value, (N_t + 1, N_d, pitch.value), ts), device="cuda")
 
 
 def tt_probe_dmma(iters: int, sink, stream=None) -> float:

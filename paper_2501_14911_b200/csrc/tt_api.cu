@@ -672,6 +672,13 @@ int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* 
     return TT_OK;
 }
 
+int tt_debug_spectrum_view(const tt_plan* p, void** ptr, int64_t* row_pitch) {
+    if (!p || !ptr || !row_pitch) return TT_ERR_NULL;
+    *ptr = p->Fhat;
+    *row_pitch = p->ldp;
+    return TT_OK;
+}
+
 int tt_probe_dmma(int iters, void* sink, double* flops, void* stream) {
     if (!sink) return TT_ERR_NULL;
     if (iters < 1) return TT_ERR_SHAPE;
