@@ -339,7 +339,7 @@ def main() -> int:
     if K == 1:
         xhat_bytes = n_f * ldp * 2 * es
         dhat_bytes = n_f * w.N_d * 2 * es
-        n_chunks = (ldp + 2047) // 2048
+        n_chunks = (ldp + 4095) // 4096
         part_bytes = n_f * n_chunks * w.N_d * 2 * es
         bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
         bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written

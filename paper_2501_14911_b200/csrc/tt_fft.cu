@@ -353,23 +353,24 @@ cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int 
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
-static int g_force_T = 0;
+static int g_force_T = 0, g_force_NT = 0;
 void fft_debug_force_T(int T) { g_force_T = T; }
+void fft_debug_force_threads(int NT) { g_force_NT = NT; }
 
 FftChoice fft_choose(int N, size_t elem) {
-    const int Ts[3] = {32, 16, 8};
-    FftChoice c{0, elem == 8 ? 512 : 256, 0};
+    // Measured on B200 (C2, C3, C5 shapes, both precisions): 256 threads and T = 16 series per CTA win as
+    // long as >= 3 CTAs fit one SM's shared memory; the phases of a CTA (global load, passes, store) are
+    // serial, so several resident CTAs are what overlaps HBM traffic with the butterflies.
+    FftChoice c{0, 256, 0};
+    auto bytes = [&](int T) { return size_t(N + 1) * T * elem; };
     if (g_force_T) {
-        const size_t bytes = size_t(N + 1) * g_force_T * elem;
-        if (bytes <= size_t(kMaxSmem)) { c.T = g_force_T; c.smem = bytes; return c; }
+        if (bytes(g_force_T) <= size_t(kMaxSmem)) { c.T = g_force_T; c.smem = bytes(g_force_T); return c; }
     }
-    for (int pass = 0; pass < 2; ++pass) {
-        const size_t limit = pass == 0 ? size_t(113) * 1024 : size_t(kMaxSmem);
-        for (int i = 0; i < 3; ++i) {
-            const size_t bytes = size_t(N + 1) * Ts[i] * elem;
-            if (bytes <= limit) { c.T = Ts[i]; c.smem = bytes; return c; }
-        }
-    }
+    const int order[3] = {16, 8, 32};
+    const size_t limits[3] = {size_t(76) * 1024, size_t(113) * 1024, size_t(kMaxSmem)};
+    for (int pass = 0; pass < 3; ++pass)
+        for (int i = 0; i < (pass == 0 ? 3 : 2); ++i)
+            if (bytes(order[i]) <= limits[pass]) { c.T = order[i]; c.smem = bytes(order[i]); return c; }
     return c;
 }
 
@@ -377,17 +378,18 @@ template <typename Tin, typename Tc, typename Tout>
 static cudaError_t r2c_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
     if (c.T == 0) return cudaErrorInvalidValue;
-    constexpr int NT = sizeof(Tc) == 4 ? 512 : 256;
+    const int nt = g_force_NT ? g_force_NT : 256;
     const long long nb = (P.B_store > P.B ? P.B_store : P.B);
     dim3 grid((unsigned)((nb + c.T - 1) / c.T), (unsigned)ny);
-#define TT_R2C(TT)                                                                                           \
+#define TT_R2C(TT, NT)                                                                                       \
     {                                                                                                        \
         auto k = fft_r2c_kernel<Tin, Tc, Tout, TT, NT>;                                                      \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Tin*>(in), static_cast<Cx<Tout>*>(out), P);             \
     }
-    if (c.T == 32) TT_R2C(32) else if (c.T == 16) TT_R2C(16) else TT_R2C(8)
+    if (nt == 512) { if (c.T == 32) TT_R2C(32, 512) else if (c.T == 16) TT_R2C(16, 512) else TT_R2C(8, 512) }
+    else           { if (c.T == 32) TT_R2C(32, 256) else if (c.T == 16) TT_R2C(16, 256) else TT_R2C(8, 256) }
 #undef TT_R2C
     return cudaGetLastError();
 }
@@ -404,16 +406,17 @@ template <typename Tc>
 static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
     if (c.T == 0) return cudaErrorInvalidValue;
-    constexpr int NT = sizeof(Tc) == 4 ? 512 : 256;
+    const int nt = g_force_NT ? g_force_NT : 256;
     dim3 grid((unsigned)((P.B + c.T - 1) / c.T), (unsigned)ny);
-#define TT_C2R(TT)                                                                                           \
+#define TT_C2R(TT, NT)                                                                                       \
     {                                                                                                        \
         auto k = fft_c2r_kernel<Tc, TT, NT>;                                                                 \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P);                \
     }
-    if (c.T == 32) TT_C2R(32) else if (c.T == 16) TT_C2R(16) else TT_C2R(8)
+    if (nt == 512) { if (c.T == 32) TT_C2R(32, 512) else if (c.T == 16) TT_C2R(16, 512) else TT_C2R(8, 512) }
+    else           { if (c.T == 32) TT_C2R(32, 256) else if (c.T == 16) TT_C2R(16, 256) else TT_C2R(8, 256) }
 #undef TT_C2R
     return cudaGetLastError();
 }

@@ -18,8 +18,8 @@ namespace tt {
 // shuffle reduction per row.  Cross-chunk sums are formed in fixed order by the inverse-FFT
 // kernel (no atomics: results are bit-reproducible run to run).
 // ---------------------------------------------------------------------------------------
-template <typename R, int NWARPS, int UNROLL>
-__global__ void __launch_bounds__(NWARPS * 32)
+template <typename R, int UNROLL>
+__global__ void __launch_bounds__(1024)
 gemv_fwd_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ xhat, Cx<R>* __restrict__ partial,
                 const GemvGeom g) {
     using V = typename Vec16<R>::type;
@@ -34,7 +34,8 @@ gemv_fwd_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ xhat, 
     const int nvec = len / VN;
 
     const V* xsrc = reinterpret_cast<const V*>(xhat + (long long)w * g.ldp + p0);
-    for (int i = threadIdx.x; i < nvec; i += NWARPS * 32) xs[i] = xsrc[i];
+    const int NWARPS = blockDim.x >> 5;
+    for (int i = threadIdx.x; i < nvec; i += blockDim.x) xs[i] = xsrc[i];
     __syncthreads();
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -75,8 +76,8 @@ gemv_fwd_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ xhat, 
 // reads 512 contiguous bytes of every row.  dhat_w (N_d complex numbers) sits in shared
 // memory and is broadcast.  No reduction across threads.
 // ---------------------------------------------------------------------------------------
-template <typename R, int NT, int UNROLL>
-__global__ void __launch_bounds__(NT)
+template <typename R, int UNROLL>
+__global__ void __launch_bounds__(512)
 gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, Cx<R>* __restrict__ xout,
                 const GemvGeom g) {
     using V = typename Vec16<R>::type;
@@ -85,6 +86,7 @@ gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, 
     Cx<R>* ds = reinterpret_cast<Cx<R>*>(smem_raw);
 
     const int w = blockIdx.y;
+    const int NT = blockDim.x;
     for (int i = threadIdx.x; i < g.N_d; i += NT) ds[i] = dhat[(long long)w * g.N_d + i];
     __syncthreads();
 
@@ -145,11 +147,22 @@ __global__ void __launch_bounds__(512) probe_read_kernel(const float4* __restric
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
+static int g_fwd_warps = 0, g_adj_threads = 0;
+void gemv_debug_set(int fwd_warps, int adj_threads) {
+    if (fwd_warps >= 0) g_fwd_warps = fwd_warps;
+    if (adj_threads >= 0) g_adj_threads = adj_threads;
+}
+
+// Warps per CTA of the forward kernel.  Measured at C3 on B200 (N_d = 100): 10, 16 and 20 warps are within
+// 1 % of each other (11.5-11.6 ms), 25 and 32 warps (one CTA per SM) lose 20 %; 16 it is.
+static int fwd_warps(int) { return g_fwd_warps ? g_fwd_warps : 16; }
+
 template <typename R>
 static cudaError_t fwd_dispatch(const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,
                                 cudaStream_t s) {
-    constexpr int NW = 16, UN = 8;
-    auto k = gemv_fwd_kernel<R, NW, UN>;
+    constexpr int UN = 8;
+    const int NW = fwd_warps(g.N_d);
+    auto k = gemv_fwd_kernel<R, UN>;
     const size_t smem = (size_t)g.chunk * sizeof(Cx<R>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -162,8 +175,9 @@ static cudaError_t fwd_dispatch(const void* Fhat, const void* xhat, void* partia
 template <typename R>
 static cudaError_t adj_dispatch(const void* Fhat, const void* dhat, void* xout, const GemvGeom& g,
                                 cudaStream_t s) {
-    constexpr int NT = 256, UN = 10;
-    auto k = gemv_adj_kernel<R, NT, UN>;
+    constexpr int UN = 10;
+    const int NT = g_adj_threads ? g_adj_threads : 256;
+    auto k = gemv_adj_kernel<R, UN>;
     const size_t smem = (size_t)g.N_d * sizeof(Cx<R>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

@@ -49,6 +49,7 @@ cudaError_t fft_c2r_launch(int tc, const void* cplx_in, void* real_out, const Ff
 cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int n_f, int n_chunks, int N_d,
                                    cudaStream_t s);
 void fft_debug_force_T(int T);  // 0 = planner's choice
+void fft_debug_force_threads(int NT);  // 256 or 512; 0 = default (512 for fp32, 256 for fp64)
 double debug_cos2pi(long long k, long long n);
 double debug_sin2pi(long long k, long long n);
 
@@ -61,6 +62,7 @@ struct GemvGeom {
     int chunk;      // forward: elements of p per CTA (multiple of 64)
     int n_chunks;
 };
+void gemv_debug_set(int fwd_warps, int adj_threads);  // -1 = leave, 0 = planner's choice
 cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,
                             cudaStream_t s);
 cudaError_t gemv_adj_launch(int dt, const void* Fhat, const void* dhat, void* xhat_out, const GemvGeom& g,
