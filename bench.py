@@ -432,7 +432,7 @@ def main() -> int:
         "config": config_dict(w, args),
         "e2e": {"value": ms_e2e / args.gpus, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": n_e2e, "api": e2e_api},
-        "gpu_launches": (6 if K == 1 else 7) * args.steps,
+        "gpu_launches": 7 * args.steps,   # A1, A2, partial reduce, A3, B1, B2, B3
         "clocks": clocks.summary(),
         "roofline": roofline,
         "ops": {
