@@ -179,13 +179,14 @@ int tt_debug_spectrum_view(const tt_plan* plan, void** ptr, int64_t* row_pitch);
 int tt_probe_dmma(int iters, void* sink, double* flops, void* stream);
 
 /* Test hook for the planner's host logic (needs no GPU): the FFT plan of an N_t-point series.
+ *   max_radix largest register butterfly allowed: 25 = the fp32 kernels' plan, 8 = the fp64 kernels' plan
  *   n_stages  receives the number of decimation-in-frequency stages
  *   radix     int[16], receives their radices (product = N_t)
  *   pos       unsigned short[N_t], pos[k] = slot of the in-place DIF output holding bin k
  *   tw        double[4*N_t], interleaved (re, im) of exp(-2 pi i k / (2 N_t)), k < 2 N_t
  * Returns TT_ERR_UNSUPPORTED_NT if N_t does not factor into {2,3,5,7} or exceeds 65535.
- * The radices are taken from {25,20,16,8,7,5,4,3,2}, largest first. */
-int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* pos, double* tw);
+ * The radices are taken from {25,20,16,8,7,5,4,3,2} (those <= max_radix), largest first. */
+int tt_debug_fft_tables(int64_t N_t, int max_radix, int* n_stages, int* radix, unsigned short* pos, double* tw);
 
 /* Test hook (no GPU): the compile-time trigonometry the register butterflies use for their
  * internal twiddles, evaluated on the host: *c = cos(2 pi k / n), *s = sin(2 pi k / n). */

@@ -67,7 +67,7 @@ def lib() -> ctypes.CDLL:
         "tt_plan_set_profiling": (ci, [vp, ci]),
         "tt_plan_stage_ms": (ci, [vp, ci, ctypes.POINTER(ctypes.c_float), ci]),
         "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
-        "tt_debug_fft_tables": (ci, [i64, ctypes.POINTER(ci), ctypes.POINTER(ci),
+        "tt_debug_fft_tables": (ci, [i64, ci, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_spectrum_view": (ci, [vp, pp, ctypes.POINTER(i64)]),
         "tt_probe_dmma": (ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]),
@@ -211,14 +211,14 @@ def tt_probe_dmma(iters: int, sink, stream=None) -> float:
     return fl.value
 
 
-def tt_debug_fft_tables(N_t: int):
+def tt_debug_fft_tables(N_t: int, max_radix: int = 25):
     """(radices, pos, tw) of the planner's FFT plan for an N_t-point series; runs without a GPU."""
     import numpy as np
     n = ctypes.c_int()
     radix = (ctypes.c_int * 16)()
     pos = (ctypes.c_ushort * max(1, N_t))()
     tw = (ctypes.c_double * (4 * max(1, N_t)))()
-    st = lib().tt_debug_fft_tables(N_t, ctypes.byref(n), radix, pos, tw)
+    st = lib().tt_debug_fft_tables(N_t, max_radix, ctypes.byref(n), radix, pos, tw)
     _check("tt_debug_fft_tables", st)
     return (list(radix[: n.value]), np.array(pos[:N_t], dtype=np.int64),
             np.array(tw[: 4 * N_t]).reshape(2 * N_t, 2) @ np.array([1.0, 1.0j]))

@@ -30,11 +30,12 @@ struct tt_plan {
     int dtype = 0, layout = 0, k_max = 1;
     int n_f = 0;
     long long ldp = 0;  // padded N_m: row pitch of Fhat and of the single-vector spectrum
-    int n_stages = 0;
-    int radix[kMaxStages] = {};
+    // FFT plans: index 0 = fp32 kernels (radices up to 25), 1 = fp64 kernels (up to 8)
+    int n_stages[2] = {0, 0};
+    int radix[2][kMaxStages] = {};
+    unsigned short* pos[2] = {nullptr, nullptr};
     void* tw_d = nullptr;  // c128[2N]
     void* tw_f = nullptr;  // c64[2N] (TT_F32 only)
-    unsigned short* pos = nullptr;
     void* Fhat = nullptr;
     void* xhat = nullptr;     // [n_f][ldp] complex
     void* dhat = nullptr;     // [n_f][N_d] complex
@@ -78,12 +79,13 @@ int dev_alloc(tt_plan* p, void** ptr, size_t bytes) {
 
 // Radices of the N-point complex FFT, largest register butterflies first (fewest passes over
 // shared memory): N = 400 -> 25*16, 500 -> 25*20, 256 -> 16*16, 512 -> 16*16*2.
-bool factorise(long long N, int* radix, int* n_stages) {
+bool factorise(long long N, int max_radix, int* radix, int* n_stages) {
     int n = 0;
     long long r = N;
     const int cand[9] = {25, 20, 16, 8, 7, 5, 4, 3, 2};
+    if (g_fft_max_radix && g_fft_max_radix < max_radix) max_radix = g_fft_max_radix;
     for (int c = 0; c < 9; ++c)
-        while (r % cand[c] == 0 && r > 1 && (g_fft_max_radix == 0 || cand[c] <= g_fft_max_radix)) {
+        while (r % cand[c] == 0 && r > 1 && cand[c] <= max_radix) {
             if (n >= kMaxStages) return false;
             radix[n++] = cand[c];
             r /= cand[c];
@@ -134,15 +136,16 @@ void build_twiddles(int L, std::vector<double>& tw) {
 void fill_fft_common(const tt_plan* p, FftParams& P, bool fp32_tables) {
     std::memset(&P, 0, sizeof(P));
     P.N = (int)p->N_t;
-    P.n_stages = p->n_stages;
+    const int which = fp32_tables ? 0 : 1;
+    P.n_stages = p->n_stages[which];
     int Ns = P.N;
-    for (int i = 0; i < p->n_stages; ++i) {
-        P.radix[i] = p->radix[i];
-        Ns /= p->radix[i];
+    for (int i = 0; i < P.n_stages; ++i) {
+        P.radix[i] = p->radix[which][i];
+        Ns /= P.radix[i];
         P.magic[i] = Ns > 1 ? (unsigned)((0x100000000ULL + (unsigned long long)Ns - 1) / (unsigned long long)Ns) : 0u;
     }
     P.tw = fp32_tables ? p->tw_f : p->tw_d;
-    P.pos = p->pos;
+    P.pos = p->pos[which];
     P.scale = 1.0 / (2.0 * (double)p->N_t);
 }
 
@@ -372,7 +375,7 @@ const char* tt_status_string(int status) {
 
 void tt_plan_destroy(tt_plan* p) {
     if (!p) return;
-    void* bufs[] = {p->tw_d, p->tw_f, p->pos, p->Fhat, p->xhat, p->dhat, p->partial,
+    void* bufs[] = {p->tw_d, p->tw_f, p->pos[0], p->pos[1], p->Fhat, p->xhat, p->dhat, p->partial,
                     p->dwork, p->m_stage, p->m_stage2, p->d_stage};
     for (void* b : bufs)
         if (b) cudaFree(b);
@@ -399,9 +402,10 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     if ((long double)N_d * (long double)(N_m + 16) * (long double)(N_t + 1) * 16.0L > lim) return TT_ERR_SHAPE;
     if ((long double)(N_m + 16) * (long double)(N_t + 1) * (long double)k_max * 16.0L > lim) return TT_ERR_SHAPE;
 
-    int radix[kMaxStages] = {};
-    int n_stages = 0;
-    if (N_t > 65535 || !factorise(N_t, radix, &n_stages)) return TT_ERR_UNSUPPORTED_NT;
+    int radix[2][kMaxStages] = {};
+    int n_stages[2] = {0, 0};
+    if (N_t > 65535 || !factorise(N_t, 25, radix[0], &n_stages[0]) || !factorise(N_t, 8, radix[1], &n_stages[1]))
+        return TT_ERR_UNSUPPORTED_NT;
     const FftChoice cd = fft_choose((int)N_t, 16);  // the fp64 transform of the matrix is the largest user
     if (cd.T == 0) return TT_ERR_UNSUPPORTED_NT;
 
@@ -421,8 +425,10 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     p->dtype = dtype; p->layout = layout; p->k_max = k_max;
     p->n_f = (int)N_t + 1;
     p->ldp = (N_m + 15) / 16 * 16;
-    p->n_stages = n_stages;
-    for (int i = 0; i < n_stages; ++i) p->radix[i] = radix[i];
+    for (int wch = 0; wch < 2; ++wch) {
+        p->n_stages[wch] = n_stages[wch];
+        for (int i = 0; i < n_stages[wch]; ++i) p->radix[wch][i] = radix[wch][i];
+    }
     p->chunk = g_gemv_chunk > 0 ? g_gemv_chunk / 64 * 64 : 4096;  // measured: 4096/8192 ~1 % ahead of 2048 at C3
     if (p->chunk < 64) p->chunk = 64;
     p->n_chunks = (int)((p->ldp + p->chunk - 1) / p->chunk);
@@ -447,8 +453,8 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     {
         std::vector<double> tw;
         build_twiddles(L, tw);
-        std::vector<unsigned short> pos;
-        build_pos((int)N_t, radix, n_stages, pos);
+        std::vector<unsigned short> pos[2];
+        for (int wch = 0; wch < 2; ++wch) build_pos((int)N_t, radix[wch], n_stages[wch], pos[wch]);
         TT_TRY(dev_alloc(p, &p->tw_d, tw.size() * sizeof(double)));
         TT_TRYC(cudaMemcpyAsync(p->tw_d, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         std::vector<float> twf(tw.size());
@@ -457,8 +463,11 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
             TT_TRY(dev_alloc(p, &p->tw_f, twf.size() * sizeof(float)));
             TT_TRYC(cudaMemcpyAsync(p->tw_f, twf.data(), twf.size() * sizeof(float), cudaMemcpyHostToDevice, s));
         }
-        TT_TRY(dev_alloc(p, reinterpret_cast<void**>(&p->pos), pos.size() * sizeof(unsigned short)));
-        TT_TRYC(cudaMemcpyAsync(p->pos, pos.data(), pos.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, s));
+        for (int wch = 0; wch < 2; ++wch) {
+            TT_TRY(dev_alloc(p, reinterpret_cast<void**>(&p->pos[wch]), pos[wch].size() * sizeof(unsigned short)));
+            TT_TRYC(cudaMemcpyAsync(p->pos[wch], pos[wch].data(), pos[wch].size() * sizeof(unsigned short),
+                                    cudaMemcpyHostToDevice, s));
+        }
         TT_TRYC(cudaStreamSynchronize(s));  // the host vectors die at the end of this scope
     }
 
@@ -658,11 +667,12 @@ int tt_plan_stage_ms(const tt_plan* p, int op, float* ms, int n) {
     return TT_OK;
 }
 
-int tt_debug_fft_tables(int64_t N_t, int* n_stages, int* radix, unsigned short* pos, double* tw) {
+int tt_debug_fft_tables(int64_t N_t, int max_radix, int* n_stages, int* radix, unsigned short* pos, double* tw) {
     if (!n_stages || !radix || !pos || !tw) return TT_ERR_NULL;
     if (N_t < 1) return TT_ERR_SHAPE;
     int rx[kMaxStages] = {};
-    if (N_t > 65535 || !factorise(N_t, rx, n_stages)) return TT_ERR_UNSUPPORTED_NT;
+    if (max_radix < 2) return TT_ERR_SHAPE;
+    if (N_t > 65535 || !factorise(N_t, max_radix, rx, n_stages)) return TT_ERR_UNSUPPORTED_NT;
     for (int i = 0; i < kMaxStages; ++i) radix[i] = i < *n_stages ? rx[i] : 0;
     std::vector<unsigned short> pv;
     build_pos((int)N_t, rx, *n_stages, pv);

@@ -165,8 +165,13 @@ __device__ __forceinline__ void fft_stage(Cx<R>* __restrict__ sm, const Cx<R>* _
     }
 }
 
+// MAXR = largest register butterfly compiled into the kernel: fp32 kernels take up to radix 25; fp64
+// kernels stop at radix 8 so that they stay near 64 registers and four CTAs fit one SM.
+template <typename R> struct MaxRadix { static constexpr int value = sizeof(R) == 4 ? 25 : 8; };
+
 template <typename R, int T>
 __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int lane_s, int g, int G) {
+    constexpr int MAXR = MaxRadix<R>::value;
     const Cx<R>* tw = reinterpret_cast<const Cx<R>*>(P.tw);
     int Ns = P.N;
     for (int st = 0; st < P.n_stages; ++st) {
@@ -181,9 +186,13 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
             case 5: fft_stage<R, T, 5>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
             case 7: fft_stage<R, T, 7>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
             case 8: fft_stage<R, T, 8>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
-            case 16: fft_stage<R, T, 16>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
-            case 20: fft_stage<R, T, 20>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
-            default: fft_stage<R, T, 25>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            default:
+                if constexpr (MAXR >= 25) {
+                    if (r == 16) fft_stage<R, T, 16>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                    else if (r == 20) fft_stage<R, T, 20>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                    else fft_stage<R, T, 25>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                }
+                break;
         }
         Ns = M;
     }

@@ -74,11 +74,12 @@ def replay_dif(z, radices, tw):
     return x
 
 
+@pytest.mark.parametrize("max_radix", [25, 8], ids=["fp32plan", "fp64plan"])
 @pytest.mark.parametrize("N_t", [1, 2, 3, 4, 5, 6, 7, 8, 12, 15, 21, 32, 35, 49, 50, 60, 64, 100, 210, 256, 400, 500, 512])
-def test_fft_plan_tables_reproduce_numpy_fft(tt, N_t):
-    radices, pos, tw = tt.tt_debug_fft_tables(N_t)
+def test_fft_plan_tables_reproduce_numpy_fft(tt, N_t, max_radix):
+    radices, pos, tw = tt.tt_debug_fft_tables(N_t, max_radix)
     assert int(np.prod(radices)) == N_t if radices else N_t == 1
-    assert all(r in (2, 3, 4, 5, 7, 8, 16, 20, 25) for r in radices)
+    assert all(r in (2, 3, 4, 5, 7, 8, 16, 20, 25) and r <= max_radix for r in radices)
     assert sorted(pos.tolist()) == list(range(N_t))                     # a permutation
     L = 2 * N_t
     k = np.arange(L)
