@@ -171,10 +171,11 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
             const int ns = g.N_d - sb < kAdjSB ? g.N_d - sb : kAdjSB;
             const int nsteps = (ns + 3) / 4;
             const c128* col = Fw + (long long)(sb + (lane & 3)) * g.ldp + (pok ? p : 0);
-            for (int t0 = 0; t0 < nsteps; t0 += 8) {
-                c128 af[8];
+            // software pipeline over batches of 4 k-steps: the A fragments of batch b+1 are in flight
+            // while the DMMAs of batch b issue
+            auto load_batch = [&](c128 (&af)[4], int t0) {
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
+                for (int u = 0; u < 4; ++u) {
                     const int t = t0 + u;
                     af[u] = mk<double>(0.0, 0.0);
                     if (pok && t < nsteps && sb + 4 * t + (lane & 3) < g.N_d) {
@@ -182,8 +183,10 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
                         af[u] = mk<double>(v.x, v.y);
                     }
                 }
+            };
+            auto mma_batch = [&](const c128 (&af)[4], int t0) {
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
+                for (int u = 0; u < 4; ++u) {
                     const int t = t0 + u;
                     if (t < nsteps) {
                         const c128* b = Ds + (4 * t + (lane & 3)) * BP + (lane >> 2);
@@ -197,6 +200,14 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
                         }
                     }
                 }
+            };
+            c128 a0[4], a1[4];
+            load_batch(a0, 0);
+            for (int t0 = 0; t0 < nsteps; t0 += 8) {
+                load_batch(a1, t0 + 4);
+                mma_batch(a0, t0);
+                load_batch(a0, t0 + 8);
+                mma_batch(a1, t0 + 4);
             }
         }
         if (pok) {
