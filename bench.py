@@ -38,6 +38,7 @@ from paper_2501_14911_b200 import synth  # noqa: E402
 METRIC = "ms per F·m and F^T·d at ~1e8 params; achieved HBM GB/s vs B200 peak"
 NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0    # B200_PROFILING.md fallback
+SAMPLE_SENSORS, SAMPLE_PARAMS = 40, 75000   # largest CPU-baseline sample (about 10-20 s on 16 host cores at C3)
 
 
 def measured_peaks():
@@ -111,12 +112,12 @@ def oracle_sample(w, F_s, m_s, d_s):
 
 def cpu_baseline(w, draw, target_s=15.0):
     """draw(ns, npar) -> (F_s [N_t,ns,npar], m_s [N_t,npar], d_s [N_t,ns]) numpy.  Extrapolates by MAC count."""
-    npar = min(w.N_m, 25000)
-    ns = min(w.N_d, 8)
+    npar = min(w.N_m, SAMPLE_PARAMS)
+    ns = min(w.N_d, 4)
     ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # warms the library and the caches
     ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # calibration
     per_sensor = max(1e-3, (ta + tb) / ns)
-    ns2 = int(max(ns, min(w.N_d, 40, round(target_s / per_sensor))))
+    ns2 = int(max(ns, min(w.N_d, SAMPLE_SENSORS, round(target_s / per_sensor))))
     ta, tb, thr = oracle_sample(w, *draw(ns2, npar))
     scale = (w.N_d * w.N_m) / float(ns2 * npar) * w.k_rhs   # k-RHS: the oracle does the columns one by one
     return {
@@ -219,7 +220,7 @@ def main() -> int:
     samples = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # fetch the largest sample cpu_baseline() may ask for before the column is freed
-        samples = draw(min(w.N_d, 40), min(w.N_m, 25000))
+        samples = draw(min(w.N_d, SAMPLE_SENSORS), min(w.N_m, SAMPLE_PARAMS))
 
     t0 = time.perf_counter()
     plan = tt.Plan(F, k_max=K)
