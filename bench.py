@@ -38,6 +38,9 @@ from paper_2501_14911_b200 import synth  # noqa: E402
 METRIC = "ms per F·m and F^T·d at ~1e8 params; achieved HBM GB/s vs B200 peak"
 NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0    # B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum of one gemv_fwd_kernel launch at C3, from the ncu --set full capture
+# summarised in profiles/r1_e_c3_ncu_full.md (81.003920 GB read + 22.305280 MB written); algorithmic: 81.02 GB
+NCU_TRAFFIC_BYTES = {"C3": 81.003920e9 + 22.305280e6}
 SAMPLE_SENSORS, SAMPLE_PARAMS = 40, 75000   # largest CPU-baseline sample (about 10-20 s on 16 host cores at C3)
 
 
@@ -348,7 +351,8 @@ def main() -> int:
         ach_adj = bytes_adj_kernel / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
         roofline = {
             "bound": "hbm", "kernel": "gemv_fwd_kernel (A2, per-frequency matvec streaming Fhat)",
-            "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak, "traffic": None,
+            "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak,
+            "traffic": NCU_TRAFFIC_BYTES.get(args.config),
             "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
                          else "fallback 6.65 TB/s (B200_PROFILING.md)",
             "algorithmic_bytes_per_launch": bytes_fwd_kernel, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
