@@ -170,7 +170,9 @@ def config_dict(w, args):
             "baseline_config": args.config,
             "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)" if w.k_rhs == 1
                     else f"one batched F.M + one batched F^T.D, k={w.k_rhs} (batched FFTs + per-frequency DMMA GEMMs)",
-            "layout": "time-major", "parallelism": "replicas only" if args.gpus > 1 else "single GPU",
+            "layout": "time-major",
+            "parallelism": ("single GPU" if args.gpus == 1 else "replicas only" if args.parallel == "replicas"
+                            else f"N_m sharded over {args.gpus} ranks, one all-reduce of d per F.m"),
             "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
 
 
@@ -181,6 +183,9 @@ def main() -> int:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C3", choices=sorted(synth.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
+                    help="N>1: independent replicas (default, the north star's one-GPU path) or the parameter axis "
+                         "sharded over the ranks with one all-reduce of d per F.m (paper_2501_14911_b200/sharded.py)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-library-baseline", action="store_true")
     args = ap.parse_args()
@@ -207,9 +212,17 @@ def main() -> int:
 
     # ---- inputs, resident in HBM ----------------------------------------------------------
     t0 = time.perf_counter()
-    F = synth.block_column(w, device=dev)
+    shard = args.parallel == "shard" and world > 1
     K = w.k_rhs                                   # > 1: the k-RHS batched calls (C4)
-    m = synth.vector_m(w, device=dev)             # [N_t, N_m] or [N_t, N_m, K]
+    if shard:
+        from paper_2501_14911_b200 import sharded
+        p0, p1 = sharded.shard_range(w.N_m, rank, world)
+        F = synth.block_column(w, device=dev, p_range=(p0, p1))
+        m = synth.vector_m(w, device=dev)[:, p0:p1].contiguous()
+        w_full, w = w, w.scaled(N_m=p1 - p0)      # byte counts below are this rank's
+    else:
+        F = synth.block_column(w, device=dev)
+        m = synth.vector_m(w, device=dev)         # [N_t, N_m] or [N_t, N_m, K]
     d = synth.vector_d(w, device=dev)
     torch.cuda.synchronize()
     t_gen = time.perf_counter() - t0
@@ -245,6 +258,14 @@ def main() -> int:
         op_fwd = lambda: tt.tt_matvec_batched(h, K, m, d_out, stream)
         op_adj = lambda: tt.tt_rmatvec_batched(h, K, d, m_out, stream)
         tag_fwd, tag_adj = tt.TT_OP_MATVEC_BATCHED, tt.TT_OP_RMATVEC_BATCHED
+
+    if shard:  # F.m = local partial + the path's one exchange step; F^T.d needs no collective
+        local_fwd = op_fwd
+
+        def op_fwd():
+            local_fwd()
+            with torch.cuda.stream(stream):
+                dist.all_reduce(d_out, op=dist.ReduceOp.SUM)
 
     def step():
         op_fwd()
@@ -402,7 +423,7 @@ def main() -> int:
     # ---- comparison row: the same operation with library FFTs and batched library matmuls ------
     # (torch.fft = cuFFT, torch.bmm = cuBLAS; timed on the plan's own spectrum, never linked into libtt)
     libs = None
-    if K == 1 and not args.no_library_baseline:
+    if K == 1 and world == 1 and not args.no_library_baseline:
         try:
             Fv = tt.tt_debug_spectrum_view(h, w.N_t, w.N_d, w.dtype)[:, :, :w.N_m]
             L2 = 2 * w.N_t
@@ -431,10 +452,11 @@ def main() -> int:
             torch.cuda.empty_cache()
 
     out = {
-        "metric": METRIC, "value": ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "metric": METRIC, "value": ms_step if shard else ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus,
+        "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "strong" if shard else "weak",
         "vs_baseline": None, "dtype": "f32" if w.dtype == torch.float32 else "f64", "data": "synthetic",
-        "config": config_dict(w, args),
+        "config": config_dict(w_full if shard else w, args),
         "e2e": {"value": ms_e2e / args.gpus, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": n_e2e, "api": e2e_api},
         "gpu_launches": 7 * args.steps,   # A1, A2, partial reduce, A3, B1, B2, B3

@@ -1,0 +1,60 @@
+"""N_m-sharded application of F and F^T over several ranks (one process per GPU).
+
+How the path shards: along the spatial parameter axis.
+Rank g holds the spectrum of its own parameter slice, Fhat[:, :, P_g], and the slice m[:, P_g]:
+
+    F m    = sum_g F[:, :, P_g] m[:, P_g]   -> local tt_matvec, then ONE all-reduce (sum) of d
+                                               (N_d*N_t reals: 160 KB at C3, latency-bound)
+    F^T d  -> d is replicated, every rank produces its own slice of m': no collective at all
+    F^T F m = rmatvec(matvec(m))            -> one all-reduce in the middle
+
+The north star of this build is the one-GPU path (bench.py's default is independent replicas);
+this wrapper is the recorded, tested route to more GPUs: torch.distributed (NCCL on GPUs, gloo in
+the CPU tests) does the only exchange step the method has.  It holds none of the method's
+arithmetic: the local operator is passed in (a tt Plan on a GPU; the CPU oracle in the gloo test).
+"""
+from __future__ import annotations
+
+import torch
+import torch.distributed as dist
+
+
+def shard_range(N_m: int, rank: int, world: int, align: int = 16) -> tuple[int, int]:
+    """Contiguous parameter range [p0, p1) of `rank`: equal shares, boundaries on multiples of `align`
+    (the row pitch granularity of Fhat) except the last one; empty ranges only if N_m < world*align."""
+    blocks = (N_m + align - 1) // align
+    b0 = blocks * rank // world
+    b1 = blocks * (rank + 1) // world
+    return min(N_m, b0 * align), min(N_m, b1 * align)
+
+
+class ShardedOperator:
+    """F, F^T, F^T F with the parameter axis split over the ranks of `group`.
+
+    local_matvec(m_local)  -> this rank's partial d  (tensor [N_t, N_d], same shape on all ranks)
+    local_rmatvec(d)       -> this rank's slice of m' (tensor [N_t, p1 - p0])
+    """
+
+    def __init__(self, local_matvec, local_rmatvec, group=None):
+        self.local_matvec, self.local_rmatvec, self.group = local_matvec, local_rmatvec, group
+
+    @property
+    def world(self) -> int:
+        return dist.get_world_size(self.group) if dist.is_available() and dist.is_initialized() else 1
+
+    def matvec(self, m_local: torch.Tensor) -> torch.Tensor:
+        d = self.local_matvec(m_local)
+        if self.world > 1:
+            dist.all_reduce(d, op=dist.ReduceOp.SUM, group=self.group)   # the path's only exchange step
+        return d
+
+    def rmatvec(self, d: torch.Tensor) -> torch.Tensor:
+        return self.local_rmatvec(d)
+
+    def normal(self, m_local: torch.Tensor) -> torch.Tensor:
+        return self.rmatvec(self.matvec(m_local))
+
+
+def from_plan(plan, group=None) -> ShardedOperator:
+    """Wraps a tt Plan built on this rank's slice F[:, :, p0:p1] of the block column."""
+    return ShardedOperator(plan.matvec, plan.rmatvec, group)
