@@ -73,7 +73,9 @@ typedef enum tt_status {
     TT_ERR_ALIAS = -7,          /* out aliases in (tt_normal) */
     TT_ERR_OOM = -8,            /* cudaMalloc failed */
     TT_ERR_CUDA = -9,           /* any other CUDA runtime error (see tt_plan_last_cuda_error) */
-    TT_ERR_NO_DEVICE = -10      /* no CUDA device / wrong architecture: there is no CPU path */
+    TT_ERR_NO_DEVICE = -10,     /* no CUDA device / wrong architecture: there is no CPU path */
+    TT_ERR_NOT_SPD = -11,       /* tt_chol_create: a diagonal entry of the factor is not positive and finite */
+    TT_ERR_MISMATCH = -12       /* plans / factor / vectors of one call disagree in shape, dtype or layout */
 } tt_status;
 
 /* Library version, major*10000 + minor*100 + patch. */
@@ -201,6 +203,75 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
  * "gemv_adj_threads" = threads per CTA of the adjoint matvec (multiple of 32, <= 512; 0 = default).
  * Returns TT_ERR_SHAPE for an unknown key. */
 int tt_debug_set(const char* key, int value);
+
+/* ======================================================================================
+ * Online phase: the data-space solve and the real-time MAP point.
+ *
+ *   G* := Gamma_prior F*  is block Toeplitz with the structure of F* when the prior is time
+ *   invariant: it is the TRANSPOSE-structured operator of the block column
+ *   G_k := F_k Gamma_s (N_d x N_m), i.e. a second tt_plan `G` whose tt_rmatvec applies G*.
+ *   K := Gamma_noise + F G*  (eq 4.7), Gamma_noise diagonal, of order
+ *   n = N_d N_t with the data stacking  row = i*N_d + s whatever the plans' layout;
+ *   K = L L^T is Cholesky-factorised offline and "triangular solves are done in the online phase"
+ *   (PAPER.md:294, 407).  The online inference is eq (4.13) with m_prior = 0:
+ *
+ *        m_map = (I - G* K^{-1} F) G* Gamma_noise^{-1} d_obs .
+ * ====================================================================================== */
+
+typedef struct tt_chol tt_chol;
+
+/* Takes the lower Cholesky factor L of K (K = L L^T) and prepares the two triangular solves.
+ *   n       order of K (>= 1)
+ *   L       n x n doubles, row-major with row pitch ld (>= n) elements, HOST or DEVICE (detected);
+ *           only the lower triangle is read; not retained
+ *   stream  work is enqueued here and the call returns after it has completed
+ * The factor is stored rescaled by the inverses of its 64 x 64 diagonal blocks (strictly lower
+ * blocks packed by block row: n^2/2 doubles) so that neither solve has a diagonal solve on its
+ * dependency chain (see tt_trsv.cu).  TT_ERR_NOT_SPD if a diagonal entry is <= 0 or not finite. */
+int tt_chol_create(tt_chol** out, int64_t n, const void* L, int64_t ld, void* stream);
+void tt_chol_destroy(tt_chol* c);
+size_t tt_chol_device_bytes(const tt_chol* c);
+int tt_chol_last_cuda_error(const tt_chol* c);
+
+/* x = K^{-1} b = L^{-T} (L^{-1} b).  b, x: DEVICE, n doubles; x may alias b.  Asynchronous on
+ * `stream`, no allocation, no host synchronisation.  Calls on one tt_chol must be serialised. */
+int tt_chol_solve(const tt_chol* c, const void* b, void* x, void* stream);
+
+/* One triangular solve: transposed == 0: x = L^{-1} b;  transposed != 0: x = L^{-T} b. */
+int tt_chol_trsv(const tt_chol* c, int transposed, const void* b, void* x, void* stream);
+
+/* K = Gamma_noise + F G*, "column-by-column": columns [col0, col0 + ncols) are
+ * F (G* e_c) + Gamma_noise e_c, pushed through tt_rmatvec_batched(G) and tt_matvec_batched(F) in
+ * groups of min(k_max(F), k_max(G)) unit vectors.
+ *   F, G       plans of identical shape, dtype and layout
+ *   noise_var  DEVICE, N_t*N_d reals of the plans' dtype and layout: the diagonal of Gamma_noise
+ *   K          DEVICE, n x n doubles, row-major, pitch ldk (>= n): entries K[row][c] of the requested
+ *              columns are overwritten for every row; row = i*N_d + s
+ * Offline call: allocates (and frees) its own scratch of N_t*(N_m + N_d)*k reals and synchronises. */
+int tt_assemble_K(const tt_plan* F, const tt_plan* G, const void* noise_var, int64_t col0, int64_t ncols,
+                  void* K, int64_t ldk, void* stream);
+
+typedef struct tt_map tt_map;
+typedef enum tt_map_form {
+    TT_MAP_PAPER = 0,  /* eq (4.13) as written: G*, F, K-solve, G* (footnote 14); by linearity the
+                          final subtraction is done in data space:  m_map = G* (y - K^{-1} F G* y),  y = Gamma_noise^{-1} d_obs */
+    TT_MAP_GAIN = 1    /* the algebraically equal gain form  m_map = G* K^{-1} d_obs  (K - F G* = Gamma_noise):
+                          one G* action and one K-solve; F is not needed */
+} tt_map_form;
+
+/* Binds the operators of the online phase.  F may be NULL (then only TT_MAP_GAIN is available).
+ * noise_var as in tt_assemble_K (read during the call, its reciprocal is kept).  The plans and the
+ * factor are borrowed: they must outlive the tt_map.  Allocates a few data-space vectors. */
+int tt_map_create(tt_map** out, const tt_plan* F, const tt_plan* G, const tt_chol* K, const void* noise_var,
+                  void* stream);
+void tt_map_destroy(tt_map* m);
+
+/* m_map from the observations.  d_obs: DEVICE, N_t*N_d reals; m_map: DEVICE, N_t*N_m reals (plans' dtype
+ * and layout).  Asynchronous on `stream`.  The K-solve runs in fp64 whatever the plans' dtype. */
+int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void* stream);
+
+/* Same with HOST vectors (pinned memory recommended): d_obs is copied in and m_map copied out on `stream`. */
+int tt_map_infer_host(const tt_map* m, int form, const void* d_obs_host, void* m_map_host, void* stream);
 
 #ifdef __cplusplus
 }

@@ -19,6 +19,7 @@ TT_F32, TT_F64 = 0, 1
 TT_TIME_MAJOR, TT_SPACE_MAJOR = 0, 1
 TT_OK = 0
 TT_OP_MATVEC, TT_OP_RMATVEC, TT_OP_NORMAL, TT_OP_MATVEC_BATCHED, TT_OP_RMATVEC_BATCHED = range(5)
+TT_MAP_PAPER, TT_MAP_GAIN = 0, 1
 
 _lib = None
 
@@ -73,6 +74,17 @@ def lib() -> ctypes.CDLL:
         "tt_probe_dmma": (ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]),
         "tt_debug_trig": (ci, [i64, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_set": (ci, [ctypes.c_char_p, ci]),
+        "tt_chol_create": (ci, [pp, i64, vp, i64, vp]),
+        "tt_chol_destroy": (None, [vp]),
+        "tt_chol_device_bytes": (sz, [vp]),
+        "tt_chol_last_cuda_error": (ci, [vp]),
+        "tt_chol_solve": (ci, [vp, vp, vp, vp]),
+        "tt_chol_trsv": (ci, [vp, ci, vp, vp, vp]),
+        "tt_assemble_K": (ci, [vp, vp, vp, i64, i64, vp, i64, vp]),
+        "tt_map_create": (ci, [pp, vp, vp, vp, vp, vp]),
+        "tt_map_destroy": (None, [vp]),
+        "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
+        "tt_map_infer_host": (ci, [vp, ci, vp, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(L, name)
@@ -86,7 +98,9 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy"
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
-           "tt_debug_trig", "tt_debug_set"]
+           "tt_debug_trig", "tt_debug_set",
+           "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
+           "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host"]
 
 
 def _stream(stream) -> int:
@@ -234,6 +248,61 @@ def tt_debug_set(key: str, value: int) -> None:
     _check("tt_debug_set", lib().tt_debug_set(key.encode(), value))
 
 
+def tt_chol_create(n: int, L, ld: int | None = None, stream=None) -> int:
+    """Handle of the prepared factor.  L: [n, n] float64 tensor (cpu or cuda, row-major) or raw pointer."""
+    out = ctypes.c_void_p()
+    st = lib().tt_chol_create(ctypes.byref(out), n, _ptr(L), n if ld is None else ld, _stream(stream))
+    _check("tt_chol_create", st)
+    return out.value
+
+
+def tt_chol_destroy(chol: int) -> None:
+    lib().tt_chol_destroy(chol)
+
+
+def tt_chol_device_bytes(chol: int) -> int:
+    return lib().tt_chol_device_bytes(chol)
+
+
+def tt_chol_last_cuda_error(chol: int) -> int:
+    return lib().tt_chol_last_cuda_error(chol)
+
+
+def _check_chol(call: str, status: int, chol: int):
+    if status != TT_OK:
+        raise TTError(call, status, lib().tt_chol_last_cuda_error(chol))
+
+
+def tt_chol_solve(chol: int, b, x, stream=None) -> None:
+    _check_chol("tt_chol_solve", lib().tt_chol_solve(chol, _ptr(b), _ptr(x), _stream(stream)), chol)
+
+
+def tt_chol_trsv(chol: int, transposed: bool, b, x, stream=None) -> None:
+    _check_chol("tt_chol_trsv", lib().tt_chol_trsv(chol, int(bool(transposed)), _ptr(b), _ptr(x), _stream(stream)), chol)
+
+
+def tt_assemble_K(F: int, G: int, noise_var, col0: int, ncols: int, K, ldk: int, stream=None) -> None:
+    _check("tt_assemble_K", lib().tt_assemble_K(F, G, _ptr(noise_var), col0, ncols, _ptr(K), ldk, _stream(stream)), F)
+
+
+def tt_map_create(F: int | None, G: int, chol: int, noise_var, stream=None) -> int:
+    out = ctypes.c_void_p()
+    _check("tt_map_create", lib().tt_map_create(ctypes.byref(out), F, G, chol, _ptr(noise_var), _stream(stream)))
+    return out.value
+
+
+def tt_map_destroy(m: int) -> None:
+    lib().tt_map_destroy(m)
+
+
+def tt_map_infer(m: int, form: int, d_obs, m_map, stream=None) -> None:
+    _check("tt_map_infer", lib().tt_map_infer(m, form, _ptr(d_obs), _ptr(m_map), _stream(stream)))
+
+
+def tt_map_infer_host(m: int, form: int, d_obs_host, m_map_host, stream=None) -> None:
+    _check("tt_map_infer_host", lib().tt_map_infer_host(m, form, _ptr(d_obs_host), _ptr(m_map_host), _stream(stream)))
+
+
 _DT = {torch.float32: TT_F32, torch.float64: TT_F64}
 
 
@@ -306,3 +375,65 @@ class Plan:
     @property
     def device_bytes(self) -> int:
         return tt_plan_device_bytes(self.handle)
+
+
+class Chol:
+    """RAII convenience over tt_chol_*: the two triangular solves with the Cholesky factor of K."""
+
+    def __init__(self, L: torch.Tensor, stream=None):
+        assert L.dim() == 2 and L.shape[0] == L.shape[1] and L.dtype == torch.float64 and L.stride(1) == 1
+        self.n = L.shape[0]
+        self.handle = tt_chol_create(self.n, L, L.stride(0), stream)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            torch.cuda.synchronize()
+            tt_chol_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def solve(self, b, out=None, stream=None):
+        out = torch.empty(self.n, dtype=torch.float64, device="cuda") if out is None else out
+        tt_chol_solve(self.handle, b, out, stream)
+        return out
+
+    def trsv(self, b, transposed=False, out=None, stream=None):
+        out = torch.empty(self.n, dtype=torch.float64, device="cuda") if out is None else out
+        tt_chol_trsv(self.handle, transposed, b, out, stream)
+        return out
+
+    @property
+    def device_bytes(self) -> int:
+        return tt_chol_device_bytes(self.handle)
+
+
+def assemble_K(F: Plan, G: Plan, noise_var: torch.Tensor, cols: tuple[int, int] | None = None,
+               out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """K = Gamma_noise + F G* as an [n, n] float64 CUDA tensor (columns `cols` = (col0, ncols) only, if given)."""
+    n = F.N_d * F.N_t
+    K = torch.zeros((n, n), dtype=torch.float64, device="cuda") if out is None else out
+    col0, ncols = cols if cols is not None else (0, n)
+    tt_assemble_K(F.handle, G.handle, noise_var, col0, ncols, K, K.stride(0), stream)
+    return K
+
+
+class MapInference:
+    """RAII convenience over tt_map_*: the online MAP point of eq (4.13)."""
+
+    def __init__(self, F: Plan | None, G: Plan, chol: Chol, noise_var: torch.Tensor, stream=None):
+        self.F, self.G, self.chol = F, G, chol          # keep the borrowed objects alive
+        self.handle = tt_map_create(F.handle if F is not None else None, G.handle, chol.handle, noise_var, stream)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            torch.cuda.synchronize()
+            tt_map_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def infer(self, d_obs, form: int = TT_MAP_PAPER, out=None, stream=None):
+        out = self.G._out(self.G.N_m) if out is None else out
+        tt_map_infer(self.handle, form, d_obs, out, stream)
+        return out

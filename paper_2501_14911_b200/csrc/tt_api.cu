@@ -54,6 +54,10 @@ struct tt_plan {
     mutable long long n_calls = 0;  // profiled apply calls so far
 };
 
+namespace tt {
+PlanInfo plan_info(const ::tt_plan* p) { return PlanInfo{p->N_d, p->N_m, p->N_t, p->dtype, p->layout, p->k_max}; }
+}  // namespace tt
+
 namespace {
 
 int fail_cuda(const tt_plan* p, cudaError_t e) {
@@ -369,6 +373,8 @@ const char* tt_status_string(int status) {
         case TT_ERR_OOM: return "TT_ERR_OOM";
         case TT_ERR_CUDA: return "TT_ERR_CUDA";
         case TT_ERR_NO_DEVICE: return "TT_ERR_NO_DEVICE";
+        case TT_ERR_NOT_SPD: return "TT_ERR_NOT_SPD";
+        case TT_ERR_MISMATCH: return "TT_ERR_MISMATCH";
         default: return "TT_ERR_UNKNOWN";
     }
 }

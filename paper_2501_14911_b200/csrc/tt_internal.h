@@ -4,7 +4,16 @@
 #include <stddef.h>
 #include <stdint.h>
 
+struct tt_plan;
+
 namespace tt {
+
+// What the online-phase calls (tt_online.cu) need to know about a plan.
+struct PlanInfo {
+    long long N_d, N_m, N_t;
+    int dtype, layout, k_max;
+};
+PlanInfo plan_info(const ::tt_plan* p);
 
 constexpr int kMaxStages = 16;
 constexpr int kMaxSmem = 232448;  // 227 KB: largest dynamic shared memory per CTA on sm_100
@@ -81,6 +90,28 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
                             cudaStream_t s);
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s);
+
+// Triangular solves with the rescaled Cholesky factor (tt_trsv.cu).
+constexpr int kTrsvNB = 64;  // block order
+struct TrsvGeom {
+    long long n;       // order of K
+    int nblk;          // ceil(n / kTrsvNB)
+    const double* Lt;  // packed strictly-lower blocks of D^{-1} L: block row I at NB*NB*I*(I-1)/2, pitch I*NB
+    const double* Dinv;  // [nblk][NB][NB] inverses of the diagonal blocks (identity on the padding)
+    double* bt;        // [nblk*NB] D^{-1} b
+    double* y;         // [nblk*NB] forward solution (self-flagging)
+    double* xt;        // [nblk*NB] backward solution before the D^{-T} post-step (self-flagging)
+    unsigned* ticket;  // [2] block tickets of the forward / backward chain
+};
+// Plan time: D_I^{-1} and Lt for the block rows of the slab src = rows [row0, row0 + nrows) of the row-major
+// factor (pitch ld), row0 a multiple of kTrsvNB; *bad is set to 1 if a diagonal entry is not positive and finite.
+cudaError_t trsv_prepare_launch(const double* src, long long ld, long long row0, long long nrows, long long n,
+                                double* Dinv, double* Lt, int* bad, cudaStream_t s);
+cudaError_t trsv_pre_launch(const TrsvGeom& g, const double* b, cudaStream_t s);   // bt = D^{-1} b (b may be null), resets
+cudaError_t trsv_fwd_launch(const TrsvGeom& g, cudaStream_t s);                    // y = Lt^{-1} bt
+cudaError_t trsv_bwd_launch(const TrsvGeom& g, const double* yin, cudaStream_t s); // xt = Lt^{-T} yin
+cudaError_t trsv_post_launch(const TrsvGeom& g, double* x, cudaStream_t s);        // x = D^{-T} xt
+cudaError_t trsv_copy_launch(const double* src, double* dst, long long n, cudaStream_t s);
 
 // sink: >= 148*8*256 doubles
 cudaError_t probe_dmma_launch(int iters, void* sink, double* flops, cudaStream_t s);

@@ -100,7 +100,12 @@ CONFIGS = {
     "C3": Workload("C3-paper-scale-c64", 100, 250000, 400, torch.float32, 2, 100.0, bump=True),
     "C4": Workload("C4-krhs-fp64", 64, 65536, 512, torch.float64, 3, 64.0, k_rhs=32),
     "C5": Workload("C5-normal-c64", 200, 100000, 400, torch.float32, 4, 100.0),
+    # the paper's own test configuration: 7x7 sensors, 513x513 parameters, 500 steps,
+    # 131 584 500 parameters, 24 500 data - the workload of the online phase (eq 4.13)
+    "P5": Workload("P5-paper-sec5-online-c64", 49, 263169, 500, torch.float32, 5, 100.0, sensor_scale=True),
 }
+
+NOISE_LEVEL = 0.05   # relative noise of the online workload (the paper uses 2-6 %)
 
 
 def _sensor_scale(w: Workload, s: torch.Tensor) -> torch.Tensor:
@@ -170,3 +175,36 @@ def vector_m(w: Workload, device="cpu", k_rhs: int | None = None) -> torch.Tenso
 def vector_d(w: Workload, device="cpu", k_rhs: int | None = None) -> torch.Tensor:
     """Data vector, time-major [i][s], or [i][s][r] for k RHS."""
     return _vector(w, TENSOR_D, w.N_t, w.N_d, device, w.k_rhs if k_rhs is None else k_rhs)
+
+
+# ---------------------------------------------------------------------------------------------
+# Inputs of the online phase (eq 4.13): stand-ins for what Phases 1-2 of the paper would deliver.
+# ---------------------------------------------------------------------------------------------
+def prior_gamma(w: Workload, device="cpu") -> torch.Tensor:
+    """Diagonal of a time-invariant spatial prior covariance Gamma_s (fp64, [N_m]), smooth and positive:
+    gamma_p = 0.5 + exp(-((p - N_m/2) / (N_m/4))^2).  Stands in for the paper's elliptic-operator prior
+    (eq 5.1), which needs a sparse solver; only 'time-invariant, block diagonal in time' matters here
+    (PAPER.md:368), because that is what makes G* block Toeplitz."""
+    p = torch.arange(w.N_m, device=device, dtype=torch.float64)
+    return 0.5 + torch.exp(-((p - 0.5 * w.N_m) / (0.25 * w.N_m)) ** 2)
+
+
+def gstar_block_column(w: Workload, F: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+    """Block column G_k = F_k Gamma_s of G* = Gamma_prior F* for the diagonal prior above,
+    formed in fp64 and rounded once to w.dtype.  Harness code: in the paper this is the output of N_d prior
+    solves (Phase 2), an input of the online phase.  Works plane by plane to bound scratch memory."""
+    g = prior_gamma(w, F.device)
+    out = torch.empty_like(F) if out is None else out
+    for k in range(F.shape[0]):
+        out[k] = (F[k].to(torch.float64) * g[None, : F.shape[2]]).to(w.dtype)
+    return out
+
+
+def noise_var(w: Workload, device="cpu") -> torch.Tensor:
+    """Diagonal of Gamma_noise, [N_t, N_d] in w.dtype: per sensor, constant in time (the paper adds noise
+    per sensor relative to that sensor's signal):  (NOISE_LEVEL)^2 * v_s  with
+    v_s = c_s^2 N_m tau / 2, the scale of Var(d_i[s]) for m ~ N(0, I) under the F recipe."""
+    s = torch.arange(w.N_d, device=device, dtype=torch.int64)
+    c = _sensor_scale(w, s) if w.sensor_scale else torch.ones(w.N_d, dtype=torch.float64, device=device)
+    v = (NOISE_LEVEL ** 2) * c * c * (w.N_m * w.tau * 0.5)
+    return v[None, :].expand(w.N_t, w.N_d).contiguous().to(w.dtype)

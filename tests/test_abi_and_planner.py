@@ -21,7 +21,7 @@ def tt():
 def declared_symbols():
     with open(os.path.join(ROOT, "include", "tt.h")) as f:
         src = re.sub(r"/\*.*?\*/", "", f.read(), flags=re.S)
-    return sorted(set(re.findall(r"\b(tt_[a-z_0-9]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(tt_[A-Za-z_0-9]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol(tt):

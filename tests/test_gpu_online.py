@@ -1,0 +1,202 @@
+"""GPU parity for the online phase: the triangular solves with the Cholesky
+factor of K, the assembly of K = Gamma_noise + F G* and the MAP point of eq (4.13), called through the
+C ABI and compared with oracle/online_plain.py on the same seeded inputs.
+
+Tolerances (relative L2 over the whole output; DESIGN.md section 11 derives them):
+  * triangular solves, fp64: 1e-12 on factors whose diagonal blocks are well conditioned;
+  * K: 1e-12 (fp64 plans) / 1e-5 (fp32 plans) relative to ||K||_F  (n matvec pairs, the matvec bar);
+  * m_map with the ORACLE's factor L uploaded (so that only the online arithmetic is compared):
+      gain form  G* K^{-1} d_obs            : matvec bar (1e-12 / 1e-5) + 8 u64 kappa(K) for the fp64 solve;
+      paper form (I - G* K^{-1} F) G* y     : rounding of a = G* y and b = F a is amplified by the solve,
+                                              bound  8 u kappa(K)  with u the unit roundoff of the plan dtype.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import online_plain as oo
+from oracle import toeplitz_plain as op
+from paper_2501_14911_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+U = {torch.float64: 1.1e-16, torch.float32: 6.0e-8}
+BAR = {torch.float64: 1e-12, torch.float32: 1e-5}
+
+
+@pytest.fixture(scope="module")
+def tt():
+    from paper_2501_14911_b200 import binding
+    binding.lib()
+    return binding
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    nb = np.linalg.norm(b)
+    return np.linalg.norm(a - b) / (nb if nb > 0 else 1.0)
+
+
+def random_factor(n, seed):
+    """A lower-triangular matrix with the profile of a Cholesky factor: positive diagonal, decaying off-diagonal."""
+    rng = np.random.default_rng(seed)
+    L = np.tril(rng.standard_normal((n, n))) / np.sqrt(max(n, 1))
+    L[np.arange(n), np.arange(n)] = rng.uniform(1.0, 2.0, n)
+    return L
+
+
+# ---------------------------------------------------------------------------- triangular solves
+@pytest.mark.parametrize("n", [1, 2, 63, 64, 65, 130, 200, 1000, 4097])
+@pytest.mark.parametrize("where", ["device", "host"])
+def test_trsv_and_solve(tt, n, where):
+    L = random_factor(n, n)
+    b = np.random.default_rng(n + 1).standard_normal(n)
+    Lt = torch.from_numpy(L)
+    # garbage in the upper triangle must be ignored
+    Lt = Lt + torch.triu(torch.full((n, n), 7.0, dtype=torch.float64), diagonal=1)
+    chol = tt.Chol(Lt.cuda() if where == "device" else Lt)
+    try:
+        bd = torch.from_numpy(b).cuda()
+        y = chol.trsv(bd).cpu().numpy()
+        x = chol.trsv(bd, transposed=True).cpu().numpy()
+        z = chol.solve(bd).cpu().numpy()
+        z2 = chol.solve(bd).cpu().numpy()
+    finally:
+        chol.close()
+    assert rel(y, oo.forward_substitution(L, b)) <= 1e-12
+    assert rel(x, oo.back_substitution_T(L, b)) <= 1e-12
+    assert rel(z, oo.chol_solve(L, b)) <= 1e-12
+    assert np.array_equal(z, z2)            # fixed summation order: bit-reproducible
+
+
+def test_trsv_pitch_alias_and_errors(tt):
+    n = 150
+    L = random_factor(n, 5)
+    big = torch.zeros((n, n + 9), dtype=torch.float64)
+    big[:, :n] = torch.from_numpy(L)
+    chol = tt.Chol(big.cuda()[:, :n])                      # row pitch n + 9
+    try:
+        b = torch.from_numpy(np.random.default_rng(1).standard_normal(n)).cuda()
+        ref = oo.chol_solve(L, b.cpu().numpy())
+        x = b.clone()
+        tt.tt_chol_solve(chol.handle, x, x)                # in place
+        assert rel(x.cpu().numpy(), ref) <= 1e-12
+        assert chol.device_bytes >= 8 * n * n // 2
+    finally:
+        chol.close()
+    bad = torch.from_numpy(L.copy())
+    bad[77, 77] = 0.0
+    with pytest.raises(tt.TTError) as ei:
+        tt.Chol(bad.cuda())
+    assert ei.value.status == -11                           # TT_ERR_NOT_SPD
+    bad[77, 77] = float("nan")
+    with pytest.raises(tt.TTError):
+        tt.Chol(bad)
+    with pytest.raises(tt.TTError):
+        tt.tt_chol_create(0, torch.zeros(1, dtype=torch.float64).cuda())
+
+
+def test_trsv_nan_rhs_terminates(tt):
+    # a NaN right-hand side must flow through (and not be mistaken for the 'not yet computed' pattern)
+    n = 300
+    chol = tt.Chol(torch.from_numpy(random_factor(n, 9)).cuda())
+    try:
+        b = torch.zeros(n, dtype=torch.float64)
+        b[5] = float("nan")
+        sentinel = np.array([0x7FF4A5A5DEADBEEF], dtype=np.uint64).view(np.float64)[0]
+        b[70] = float(sentinel)
+        x = chol.solve(b.cuda())
+        torch.cuda.synchronize()
+        assert torch.isnan(x).any()
+    finally:
+        chol.close()
+
+
+# ---------------------------------------------------------------------------- K and the MAP point
+def online_inputs(N_d, N_m, N_t, dtype):
+    w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
+    F = synth.block_column(w)
+    G = synth.gstar_block_column(w, F)
+    nv = synth.noise_var(w)
+    d_obs = synth.vector_d(w, k_rhs=1)
+    return w, F, G, nv, d_obs
+
+
+ONLINE_SHAPES = [(3, 40, 12), (6, 400, 50), (5, 1000, 35), (1, 64, 20), (4, 2100, 16)]
+
+
+@pytest.mark.parametrize("N_d,N_m,N_t", ONLINE_SHAPES)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("k_max", [1, 8])
+def test_assemble_K(tt, N_d, N_m, N_t, dtype, k_max):
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    K_ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
+    pF, pG = tt.Plan(F.cuda(), k_max=k_max), tt.Plan(G.cuda(), k_max=k_max)
+    try:
+        K = tt.assemble_K(pF, pG, nv.cuda()).cpu().numpy()
+        n = N_d * N_t
+        part = torch.full((n, n + 3), -1.0, dtype=torch.float64, device="cuda")      # a column range, pitched output
+        c0, nc = n // 3, min(n - n // 3, 11)
+        tt.tt_assemble_K(pF.handle, pG.handle, nv.cuda(), c0, nc, part, n + 3)
+        part = part.cpu().numpy()
+    finally:
+        pF.close(); pG.close()
+    assert rel(K, K_ref) <= BAR[dtype]
+    assert rel(K, K.T) <= 2 * BAR[dtype]
+    assert rel(part[:, c0:c0 + nc], K_ref[:, c0:c0 + nc]) <= BAR[dtype]
+    assert (part[:, :c0] == -1.0).all() and (part[:, c0 + nc:] == -1.0).all()
+
+
+@pytest.mark.parametrize("N_d,N_m,N_t", ONLINE_SHAPES)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_map_point(tt, N_d, N_m, N_t, dtype, layout):
+    w, F, G, nv, d_obs = online_inputs(N_d, N_m, N_t, dtype)
+    Fn, Gn, nvn, dn = F.numpy(), G.numpy(), nv.numpy(), d_obs.numpy()
+    K = oo.assemble_K(Fn, Gn, nvn)
+    L = oo.cholesky(K)
+    m_ref = oo.map_point(Fn, Gn, nvn, L, dn)
+    ev = np.linalg.eigvalsh(K)
+    kappa = ev[-1] / ev[0]
+    pF, pG = tt.Plan(F.cuda(), layout=layout), tt.Plan(G.cuda(), layout=layout)
+    chol = tt.Chol(torch.from_numpy(L).cuda())
+    lay = (lambda t: t.t().contiguous()) if layout == 1 else (lambda t: t)
+    unlay = (lambda t: t.t()) if layout == 1 else (lambda t: t)
+    mp = tt.MapInference(pF, pG, chol, lay(nv).cuda())
+    try:
+        m_paper = unlay(mp.infer(lay(d_obs).cuda(), tt.TT_MAP_PAPER)).cpu().numpy()
+        m_gain = unlay(mp.infer(lay(d_obs).cuda(), tt.TT_MAP_GAIN)).cpu().numpy()
+        mg = tt.MapInference(None, pG, chol, lay(nv).cuda())       # gain form needs no F
+        m_gain2 = unlay(mg.infer(lay(d_obs).cuda(), tt.TT_MAP_GAIN)).cpu().numpy()
+        with pytest.raises(tt.TTError):
+            mg.infer(lay(d_obs).cuda(), tt.TT_MAP_PAPER)
+        mg.close()
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close()
+    e_gain, e_paper = rel(m_gain, m_ref), rel(m_paper, m_ref)
+    print(f"map {N_d}x{N_m}x{N_t} {dtype} layout {layout}: kappa(K) {kappa:.1f}  gain {e_gain:.2e}  paper {e_paper:.2e}")
+    assert e_gain <= BAR[dtype] + 8 * U[torch.float64] * kappa
+    assert e_paper <= 8 * U[dtype] * kappa + BAR[dtype]
+    assert np.array_equal(m_gain, m_gain2)
+    # the MAP point solves eq (2.12): F* Gn^{-1} (d - F m) = Gamma_prior^{-1} m, checked through the oracle operators
+    g = synth.prior_gamma(w).numpy()
+    lhs = op.rmatvec(Fn, (dn - op.matvec(Fn, m_gain)) / nvn)
+    assert rel(lhs, m_gain / g[None, :]) <= 1e3 * (BAR[dtype] + 8 * U[dtype] * kappa)
+
+
+def test_map_mismatch_errors(tt):
+    w, F, G, nv, d_obs = online_inputs(3, 40, 12, torch.float64)
+    pF, pG = tt.Plan(F.cuda()), tt.Plan(G[:, :2].contiguous().cuda())
+    chol = tt.Chol(torch.eye(7, dtype=torch.float64).cuda())
+    try:
+        with pytest.raises(tt.TTError) as ei:
+            tt.MapInference(pF, pG, chol, nv.cuda())
+        assert ei.value.status == -12                       # TT_ERR_MISMATCH (plans)
+        with pytest.raises(tt.TTError) as ei:
+            tt.MapInference(None, pF, chol, nv.cuda())
+        assert ei.value.status == -12                       # factor order != N_d N_t
+        with pytest.raises(tt.TTError):
+            tt.assemble_K(pF, pG, nv.cuda())
+    finally:
+        chol.close(); pF.close(); pG.close()
