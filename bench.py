@@ -176,6 +176,162 @@ def config_dict(w, args):
             "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
 
 
+ONLINE_METRIC = "ms per online MAP inference, eq (4.13): m_map from d_obs (G*, F, K-solve, G*)"
+
+
+def run_online(args, w):
+    """--online: the online phase at the paper's own shape (P5: PAPER.md:370-381).
+
+    Inputs of the online phase, all resident in HBM before the timed region: the spectra of F and of
+    G* = Gamma_prior F* (synthetic block columns, synth.py), diag(Gamma_noise), and a Cholesky factor of the order
+    of K (n = N_d N_t).  The factor is a seeded stand-in (synth.factor_standin): assembling the true K takes n
+    matvec pairs; `--k-cols` columns of it ARE assembled with tt_assemble_K and timed.
+    A step = one tt_map_infer in the paper's form (G*, F, two triangular solves, G*).
+    """
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    from paper_2501_14911_b200 import binding as tt
+    tt.lib()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    es = 4 if w.dtype == torch.float32 else 8
+    n = w.N_d * w.N_t
+    kb = max(1, args.k_batch)
+    t0 = time.perf_counter()
+    F = synth.block_column(w, device=dev)
+    pF = tt.Plan(F, k_max=kb)
+    synth.gstar_block_column(w, F, out=F)            # in place: F now holds the block column of G*
+    pG = tt.Plan(F, k_max=kb)
+    F_s = None
+    if not args.no_cpu_baseline:
+        F_s = F[:, : min(w.N_d, 4), : min(w.N_m, SAMPLE_PARAMS)].contiguous().cpu().numpy()   # sample of G for the CPU leg
+    del F
+    torch.cuda.empty_cache()
+    nv = synth.noise_var(w, device=dev)
+    d_obs = synth.vector_d(w, device=dev, k_rhs=1)
+    L = synth.factor_standin(n, w.seed, device=dev)
+    chol = tt.Chol(L)
+    L_h = L.cpu().numpy() if not args.no_cpu_baseline else None
+    del L
+    torch.cuda.empty_cache()
+    mp = tt.MapInference(pF, pG, chol, nv)
+    torch.cuda.synchronize()
+    t_setup = time.perf_counter() - t0
+
+    stream = torch.cuda.Stream(device=dev)
+    m_map = torch.empty((w.N_t, w.N_m), dtype=w.dtype, device=dev)
+    b64 = torch.randn(n, dtype=torch.float64, device=dev)
+    x64 = torch.empty_like(b64)
+
+    def time_op(fn, k):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(stream)
+        for _ in range(k):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / k
+
+    paper = lambda: tt.tt_map_infer(mp.handle, tt.TT_MAP_PAPER, d_obs, m_map, stream)
+    gain = lambda: tt.tt_map_infer(mp.handle, tt.TT_MAP_GAIN, d_obs, m_map, stream)
+    for _ in range(args.warmup):
+        paper(); gain()
+    with ClockSampler(0) as clocks:
+        ms_paper = time_op(paper, args.steps)
+    ms_gain = time_op(gain, args.steps)
+    ms_solve = time_op(lambda: tt.tt_chol_solve(chol.handle, b64, x64, stream), 4 * args.steps)
+    ms_fwd = time_op(lambda: tt.tt_chol_trsv(chol.handle, False, b64, x64, stream), 4 * args.steps)
+    ms_bwd = time_op(lambda: tt.tt_chol_trsv(chol.handle, True, b64, x64, stream), 4 * args.steps)
+    m_tmp = torch.empty_like(m_map)
+    d_tmp = torch.empty_like(d_obs)
+    ms_G = time_op(lambda: tt.tt_rmatvec(pG.handle, d_obs, m_tmp, stream), args.steps)
+    ms_F = time_op(lambda: tt.tt_matvec(pF.handle, m_tmp, d_tmp, stream), args.steps)
+    del m_tmp
+
+    # end to end with HOST vectors: d_obs in (98 KB), m_map out (526 MB)
+    d_h = d_obs.cpu().pin_memory()
+    m_h = torch.empty((w.N_t, w.N_m), dtype=w.dtype).pin_memory()
+    tt.tt_map_infer_host(mp.handle, tt.TT_MAP_PAPER, d_h, m_h, stream)
+    stream.synchronize()
+    n_e2e = max(2, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        tt.tt_map_infer_host(mp.handle, tt.TT_MAP_PAPER, d_h, m_h, stream)
+    stream.synchronize()
+    ms_e2e = (time.perf_counter() - t0) * 1e3 / n_e2e
+
+    # K assembly: a bounded number of columns, extrapolated like the paper does (n x time per column, PAPER.md:407)
+    kcols = min(n, args.k_cols)
+    c0 = min(n // 2, n - kcols)
+    Kbuf = torch.zeros((n, n), dtype=torch.float64, device=dev)
+    t0 = time.perf_counter()
+    tt.tt_assemble_K(pF.handle, pG.handle, nv, c0, kcols, Kbuf, n, stream)
+    torch.cuda.synchronize()
+    s_cols = time.perf_counter() - t0
+    Kd = Kbuf[c0:c0 + kcols, c0:c0 + kcols]
+    sym = float((Kd - Kd.t()).abs().max() / Kd.abs().max())      # K is symmetric: its diagonal block must be
+    del Kbuf, Kd
+
+    peaks, peak_kind = measured_peaks()
+    peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
+    lt_bytes = 64 * 64 * 8 * ((n + 63) // 64) * ((n + 63) // 64 - 1) // 2
+    n_f, ldp = w.N_t + 1, (w.N_m + 15) // 16 * 16
+    fhat_bytes = n_f * w.N_d * ldp * 2 * es
+    vec = w.N_t * w.N_m * es
+    out = {
+        "metric": ONLINE_METRIC, "value": ms_paper, "unit": "ms", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_paper, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 matvecs / f64 K-solve" if w.dtype == torch.float32 else "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name}: N_d={w.N_d}, N_m={w.N_m}, N_t={w.N_t} ({w.n_params:.4g} parameters, "
+                               f"{n} data), online phase of PAPER.md:343-350",
+                   "step": "tt_map_infer TT_MAP_PAPER: y = Gn^-1 d, a = G* y, b = F a, c = K^-1 b (two triangular solves), "
+                           "m_map = G* (y - c)",
+                   "factor": "seeded stand-in of order n (synth.factor_standin); timing is value independent",
+                   "l2": "inputs larger than L2 (two 52 GB spectra + 2.4 GB factor streamed per step)"},
+        "e2e": {"value": ms_e2e, "unit": "ms", "h2d_bytes_per_step": n * es, "d2h_bytes_per_step": w.N_t * w.N_m * es,
+                "steps": n_e2e, "api": "tt_map_infer_host, pinned host vectors"},
+        "gpu_launches": (3 * 3 + 1 + 4 + 3) * args.steps,   # 2 x G* (3 each), F (4), 4 solve kernels, 3 element-wise
+        "clocks": clocks.summary(),
+        "roofline": {"bound": "hbm", "kernel": "trsv_fwd_kernel + trsv_bwd_kernel (the two triangular solves of the K-solve)",
+                     "achieved": 2 * lt_bytes / (ms_solve * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": 2 * lt_bytes / (ms_solve * 1e-3) / 1e9 / peak, "traffic": None,
+                     "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
+                     "algorithmic_bytes_per_solve": 2 * lt_bytes, "ms_per_solve": ms_solve,
+                     "forward_ms": ms_fwd, "backward_ms": ms_bwd, "chain_steps": (n + 63) // 64,
+                     "note": "latency chain of n/64 block steps on top of the stream; see DESIGN.md section 11"},
+        "ops": {"map_paper_form_ms": ms_paper, "map_gain_form_ms": ms_gain, "Gstar_ms": ms_G, "F_ms": ms_F,
+                "K_solve_ms": ms_solve,
+                "paper_form_GBs": (3 * (fhat_bytes + vec) + 2 * lt_bytes) / (ms_paper * 1e-3) / 1e9,
+                "gain_form_GBs": (fhat_bytes + vec + 2 * lt_bytes) / (ms_gain * 1e-3) / 1e9,
+                "paper_timing_context": "PAPER.md:436-438: ~53 ms on 24 A100 (11 ms per G*/F, 20 ms K-solve)"},
+        "K_assembly": {"columns_timed": kcols, "k_batch": kb, "s_per_column": s_cols / kcols,
+                       "extrapolated_total_s": s_cols / kcols * n, "symmetry_defect_of_the_diagonal_block": sym,
+                       "paper_timing_context": "PAPER.md:407: 24 500 x 0.022 s ~ 9 min on 24 A100"},
+        "setup": {"seconds": t_setup, "plan_bytes": pF.device_bytes + pG.device_bytes, "chol_bytes": chol.device_bytes},
+    }
+    if not args.no_cpu_baseline:
+        from oracle import online_plain as oo
+        from oracle import toeplitz_blocked as ob
+        ob.build()
+        d_np = d_obs.cpu().numpy()
+        t0 = time.perf_counter(); z = oo.chol_solve(L_h, d_np.reshape(n).astype("float64")); t_solve = time.perf_counter() - t0
+        ns, npar = F_s.shape[1], F_s.shape[2]
+        zz = z.reshape(w.N_t, w.N_d)[:, :ns].copy()
+        ob.rmatvec(F_s, zz)
+        t0 = time.perf_counter(); ob.rmatvec(F_s, zz); t_g = time.perf_counter() - t0
+        scale = (w.N_d * w.N_m) / float(ns * npar)
+        out["cpu_baseline"] = {
+            "value": (t_solve + 3 * t_g * scale) * 1e3, "unit": "ms", "cores": ob.num_threads(), "kind": "oracle",
+            "sample": (f"oracle/online_plain.chol_solve at full order n={n} ({t_solve:.2f} s, numpy substitution loops) + 3 x "
+                       f"oracle/toeplitz_blocked block convolution timed on {ns} sensors x {npar} parameters x {w.N_t} steps "
+                       f"({t_g:.2f} s), scaled by {scale:.1f}"),
+            "note": "reported baseline, not the optimisation target"}
+    mp.close(); chol.close(); pF.close(); pG.close()
+    print(json.dumps(out))
+    return 0
+
+
 def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,6 +342,11 @@ def main() -> int:
     ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
                     help="N>1: independent replicas (default, the north star's one-GPU path) or the parameter axis "
                          "sharded over the ranks with one all-reduce of d per F.m (paper_2501_14911_b200/sharded.py)")
+    ap.add_argument("--online", action="store_true",
+                    help="time the online phase (eq 4.13 MAP inference, K-solve, K assembly) instead of the matvec pair; "
+                         "meant for --config P5, the paper's own shape")
+    ap.add_argument("--k-cols", type=int, default=64, help="--online: columns of K assembled and timed")
+    ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-library-baseline", action="store_true")
     args = ap.parse_args()
@@ -193,6 +354,8 @@ def main() -> int:
     w = synth.CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, w)
+    if args.online:
+        return run_online(args, w)
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

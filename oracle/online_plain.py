@@ -107,19 +107,22 @@ def chol_solve(L, b) -> np.ndarray:
     return back_substitution_T(L, forward_substitution(L, b))
 
 
-def map_point(F, G, noise_var, L, d_obs) -> np.ndarray:
+def map_point(F, G, noise_var, L, d_obs, conv=tp) -> np.ndarray:
     """m_map of eq (4.13) with m_prior = 0, in the paper's order of operations
     (footnote 14: G*, F, solve with the prefactorised K, G*):
 
         y = Gamma_noise^{-1} d_obs ;  a = G* y ;  b = F a ;  c = K^{-1} b ;  m_map = a - G* c.
+
+    conv: the oracle module that supplies the block convolution (toeplitz_plain, or toeplitz_blocked - the same
+    sums in C/OpenMP - for sizes where the numpy loops are too slow).
     """
-    F, G, nv, d = _f64(F), _f64(G), _f64(noise_var), _f64(d_obs)
-    N_t, N_d, _ = F.shape
+    nv, d = _f64(noise_var), _f64(d_obs)
+    N_t, N_d = F.shape[0], F.shape[1]
     y = d / nv
-    a = apply_gstar(G, y)
-    b = tp.matvec(F, a)
+    a = conv.rmatvec(G, y)                                   # G* y
+    b = conv.matvec(F, a)
     c = chol_solve(L, b.reshape(N_t * N_d)).reshape(N_t, N_d)
-    return a - apply_gstar(G, c)
+    return a - conv.rmatvec(G, c)
 
 
 def post_cov_apply(F, G, L, Gamma_s, v) -> np.ndarray:

@@ -722,6 +722,7 @@ int tt_debug_set(const char* key, int value) {
     }
     if (!std::strcmp(key, "fft_max_radix")) { g_fft_max_radix = value; return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
+    if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_fwd_warps")) {
         if (value < 0 || value > 32) return TT_ERR_SHAPE;
         gemv_debug_set(value, -1);

@@ -96,7 +96,7 @@ constexpr int kTrsvNB = 64;  // block order
 struct TrsvGeom {
     long long n;       // order of K
     int nblk;          // ceil(n / kTrsvNB)
-    const double* Lt;  // packed strictly-lower blocks of D^{-1} L: block row I at NB*NB*I*(I-1)/2, pitch I*NB
+    const double* Lt;  // strictly-lower blocks of D^{-1} L, block (I,J) contiguous at NB*NB*(I*(I-1)/2 + J)
     const double* Dinv;  // [nblk][NB][NB] inverses of the diagonal blocks (identity on the padding)
     double* bt;        // [nblk*NB] D^{-1} b
     double* y;         // [nblk*NB] forward solution (self-flagging)
@@ -111,6 +111,7 @@ cudaError_t trsv_pre_launch(const TrsvGeom& g, const double* b, cudaStream_t s);
 cudaError_t trsv_fwd_launch(const TrsvGeom& g, cudaStream_t s);                    // y = Lt^{-1} bt
 cudaError_t trsv_bwd_launch(const TrsvGeom& g, const double* yin, cudaStream_t s); // xt = Lt^{-T} yin
 cudaError_t trsv_post_launch(const TrsvGeom& g, double* x, cudaStream_t s);        // x = D^{-T} xt
+void trsv_debug_set_U(int U);  // blocks in flight per warp: 1, 2 (default), 3
 cudaError_t trsv_copy_launch(const double* src, double* dst, long long n, cudaStream_t s);
 
 // sink: >= 148*8*256 doubles

@@ -14,8 +14,9 @@
 //     and the chain of either solve is a pure block recurrence with NO diagonal solve on it:
 //          forward   y_I  = bt_I - sum_{J<I} Lt_IJ   y_J          (bt = D^{-1} b, fully parallel pre-step)
 //          backward  xt_I = y_I  - sum_{J>I} Lt_JI^T xt_J         (x  = D^{-T} xt, fully parallel post-step)
-//     Only the strictly lower blocks of Lt are stored, packed by block row (half the memory of the
-//     square factor), plus the NB x NB inverses D_I^{-1}.
+//     Only the strictly lower blocks of Lt are stored (half the memory of the square factor), each
+//     64 x 64 block contiguous (32 KB) and the blocks of one block row one after the other, so that
+//     every CTA of the forward solve reads ONE sequential stream; plus the NB x NB inverses D_I^{-1}.
 //   * One CTA per block row (forward) / block column (backward).  A CTA takes its block index from an
 //     atomic ticket, so a CTA only ever waits for blocks owned by CTAs that have already started:
 //     no co-residency assumption, no deadlock.
@@ -37,7 +38,6 @@ namespace {
 constexpr int NB = kTrsvNB;     // block order
 constexpr int RW = 8;           // rows per warp
 constexpr int NTHREADS = (NB / RW) * 32;
-constexpr int U = 2;            // blocks of Lt in flight per warp
 constexpr unsigned long long kSentinel = 0x7FF4A5A5DEADBEEFULL;  // signalling-NaN payload: "not yet computed"
 
 __device__ __forceinline__ bool is_sentinel(double v) { return (unsigned long long)__double_as_longlong(v) == kSentinel; }
@@ -56,8 +56,6 @@ __device__ __forceinline__ double2 ld_poll2(const double* p) {
 __device__ __forceinline__ void st_publish(double* p, double v) {
     asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
-
-__device__ __forceinline__ size_t row_base(int I) { return (size_t)NB * NB * ((size_t)I * (size_t)(I - 1) / 2); }
 
 // Sum of acc[r] over the 32 lanes for r = 0..7 with 9 exchanges: afterwards the lanes with (lane & 3) == 0
 // hold the total of row  r = 4*bit4(lane) + 2*bit3(lane) + bit2(lane).
@@ -96,15 +94,29 @@ __device__ __forceinline__ double reduce8(const double (&acc)[RW], int lane) {
 // ---------------------------------------------------------------------------------------
 // forward chain:  y_I = bt_I - sum_{J<I} Lt_IJ y_J
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NTHREADS)
+// Block (I, J), J < I, of Lt: NB x NB doubles, row-major, contiguous (32 KB); the blocks of block row I follow
+// each other, so that the forward solve reads one sequential stream per CTA.
+__device__ __forceinline__ size_t blk_off(int I, int J) {
+    return (size_t)NB * NB * ((size_t)I * (size_t)(I - 1) / 2 + (size_t)J);
+}
+
+// ---------------------------------------------------------------------------------------
+// forward chain:  y_I = bt_I - sum_{J<I} Lt_IJ y_J
+// Warp w owns rows 8w..8w+7 (4 KB contiguous per block); lane owns columns 2*lane, 2*lane+1.
+// ---------------------------------------------------------------------------------------
+template <int U>
+__global__ void __launch_bounds__(NTHREADS, 2)
 trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, double* y, unsigned* ticket) {
     __shared__ int sI;
     if (threadIdx.x == 0) sI = (int)atomicAdd(ticket, 1u);
     __syncthreads();
     const int I = sI;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const size_t pitch = (size_t)I * NB;
-    const double* rowp = Lt + row_base(I) + (size_t)(warp * RW) * pitch + 2 * lane;
+    const double* rowp = Lt + blk_off(I, 0) + (size_t)(warp * RW) * NB + 2 * lane;
+    // the right-hand side of the row this lane will publish, fetched before the chain needs it
+    const int my_r = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+    const size_t my_row = (size_t)I * NB + warp * RW + my_r;
+    const double my_bt = bt[my_row];
 
     double acc[RW];
 #pragma unroll
@@ -114,7 +126,8 @@ trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, do
     for (int u = 0; u < U; ++u)
         if (u < I) {
 #pragma unroll
-            for (int r = 0; r < RW; ++r) buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(rowp + r * pitch + u * NB));
+            for (int r = 0; r < RW; ++r)
+                buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(rowp + (size_t)u * NB * NB + r * NB));
         }
     for (int J0 = 0; J0 < I; J0 += U) {
 #pragma unroll
@@ -122,6 +135,8 @@ trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, do
             const int J = J0 + u;
             if (J < I) {
                 const double* yp = y + (size_t)J * NB + 2 * lane;
+                // Every waiting warp spins at full rate: a back-off (__nanosleep) for the CTAs far from the chain
+                // head and a look-ahead poll of y_{J+1} were both measured slower (B200, n = 4096 / 24 500).
                 double2 yv = ld_poll2(yp);
                 while (is_sentinel(yv.x) || is_sentinel(yv.y)) yv = ld_poll2(yp);
 #pragma unroll
@@ -132,24 +147,21 @@ trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, do
                 if (J + U < I) {
 #pragma unroll
                     for (int r = 0; r < RW; ++r)
-                        buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(rowp + r * pitch + (J + U) * NB));
+                        buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(rowp + (size_t)(J + U) * NB * NB + r * NB));
                 }
             }
         }
     }
     const double tot = reduce8(acc, lane);
-    if ((lane & 3) == 0) {
-        const int r = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-        const size_t row = (size_t)I * NB + warp * RW + r;
-        st_publish(y + row, publishable(bt[row] - tot));
-    }
+    if ((lane & 3) == 0) st_publish(y + my_row, publishable(my_bt - tot));
 }
 
 // ---------------------------------------------------------------------------------------
 // backward chain:  xt_I = y_I - sum_{J>I} Lt_JI^T xt_J
 // Warp w sums rows 8w..8w+7 of every block (J, I); lane owns columns 2*lane, 2*lane+1.
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NTHREADS)
+template <int U>
+__global__ void __launch_bounds__(NTHREADS, 2)
 trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, double* xt, unsigned* ticket, int nblk) {
     __shared__ int sI;
     __shared__ double part[NB / RW][NB];
@@ -157,21 +169,18 @@ trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, d
     __syncthreads();
     const int I = sI;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nJ = nblk - 1 - I;  // blocks below the diagonal in block column I; t-th visited is J = nblk-1-t
+    const int nJ = nblk - 1 - I;  // blocks below the diagonal in block column I; the t-th visited is J = nblk-1-t
+    const double my_y = threadIdx.x < NB ? yin[(size_t)I * NB + threadIdx.x] : 0.0;
 
-    auto blk = [&](int t) {
-        const int J = nblk - 1 - t;
-        return Lt + row_base(J) + (size_t)(warp * RW) * ((size_t)J * NB) + (size_t)I * NB + 2 * lane;
-    };
+    auto blk = [&](int t) { return Lt + blk_off(nblk - 1 - t, I) + (size_t)(warp * RW) * NB + 2 * lane; };
     double2 acc = make_double2(0.0, 0.0);
     double2 buf[U][RW];
 #pragma unroll
     for (int u = 0; u < U; ++u)
         if (u < nJ) {
             const double* p = blk(u);
-            const size_t pitch = (size_t)(nblk - 1 - u) * NB;
 #pragma unroll
-            for (int r = 0; r < RW; ++r) buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(p + r * pitch));
+            for (int r = 0; r < RW; ++r) buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(p + r * NB));
         }
     for (int t0 = 0; t0 < nJ; t0 += U) {
 #pragma unroll
@@ -180,23 +189,26 @@ trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, d
             if (t < nJ) {
                 const int J = nblk - 1 - t;
                 const double* xp = xt + (size_t)J * NB + warp * RW;
-                double xv[RW];
+                double2 xv[RW / 2];
+                bool ok;
+                do {   // the four loads of one attempt are in flight together
 #pragma unroll
-                for (int r = 0; r < RW; r += 2) {
-                    double2 v = ld_poll2(xp + r);
-                    while (is_sentinel(v.x) || is_sentinel(v.y)) v = ld_poll2(xp + r);
-                    xv[r] = v.x; xv[r + 1] = v.y;
-                }
+                    for (int r = 0; r < RW / 2; ++r) xv[r] = ld_poll2(xp + 2 * r);
+                    ok = true;
 #pragma unroll
-                for (int r = 0; r < RW; ++r) {
-                    acc.x = fma(buf[u][r].x, xv[r], acc.x);
-                    acc.y = fma(buf[u][r].y, xv[r], acc.y);
+                    for (int r = 0; r < RW / 2; ++r) ok = ok && !is_sentinel(xv[r].x) && !is_sentinel(xv[r].y);
+                } while (!ok);
+#pragma unroll
+                for (int r = 0; r < RW / 2; ++r) {
+                    acc.x = fma(buf[u][2 * r].x, xv[r].x, acc.x);
+                    acc.y = fma(buf[u][2 * r].y, xv[r].x, acc.y);
+                    acc.x = fma(buf[u][2 * r + 1].x, xv[r].y, acc.x);
+                    acc.y = fma(buf[u][2 * r + 1].y, xv[r].y, acc.y);
                 }
                 if (t + U < nJ) {
                     const double* p = blk(t + U);
-                    const size_t pitch = (size_t)(nblk - 1 - (t + U)) * NB;
 #pragma unroll
-                    for (int r = 0; r < RW; ++r) buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(p + r * pitch));
+                    for (int r = 0; r < RW; ++r) buf[u][r] = ldg_stream(reinterpret_cast<const double2*>(p + r * NB));
                 }
             }
         }
@@ -208,8 +220,7 @@ trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, d
         double s = 0.0;
 #pragma unroll
         for (int w = 0; w < NB / RW; ++w) s += part[w][threadIdx.x];
-        const size_t row = (size_t)I * NB + threadIdx.x;
-        st_publish(xt + row, publishable(yin[row] - s));
+        st_publish(xt + (size_t)I * NB + threadIdx.x, publishable(my_y - s));
     }
 }
 
@@ -330,12 +341,11 @@ trsv_scale_kernel(const double* __restrict__ src, long long ld, long long row0, 
 #pragma unroll
             for (int j = 0; j < 4; ++j) o[i][j] = fma(a[i], b[j], o[i][j]);
     }
-    double* dst = Lt + row_base(I) + (size_t)J * NB;
-    const size_t pitch = (size_t)I * NB;
+    double* dst = Lt + blk_off(I, J);
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) dst[(size_t)(r0 + i) * pitch + c0 + j] = o[i][j];
+        for (int j = 0; j < 4; ++j) dst[(size_t)(r0 + i) * NB + c0 + j] = o[i][j];
 }
 
 }  // namespace
@@ -368,12 +378,19 @@ cudaError_t trsv_pre_launch(const TrsvGeom& g, const double* b, cudaStream_t s) 
     trsv_pre_kernel<<<g.nblk, 256, 0, s>>>(g.Dinv, b, g.bt, g.y, g.xt, g.ticket, g.n);
     return cudaGetLastError();
 }
+static int g_trsv_U = 0;
+void trsv_debug_set_U(int U) { g_trsv_U = U; }
+
 cudaError_t trsv_fwd_launch(const TrsvGeom& g, cudaStream_t s) {
-    trsv_fwd_kernel<<<g.nblk, NTHREADS, 0, s>>>(g.Lt, g.bt, g.y, g.ticket);
+    if (g_trsv_U == 3) trsv_fwd_kernel<3><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, g.bt, g.y, g.ticket);
+    else if (g_trsv_U == 1) trsv_fwd_kernel<1><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, g.bt, g.y, g.ticket);
+    else trsv_fwd_kernel<2><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, g.bt, g.y, g.ticket);
     return cudaGetLastError();
 }
 cudaError_t trsv_bwd_launch(const TrsvGeom& g, const double* yin, cudaStream_t s) {
-    trsv_bwd_kernel<<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    if (g_trsv_U == 3) trsv_bwd_kernel<3><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    else if (g_trsv_U == 1) trsv_bwd_kernel<1><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    else trsv_bwd_kernel<2><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
     return cudaGetLastError();
 }
 cudaError_t trsv_post_launch(const TrsvGeom& g, double* x, cudaStream_t s) {

@@ -26,7 +26,7 @@ from dataclasses import dataclass, replace
 
 import torch
 
-TENSOR_F, TENSOR_M, TENSOR_D, TENSOR_SCALE, TENSOR_CENTRE = 0, 1, 2, 3, 4
+TENSOR_F, TENSOR_M, TENSOR_D, TENSOR_SCALE, TENSOR_CENTRE, TENSOR_L = 0, 1, 2, 3, 4, 5
 
 _MASK64 = (1 << 64) - 1
 
@@ -208,3 +208,21 @@ def noise_var(w: Workload, device="cpu") -> torch.Tensor:
     c = _sensor_scale(w, s) if w.sensor_scale else torch.ones(w.N_d, dtype=torch.float64, device=device)
     v = (NOISE_LEVEL ** 2) * c * c * (w.N_m * w.tau * 0.5)
     return v[None, :].expand(w.N_t, w.N_d).contiguous().to(w.dtype)
+
+
+def factor_standin(n: int, seed: int, device="cpu", rows_per_chunk: int = 1024) -> torch.Tensor:
+    """A lower-triangular [n, n] fp64 matrix with the profile of a Cholesky factor (diagonal in (1, 2), strictly
+    lower entries N(0, 1/n), zeros above): stands in for the factor of K = Gamma_noise + F G* where assembling
+    the true K (N_d N_t matvec pairs) is not affordable - the cost of the triangular solves does
+    not depend on the values.  Counter-based like everything else here: entry (r, c) depends on (seed, r*n + c)."""
+    L = torch.zeros((n, n), dtype=torch.float64, device=device)
+    col = torch.arange(n, device=L.device, dtype=torch.int64)
+    for r0 in range(0, n, rows_per_chunk):
+        r1 = min(n, r0 + rows_per_chunk)
+        row = torch.arange(r0, r1, device=L.device, dtype=torch.int64)
+        lin = row[:, None] * n + col[None, :]
+        blk = normal01(seed, TENSOR_L, lin) * (1.0 / math.sqrt(n))
+        blk = torch.where(col[None, :] < row[:, None], blk, torch.zeros_like(blk))
+        L[r0:r1] = blk
+        L[row, row] = 1.0 + uniform01(seed, TENSOR_L, row * n + row)
+    return L

@@ -138,3 +138,81 @@ def test_c4_krhs_slices(tt):
     # adjoint identity over all columns at once: <F M, D> = <M, F^T D>
     lhs, rhs = float((FM * D).sum()), float((M * FtD).sum())
     assert abs(lhs - rhs) <= 1e-12 * float(FM.norm() * D.norm())
+
+
+# ------------------------------------------------------------------------------------------------
+# Online phase at sizes beyond tests/test_gpu_online.py
+# ------------------------------------------------------------------------------------------------
+def test_online_medium_true_K(tt):
+    """Everything real at a size that spans several tiles of every kernel (2 GEMV chunks, 10 blocks of the
+    triangular solves): K assembled by the GPU against the oracle's K, then m_map (both forms) with the ORACLE's
+    Cholesky factor against the oracle's eq (4.13)."""
+    from oracle import online_plain as oo
+    for dtype in (torch.float64, torch.float32):
+        w = synth.CONFIGS["P5"].scaled(N_d=8, N_m=4160, N_t=80, dtype=dtype)
+        F = synth.block_column(w)
+        G = synth.gstar_block_column(w, F)
+        nv, d_obs = synth.noise_var(w), synth.vector_d(w, k_rhs=1)
+        Fn, Gn = F.numpy(), G.numpy()
+        K_ref = oo.assemble_K(Fn, Gn, nv.numpy())
+        L = oo.cholesky(K_ref)
+        m_ref = oo.map_point(Fn, Gn, nv.numpy(), L, d_obs.numpy(), conv=ob)
+        ev = np.linalg.eigvalsh(K_ref)
+        kappa = ev[-1] / ev[0]
+        pF, pG = tt.Plan(F.cuda(), k_max=16), tt.Plan(G.cuda(), k_max=16)
+        chol = tt.Chol(torch.from_numpy(L))          # host factor: goes through the slab path
+        mp = tt.MapInference(pF, pG, chol, nv.cuda())
+        try:
+            K = tt.assemble_K(pF, pG, nv.cuda()).cpu().numpy()
+            m_paper = mp.infer(d_obs.cuda(), tt.TT_MAP_PAPER).cpu().numpy()
+            m_gain = mp.infer(d_obs.cuda(), tt.TT_MAP_GAIN).cpu().numpy()
+        finally:
+            mp.close(); chol.close(); pF.close(); pG.close()
+        u = 1.1e-16 if dtype == torch.float64 else 6e-8
+        print(f"online medium {dtype}: kappa {kappa:.0f}  K {rel(K, K_ref):.2e}  gain {rel(m_gain, m_ref):.2e}  "
+              f"paper {rel(m_paper, m_ref):.2e}")
+        assert rel(K, K_ref) <= TOL[dtype]
+        assert rel(m_gain, m_ref) <= TOL[dtype] + 8 * 1.1e-16 * kappa
+        assert rel(m_paper, m_ref) <= TOL[dtype] + 8 * u * kappa
+
+
+def test_online_p5_full_size_sampled(tt):
+    """The paper's own shape (N_d=49, N_m=263169, N_t=500: 131 584 500 parameters, 24 500 data), in the launch
+    configuration `bench.py --config P5 --online` times: the K-solve against the oracle over the whole vector, and
+    m_map = G* K^{-1} d_obs (gain form) on sampled outputs the oracle computes one by one from single columns
+    G[:, :, p] of the block column.  The factor is the seeded stand-in the bench uses."""
+    from oracle import online_plain as oo
+    from oracle import toeplitz_plain as op
+    w = synth.CONFIGS["P5"]
+    need_memory(120)
+    n = w.N_d * w.N_t
+    L = synth.factor_standin(n, w.seed, device="cuda")
+    chol = tt.Chol(L)
+    L_h = L.cpu().numpy()
+    del L
+    d_obs = synth.vector_d(w, device="cuda", k_rhs=1)
+    d_np = d_obs.cpu().numpy().astype(np.float64)
+    z_ref = oo.chol_solve(L_h, d_np.reshape(n))
+    del L_h
+    z = chol.solve(torch.from_numpy(d_np.reshape(n)).cuda()).cpu().numpy()
+    assert rel(z, z_ref) <= 1e-12
+    G = synth.block_column(w, device="cuda")
+    synth.gstar_block_column(w, G, out=G)
+    rng = np.random.default_rng(5)
+    ps = sorted(set(int(p) for p in rng.integers(0, w.N_m, 12)) | {0, w.N_m - 1})
+    cols = {p: G[:, :, p:p + 1].cpu().numpy() for p in ps}
+    pG = tt.Plan(G)
+    del G
+    torch.cuda.empty_cache()
+    mp = tt.MapInference(None, pG, chol, synth.noise_var(w, device="cuda"))
+    try:
+        m_map = mp.infer(d_obs, tt.TT_MAP_GAIN)
+        got = {p: m_map[:, p].cpu().numpy() for p in ps}
+        scale = float(m_map.double().pow(2).mean().sqrt())
+    finally:
+        mp.close(); pG.close(); chol.close()
+    zr = z_ref.reshape(w.N_t, w.N_d)
+    for p in ps:
+        ref = np.array([op.rmatvec_entry(cols[p], zr, j, 0) for j in range(0, w.N_t, 7)])
+        err = np.linalg.norm(got[p][::7] - ref) / max(np.linalg.norm(ref), 1e-3 * scale * np.sqrt(len(ref)))
+        assert err <= 1e-5, (p, err)
