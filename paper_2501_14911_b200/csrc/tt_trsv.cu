@@ -137,8 +137,9 @@ trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, do
                 const double* yp = y + (size_t)J * NB + 2 * lane;
                 // Every waiting warp spins at full rate: a back-off (__nanosleep) for the CTAs far from the chain
                 // head and a look-ahead poll of y_{J+1} were both measured slower (B200, n = 4096 / 24 500).
-                double2 yv = ld_poll2(yp);
-                while (is_sentinel(yv.x) || is_sentinel(yv.y)) yv = ld_poll2(yp);
+                double2 yv;
+#pragma unroll 1
+                do { yv = ld_poll2(yp); } while (is_sentinel(yv.x) || is_sentinel(yv.y));   // one load per attempt
 #pragma unroll
                 for (int r = 0; r < RW; ++r) {
                     acc[r] = fma(buf[u][r].x, yv.x, acc[r]);
@@ -191,6 +192,7 @@ trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, d
                 const double* xp = xt + (size_t)J * NB + warp * RW;
                 double2 xv[RW / 2];
                 bool ok;
+#pragma unroll 1
                 do {   // the four loads of one attempt are in flight together
 #pragma unroll
                     for (int r = 0; r < RW / 2; ++r) xv[r] = ld_poll2(xp + 2 * r);
