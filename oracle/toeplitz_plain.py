@@ -94,3 +94,43 @@ def rmatvec_entry(F, d, j: int, p: int) -> float:
         acc += float(np.dot(np.asarray(F[i - j][:, p], dtype=np.float64),
                             np.asarray(d[i], dtype=np.float64)))
     return acc
+
+
+# ---------------------------------------------------------------------------------------------
+# Output on a coarser time grid: the p2q map of the paper's example (N_t^q = 50 << N_t = 500,
+# PAPER.md:162, 381).  The paper says only that "the block structure ... changes correspondingly";
+# DESIGN.md reading R19: the QoI is the fine-grid output sampled at the end of every r-th step,
+#     q_I = (F_q m)_{r(I+1)-1} = sum_{j=0..r(I+1)-1} F_{r(I+1)-1-j} m_j ,   I = 0..N_t/r - 1,
+# (the paper's 1-based q_I at time I*r*dt), the stored block column staying the fine-grid one
+# (N_t blocks of N_q x N_m: the 16 x 1.05 GB = 17 GB of PAPER.md:393).  Its transpose is
+#     m'_j = sum_{I : r(I+1)-1 >= j} F_{r(I+1)-1-j}^T q_I .
+# ---------------------------------------------------------------------------------------------
+def matvec_decimated(F, m, r: int) -> np.ndarray:
+    """q = S F m with S = 'keep fine steps r-1, 2r-1, ...'.  Returns fp64 [N_t // r, N_q(, k)]."""
+    F, m = _f64(F), _f64(m)
+    N_t, N_q, N_m = F.shape
+    assert N_t % r == 0 and m.shape[0] == N_t and m.shape[1] == N_m
+    q = np.zeros((N_t // r, N_q) + m.shape[2:], dtype=np.float64)
+    for I in range(N_t // r):
+        i = r * (I + 1) - 1
+        acc = np.zeros((N_q,) + m.shape[2:], dtype=np.float64)
+        for j in range(i + 1):
+            acc += F[i - j] @ m[j]
+        q[I] = acc
+    return q
+
+
+def rmatvec_decimated(F, q, r: int) -> np.ndarray:
+    """m' = F^T S^T q.  q: [N_t // r, N_q(, k)].  Returns fp64 [N_t, N_m(, k)]."""
+    F, q = _f64(F), _f64(q)
+    N_t, N_q, N_m = F.shape
+    assert N_t % r == 0 and q.shape[0] == N_t // r and q.shape[1] == N_q
+    out = np.zeros((N_t, N_m) + q.shape[2:], dtype=np.float64)
+    for j in range(N_t):
+        acc = np.zeros((N_m,) + q.shape[2:], dtype=np.float64)
+        for I in range(N_t // r):
+            i = r * (I + 1) - 1
+            if i >= j:
+                acc += F[i - j].T @ q[I]
+        out[j] = acc
+    return out

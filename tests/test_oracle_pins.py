@@ -229,3 +229,37 @@ def test_entry_helpers_and_multi_rhs():
         assert abs(op.matvec_entry(F, M[..., 0], i, s) - d[i * N_d + s]) <= 1e-13
     for j, p in itertools.product((0, 2, N_t - 1), (0, N_m - 1)):
         assert abs(op.rmatvec_entry(F, D[..., 0], j, p) - mm[j * N_m + p]) <= 1e-13
+
+
+# ---------------------------------------------------------------- coarser output grid (p2q, reading R19)
+@pytest.mark.parametrize("N_q,N_m,N_t,r", [(2, 3, 6, 2), (1, 4, 9, 3), (3, 2, 8, 8), (2, 5, 10, 5), (2, 3, 7, 1)])
+def test_decimated_output_dense_and_adjoint(N_q, N_m, N_t, r):
+    F = RNG.standard_normal((N_t, N_q, N_m))
+    m = RNG.standard_normal((N_t, N_m))
+    q = RNG.standard_normal((N_t // r, N_q))
+    A = dense_from_block_column(F)
+    keep = np.concatenate([np.arange(N_q) + (r * (I + 1) - 1) * N_q for I in range(N_t // r)])
+    Aq = A[keep]                                             # S A: the rows of the fine steps r-1, 2r-1, ...
+    assert rel(op.matvec_decimated(F, m, r), Aq @ m.ravel()) <= 1e-14
+    assert rel(op.rmatvec_decimated(F, q, r), Aq.T @ q.ravel()) <= 1e-14
+    lhs = np.vdot(op.matvec_decimated(F, m, r), q)
+    assert abs(lhs - np.vdot(m, op.rmatvec_decimated(F, q, r))) <= 1e-13 * max(1.0, abs(lhs))
+    if r == 1:
+        assert np.array_equal(op.matvec_decimated(F, m, 1), op.matvec(F, m))
+        assert np.array_equal(op.rmatvec_decimated(F, q, 1), op.rmatvec(F, q))
+
+
+def test_decimated_output_is_the_sampled_recurrence():
+    # eq (2.2)-(2.3) with a QoI observation operator B_q (eq 2.14-2.16), sampled every r steps:
+    # q_I = B_q w_{r(I+1)} in the paper's 1-based state index, i.e. after r(I+1) steps of the recurrence
+    n_w, N_q, N_m, N_t, r = 5, 2, 3, 12, 4
+    A = RNG.standard_normal((n_w, n_w)); A *= 0.9 / np.abs(np.linalg.eigvals(A)).max()
+    Bq, C = RNG.standard_normal((N_q, n_w)), RNG.standard_normal((n_w, N_m))
+    F = np.stack([Bq @ np.linalg.matrix_power(A, k) @ C for k in range(N_t)])
+    m = RNG.standard_normal((N_t, N_m))
+    w, out = np.zeros(n_w), []
+    for k in range(N_t):
+        w = A @ w + C @ m[k]
+        if (k + 1) % r == 0:
+            out.append(Bq @ w)
+    assert rel(op.matvec_decimated(F, m, r), np.array(out)) <= 1e-13
