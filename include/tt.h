@@ -103,6 +103,20 @@ const char* tt_status_string(int status);
 int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dtype, int layout,
                    int k_max, const void* first_block_column, void* stream);
 
+/* The same operator with its OUTPUT on a coarser time grid - the p2q map of the paper's example, whose QoIs are
+ * sampled at 1 Hz while parameters and data live at 10 Hz (N_t^q = 50 << N_t = 500).
+ * The paper gives no formula ("the block structure ... changes correspondingly"); reading R19: the
+ * data side keeps the fine-grid steps out_every-1, 2*out_every-1, ... (the end of every out_every-th step),
+ *
+ *        q_I = (F m)_{out_every*(I+1)-1} ,   I = 0 .. N_t/out_every - 1 ,
+ *
+ * and the block column stays the fine-grid one (N_t blocks).  out_every must divide N_t.  Every data-side vector of
+ * the plan (d of tt_matvec / tt_rmatvec, D of the k-RHS calls, the intermediate of tt_normal) then has
+ * N_t/out_every time steps; tt_rmatvec applies the exact transpose (zeros at the steps that are not sampled).
+ * The sampling and the zero-stuffing live in the load / store of the data-side FFT kernels. */
+int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int64_t out_every, int dtype,
+                          int layout, int k_max, const void* first_block_column, void* stream);
+
 /* Frees Fhat and all scratch.  NULL-safe.  The caller must have synchronised any stream
  * that still runs work of this plan. */
 void tt_plan_destroy(tt_plan* plan);

@@ -53,6 +53,7 @@ def lib() -> ctypes.CDLL:
         "tt_version": (ci, []),
         "tt_status_string": (ctypes.c_char_p, [ci]),
         "tt_plan_create": (ci, [pp, i64, i64, i64, ci, ci, ci, vp, vp]),
+        "tt_plan_create_coarse": (ci, [pp, i64, i64, i64, i64, ci, ci, ci, vp, vp]),
         "tt_plan_destroy": (None, [vp]),
         "tt_plan_device_bytes": (sz, [vp]),
         "tt_plan_last_cuda_error": (ci, [vp]),
@@ -94,7 +95,7 @@ def lib() -> ctypes.CDLL:
     return L
 
 
-EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_destroy", "tt_plan_device_bytes",
+EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_coarse", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
@@ -132,6 +133,17 @@ def tt_plan_create(N_d: int, N_m: int, N_t: int, dtype: int, layout: int, k_max:
     out = ctypes.c_void_p()
     st = lib().tt_plan_create(ctypes.byref(out), N_d, N_m, N_t, dtype, layout, k_max, ptr, _stream(stream))
     _check("tt_plan_create", st)
+    return out.value
+
+
+def tt_plan_create_coarse(N_d: int, N_m: int, N_t: int, out_every: int, dtype: int, layout: int, k_max: int,
+                          first_block_column, stream=None) -> int:
+    """tt_plan_create with the data side on every out_every-th time step (the p2q map, reading R19)."""
+    ptr = first_block_column if isinstance(first_block_column, int) else first_block_column.data_ptr()
+    out = ctypes.c_void_p()
+    st = lib().tt_plan_create_coarse(ctypes.byref(out), N_d, N_m, N_t, out_every, dtype, layout, k_max, ptr,
+                                     _stream(stream))
+    _check("tt_plan_create_coarse", st)
     return out.value
 
 
@@ -314,13 +326,13 @@ class Plan:
     """
 
     def __init__(self, first_block_column: torch.Tensor, layout: int = TT_TIME_MAJOR, k_max: int = 1,
-                 stream=None):
+                 stream=None, out_every: int = 1):
         assert first_block_column.dim() == 3 and first_block_column.is_contiguous()
         self.N_t, self.N_d, self.N_m = first_block_column.shape
         self.dtype = first_block_column.dtype
-        self.layout, self.k_max = layout, k_max
-        self.handle = tt_plan_create(self.N_d, self.N_m, self.N_t, _DT[self.dtype], layout, k_max,
-                                     first_block_column, stream)
+        self.layout, self.k_max, self.out_every = layout, k_max, out_every
+        self.handle = tt_plan_create_coarse(self.N_d, self.N_m, self.N_t, out_every, _DT[self.dtype], layout, k_max,
+                                            first_block_column, stream)
 
     def close(self):
         if getattr(self, "handle", None):
@@ -330,17 +342,18 @@ class Plan:
 
     __del__ = close
 
-    def _shape(self, n_space: int, k: int | None):
-        base = (self.N_t, n_space) if self.layout == TT_TIME_MAJOR else (n_space, self.N_t)
+    def _shape(self, n_space: int, k: int | None, data: bool = False):
+        n_time = self.N_t // self.out_every if data else self.N_t
+        base = (n_time, n_space) if self.layout == TT_TIME_MAJOR else (n_space, n_time)
         if k is None:
             return base
         return base + (k,) if self.layout == TT_TIME_MAJOR else (k,) + base
 
-    def _out(self, n_space: int, k: int | None = None):
-        return torch.empty(self._shape(n_space, k), dtype=self.dtype, device="cuda")
+    def _out(self, n_space: int, k: int | None = None, data: bool = False):
+        return torch.empty(self._shape(n_space, k, data), dtype=self.dtype, device="cuda")
 
     def matvec(self, m, out=None, stream=None):
-        out = self._out(self.N_d) if out is None else out
+        out = self._out(self.N_d, data=True) if out is None else out
         tt_matvec(self.handle, m, out, stream)
         return out
 
@@ -356,7 +369,7 @@ class Plan:
 
     def matvec_batched(self, M, out=None, stream=None):
         k = M.shape[-1] if self.layout == TT_TIME_MAJOR else M.shape[0]
-        out = self._out(self.N_d, k) if out is None else out
+        out = self._out(self.N_d, k, data=True) if out is None else out
         tt_matvec_batched(self.handle, k, M, out, stream)
         return out
 

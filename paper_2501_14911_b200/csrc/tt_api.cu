@@ -27,6 +27,7 @@ int g_fft_max_radix = 0;  // tt_debug_set("fft_max_radix"): 0 = no limit
 
 struct tt_plan {
     long long N_d = 0, N_m = 0, N_t = 0;
+    long long dec = 1, N_td = 0;  // data vectors live on every dec-th time step: N_td = N_t / dec of them (p2q, reading R19)
     int dtype = 0, layout = 0, k_max = 1;
     int n_f = 0;
     long long ldp = 0;  // padded N_m: row pitch of Fhat and of the single-vector spectrum
@@ -55,7 +56,7 @@ struct tt_plan {
 };
 
 namespace tt {
-PlanInfo plan_info(const ::tt_plan* p) { return PlanInfo{p->N_d, p->N_m, p->N_t, p->dtype, p->layout, p->k_max}; }
+PlanInfo plan_info(const ::tt_plan* p) { return PlanInfo{p->N_d, p->N_m, p->N_t, p->dtype, p->layout, p->k_max, p->dec}; }
 }  // namespace tt
 
 namespace {
@@ -151,14 +152,15 @@ void fill_fft_common(const tt_plan* p, FftParams& P, bool fp32_tables) {
     P.tw = fp32_tables ? p->tw_f : p->tw_d;
     P.pos = p->pos[which];
     P.scale = 1.0 / (2.0 * (double)p->N_t);
+    P.dec = 1;
 }
 
 // Where column r of a (k-RHS) vector lives: element (b, j) is base[b*bs + j*ts] (in elements).
 struct VecView {
     long long off, bs, ts;
 };
-VecView view(const tt_plan* p, long long n_space, int k, int r) {
-    if (p->layout == TT_SPACE_MAJOR) return VecView{(long long)r * n_space * p->N_t, p->N_t, 1};
+VecView view(const tt_plan* p, long long n_space, long long n_time, int k, int r) {
+    if (p->layout == TT_SPACE_MAJOR) return VecView{(long long)r * n_space * n_time, n_time, 1};
     return VecView{(long long)r, (long long)k, n_space * k};
 }
 inline const void* at(const void* base, long long off, size_t es) { return static_cast<const char*>(base) + (size_t)off * es; }
@@ -188,7 +190,7 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
     const bool f32 = p->dtype == TT_F32;
     const int t = f32 ? 0 : 1;
     const size_t es = esize(p->dtype);
-    const VecView vm = view(p, p->N_m, k, r), vd = view(p, p->N_d, k, r);
+    const VecView vm = view(p, p->N_m, p->N_t, k, r), vd = view(p, p->N_d, p->N_td, k, r);
     Prof pr{p, s, ev_base};
     pr.mark(0);
     FftParams P;
@@ -205,7 +207,7 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
     fill_fft_common(p, P, f32);
     P.B = p->N_d; P.B_store = p->N_d;
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
-    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
     TT_CUDA(p, fft_c2r_launch(t, p->dhat, at(d, vd.off, es), P, 1, s));
     pr.mark(3);
     return TT_OK;
@@ -216,13 +218,13 @@ int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev
     const bool f32 = p->dtype == TT_F32;
     const int t = f32 ? 0 : 1;
     const size_t es = esize(p->dtype);
-    const VecView vm = view(p, p->N_m, k, r), vd = view(p, p->N_d, k, r);
+    const VecView vm = view(p, p->N_m, p->N_t, k, r), vd = view(p, p->N_d, p->N_td, k, r);
     Prof pr{p, s, ev_base};
     pr.mark(0);
     FftParams P;
     fill_fft_common(p, P, f32);
     P.B = p->N_d; P.B_store = p->N_d;
-    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
     TT_CUDA(p, fft_r2c_launch(t, t, t, at(d, vd.off, es), p->dhat, P, 1, s));
     pr.mark(1);
@@ -257,12 +259,15 @@ GemmGeom gemm_geom(const tt_plan* p, int k) {
     return g;
 }
 
-void batched_views(const tt_plan* p, FftParams& P, long long n_space, int k, long long c_pitch, int* ny) {
+void batched_views(const tt_plan* p, FftParams& P, long long n_space, int k, long long c_pitch, int* ny,
+                   bool data_side = false) {
+    const long long n_time = data_side ? p->N_td : p->N_t;
+    P.dec = data_side ? (int)p->dec : 1;
     // series b = x*k + r (x = space index): time-major vectors have it contiguous; space-major ones
     // are [r][x][j], addressed with one grid row per r.
     if (p->layout == TT_SPACE_MAJOR) {
         P.B = n_space; P.B_store = n_space;
-        P.r_ys = n_space * p->N_t; P.r_bs = p->N_t; P.r_ts = 1;
+        P.r_ys = n_space * n_time; P.r_bs = n_time; P.r_ts = 1;
         P.c_ys = 1; P.c_bs = k; P.c_fs = c_pitch;
         *ny = k;
     } else {
@@ -287,7 +292,7 @@ int run_matvec_gemm(const tt_plan* p, int k, const void* M, void* D, cudaStream_
     pr.mark(2);
     TT_CUDA(p, reduce_partials_launch(1, p->partial, p->dhat, p->n_f, g.split, (int)(p->N_d * k), s));
     fill_fft_common(p, P, false);
-    batched_views(p, P, p->N_d, k, p->N_d * k, &ny);
+    batched_views(p, P, p->N_d, k, p->N_d * k, &ny, true);
     TT_CUDA(p, fft_c2r_launch(1, p->dhat, D, P, ny, s));
     pr.mark(3);
     return TT_OK;
@@ -300,7 +305,7 @@ int run_rmatvec_gemm(const tt_plan* p, int k, const void* D, void* M, cudaStream
     pr.mark(0);
     FftParams P;
     fill_fft_common(p, P, false);
-    batched_views(p, P, p->N_d, k, p->N_d * k, &ny);
+    batched_views(p, P, p->N_d, k, p->N_d * k, &ny, true);
     TT_CUDA(p, fft_r2c_launch(1, 1, 1, D, p->dhat, P, ny, s));
     pr.mark(1);
     TT_CUDA(p, gemm_adj_launch(1, p->Fhat, p->dhat, p->xhat, g, s));
@@ -395,10 +400,16 @@ void tt_plan_destroy(tt_plan* p) {
 
 int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dtype, int layout, int k_max,
                    const void* first_block_column, void* stream) {
+    return tt_plan_create_coarse(out, N_d, N_m, N_t, 1, dtype, layout, k_max, first_block_column, stream);
+}
+
+int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int64_t out_every, int dtype, int layout,
+                          int k_max, const void* first_block_column, void* stream) {
     if (!out) return TT_ERR_NULL;
     *out = nullptr;
     if (!first_block_column) return TT_ERR_NULL;
     if (N_d < 1 || N_m < 1 || N_t < 1) return TT_ERR_SHAPE;
+    if (out_every < 1 || N_t % out_every != 0) return TT_ERR_SHAPE;
     if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
     if (layout != TT_TIME_MAJOR && layout != TT_SPACE_MAJOR) return TT_ERR_LAYOUT;
     if (k_max < 1) return TT_ERR_K;
@@ -428,6 +439,7 @@ int tt_plan_create(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, int dty
     tt_plan* p = new (std::nothrow) tt_plan();
     if (!p) return TT_ERR_OOM;
     p->N_d = N_d; p->N_m = N_m; p->N_t = N_t;
+    p->dec = out_every; p->N_td = N_t / out_every;
     p->dtype = dtype; p->layout = layout; p->k_max = k_max;
     p->n_f = (int)N_t + 1;
     p->ldp = (N_m + 15) / 16 * 16;
@@ -602,7 +614,7 @@ int tt_matvec_host(const tt_plan* p, const void* m_host, void* d_host, void* str
     TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
     r = run_matvec(p, p->m_stage, p->d_stage, s, begin_call(p, TT_OP_MATVEC, 1));
     if (r) return r;
-    TT_CUDA(p, cudaMemcpyAsync(d_host, p->d_stage, (size_t)p->N_t * p->N_d * es, cudaMemcpyDeviceToHost, s));
+    TT_CUDA(p, cudaMemcpyAsync(d_host, p->d_stage, (size_t)p->N_td * p->N_d * es, cudaMemcpyDeviceToHost, s));
     return TT_OK;
 }
 
@@ -613,7 +625,7 @@ int tt_rmatvec_host(const tt_plan* p, const void* d_host, void* m_host, void* st
     if (r) return r;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
-    TT_CUDA(p, cudaMemcpyAsync(p->d_stage, d_host, (size_t)p->N_t * p->N_d * es, cudaMemcpyHostToDevice, s));
+    TT_CUDA(p, cudaMemcpyAsync(p->d_stage, d_host, (size_t)p->N_td * p->N_d * es, cudaMemcpyHostToDevice, s));
     r = run_rmatvec(p, p->d_stage, p->m_stage, s, begin_call(p, TT_OP_RMATVEC, 1));
     if (r) return r;
     TT_CUDA(p, cudaMemcpyAsync(m_host, p->m_stage, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));

@@ -213,6 +213,11 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
     const bool live = b < P.B;
     const int N = P.N;
     const Tin* src = in + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
+    const int dec = P.dec;
+    auto ld_real = [&](int j) -> Tin {   // time step j of the series; on a coarser grid only every dec-th step exists
+        if (dec == 1) return src[(long long)j * P.r_ts];
+        return ((j + 1) % dec == 0) ? src[(long long)((j + 1) / dec - 1) * P.r_ts] : Tin(0);
+    };
 
     // z_n = x_{2n} + i x_{2n+1}; x_j = 0 for j >= N_t = N (the zero padding).  The global loads are
     // issued in batches of 2*UB independent requests per thread before any of them is consumed.
@@ -225,8 +230,8 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
             const int n = n0 + u * G;
             v0[u] = Tin(0); v1[u] = Tin(0);
             if (live && n < nh) {
-                v0[u] = src[(long long)(2 * n) * P.r_ts];
-                if (2 * n + 1 < N) v1[u] = src[(long long)(2 * n + 1) * P.r_ts];
+                v0[u] = ld_real(2 * n);
+                if (2 * n + 1 < N) v1[u] = ld_real(2 * n + 1);
             }
         }
 #pragma unroll
@@ -313,10 +318,15 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
     if (live) {
         Tc* dst = out + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
         const Tc sc = Tc(P.scale);
+        const int dec = P.dec;
+        auto st_real = [&](int j, Tc val) {   // on a coarser grid only every dec-th time step is kept
+            if (dec == 1) dst[(long long)j * P.r_ts] = val;
+            else if ((j + 1) % dec == 0) dst[(long long)((j + 1) / dec - 1) * P.r_ts] = val;
+        };
         for (int n = g; 2 * n < N; n += G) {
             const Cx<Tc> v = sm[(int)P.pos[n] * T + lane_s];
-            dst[(long long)(2 * n) * P.r_ts] = v.re * sc;
-            if (2 * n + 1 < N) dst[(long long)(2 * n + 1) * P.r_ts] = -v.im * sc;
+            st_real(2 * n, v.re * sc);
+            if (2 * n + 1 < N) st_real(2 * n + 1, -v.im * sc);
         }
     }
 }

@@ -12,6 +12,7 @@ namespace tt {
 struct PlanInfo {
     long long N_d, N_m, N_t;
     int dtype, layout, k_max;
+    long long dec;  // data vectors on every dec-th time step (tt_plan_create_coarse)
 };
 PlanInfo plan_info(const ::tt_plan* p);
 
@@ -39,6 +40,8 @@ struct FftParams {
     long long r_ys, r_bs, r_ts;
     long long c_ys, c_bs, c_fs;
     double scale;           // inverse only: factor applied to the real output (1/L)
+    int dec;                // real side on a coarser time grid: only the time steps j with (j+1) % dec == 0 exist, stored
+                            // at index (j+1)/dec - 1 (forward: the others are zeros; inverse: the others are dropped); 1 = all
 };
 
 struct FftChoice {

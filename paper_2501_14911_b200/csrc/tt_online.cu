@@ -135,7 +135,8 @@ __global__ void scatter_K_kernel(const T* __restrict__ D, const T* __restrict__ 
 inline unsigned nblocks(long long n, int t = 256) { return (unsigned)((n + t - 1) / t); }
 
 bool same_shape(const PlanInfo& a, const PlanInfo& b) {
-    return a.N_d == b.N_d && a.N_m == b.N_m && a.N_t == b.N_t && a.dtype == b.dtype && a.layout == b.layout;
+    return a.N_d == b.N_d && a.N_m == b.N_m && a.N_t == b.N_t && a.dtype == b.dtype && a.layout == b.layout &&
+           a.dec == 1 && b.dec == 1;   // the online phase is defined on the data grid of F (N_t^d = N_t^m)
 }
 
 template <typename T>
@@ -349,7 +350,7 @@ int tt_map_create(tt_map** out, const tt_plan* F, const tt_plan* G, const tt_cho
     const PlanInfo pg = plan_info(G);
     if (F && !same_shape(plan_info(F), pg)) return TT_ERR_MISMATCH;
     const long long n = pg.N_d * pg.N_t;
-    if (K->n != n) return TT_ERR_MISMATCH;
+    if (K->n != n || pg.dec != 1) return TT_ERR_MISMATCH;
     tt_map* m = new (std::nothrow) tt_map();
     if (!m) return TT_ERR_OOM;
     m->F = F; m->G = G; m->K = K; m->pi = pg;

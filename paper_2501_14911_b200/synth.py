@@ -103,6 +103,9 @@ CONFIGS = {
     # the paper's own test configuration: 7x7 sensors, 513x513 parameters, 500 steps,
     # 131 584 500 parameters, 24 500 data - the workload of the online phase (eq 4.13)
     "P5": Workload("P5-paper-sec5-online-c64", 49, 263169, 500, torch.float32, 5, 100.0, sensor_scale=True),
+    # the paper's p2q map: 4x4 QoI locations, the same parameter grid and fine time grid,
+    # QoIs sampled at 1 Hz (every 10th step): 800 QoIs; 17 GB block column in fp64, 8.4 GB here in fp32
+    "Q5": Workload("Q5-paper-sec5-p2q-c64", 16, 263169, 500, torch.float32, 6, 100.0, sensor_scale=True),
 }
 
 NOISE_LEVEL = 0.05   # relative noise of the online workload (the paper uses 2-6 %)

@@ -244,6 +244,9 @@ def test_decimated_output_dense_and_adjoint(N_q, N_m, N_t, r):
     assert rel(op.rmatvec_decimated(F, q, r), Aq.T @ q.ravel()) <= 1e-14
     lhs = np.vdot(op.matvec_decimated(F, m, r), q)
     assert abs(lhs - np.vdot(m, op.rmatvec_decimated(F, q, r))) <= 1e-13 * max(1.0, abs(lhs))
+    assert np.array_equal(op.matvec_decimated(F, m, r), op.matvec(F, m)[r - 1::r])       # S (F m): the same sums
+    up = np.zeros((N_t, N_q)); up[r - 1::r] = q
+    assert rel(op.rmatvec_decimated(F, q, r), op.rmatvec(F, up)) <= 1e-15                  # F^T (S^T q)
     if r == 1:
         assert np.array_equal(op.matvec_decimated(F, m, 1), op.matvec(F, m))
         assert np.array_equal(op.rmatvec_decimated(F, q, 1), op.rmatvec(F, q))
