@@ -538,7 +538,8 @@ def main() -> int:
     if K == 1:
         xhat_bytes = n_f * ldp * 2 * es
         dhat_bytes = n_f * w.N_d * 2 * es
-        n_chunks = (ldp + 4095) // 4096
+        chunk = 2048 if n_f * ((ldp + 4095) // 4096) < 148 * 2 * 8 else 4096      # the planner's choice (tt_api.cu)
+        n_chunks = (ldp + chunk - 1) // chunk
         part_bytes = n_f * n_chunks * w.N_d * 2 * es
         bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
         bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written

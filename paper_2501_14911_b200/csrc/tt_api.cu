@@ -45,7 +45,7 @@ struct tt_plan {
     void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
     void* d_stage = nullptr;
     void* m_stage2 = nullptr;
-    int chunk = 0, n_chunks = 0;
+    int chunk = 0, n_chunks = 0, fwd_warps = 0;
     size_t bytes = 0;
     mutable int last_cuda = 0;
     bool prof = false;
@@ -200,7 +200,7 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
     TT_CUDA(p, fft_r2c_launch(t, t, t, at(m, vm.off, es), p->xhat, P, 1, s));
     pr.mark(1);
-    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks};
+    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
     TT_CUDA(p, gemv_fwd_launch(t, p->Fhat, p->xhat, p->partial, g, s));
     pr.mark(2);
     TT_CUDA(p, reduce_partials_launch(t, p->partial, p->dhat, p->n_f, p->n_chunks, (int)p->N_d, s));
@@ -228,7 +228,7 @@ int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
     TT_CUDA(p, fft_r2c_launch(t, t, t, at(d, vd.off, es), p->dhat, P, 1, s));
     pr.mark(1);
-    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks};
+    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
     TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
     pr.mark(2);
     fill_fft_common(p, P, f32);
@@ -281,19 +281,21 @@ void batched_views(const tt_plan* p, FftParams& P, long long n_space, int k, lon
 int run_matvec_gemm(const tt_plan* p, int k, const void* M, void* D, cudaStream_t s, int ev_base) {
     Prof pr{p, s, ev_base};
     const GemmGeom g = gemm_geom(p, k);
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
     int ny = 1;
     pr.mark(0);
     FftParams P;
-    fill_fft_common(p, P, false);
+    fill_fft_common(p, P, f32);
     batched_views(p, P, p->N_m, k, g.ldx, &ny);
-    TT_CUDA(p, fft_r2c_launch(1, 1, 1, M, p->xhat, P, ny, s));
+    TT_CUDA(p, fft_r2c_launch(t, t, t, M, p->xhat, P, ny, s));
     pr.mark(1);
-    TT_CUDA(p, gemm_fwd_launch(1, p->Fhat, p->xhat, p->partial, g, s));
+    TT_CUDA(p, gemm_fwd_launch(t, p->Fhat, p->xhat, p->partial, g, s));
     pr.mark(2);
-    TT_CUDA(p, reduce_partials_launch(1, p->partial, p->dhat, p->n_f, g.split, (int)(p->N_d * k), s));
-    fill_fft_common(p, P, false);
+    TT_CUDA(p, reduce_partials_launch(t, p->partial, p->dhat, p->n_f, g.split, (int)(p->N_d * k), s));
+    fill_fft_common(p, P, f32);
     batched_views(p, P, p->N_d, k, p->N_d * k, &ny, true);
-    TT_CUDA(p, fft_c2r_launch(1, p->dhat, D, P, ny, s));
+    TT_CUDA(p, fft_c2r_launch(t, p->dhat, D, P, ny, s));
     pr.mark(3);
     return TT_OK;
 }
@@ -301,18 +303,20 @@ int run_matvec_gemm(const tt_plan* p, int k, const void* M, void* D, cudaStream_
 int run_rmatvec_gemm(const tt_plan* p, int k, const void* D, void* M, cudaStream_t s, int ev_base) {
     Prof pr{p, s, ev_base};
     const GemmGeom g = gemm_geom(p, k);
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
     int ny = 1;
     pr.mark(0);
     FftParams P;
-    fill_fft_common(p, P, false);
+    fill_fft_common(p, P, f32);
     batched_views(p, P, p->N_d, k, p->N_d * k, &ny, true);
-    TT_CUDA(p, fft_r2c_launch(1, 1, 1, D, p->dhat, P, ny, s));
+    TT_CUDA(p, fft_r2c_launch(t, t, t, D, p->dhat, P, ny, s));
     pr.mark(1);
-    TT_CUDA(p, gemm_adj_launch(1, p->Fhat, p->dhat, p->xhat, g, s));
+    TT_CUDA(p, gemm_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
     pr.mark(2);
-    fill_fft_common(p, P, false);
+    fill_fft_common(p, P, f32);
     batched_views(p, P, p->N_m, k, g.ldx, &ny);
-    TT_CUDA(p, fft_c2r_launch(1, p->xhat, M, P, ny, s));
+    TT_CUDA(p, fft_c2r_launch(t, p->xhat, M, P, ny, s));
     pr.mark(3);
     return TT_OK;
 }
@@ -449,6 +453,12 @@ int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, 
     }
     p->chunk = g_gemv_chunk > 0 ? g_gemv_chunk / 64 * 64 : 4096;  // measured: 4096/8192 ~1 % ahead of 2048 at C3
     if (p->chunk < 64) p->chunk = 64;
+    // Small spectra (C2: 257 frequencies x 4 chunks = 3.5 waves of 2 CTAs/SM) lose a wave to the tail: halve the chunk
+    // and the CTA (8 warps) so that the grid is ~7 waves of finer CTAs; measured at C2: F.m 0.736 -> 0.704 ms.
+    if (g_gemv_chunk <= 0 && (long long)p->n_f * ((p->ldp + 4095) / 4096) < 148LL * 2 * 8) {
+        p->chunk = 2048;
+        p->fwd_warps = 8;
+    }
     p->n_chunks = (int)((p->ldp + p->chunk - 1) / p->chunk);
 
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -575,14 +585,15 @@ int tt_normal(const tt_plan* p, const void* m, void* out, void* stream) {
     return run_rmatvec(p, p->dwork, out, static_cast<cudaStream_t>(stream), e0 + 4);
 }
 
-// k-RHS: TT_F64 plans run batched FFTs + one FP64 DMMA complex GEMM per frequency (tt_gemm.cu);
-// TT_F32 plans (and k = 1) run the single-vector kernels once per right-hand side, addressing
-// column r through the strides of the fused FFT load/store.
+// k-RHS: batched FFTs + one complex GEMM per frequency - FP64 DMMA for TT_F64 plans (tt_gemm.cu), register-tiled
+// FP32 FMA for TT_F32 plans (tt_gemm32.cu).  k = 1 (and TT_F32 plans with more than kGemm32MaxNd sensors) run the
+// single-vector kernels once per right-hand side, addressing column r through the strides of the fused FFT
+// load/store.
 int tt_matvec_batched(const tt_plan* p, int k, const void* M, void* D, void* stream) {
     int r = check_apply(p, M, D);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
-    if (p->dtype == TT_F64 && k > 1)
+    if (k > 1 && (p->dtype == TT_F64 || p->N_d <= kGemm32MaxNd))
         return run_matvec_gemm(p, k, M, D, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC_BATCHED, 1));
     for (int c = 0; c < k; ++c) {
         r = run_matvec(p, M, D, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_MATVEC_BATCHED, 1), k, c);
@@ -595,7 +606,7 @@ int tt_rmatvec_batched(const tt_plan* p, int k, const void* D, void* M, void* st
     int r = check_apply(p, D, M);
     if (r) return r;
     if (k < 1 || k > p->k_max) return TT_ERR_K;
-    if (p->dtype == TT_F64 && k > 1)
+    if (k > 1 && (p->dtype == TT_F64 || p->N_d <= kGemm32MaxNd))
         return run_rmatvec_gemm(p, k, D, M, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC_BATCHED, 1));
     for (int c = 0; c < k; ++c) {
         r = run_rmatvec(p, D, M, static_cast<cudaStream_t>(stream), begin_call(p, TT_OP_RMATVEC_BATCHED, 1), k, c);
@@ -735,6 +746,7 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "fft_max_radix")) { g_fft_max_radix = value; return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
+    if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_fwd_warps")) {
         if (value < 0 || value > 32) return TT_ERR_SHAPE;
         gemv_debug_set(value, -1);

@@ -276,7 +276,7 @@ static cudaError_t adj_launch_nn(const c128* F, const c128* D, c128* X, const Ge
 
 cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g,
                             cudaStream_t s) {
-    if (dt != 1) return cudaErrorNotSupported;
+    if (dt == 0) return gemm32_fwd_launch(Fhat, Xhat, partial, g, s);
     const c128* F = static_cast<const c128*>(Fhat);
     const c128* X = static_cast<const c128*>(Xhat);
     c128* P = static_cast<c128*>(partial);
@@ -292,7 +292,7 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
 
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s) {
-    if (dt != 1) return cudaErrorNotSupported;
+    if (dt == 0) return gemm32_adj_launch(Fhat, Dhat, Xhat_out, g, s);
     const c128* F = static_cast<const c128*>(Fhat);
     const c128* D = static_cast<const c128*>(Dhat);
     c128* X = static_cast<c128*>(Xhat_out);

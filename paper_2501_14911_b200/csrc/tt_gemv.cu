@@ -161,7 +161,7 @@ template <typename R>
 static cudaError_t fwd_dispatch(const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,
                                 cudaStream_t s) {
     constexpr int UN = 8;
-    const int NW = fwd_warps(g.N_d);
+    const int NW = g_fwd_warps ? g_fwd_warps : g.warps ? g.warps : fwd_warps(g.N_d);
     auto k = gemv_fwd_kernel<R, UN>;
     const size_t smem = (size_t)g.chunk * sizeof(Cx<R>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -73,6 +73,7 @@ struct GemvGeom {
     long long ldp;  // padded N_m (multiple of 16 elements)
     int chunk;      // forward: elements of p per CTA (multiple of 64)
     int n_chunks;
+    int warps;      // forward: warps per CTA (0 = kernel default)
 };
 void gemv_debug_set(int fwd_warps, int adj_threads);  // -1 = leave, 0 = planner's choice
 cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,
@@ -93,6 +94,12 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
                             cudaStream_t s);
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s);
+
+// complex64 FMA GEMMs of TT_F32 plans (tt_gemm32.cu); N_d <= kGemm32MaxNd for the adjoint (Dhat_w lives in shared memory)
+constexpr int kGemm32MaxNd = 768;
+cudaError_t gemm32_fwd_launch(const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g, cudaStream_t s);
+cudaError_t gemm32_adj_launch(const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g, cudaStream_t s);
+void gemm32_debug_set(int fwd_variant);
 
 // Triangular solves with the rescaled Cholesky factor (tt_trsv.cu).
 constexpr int kTrsvNB = 64;  // block order

@@ -251,6 +251,29 @@ def test_dmma_gemm_path_shapes(tt, N_d, N_m, N_t, k):
     assert rel(gd[..., 1], one_d) <= 1e-13 and rel(gm[..., 1], one_m) <= 1e-13
 
 
+@pytest.mark.parametrize("N_d,N_m,N_t,k", [(70, 5000, 16, 5), (130, 4500, 12, 33), (64, 8192, 64, 32), (49, 2049, 20, 32),
+                                            (9, 257, 20, 17), (3, 31, 6, 40), (200, 700, 8, 7), (16, 3001, 10, 2)])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_fp32_gemm_path_shapes(tt, N_d, N_m, N_t, k, layout):
+    """fp32 k-RHS path (batched FFTs + per-frequency complex64 FMA GEMMs, tt_gemm32.cu): every sensor-tile variant
+    (N_d <= 32, <= 64, > 64, > 128), ragged tiles, several p-splits, odd N_m, odd k, k > 32, both layouts."""
+    w = workload("C4", N_d, N_m, N_t, torch.float32)
+    F = synth.block_column(w)
+    M = synth.vector_m(w, k_rhs=k)
+    D = synth.vector_d(w, k_rhs=k)
+    lay = (lambda t: t.permute(2, 1, 0).contiguous()) if layout == 1 else (lambda t: t)
+    unlay = (lambda t: t.permute(2, 1, 0)) if layout == 1 else (lambda t: t)
+    plan = tt.Plan(F.cuda(), layout=layout, k_max=k)
+    try:
+        gd = unlay(plan.matvec_batched(lay(M).cuda())).cpu().numpy()
+        gm = unlay(plan.rmatvec_batched(lay(D).cuda())).cpu().numpy()
+    finally:
+        plan.close()
+    for r in sorted({0, 1, k // 2, k - 1}):
+        assert rel(gd[..., r], ob.matvec(F.numpy(), M[..., r].contiguous().numpy())) <= 1e-5
+        assert rel(gm[..., r], ob.rmatvec(F.numpy(), D[..., r].contiguous().numpy())) <= 1e-5
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
 def test_space_major_layout(tt, dtype):
     """TT_SPACE_MAJOR (time contiguous, the 'm (64x32)' shapes of BASELINE.json) gives the same numbers."""
