@@ -33,7 +33,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 constexpr int KP = 32;        // forward: parameters per pipeline stage
 constexpr int AP = KP + 2;    // A-tile pitch in complex elements (272 B: 16-byte aligned rows, skewed banks)
-constexpr int NC = 32;        // columns per launch (8 column groups of 4)
+constexpr int NC = 32;        // columns per launch: NCG = 8 column groups of 4 (NCG = 4 when only <= 16 are left)
 
 // ---------------------------------------------------------------------------------------
 // forward: partial[((w*nsplit + c)*N_d + s)*k + r0 + r] = sum_{p in split c} Fhat_w[s,p] Xhat_w[p, r0 + r]
@@ -41,16 +41,16 @@ constexpr int NC = 32;        // columns per launch (8 column groups of 4)
 // sensors (ty, ty + TY, ...) x 4 columns.  Shared-memory bandwidth bounds this kernel (every thread re-reads its
 // 4 columns of the Xhat tile per parameter), so the sensor tile per thread is made as tall as N_d allows.
 // ---------------------------------------------------------------------------------------
-template <int TS, int TY>
-__global__ void __launch_bounds__(8 * TY)
+template <int TS, int TY, int NCG>
+__global__ void __launch_bounds__(NCG * TY)
 gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c64* __restrict__ partial,
                   const GemmGeom g, const int r0, const int kk) {
-    constexpr int ROWS = TY * TS, NT = 8 * TY;
+    constexpr int ROWS = TY * TS, NT = NCG * TY, NCW = 4 * NCG;   // NCW = columns of the Xhat tile
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c64* As = reinterpret_cast<c64*>(smem_raw);          // [2][ROWS][AP]
-    c64* Bs = As + 2 * ROWS * AP;                         // [2][KP][NC]
+    c64* Bs = As + 2 * ROWS * AP;                         // [2][KP][NCW]
 
-    const int tid = threadIdx.x, tx = tid & 7, ty = tid >> 3;
+    const int tid = threadIdx.x, tx = tid % NCG, ty = tid / NCG;
     const int w = blockIdx.y, c = blockIdx.x, s0 = blockIdx.z * ROWS;
     const long long p_lo = (long long)c * g.p_per_split;
     long long p_hi = p_lo + g.p_per_split;
@@ -68,12 +68,12 @@ gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c6
             const bool ok = (s0 + row < g.N_d) && (p0 + col < p_hi);
             cp_async16(a + row * AP + col, ok ? Abase + (long long)row * g.ldp + p0 + col : Abase, ok);
         }
-        c64* b = Bs + st * KP * NC;
+        c64* b = Bs + st * KP * NCW;
 #pragma unroll
-        for (int i = 0; i < (KP * NC) / NT; ++i) {              // 8-byte chunks: rows of Xhat_w need not be 16-byte aligned
-            const int e = i * NT + tid, row = e / NC, col = e % NC;
+        for (int i = 0; i < (KP * NCW) / NT; ++i) {             // 8-byte chunks: rows of Xhat_w need not be 16-byte aligned
+            const int e = i * NT + tid, row = e / NCW, col = e % NCW;
             const bool ok = (p0 + row < p_hi) && (col < kk);
-            cp_async8(b + row * NC + col, ok ? Bbase + (p0 + row) * (long long)g.k + col : Bbase, ok);
+            cp_async8(b + row * NCW + col, ok ? Bbase + (p0 + row) * (long long)g.k + col : Bbase, ok);
         }
     };
 
@@ -91,10 +91,10 @@ gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c6
         if (it + 1 < n_it) load_stage((it + 1) & 1, it + 1);
         cp_async_commit();
         const c64* a = As + (it & 1) * ROWS * AP + ty * AP;
-        const float4* b = reinterpret_cast<const float4*>(Bs + (it & 1) * KP * NC + 4 * tx);
+        const float4* b = reinterpret_cast<const float4*>(Bs + (it & 1) * KP * NCW + 4 * tx);
 #pragma unroll 8
         for (int p = 0; p < KP; ++p) {
-            const float4 b01 = b[p * (NC / 2)], b23 = b[p * (NC / 2) + 1];
+            const float4 b01 = b[p * (NCW / 2)], b23 = b[p * (NCW / 2) + 1];
             const c64 bv[4] = {mk<float>(b01.x, b01.y), mk<float>(b01.z, b01.w), mk<float>(b23.x, b23.y),
                                mk<float>(b23.z, b23.w)};
 #pragma unroll
@@ -123,24 +123,25 @@ gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c6
 // Fhat_w rows (2 KB contiguous per sensor) go through a 2-stage cp.async pipeline, KS sensors per stage.
 // ---------------------------------------------------------------------------------------
 constexpr int KS = 8;
-constexpr int PT = 256;
 
+template <int NCG>
 __global__ void __launch_bounds__(256, 2)
 gemm32_adj_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Dhat, c64* __restrict__ Xout,
                   const GemmGeom g, const int r0, const int kk) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int PT = 8 * (256 / NCG), NCW = 4 * NCG;    // parameters per CTA, columns of the Dhat tile
     c64* As = reinterpret_cast<c64*>(smem_raw);          // [2][KS][PT]
-    c64* Ds = As + 2 * KS * PT;                           // [N_d][NC]
+    c64* Ds = As + 2 * KS * PT;                           // [N_d][NCW]
 
-    const int tid = threadIdx.x, tx = tid & 7, ty = tid >> 3;
+    const int tid = threadIdx.x, tx = tid % NCG, ty = tid / NCG;
     const int w = blockIdx.y;
     const long long p0 = (long long)blockIdx.x * PT;
     const c64* Abase = Fhat + (long long)w * g.N_d * g.ldp + p0;
     const c64* Dbase = Dhat + (long long)w * g.N_d * g.k + r0;
     const int n_it = (g.N_d + KS - 1) / KS;
 
-    for (int e = tid; e < g.N_d * NC; e += 256) {
-        const int s = e / NC, col = e % NC;
+    for (int e = tid; e < g.N_d * NCW; e += 256) {
+        const int s = e / NCW, col = e % NCW;
         Ds[e] = col < kk ? Dbase[(long long)s * g.k + col] : mk<float>(0.f, 0.f);
     }
     auto load_stage = [&](int st, int it) {
@@ -168,11 +169,11 @@ gemm32_adj_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Dhat, c6
         if (it + 1 < n_it) load_stage((it + 1) & 1, it + 1);
         cp_async_commit();
         const float4* a = reinterpret_cast<const float4*>(As + (it & 1) * KS * PT + ty * 8);
-        const float4* d = reinterpret_cast<const float4*>(Ds + (it * KS) * NC + 4 * tx);
+        const float4* d = reinterpret_cast<const float4*>(Ds + (it * KS) * NCW + 4 * tx);
 #pragma unroll
         for (int sl = 0; sl < KS; ++sl) {                  // rows beyond N_d are zero-filled tiles: they add nothing
             if (it * KS + sl >= g.N_d) break;
-            const float4 d01 = d[sl * (NC / 2)], d23 = d[sl * (NC / 2) + 1];
+            const float4 d01 = d[sl * (NCW / 2)], d23 = d[sl * (NCW / 2) + 1];
             const c64 dv[4] = {mk<float>(d01.x, d01.y), mk<float>(d01.z, d01.w), mk<float>(d23.x, d23.y),
                                mk<float>(d23.z, d23.w)};
 #pragma unroll
@@ -198,14 +199,14 @@ gemm32_adj_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Dhat, c6
     }
 }
 
-template <int TS, int TY>
+template <int TS, int TY, int NCG = 8>
 cudaError_t fwd32_launch(const c64* F, const c64* X, c64* P, const GemmGeom& g, int r0, int kk, cudaStream_t s) {
-    auto k = gemm32_fwd_kernel<TS, TY>;
-    const size_t smem = sizeof(c64) * (2 * TY * TS * AP + 2 * KP * NC);
+    auto k = gemm32_fwd_kernel<TS, TY, NCG>;
+    const size_t smem = sizeof(c64) * (2 * TY * TS * AP + 2 * KP * 4 * NCG);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + TY * TS - 1) / (TY * TS)));
-    k<<<grid, 8 * TY, smem, s>>>(F, X, P, g, r0, kk);
+    k<<<grid, NCG * TY, smem, s>>>(F, X, P, g, r0, kk);
     return cudaGetLastError();
 }
 
@@ -220,7 +221,11 @@ cudaError_t gemm32_fwd_launch(const void* Fhat, const void* Xhat, void* partial,
     for (int r0 = 0; r0 < g.k; r0 += NC) {
         const int kk = g.k - r0 < NC ? g.k - r0 : NC;
         cudaError_t e;
-        if (g_fwd_variant == 1) e = g.N_d <= 32 ? fwd32_launch<1, 32>(F, X, P, g, r0, kk, s)
+        if (kk <= 16 && g_fwd_variant == 0)   // half-width tile: 4 column groups, twice the sensor rows per CTA
+            e = g.N_d <= 32 ? fwd32_launch<2, 16, 4>(F, X, P, g, r0, kk, s)
+              : g.N_d <= 64 ? fwd32_launch<4, 16, 4>(F, X, P, g, r0, kk, s)
+                            : fwd32_launch<8, 16, 4>(F, X, P, g, r0, kk, s);
+        else if (g_fwd_variant == 1) e = g.N_d <= 32 ? fwd32_launch<1, 32>(F, X, P, g, r0, kk, s)
                                   : g.N_d <= 64 ? fwd32_launch<2, 32>(F, X, P, g, r0, kk, s)
                                                 : fwd32_launch<4, 32>(F, X, P, g, r0, kk, s);
         else if (g_fwd_variant == 2) e = g.N_d <= 32 ? fwd32_launch<4, 8>(F, X, P, g, r0, kk, s)
@@ -235,15 +240,18 @@ cudaError_t gemm32_fwd_launch(const void* Fhat, const void* Xhat, void* partial,
 }
 
 cudaError_t gemm32_adj_launch(const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g, cudaStream_t s) {
-    const size_t smem = sizeof(c64) * (2 * KS * PT + (size_t)g.N_d * NC);
-    if (smem > (size_t)kMaxSmem) return cudaErrorInvalidValue;   // N_d > ~770: callers fall back to the per-column path
-    cudaError_t e = cudaFuncSetAttribute(gemm32_adj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)((g.ldp + PT - 1) / PT), (unsigned)g.n_f);
     for (int r0 = 0; r0 < g.k; r0 += NC) {
         const int kk = g.k - r0 < NC ? g.k - r0 : NC;
-        gemm32_adj_kernel<<<grid, 256, smem, s>>>(static_cast<const c64*>(Fhat), static_cast<const c64*>(Dhat),
-                                                  static_cast<c64*>(Xhat_out), g, r0, kk);
+        const int ncg = kk <= 16 ? 4 : 8;
+        const int PT = 8 * (256 / ncg);
+        const size_t smem = sizeof(c64) * (2 * KS * PT + (size_t)g.N_d * 4 * ncg);
+        if (smem > (size_t)kMaxSmem) return cudaErrorInvalidValue;   // N_d > kGemm32MaxNd: callers use the per-column path
+        auto k = ncg == 4 ? gemm32_adj_kernel<4> : gemm32_adj_kernel<8>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        dim3 grid((unsigned)((g.ldp + PT - 1) / PT), (unsigned)g.n_f);
+        k<<<grid, 256, smem, s>>>(static_cast<const c64*>(Fhat), static_cast<const c64*>(Dhat),
+                                  static_cast<c64*>(Xhat_out), g, r0, kk);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
