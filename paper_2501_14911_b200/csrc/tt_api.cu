@@ -744,6 +744,7 @@ int tt_debug_set(const char* key, int value) {
         return TT_OK;
     }
     if (!std::strcmp(key, "fft_max_radix")) { g_fft_max_radix = value; return TT_OK; }
+    if (!std::strcmp(key, "fft_no_static")) { fft_debug_no_static(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }

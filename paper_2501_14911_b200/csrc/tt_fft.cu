@@ -141,14 +141,17 @@ __device__ __forceinline__ void butterfly(Cx<R> (&x)[RAD]) {
 
 // One decimation-in-frequency pass on every length-Ns block of the N-point array:
 //   y_q[j] = w_Ns^{j q} * sum_a x[j + a M] w_R^{a q},  M = Ns/R,  stored in place at j + q M.
-template <typename R, int T, int RAD>
+// STATIC: N, Ns, M are literals at the call site (this function is inlined), so every stride, bound and division
+// below folds to a constant - the planner's common lengths take this route (see fft_inplace).
+template <typename R, int T, int RAD, bool STATIC = false>
 __device__ __forceinline__ void fft_stage(Cx<R>* __restrict__ sm, const Cx<R>* __restrict__ tw, int N, int Ns,
                                           int M, unsigned magic, int lane_s, int g, int G) {
     const int nb = N / RAD;
     const int tws = (N / Ns) * 2;  // w_Ns = w_L^(2N/Ns)
     const int MT = M * T;
+#pragma unroll 1   // one butterfly's registers at a time (the static variants would otherwise unroll this loop)
     for (int u = g; u < nb; u += G) {
-        const int blk = M == 1 ? u : (int)__umulhi((unsigned)u, magic);  // u / M
+        const int blk = M == 1 ? u : STATIC ? u / M : (int)__umulhi((unsigned)u, magic);  // u / M
         const int j = u - blk * M;
         Cx<R>* p = sm + (blk * Ns + j) * T + lane_s;
         Cx<R> x[RAD];
@@ -169,10 +172,35 @@ __device__ __forceinline__ void fft_stage(Cx<R>* __restrict__ sm, const Cx<R>* _
 // kernels stop at radix 8 so that they stay near 64 registers and four CTAs fit one SM.
 template <typename R> struct MaxRadix { static constexpr int value = sizeof(R) == 4 ? 25 : 8; };
 
-template <typename R, int T>
+// Lengths with a fully static kernel variant (NS template parameter), and their radices - which must be the
+// planner's own sequence for that length (tt_api.cu factorise(): largest butterflies first), because the `pos`
+// table is built from it; the host only picks a static variant when the plan's radices match.
+template <typename R, int NS> struct StaticPlan { static constexpr int r1 = 0, r2 = 0, r3 = 0; };
+template <> struct StaticPlan<float, 400> { static constexpr int r1 = 25, r2 = 16, r3 = 1; };
+template <> struct StaticPlan<float, 500> { static constexpr int r1 = 25, r2 = 20, r3 = 1; };
+template <> struct StaticPlan<float, 256> { static constexpr int r1 = 16, r2 = 16, r3 = 1; };
+template <> struct StaticPlan<double, 512> { static constexpr int r1 = 8, r2 = 8, r3 = 8; };
+template <> struct StaticPlan<double, 256> { static constexpr int r1 = 8, r2 = 8, r3 = 4; };
+
+template <typename R, int T, int NS = 0>
 __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int lane_s, int g, int G) {
     constexpr int MAXR = MaxRadix<R>::value;
     const Cx<R>* tw = reinterpret_cast<const Cx<R>*>(P.tw);
+    if constexpr (NS != 0) {
+        using SP = StaticPlan<R, NS>;
+        constexpr int R1 = SP::r1, R2 = SP::r2, R3 = SP::r3;
+        static_assert(R1 * R2 * R3 == NS, "static FFT plan does not match its length");
+        __syncthreads();
+        fft_stage<R, T, R1, true>(sm, tw, NS, NS, NS / R1, 0u, lane_s, g, G);
+        __syncthreads();
+        fft_stage<R, T, R2, true>(sm, tw, NS, NS / R1, NS / (R1 * R2), 0u, lane_s, g, G);
+        if constexpr (R3 > 1) {
+            __syncthreads();
+            fft_stage<R, T, R3, true>(sm, tw, NS, R3, 1, 0u, lane_s, g, G);
+        }
+        __syncthreads();
+        return;
+    }
     int Ns = P.N;
     for (int st = 0; st < P.n_stages; ++st) {
         __syncthreads();
@@ -202,8 +230,9 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
 // ---------------------------------------------------------------------------------------
 // forward: zero-pad + real-to-complex FFT + frequency-major store          (P0, A1, B1)
 // ---------------------------------------------------------------------------------------
-template <typename Tin, typename Tc, typename Tout, int T, int NT>
-__global__ void __launch_bounds__(NT)
+// The static 400/500 variants are held to the register budget of three resident CTAs (measured best on B200).
+template <typename Tin, typename Tc, typename Tout, int T, int NT, int NS = 0>
+__global__ void __launch_bounds__(NT, (NS == 400 || NS == 500) ? 3 : 0)
 fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
@@ -211,7 +240,7 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
     const int lane_s = threadIdx.x % T, g = threadIdx.x / T;
     const long long b = (long long)blockIdx.x * T + lane_s;
     const bool live = b < P.B;
-    const int N = P.N;
+    const int N = NS ? NS : P.N;
     const Tin* src = in + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
     const int dec = P.dec;
     auto ld_real = [&](int j) -> Tin {   // time step j of the series; on a coarser grid only every dec-th step exists
@@ -241,7 +270,7 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
         }
     }
     for (int n = nh + g; n < N; n += G) sm[n * T + lane_s] = mk<Tc>(Tc(0), Tc(0));
-    fft_inplace<Tc, T>(sm, P, lane_s, g, G);
+    fft_inplace<Tc, T, NS>(sm, P, lane_s, g, G);
 
     const Cx<Tc>* tw = reinterpret_cast<const Cx<Tc>*>(P.tw);
     Cx<Tout>* dst = out + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
@@ -265,8 +294,8 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
 // ---------------------------------------------------------------------------------------
 // inverse: complex-to-real inverse FFT + truncate + scale                               (A3, B3)
 // ---------------------------------------------------------------------------------------
-template <typename Tc, int T, int NT>
-__global__ void __launch_bounds__(NT)
+template <typename Tc, int T, int NT, int NS = 0>
+__global__ void __launch_bounds__(NT, (NS == 400 || NS == 500) ? 3 : 0)
 fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
@@ -274,7 +303,7 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
     const int lane_s = threadIdx.x % T, g = threadIdx.x / T;
     const long long b = (long long)blockIdx.x * T + lane_s;
     const bool live = b < P.B;
-    const int N = P.N;
+    const int N = NS ? NS : P.N;
     const Cx<Tc>* src = in + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
 
     constexpr int UB = 8;
@@ -312,7 +341,7 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
             sm[k * T + lane_s] = conj(Zk);
         }
     }
-    fft_inplace<Tc, T>(sm, P, lane_s, g, G);
+    fft_inplace<Tc, T, NS>(sm, P, lane_s, g, G);
 
     // conj(result)_n = z_n * N:  x_{2n} = Re z_n, x_{2n+1} = Im z_n; keep j < N_t (truncation)
     if (live) {
@@ -372,7 +401,8 @@ cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int 
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
-static int g_force_T = 0, g_force_NT = 0;
+static int g_force_T = 0, g_force_NT = 0, g_no_static = 0;
+void fft_debug_no_static(int v) { g_no_static = v; }
 void fft_debug_force_T(int T) { g_force_T = T; }
 void fft_debug_force_threads(int NT) { g_force_NT = NT; }
 
@@ -393,6 +423,20 @@ FftChoice fft_choose(int N, size_t elem) {
     return c;
 }
 
+// The static variant for this plan, or 0: T = 16 / 256 threads only (the planner's choice for these lengths), and the
+// plan's radices must be the ones compiled in.
+template <typename Tc>
+static int static_length(const FftParams& P, const FftChoice& c, int nt) {
+    if (g_no_static > 0 || c.T != 16 || nt != 256) return 0;
+    auto is = [&](int n, int r1, int r2, int r3) {
+        return P.N == n && P.n_stages == (r3 > 1 ? 3 : 2) && P.radix[0] == r1 && P.radix[1] == r2 &&
+               (r3 == 1 || P.radix[2] == r3);
+    };
+    // (the 500 = 25 x 20 variant needs ~130 registers - it spills under the three-CTA budget and was measured slower)
+    if (sizeof(Tc) == 4) return is(400, 25, 16, 1) ? 400 : g_no_static == -1 && is(500, 25, 20, 1) ? 500 : is(256, 16, 16, 1) ? 256 : 0;
+    return is(512, 8, 8, 8) ? 512 : is(256, 8, 8, 4) ? 256 : 0;
+}
+
 template <typename Tin, typename Tc, typename Tout>
 static cudaError_t r2c_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
@@ -400,15 +444,20 @@ static cudaError_t r2c_dispatch(const void* in, void* out, const FftParams& P, i
     const int nt = g_force_NT ? g_force_NT : 256;
     const long long nb = (P.B_store > P.B ? P.B_store : P.B);
     dim3 grid((unsigned)((nb + c.T - 1) / c.T), (unsigned)ny);
-#define TT_R2C(TT, NT)                                                                                       \
+#define TT_R2C(TT, NT, ...)                                                                                  \
     {                                                                                                        \
-        auto k = fft_r2c_kernel<Tin, Tc, Tout, TT, NT>;                                                      \
+        auto k = fft_r2c_kernel<Tin, Tc, Tout, TT, NT, ##__VA_ARGS__>;                                                    \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Tin*>(in), static_cast<Cx<Tout>*>(out), P);             \
     }
-    if (nt == 512) { if (c.T == 32) TT_R2C(32, 512) else if (c.T == 16) TT_R2C(16, 512) else TT_R2C(8, 512) }
-    else           { if (c.T == 32) TT_R2C(32, 256) else if (c.T == 16) TT_R2C(16, 256) else TT_R2C(8, 256) }
+    const int ns = static_length<Tc>(P, c, nt);
+    if (ns) {
+        if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_R2C(16, 256, 400) else if (ns == 500) TT_R2C(16, 256, 500) else TT_R2C(16, 256, 256) }
+        else                           { if (ns == 512) TT_R2C(16, 256, 512) else TT_R2C(16, 256, 256) }
+    }
+    else if (nt == 512) { if (c.T == 32) TT_R2C(32, 512) else if (c.T == 16) TT_R2C(16, 512) else TT_R2C(8, 512) }
+    else                { if (c.T == 32) TT_R2C(32, 256) else if (c.T == 16) TT_R2C(16, 256) else TT_R2C(8, 256) }
 #undef TT_R2C
     return cudaGetLastError();
 }
@@ -427,15 +476,20 @@ static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, i
     if (c.T == 0) return cudaErrorInvalidValue;
     const int nt = g_force_NT ? g_force_NT : 256;
     dim3 grid((unsigned)((P.B + c.T - 1) / c.T), (unsigned)ny);
-#define TT_C2R(TT, NT)                                                                                       \
+#define TT_C2R(TT, NT, ...)                                                                                  \
     {                                                                                                        \
-        auto k = fft_c2r_kernel<Tc, TT, NT>;                                                                 \
+        auto k = fft_c2r_kernel<Tc, TT, NT, ##__VA_ARGS__>;                                                               \
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P);                \
     }
-    if (nt == 512) { if (c.T == 32) TT_C2R(32, 512) else if (c.T == 16) TT_C2R(16, 512) else TT_C2R(8, 512) }
-    else           { if (c.T == 32) TT_C2R(32, 256) else if (c.T == 16) TT_C2R(16, 256) else TT_C2R(8, 256) }
+    const int ns = static_length<Tc>(P, c, nt);
+    if (ns) {
+        if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_C2R(16, 256, 400) else if (ns == 500) TT_C2R(16, 256, 500) else TT_C2R(16, 256, 256) }
+        else                           { if (ns == 512) TT_C2R(16, 256, 512) else TT_C2R(16, 256, 256) }
+    }
+    else if (nt == 512) { if (c.T == 32) TT_C2R(32, 512) else if (c.T == 16) TT_C2R(16, 512) else TT_C2R(8, 512) }
+    else                { if (c.T == 32) TT_C2R(32, 256) else if (c.T == 16) TT_C2R(16, 256) else TT_C2R(8, 256) }
 #undef TT_C2R
     return cudaGetLastError();
 }

@@ -62,6 +62,7 @@ cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int 
                                    cudaStream_t s);
 void fft_debug_force_T(int T);  // 0 = planner's choice
 void fft_debug_force_threads(int NT);  // 256 or 512; 0 = default (512 for fp32, 256 for fp64)
+void fft_debug_no_static(int v);  // 1 = never use the statically specialised FFT variants
 double debug_cos2pi(long long k, long long n);
 double debug_sin2pi(long long k, long long n);
 

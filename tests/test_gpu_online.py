@@ -200,3 +200,49 @@ def test_map_mismatch_errors(tt):
             tt.assemble_K(pF, pG, nv.cuda())
     finally:
         chol.close(); pF.close(); pG.close()
+
+
+def _guarded(shape, dtype):
+    """An output tensor surrounded by 4096-element canary zones (compute-sanitizer is not available on the pool)."""
+    n = int(np.prod(shape))
+    buf = torch.full((n + 8192,), -7.0, dtype=dtype, device="cuda")
+    return buf, buf[4096:4096 + n].view(shape)
+
+
+def test_outputs_stay_inside_their_buffers(tt):
+    """Every kernel that writes a caller's vector, at ragged shapes: the bytes before and after the output are untouched."""
+    for dtype in (torch.float32, torch.float64):
+        N_d, N_m, N_t, k = 5, 1001, 35, 7
+        w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
+        F = synth.block_column(w)
+        G = synth.gstar_block_column(w, F)
+        nv = synth.noise_var(w)
+        L = oo.cholesky(oo.assemble_K(F.numpy(), G.numpy(), nv.numpy()))
+        pF, pG = tt.Plan(F.cuda(), k_max=k), tt.Plan(G.cuda(), k_max=k)
+        chol = tt.Chol(torch.from_numpy(L).cuda())
+        mp = tt.MapInference(pF, pG, chol, nv.cuda())
+        bufs = []
+        try:
+            m, d = synth.vector_m(w, k_rhs=1).cuda(), synth.vector_d(w, k_rhs=1).cuda()
+            M, D = synth.vector_m(w, k_rhs=k).cuda(), synth.vector_d(w, k_rhs=k).cuda()
+            for shape, call in (((N_t, N_d), lambda o: tt.tt_matvec(pF.handle, m, o)),
+                                ((N_t, N_m), lambda o: tt.tt_rmatvec(pF.handle, d, o)),
+                                ((N_t, N_m), lambda o: tt.tt_normal(pF.handle, m, o)),
+                                ((N_t, N_d, k), lambda o: tt.tt_matvec_batched(pF.handle, k, M, o)),
+                                ((N_t, N_m, k), lambda o: tt.tt_rmatvec_batched(pF.handle, k, D, o)),
+                                ((N_t, N_m), lambda o: tt.tt_map_infer(mp.handle, tt.TT_MAP_PAPER, d, o)),
+                                ((N_t, N_m), lambda o: tt.tt_map_infer(mp.handle, tt.TT_MAP_GAIN, d, o))):
+                buf, out = _guarded(shape, dtype)
+                call(out)
+                bufs.append((buf, out.numel()))
+            b64 = torch.randn(N_d * N_t, dtype=torch.float64, device="cuda")
+            for tr in (None, False, True):
+                buf, out = _guarded((N_d * N_t,), torch.float64)
+                tt.tt_chol_solve(chol.handle, b64, out) if tr is None else tt.tt_chol_trsv(chol.handle, tr, b64, out)
+                bufs.append((buf, out.numel()))
+            torch.cuda.synchronize()
+        finally:
+            mp.close(); chol.close(); pF.close(); pG.close()
+        for buf, n in bufs:
+            assert (buf[:4096] == -7.0).all() and (buf[4096 + n:] == -7.0).all()
+            assert torch.isfinite(buf[4096:4096 + n]).all()
