@@ -284,6 +284,16 @@ void tt_map_destroy(tt_map* m);
  * and layout).  Asynchronous on `stream`.  The K-solve runs in fp64 whatever the plans' dtype. */
 int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void* stream);
 
+/* eq (4.13) in two halves, split at the one exchange step of the N_m-sharded path (DESIGN.md section 6 / 11):
+ *   tt_map_infer_partial:  y = Gamma_noise^{-1} d_obs (kept in the tt_map), a = G* y -> a_scratch (N_t*N_m reals),
+ *                          b = F a -> b (N_t*N_d reals).  On a rank that holds a parameter slice, b is its PARTIAL
+ *                          data vector: all-reduce (sum) it over the ranks before the second half.
+ *   tt_map_infer_finish:   c = K^{-1} b, m_map = G* (y - c), with the y of the preceding tt_map_infer_partial.
+ *                          m_map may be the a_scratch of the first half.
+ * tt_map_infer(TT_MAP_PAPER) is exactly these two calls back to back.  All pointers DEVICE, plans' dtype and layout. */
+int tt_map_infer_partial(const tt_map* m, const void* d_obs, void* a_scratch, void* b, void* stream);
+int tt_map_infer_finish(const tt_map* m, const void* b, void* m_map, void* stream);
+
 /* Same with HOST vectors (pinned memory recommended): d_obs is copied in and m_map copied out on `stream`. */
 int tt_map_infer_host(const tt_map* m, int form, const void* d_obs_host, void* m_map_host, void* stream);
 

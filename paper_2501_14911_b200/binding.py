@@ -86,6 +86,8 @@ def lib() -> ctypes.CDLL:
         "tt_map_destroy": (None, [vp]),
         "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
         "tt_map_infer_host": (ci, [vp, ci, vp, vp, vp]),
+        "tt_map_infer_partial": (ci, [vp, vp, vp, vp, vp]),
+        "tt_map_infer_finish": (ci, [vp, vp, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(L, name)
@@ -101,7 +103,8 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
-           "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host"]
+           "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
+           "tt_map_infer_partial", "tt_map_infer_finish"]
 
 
 def _stream(stream) -> int:
@@ -311,6 +314,14 @@ def tt_map_infer(m: int, form: int, d_obs, m_map, stream=None) -> None:
     _check("tt_map_infer", lib().tt_map_infer(m, form, _ptr(d_obs), _ptr(m_map), _stream(stream)))
 
 
+def tt_map_infer_partial(m: int, d_obs, a_scratch, b, stream=None) -> None:
+    _check("tt_map_infer_partial", lib().tt_map_infer_partial(m, _ptr(d_obs), _ptr(a_scratch), _ptr(b), _stream(stream)))
+
+
+def tt_map_infer_finish(m: int, b, m_map, stream=None) -> None:
+    _check("tt_map_infer_finish", lib().tt_map_infer_finish(m, _ptr(b), _ptr(m_map), _stream(stream)))
+
+
 def tt_map_infer_host(m: int, form: int, d_obs_host, m_map_host, stream=None) -> None:
     _check("tt_map_infer_host", lib().tt_map_infer_host(m, form, _ptr(d_obs_host), _ptr(m_map_host), _stream(stream)))
 
@@ -449,4 +460,14 @@ class MapInference:
     def infer(self, d_obs, form: int = TT_MAP_PAPER, out=None, stream=None):
         out = self.G._out(self.G.N_m) if out is None else out
         tt_map_infer(self.handle, form, d_obs, out, stream)
+        return out
+
+    def infer_partial(self, d_obs, stream=None):
+        """First half of eq (4.13): returns (a_scratch, b); b is this rank's partial F G* y."""
+        a, b = self.G._out(self.G.N_m), self.G._out(self.G.N_d, data=True)
+        tt_map_infer_partial(self.handle, d_obs, a, b, stream)
+        return a, b
+
+    def infer_finish(self, b, out, stream=None):
+        tt_map_infer_finish(self.handle, b, out, stream)
         return out

@@ -170,27 +170,41 @@ int assemble_K_typed(const tt_plan* F, const tt_plan* G, const PlanInfo& pi, con
     return rc;
 }
 
+// eq (4.13) in two halves, split where the N_m-sharded path has its one exchange step (the all-reduce of b = F a):
+//   partial:  y = Gamma_noise^{-1} d_obs (kept in the tt_map),  a = G* y,  b = F a
+//   finish :  c = K^{-1} b,  z = y - c,  m_map = G* z
 template <typename T>
-int map_infer_typed(const tt_map* m, int form, const T* d_obs, T* m_map, cudaStream_t s) {
+int map_partial_typed(const tt_map* m, const T* d_obs, T* a, T* b, cudaStream_t s) {
+    const long long n = m->pi.N_d * m->pi.N_t;
+    T* yv = static_cast<T*>(m->yv);
+    mul_kernel<T><<<nblocks(n), 256, 0, s>>>(d_obs, static_cast<const T*>(m->inv_nv), yv, n);      // y = Gamma_noise^{-1} d_obs
+    TTO_CUDA(m, cudaGetLastError());
+    int rc;
+    if ((rc = tt_rmatvec(m->G, yv, a, s)) != TT_OK) return rc;                                      // a = G* y
+    return tt_matvec(m->F, a, b, s);                                                                // b = F a
+}
+
+template <typename T>
+int map_finish_typed(const tt_map* m, const T* y /* nullptr: gain form, z = K^{-1} b */, const T* b, T* m_map,
+                     cudaStream_t s) {
     const PlanInfo& pi = m->pi;
     const long long n = pi.N_d * pi.N_t;
-    T* yv = static_cast<T*>(m->yv);
     T* dv = static_cast<T*>(m->dv);
+    to_k_kernel<T><<<nblocks(n), 256, 0, s>>>(b, m->k64, pi.N_d, pi.N_t, pi.layout);
     int rc;
-    if (form == TT_MAP_PAPER) {
-        mul_kernel<T><<<nblocks(n), 256, 0, s>>>(d_obs, static_cast<const T*>(m->inv_nv), yv, n);  // y = Gamma_noise^{-1} d_obs
-        if ((rc = tt_rmatvec(m->G, yv, m_map, s)) != TT_OK) return rc;                              // a = G* y
-        if ((rc = tt_matvec(m->F, m_map, dv, s)) != TT_OK) return rc;                               // b = F a
-        to_k_kernel<T><<<nblocks(n), 256, 0, s>>>(dv, m->k64, pi.N_d, pi.N_t, pi.layout);
-        if ((rc = tt_chol_solve(m->K, m->k64, m->k64, s)) != TT_OK) return rc;                      // c = K^{-1} b
-        from_k_kernel<T><<<nblocks(n), 256, 0, s>>>(yv, m->k64, dv, pi.N_d, pi.N_t, pi.layout);     // z = y - c
-    } else {
-        to_k_kernel<T><<<nblocks(n), 256, 0, s>>>(d_obs, m->k64, pi.N_d, pi.N_t, pi.layout);
-        if ((rc = tt_chol_solve(m->K, m->k64, m->k64, s)) != TT_OK) return rc;                      // z = K^{-1} d_obs
-        from_k_kernel<T><<<nblocks(n), 256, 0, s>>>(static_cast<const T*>(nullptr), m->k64, dv, pi.N_d, pi.N_t, pi.layout);
-    }
+    if ((rc = tt_chol_solve(m->K, m->k64, m->k64, s)) != TT_OK) return rc;                          // c = K^{-1} b
+    from_k_kernel<T><<<nblocks(n), 256, 0, s>>>(y, m->k64, dv, pi.N_d, pi.N_t, pi.layout);          // z = y - c  (or c)
     TTO_CUDA(m, cudaGetLastError());
     return tt_rmatvec(m->G, dv, m_map, s);                                                          // m_map = G* z
+}
+
+template <typename T>
+int map_infer_typed(const tt_map* m, int form, const T* d_obs, T* m_map, cudaStream_t s) {
+    if (form == TT_MAP_GAIN) return map_finish_typed<T>(m, nullptr, d_obs, m_map, s);               // G* K^{-1} d_obs
+    T* dv = static_cast<T*>(m->dv);
+    const int rc = map_partial_typed<T>(m, d_obs, m_map, dv, s);                                    // a lives in m_map
+    if (rc != TT_OK) return rc;
+    return map_finish_typed<T>(m, static_cast<const T*>(m->yv), dv, m_map, s);
 }
 
 }  // namespace
@@ -387,6 +401,26 @@ int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void
     if (m->pi.dtype == TT_F32)
         return map_infer_typed<float>(m, form, static_cast<const float*>(d_obs), static_cast<float*>(m_map), s);
     return map_infer_typed<double>(m, form, static_cast<const double*>(d_obs), static_cast<double*>(m_map), s);
+}
+
+int tt_map_infer_partial(const tt_map* m, const void* d_obs, void* a_scratch, void* b, void* stream) {
+    if (!m || !d_obs || !a_scratch || !b || !m->F) return TT_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (m->pi.dtype == TT_F32)
+        return map_partial_typed<float>(m, static_cast<const float*>(d_obs), static_cast<float*>(a_scratch),
+                                        static_cast<float*>(b), s);
+    return map_partial_typed<double>(m, static_cast<const double*>(d_obs), static_cast<double*>(a_scratch),
+                                     static_cast<double*>(b), s);
+}
+
+int tt_map_infer_finish(const tt_map* m, const void* b, void* m_map, void* stream) {
+    if (!m || !b || !m_map) return TT_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (m->pi.dtype == TT_F32)
+        return map_finish_typed<float>(m, static_cast<const float*>(m->yv), static_cast<const float*>(b),
+                                       static_cast<float*>(m_map), s);
+    return map_finish_typed<double>(m, static_cast<const double*>(m->yv), static_cast<const double*>(b),
+                                    static_cast<double*>(m_map), s);
 }
 
 int tt_map_infer_host(const tt_map* cm, int form, const void* d_obs_host, void* m_map_host, void* stream) {

@@ -58,3 +58,45 @@ class ShardedOperator:
 def from_plan(plan, group=None) -> ShardedOperator:
     """Wraps a tt Plan built on this rank's slice F[:, :, p0:p1] of the block column."""
     return ShardedOperator(plan.matvec, plan.rmatvec, group)
+
+
+class ShardedMapInference:
+    """The online MAP point of eq (4.13) with the parameter axis split over the ranks.
+
+    G* and F shard exactly like F^T and F above: G* y needs no collective (every rank owns its slice of the
+    parameter field), b = F G* y is the local partial followed by the ONE all-reduce of the data vector; the
+    data-space steps (Gamma_noise^{-1}, the K-solve with the replicated Cholesky factor) are replicated - they
+    act on n = N_d N_t numbers.  This is what lets the paper's fp64 spectra (2 x 103 GB at its test shape) be
+    held by two or more GPUs.  Like ShardedOperator this class holds none of the method's arithmetic:
+
+      partial(d_obs) -> b_partial      the first half of eq (4.13) on the local slices (tt_map_infer_partial)
+      finish(b)      -> m_map slice    the second half (tt_map_infer_finish)
+      gain(d_obs)    -> m_map slice    G* K^{-1} d_obs (tt_map_infer TT_MAP_GAIN): no collective at all
+    """
+
+    def __init__(self, partial, finish, gain, group=None):
+        self.partial, self.finish, self.gain, self.group = partial, finish, gain, group
+
+    def infer(self, d_obs: torch.Tensor, gain_form: bool = False) -> torch.Tensor:
+        """This rank's slice of m_map."""
+        if gain_form:
+            return self.gain(d_obs)
+        b = self.partial(d_obs)
+        if dist.is_available() and dist.is_initialized() and dist.get_world_size(self.group) > 1:
+            dist.all_reduce(b, op=dist.ReduceOp.SUM, group=self.group)       # the path's only exchange step
+        return self.finish(b)
+
+
+def map_from_binding(mp, group=None) -> ShardedMapInference:
+    """Wraps a binding.MapInference built on this rank's slices of the block columns of F and G*."""
+    from . import binding as tt
+    state = {}
+
+    def partial(d_obs):
+        state["a"], b = mp.infer_partial(d_obs)
+        return b
+
+    def finish(b):
+        return mp.infer_finish(b, state.pop("a"))
+
+    return ShardedMapInference(partial, finish, lambda d: mp.infer(d, tt.TT_MAP_GAIN), group)

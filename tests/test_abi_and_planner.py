@@ -118,3 +118,26 @@ def test_unsupported_nt(tt, N_t):
     with pytest.raises(tt.TTError) as e:
         tt.tt_debug_fft_tables(N_t)
     assert e.value.status == -5
+
+
+def test_online_phase_argument_validation_without_a_gpu(tt):
+    """Host logic of the second half of include/tt.h: shape / NULL checks come before any device work."""
+    import ctypes
+    L = tt.lib()
+    out = ctypes.c_void_p()
+    buf = (ctypes.c_double * 16)()
+    assert tt.tt_status_string(L.tt_chol_create(ctypes.byref(out), 0, buf, 4, None)) == "TT_ERR_SHAPE"
+    assert tt.tt_status_string(L.tt_chol_create(ctypes.byref(out), 4, buf, 3, None)) == "TT_ERR_SHAPE"     # ld < n
+    assert tt.tt_status_string(L.tt_chol_create(ctypes.byref(out), 4, None, 4, None)) == "TT_ERR_NULL"
+    assert tt.tt_status_string(L.tt_chol_create(None, 4, buf, 4, None)) == "TT_ERR_NULL"
+    assert tt.tt_status_string(L.tt_chol_solve(None, buf, buf, None)) == "TT_ERR_NULL"
+    assert tt.tt_status_string(L.tt_map_create(ctypes.byref(out), None, None, None, buf, None)) == "TT_ERR_NULL"
+    assert tt.tt_status_string(L.tt_map_infer(None, 0, buf, buf, None)) == "TT_ERR_NULL"
+    assert tt.tt_status_string(L.tt_assemble_K(None, None, buf, 0, 1, buf, 4, None)) == "TT_ERR_NULL"
+    # coarse output grid: out_every must divide N_t (checked before the device is touched)
+    for bad in (0, 3, 64):
+        st = L.tt_plan_create_coarse(ctypes.byref(out), 2, 8, 32, bad, tt.TT_F64, tt.TT_TIME_MAJOR, 1, buf, None)
+        assert tt.tt_status_string(st) == "TT_ERR_SHAPE"
+    L.tt_chol_destroy(None); L.tt_map_destroy(None)        # NULL-safe
+    assert L.tt_chol_device_bytes(None) == 0
+    assert tt.tt_status_string(-11) == "TT_ERR_NOT_SPD" and tt.tt_status_string(-12) == "TT_ERR_MISMATCH"

@@ -246,3 +246,23 @@ def test_outputs_stay_inside_their_buffers(tt):
         for buf, n in bufs:
             assert (buf[:4096] == -7.0).all() and (buf[4096 + n:] == -7.0).all()
             assert torch.isfinite(buf[4096:4096 + n]).all()
+
+
+def test_map_two_halves_equal_the_whole(tt):
+    """tt_map_infer_partial + tt_map_infer_finish (the split at the sharded path's all-reduce) == tt_map_infer."""
+    from paper_2501_14911_b200 import sharded
+    w, F, G, nv, d_obs = online_inputs(4, 700, 24, torch.float32)
+    L = oo.cholesky(oo.assemble_K(F.numpy(), G.numpy(), nv.numpy()))
+    pF, pG, chol = tt.Plan(F.cuda()), tt.Plan(G.cuda()), tt.Chol(torch.from_numpy(L).cuda())
+    mp = tt.MapInference(pF, pG, chol, nv.cuda())
+    try:
+        whole = mp.infer(d_obs.cuda(), tt.TT_MAP_PAPER).cpu()
+        a, b = mp.infer_partial(d_obs.cuda())
+        halves = mp.infer_finish(b, a).cpu()
+        sm = sharded.map_from_binding(mp)                      # world size 1: no collective
+        via = sm.infer(d_obs.cuda()).cpu()
+        gain = sm.infer(d_obs.cuda(), gain_form=True).cpu()
+        ref_gain = mp.infer(d_obs.cuda(), tt.TT_MAP_GAIN).cpu()
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close()
+    assert torch.equal(whole, halves) and torch.equal(whole, via) and torch.equal(gain, ref_gain)

@@ -46,6 +46,29 @@ def _worker(rank, world, port, out_dir):
         ok = (np.allclose(got_d, ref_d, rtol=0, atol=1e-12 * np.abs(ref_d).max())
               and np.allclose(got_m, ref_m[:, p0:p1], rtol=0, atol=1e-12 * np.abs(ref_m).max())
               and np.allclose(got_n, ref_n[:, p0:p1], rtol=0, atol=1e-11 * np.abs(ref_n).max()))
+        # the online phase (eq 4.13) on the same two ranks: replicated K-solve, sharded G* and F
+        from oracle import online_plain as oo
+        wo = synth.CONFIGS["P5"].scaled(N_d=3, N_m=70, N_t=12, dtype=torch.float64)
+        Fo = synth.block_column(wo)
+        Go = synth.gstar_block_column(wo, Fo).numpy()
+        Fo = Fo.numpy()
+        nv, dob = synth.noise_var(wo).numpy(), synth.vector_d(wo, k_rhs=1).numpy()
+        Lc = oo.cholesky(oo.assemble_K(Fo, Go, nv))
+        m_ref = oo.map_point(Fo, Go, nv, Lc, dob)
+        Fl2, Gl2 = Fo[:, :, p0:p1], Go[:, :, p0:p1]
+        solve = lambda b: oo.chol_solve(Lc, b.reshape(-1)).reshape(b.shape)
+        st = {}
+
+        def partial(dd):                                   # the oracle as the local first half
+            st["y"] = dd.numpy() / nv
+            return torch.from_numpy(op.matvec(Fl2, op.rmatvec(Gl2, st["y"])))
+
+        finish = lambda b: torch.from_numpy(op.rmatvec(Gl2, st["y"] - solve(b.numpy())))
+        gain = lambda dd: torch.from_numpy(op.rmatvec(Gl2, solve(dd.numpy())))
+        smap = sharded.ShardedMapInference(partial, finish, gain)
+        for gain in (False, True):
+            got = smap.infer(torch.from_numpy(dob), gain_form=gain).numpy()
+            ok = ok and np.allclose(got, m_ref[:, p0:p1], rtol=0, atol=1e-10 * np.abs(m_ref).max())
         with open(os.path.join(out_dir, f"rank{rank}.ok"), "w") as f:
             f.write("1" if ok else "0")
     finally:
