@@ -153,9 +153,11 @@ int tt_normal(const tt_plan* plan, const void* m, void* out, void* stream);
 int tt_matvec_batched(const tt_plan* plan, int k, const void* M, void* D, void* stream);
 int tt_rmatvec_batched(const tt_plan* plan, int k, const void* D, void* M, void* stream);
 
-/* Convenience calls with HOST vectors (pinned memory recommended): copy the input to a
- * device staging buffer on `stream`, apply, copy the result back; all asynchronous on
- * `stream` when the host memory is pinned.  The staging buffers are allocated on first
+/* The same calls with HOST vectors (pinned memory recommended; what bench.py's `e2e` times).  The parameter-sized
+ * vector crosses PCIe in 8 ranges of the parameter axis on a copy stream owned by the plan, overlapped with the kernels
+ * of the neighbouring range on `stream` (H2D of range c+1 under the FFT + matvec of range c; D2H of range c under the
+ * matvec + inverse FFT of range c+1); `stream` waits for the last copy, so synchronising it is enough.  Results are
+ * bit-identical to the device-pointer calls.  The staging buffers, the copy stream and its events are created on first
  * use (the only apply-time allocation in the library) and freed with the plan. */
 int tt_matvec_host(const tt_plan* plan, const void* m_host, void* d_host, void* stream);
 int tt_rmatvec_host(const tt_plan* plan, const void* d_host, void* m_host, void* stream);

@@ -18,6 +18,7 @@ namespace {
 constexpr int kVersion = 100;  // 0.1.0
 constexpr int kRing = 64;       // profiled apply calls remembered
 constexpr int kSlotEvents = 8;  // two kernel triples (tt_normal) x 4 marks
+constexpr int kHostChunks = 8;  // parameter ranges of the pipelined *_host calls
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
 int g_gemv_chunk = 0;  // tt_debug_set("gemv_chunk"): 0 = planner's choice
@@ -45,6 +46,8 @@ struct tt_plan {
     void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
     void* d_stage = nullptr;
     void* m_stage2 = nullptr;
+    cudaStream_t copy_stream = nullptr;   // *_host calls: the PCIe copies of the parameter-sized vector run here, chunk by
+    cudaEvent_t cev[kHostChunks + 2] = {};  // chunk over ranges of the parameter axis, overlapped with the kernels (lazily created)
     int chunk = 0, n_chunks = 0, fwd_warps = 0;
     size_t bytes = 0;
     mutable int last_cuda = 0;
@@ -352,18 +355,122 @@ int ensure_staging(const tt_plan* cp) {
         int r = dev_alloc(p, &p->m_stage, (size_t)p->N_t * p->N_m * es);
         if (r) return r;
     }
-    if (!p->m_stage2) {
-        int r = dev_alloc(p, &p->m_stage2, (size_t)p->N_t * p->N_m * es);
+    if (!p->d_stage) {
+        int r = dev_alloc(p, &p->d_stage, (size_t)p->N_td * p->N_d * es);
         if (r) return r;
     }
-    if (!p->d_stage) {
-        int r = dev_alloc(p, &p->d_stage, (size_t)p->N_t * p->N_d * es);
-        if (r) return r;
+    if (!p->copy_stream) {
+        TT_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : p->cev) TT_CUDA(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
     return TT_OK;
 }
 
+// Parameter range c of the pipelined host calls: boundaries on multiples of 4096 (a multiple of the GEMV chunk, of the
+// 512-parameter tile of the adjoint kernel and of the 16-element row pitch), the last range ends at ldp.
+void host_chunk(const tt_plan* p, int c, long long* p0, long long* p1) {
+    long long per = (p->ldp + kHostChunks - 1) / kHostChunks;
+    per = (per + 4095) / 4096 * 4096;
+    *p0 = per * c < p->ldp ? per * c : p->ldp;
+    *p1 = per * (c + 1) < p->ldp ? per * (c + 1) : p->ldp;
+}
+
+// Copy of the parameters [p0, p1) of a parameter-sized vector between host and device staging (either direction).
+cudaError_t copy_m_range(const tt_plan* p, void* dst, const void* src, long long p0, long long p1, cudaMemcpyKind kind,
+                         cudaStream_t s) {
+    const size_t es = esize(p->dtype);
+    if (p1 > p->N_m) p1 = p->N_m;
+    if (p1 <= p0) return cudaSuccess;
+    if (p->layout == TT_SPACE_MAJOR)   // [p][j]: the range is contiguous
+        return cudaMemcpyAsync(static_cast<char*>(dst) + (size_t)p0 * p->N_t * es,
+                               static_cast<const char*>(src) + (size_t)p0 * p->N_t * es, (size_t)(p1 - p0) * p->N_t * es, kind, s);
+    return cudaMemcpy2DAsync(static_cast<char*>(dst) + (size_t)p0 * es, (size_t)p->N_m * es,
+                             static_cast<const char*>(src) + (size_t)p0 * es, (size_t)p->N_m * es, (size_t)(p1 - p0) * es,
+                             (size_t)p->N_t, kind, s);
+}
+
+// d = F m with m on the HOST: the H2D copy of parameter range c+1 (copy stream) overlaps the FFT and the per-frequency
+// matvec of range c (caller's stream); A2 already sums per chunk, so the ranges only restrict its grid.
+int run_matvec_from_host(const tt_plan* p, const void* m_host, void* d_dev, cudaStream_t s) {
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
+    const size_t es = esize(p->dtype);
+    const VecView vm = view(p, p->N_m, p->N_t, 1, 0), vd = view(p, p->N_d, p->N_td, 1, 0);
+    TT_CUDA(p, cudaEventRecord(p->cev[kHostChunks], s));                 // the staging buffer is free once s gets here
+    TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[kHostChunks], 0));
+    for (int c = 0; c < kHostChunks; ++c) {
+        long long p0, p1;
+        host_chunk(p, c, &p0, &p1);
+        if (p1 <= p0) continue;
+        TT_CUDA(p, copy_m_range(p, p->m_stage, m_host, p0, p1, cudaMemcpyHostToDevice, p->copy_stream));
+        TT_CUDA(p, cudaEventRecord(p->cev[c], p->copy_stream));
+        TT_CUDA(p, cudaStreamWaitEvent(s, p->cev[c], 0));
+        FftParams P;
+        fill_fft_common(p, P, f32);
+        const long long b1 = p1 < p->N_m ? p1 : p->N_m;
+        P.B = b1 > p0 ? b1 - p0 : 0; P.B_store = p1 - p0;                  // the last range also zeroes the row padding
+        P.r_ys = 0; P.r_bs = vm.bs; P.r_ts = vm.ts;
+        P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
+        TT_CUDA(p, fft_r2c_launch(t, t, t, at(p->m_stage, p0 * vm.bs, es), at(p->xhat, p0, 2 * es), P, 1, s));
+        GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
+        g.p_begin = p0; g.p_end = p1;
+        TT_CUDA(p, gemv_fwd_launch(t, p->Fhat, p->xhat, p->partial, g, s));
+    }
+    TT_CUDA(p, reduce_partials_launch(t, p->partial, p->dhat, p->n_f, p->n_chunks, (int)p->N_d, s));
+    FftParams P;
+    fill_fft_common(p, P, f32);
+    P.B = p->N_d; P.B_store = p->N_d;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
+    TT_CUDA(p, fft_c2r_launch(t, p->dhat, d_dev, P, 1, s));
+    return TT_OK;
+}
+
+// m = F^T d with m delivered to the HOST: per parameter range, B2 and B3 on the caller's stream, then the D2H copy of
+// that range on the copy stream while the next range computes.  The caller's stream waits for the last copy.
+int run_rmatvec_to_host(const tt_plan* p, const void* d_dev, void* m_host, cudaStream_t s) {
+    const bool f32 = p->dtype == TT_F32;
+    const int t = f32 ? 0 : 1;
+    const size_t es = esize(p->dtype);
+    const VecView vm = view(p, p->N_m, p->N_t, 1, 0), vd = view(p, p->N_d, p->N_td, 1, 0);
+    FftParams P;
+    fill_fft_common(p, P, f32);
+    P.B = p->N_d; P.B_store = p->N_d;
+    P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
+    P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
+    TT_CUDA(p, fft_r2c_launch(t, t, t, d_dev, p->dhat, P, 1, s));
+    for (int c = 0; c < kHostChunks; ++c) {
+        long long p0, p1;
+        host_chunk(p, c, &p0, &p1);
+        if (p1 <= p0) continue;
+        GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
+        g.p_begin = p0; g.p_end = p1;
+        TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
+        const long long b1 = p1 < p->N_m ? p1 : p->N_m;
+        if (b1 > p0) {
+            fill_fft_common(p, P, f32);
+            P.B = b1 - p0; P.B_store = b1 - p0;
+            P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
+            P.r_ys = 0; P.r_bs = vm.bs; P.r_ts = vm.ts;
+            TT_CUDA(p, fft_c2r_launch(t, at(p->xhat, p0, 2 * es), at(p->m_stage, p0 * vm.bs, es), P, 1, s));
+        }
+        TT_CUDA(p, cudaEventRecord(p->cev[c], s));
+        TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[c], 0));
+        TT_CUDA(p, copy_m_range(p, m_host, p->m_stage, p0, p1, cudaMemcpyDeviceToHost, p->copy_stream));
+    }
+    TT_CUDA(p, cudaEventRecord(p->cev[kHostChunks + 1], p->copy_stream));
+    TT_CUDA(p, cudaStreamWaitEvent(s, p->cev[kHostChunks + 1], 0));
+    return TT_OK;
+}
+
 }  // namespace
+
+namespace tt {
+int plan_rmatvec_to_host(const ::tt_plan* p, const void* d_dev, void* m_host, cudaStream_t s) {
+    const int r = ensure_staging(p);
+    return r ? r : run_rmatvec_to_host(p, d_dev, m_host, s);
+}
+}  // namespace tt
 
 extern "C" {
 
@@ -394,6 +501,9 @@ void tt_plan_destroy(tt_plan* p) {
                     p->dwork, p->m_stage, p->m_stage2, p->d_stage};
     for (void* b : bufs)
         if (b) cudaFree(b);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (cudaEvent_t e : p->cev)
+        if (e) cudaEventDestroy(e);
     if (p->ev) {
         for (int i = 0; i < kRing * kSlotEvents; ++i)
             if (p->ev[i]) cudaEventDestroy(p->ev[i]);
@@ -622,8 +732,7 @@ int tt_matvec_host(const tt_plan* p, const void* m_host, void* d_host, void* str
     if (r) return r;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
-    TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
-    r = run_matvec(p, p->m_stage, p->d_stage, s, begin_call(p, TT_OP_MATVEC, 1));
+    r = run_matvec_from_host(p, m_host, p->d_stage, s);
     if (r) return r;
     TT_CUDA(p, cudaMemcpyAsync(d_host, p->d_stage, (size_t)p->N_td * p->N_d * es, cudaMemcpyDeviceToHost, s));
     return TT_OK;
@@ -637,10 +746,7 @@ int tt_rmatvec_host(const tt_plan* p, const void* d_host, void* m_host, void* st
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
     TT_CUDA(p, cudaMemcpyAsync(p->d_stage, d_host, (size_t)p->N_td * p->N_d * es, cudaMemcpyHostToDevice, s));
-    r = run_rmatvec(p, p->d_stage, p->m_stage, s, begin_call(p, TT_OP_RMATVEC, 1));
-    if (r) return r;
-    TT_CUDA(p, cudaMemcpyAsync(m_host, p->m_stage, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
-    return TT_OK;
+    return run_rmatvec_to_host(p, p->d_stage, m_host, s);
 }
 
 int tt_normal_host(const tt_plan* p, const void* m_host, void* out_host, void* stream) {
@@ -650,14 +756,9 @@ int tt_normal_host(const tt_plan* p, const void* m_host, void* out_host, void* s
     if (r) return r;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const size_t es = esize(p->dtype);
-    TT_CUDA(p, cudaMemcpyAsync(p->m_stage, m_host, (size_t)p->N_t * p->N_m * es, cudaMemcpyHostToDevice, s));
-    const int e0 = begin_call(p, TT_OP_NORMAL, 2);
-    r = run_matvec(p, p->m_stage, p->dwork, s, e0);
+    r = run_matvec_from_host(p, m_host, p->dwork, s);
     if (r) return r;
-    r = run_rmatvec(p, p->dwork, p->m_stage2, s, e0 + 4);
-    if (r) return r;
-    TT_CUDA(p, cudaMemcpyAsync(out_host, p->m_stage2, (size_t)p->N_t * p->N_m * es, cudaMemcpyDeviceToHost, s));
-    return TT_OK;
+    return run_rmatvec_to_host(p, p->dwork, out_host, s);
 }
 
 int tt_plan_set_profiling(tt_plan* p, int enabled) {

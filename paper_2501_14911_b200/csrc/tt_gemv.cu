@@ -27,7 +27,7 @@ gemv_fwd_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ xhat, 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V* xs = reinterpret_cast<V*>(smem_raw);
 
-    const int w = blockIdx.y, c = blockIdx.x;
+    const int w = blockIdx.y, c = blockIdx.x + (int)(g.p_begin / g.chunk);
     const long long p0 = (long long)c * g.chunk;
     const long long rem = g.ldp - p0;
     const int len = rem < g.chunk ? (int)rem : g.chunk;
@@ -91,8 +91,8 @@ gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, 
     __syncthreads();
 
     const long long rowv = g.ldp / VN;
-    const long long v = (long long)blockIdx.x * NT + threadIdx.x;
-    if (v >= rowv) return;
+    const long long v = (long long)blockIdx.x * NT + threadIdx.x + g.p_begin / VN;
+    if (v >= (g.p_end ? g.p_end / VN : rowv)) return;
     const V* col = reinterpret_cast<const V*>(Fhat + (long long)w * g.N_d * g.ldp) + v;
 
     Cx<R> acc[VN];
@@ -166,7 +166,8 @@ static cudaError_t fwd_dispatch(const void* Fhat, const void* xhat, void* partia
     const size_t smem = (size_t)g.chunk * sizeof(Cx<R>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    dim3 grid((unsigned)g.n_chunks, (unsigned)g.n_f);
+    const long long pe = g.p_end ? g.p_end : g.ldp;
+    dim3 grid((unsigned)((pe - g.p_begin + g.chunk - 1) / g.chunk), (unsigned)g.n_f);
     k<<<grid, NW * 32, smem, s>>>(static_cast<const Cx<R>*>(Fhat), static_cast<const Cx<R>*>(xhat),
                                  static_cast<Cx<R>*>(partial), g);
     return cudaGetLastError();
@@ -182,7 +183,8 @@ static cudaError_t adj_dispatch(const void* Fhat, const void* dhat, void* xout, 
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long rowv = g.ldp / Vec16<R>::n;
-    dim3 grid((unsigned)((rowv + NT - 1) / NT), (unsigned)g.n_f);
+    const long long nv = (g.p_end ? g.p_end : g.ldp) / Vec16<R>::n - g.p_begin / Vec16<R>::n;
+    dim3 grid((unsigned)((nv + NT - 1) / NT), (unsigned)g.n_f);
     k<<<grid, NT, smem, s>>>(static_cast<const Cx<R>*>(Fhat), static_cast<const Cx<R>*>(dhat),
                              static_cast<Cx<R>*>(xout), g);
     return cudaGetLastError();

@@ -15,6 +15,8 @@ struct PlanInfo {
     long long dec;  // data vectors on every dec-th time step (tt_plan_create_coarse)
 };
 PlanInfo plan_info(const ::tt_plan* p);
+// m_host = F^T d_dev, delivered to HOST memory with the D2H copies pipelined behind the kernels (tt_api.cu); returns a tt_status
+int plan_rmatvec_to_host(const ::tt_plan* p, const void* d_dev, void* m_host, cudaStream_t s);
 
 constexpr int kMaxStages = 16;
 constexpr int kMaxSmem = 232448;  // 227 KB: largest dynamic shared memory per CTA on sm_100
@@ -75,6 +77,8 @@ struct GemvGeom {
     int chunk;      // forward: elements of p per CTA (multiple of 64)
     int n_chunks;
     int warps;      // forward: warps per CTA (0 = kernel default)
+    long long p_begin = 0, p_end = 0;  // restrict the launch to parameters [p_begin, p_end) (p_end == 0: all); p_begin must be
+                                       // a multiple of `chunk` (forward) and of 512 (adjoint) - the pipelined *_host calls
 };
 void gemv_debug_set(int fwd_warps, int adj_threads);  // -1 = leave, 0 = planner's choice
 cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,

@@ -186,7 +186,7 @@ int map_partial_typed(const tt_map* m, const T* d_obs, T* a, T* b, cudaStream_t 
 
 template <typename T>
 int map_finish_typed(const tt_map* m, const T* y /* nullptr: gain form, z = K^{-1} b */, const T* b, T* m_map,
-                     cudaStream_t s) {
+                     cudaStream_t s, void* m_host = nullptr /* deliver m_map to host memory instead, copies pipelined */) {
     const PlanInfo& pi = m->pi;
     const long long n = pi.N_d * pi.N_t;
     T* dv = static_cast<T*>(m->dv);
@@ -195,16 +195,17 @@ int map_finish_typed(const tt_map* m, const T* y /* nullptr: gain form, z = K^{-
     if ((rc = tt_chol_solve(m->K, m->k64, m->k64, s)) != TT_OK) return rc;                          // c = K^{-1} b
     from_k_kernel<T><<<nblocks(n), 256, 0, s>>>(y, m->k64, dv, pi.N_d, pi.N_t, pi.layout);          // z = y - c  (or c)
     TTO_CUDA(m, cudaGetLastError());
+    if (m_host) return plan_rmatvec_to_host(m->G, dv, m_host, s);
     return tt_rmatvec(m->G, dv, m_map, s);                                                          // m_map = G* z
 }
 
 template <typename T>
-int map_infer_typed(const tt_map* m, int form, const T* d_obs, T* m_map, cudaStream_t s) {
-    if (form == TT_MAP_GAIN) return map_finish_typed<T>(m, nullptr, d_obs, m_map, s);               // G* K^{-1} d_obs
+int map_infer_typed(const tt_map* m, int form, const T* d_obs, T* m_map, cudaStream_t s, void* m_host = nullptr) {
+    if (form == TT_MAP_GAIN) return map_finish_typed<T>(m, nullptr, d_obs, m_map, s, m_host);       // G* K^{-1} d_obs
     T* dv = static_cast<T*>(m->dv);
     const int rc = map_partial_typed<T>(m, d_obs, m_map, dv, s);                                    // a lives in m_map
     if (rc != TT_OK) return rc;
-    return map_finish_typed<T>(m, static_cast<const T*>(m->yv), dv, m_map, s);
+    return map_finish_typed<T>(m, static_cast<const T*>(m->yv), dv, m_map, s, m_host);
 }
 
 }  // namespace
@@ -425,17 +426,21 @@ int tt_map_infer_finish(const tt_map* m, const void* b, void* m_map, void* strea
 
 int tt_map_infer_host(const tt_map* cm, int form, const void* d_obs_host, void* m_map_host, void* stream) {
     if (!cm || !d_obs_host || !m_map_host) return TT_ERR_NULL;
+    if (form != TT_MAP_PAPER && form != TT_MAP_GAIN) return TT_ERR_SHAPE;
+    if (form == TT_MAP_PAPER && !cm->F) return TT_ERR_NULL;
     tt_map* m = const_cast<tt_map*>(cm);
     const size_t es = esize(m->pi.dtype);
     const size_t nd = (size_t)m->pi.N_d * m->pi.N_t * es, nm = (size_t)m->pi.N_m * m->pi.N_t * es;
     if (!m->d_stage) TTO_CUDA(m, cudaMalloc(&m->d_stage, nd));
-    if (!m->m_stage) TTO_CUDA(m, cudaMalloc(&m->m_stage, nm));
+    if (form == TT_MAP_PAPER && !m->m_stage) TTO_CUDA(m, cudaMalloc(&m->m_stage, nm));   // a = G* y lives here
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     TTO_CUDA(m, cudaMemcpyAsync(m->d_stage, d_obs_host, nd, cudaMemcpyHostToDevice, s));
-    const int rc = tt_map_infer(m, form, m->d_stage, m->m_stage, stream);
-    if (rc != TT_OK) return rc;
-    TTO_CUDA(m, cudaMemcpyAsync(m_map_host, m->m_stage, nm, cudaMemcpyDeviceToHost, s));
-    return TT_OK;
+    // the final G* action delivers m_map range by range to the host while the next range computes
+    if (m->pi.dtype == TT_F32)
+        return map_infer_typed<float>(m, form, static_cast<const float*>(m->d_stage), static_cast<float*>(m->m_stage), s,
+                                      m_map_host);
+    return map_infer_typed<double>(m, form, static_cast<const double*>(m->d_stage), static_cast<double*>(m->m_stage), s,
+                                   m_map_host);
 }
 
 }  // extern "C"

@@ -266,3 +266,85 @@ def test_map_two_halves_equal_the_whole(tt):
     finally:
         mp.close(); chol.close(); pF.close(); pG.close()
     assert torch.equal(whole, halves) and torch.equal(whole, via) and torch.equal(gain, ref_gain)
+
+
+def test_apply_calls_are_cuda_graph_capturable(tt):
+    """No allocation, no host synchronisation after plan creation: the whole online step (and the plain matvec pair)
+    can be captured once in a CUDA graph and replayed - what a launch-bound small problem (C1: 7 launches) wants."""
+    w, F, G, nv, d_obs = online_inputs(4, 64, 32, torch.float64)
+    L = oo.cholesky(oo.assemble_K(F.numpy(), G.numpy(), nv.numpy()))
+    pF, pG, chol = tt.Plan(F.cuda()), tt.Plan(G.cuda()), tt.Chol(torch.from_numpy(L).cuda())
+    mp = tt.MapInference(pF, pG, chol, nv.cuda())
+    try:
+        d_in = d_obs.cuda().clone()
+        m_in = synth.vector_m(w, k_rhs=1).cuda()
+        out_map = torch.empty((w.N_t, w.N_m), dtype=torch.float64, device="cuda")
+        out_d = torch.empty((w.N_t, w.N_d), dtype=torch.float64, device="cuda")
+        out_m = torch.empty_like(out_map)
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            for _ in range(2):                                    # warm-up outside the capture
+                tt.tt_map_infer(mp.handle, tt.TT_MAP_PAPER, d_in, out_map, s)
+        s.synchronize()
+        ref_map = out_map.clone()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            tt.tt_matvec(pF.handle, m_in, out_d, s)
+            tt.tt_rmatvec(pF.handle, out_d, out_m, s)
+            tt.tt_map_infer(mp.handle, tt.TT_MAP_PAPER, d_in, out_map, s)
+        out_map.zero_(); out_d.zero_(); out_m.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out_map, ref_map)
+        d_in.mul_(2.0)                                            # new data, same graph
+        graph.replay()
+        torch.cuda.synchronize()
+        assert rel(out_map.cpu().numpy(), 2.0 * ref_map.cpu().numpy()) <= 1e-13
+        assert rel(out_m.cpu().numpy(), op.rmatvec(F.numpy(), op.matvec(F.numpy(), m_in.cpu().numpy()))) <= 1e-12
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_pipelined_host_calls_equal_device_calls(tt, dtype, layout):
+    """The *_host calls move the parameter-sized vector range by range (8 ranges of the parameter axis) on a copy stream
+    while the kernels of the neighbouring range run; the result must be bit-identical to the device-pointer calls.
+    N_m = 40007 gives five non-empty ranges with a ragged last one."""
+    N_d, N_m, N_t, r = 3, 40007, 20, 2
+    w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
+    F = synth.block_column(w)
+    G = synth.gstar_block_column(w, F)
+    nv, d_obs = synth.noise_var(w), synth.vector_d(w, k_rhs=1)
+    m = synth.vector_m(w, k_rhs=1)
+    lay = (lambda t: t.t().contiguous()) if layout == 1 else (lambda t: t)
+    mh, dh = lay(m).pin_memory(), lay(d_obs).pin_memory()
+    pF, pG = tt.Plan(F.cuda(), layout=layout), tt.Plan(G.cuda(), layout=layout)
+    pC = tt.Plan(F.cuda(), layout=layout, out_every=r)
+    n = N_d * N_t
+    Lf = torch.eye(n, dtype=torch.float64) * 3.0 + torch.tril(torch.full((n, n), 0.01, dtype=torch.float64), -1)
+    chol = tt.Chol(Lf.cuda())
+    mp = tt.MapInference(pF, pG, chol, lay(nv).cuda())
+    try:
+        for plan, dvec in ((pF, dh), (pC, lay(d_obs[: N_t // r]).pin_memory())):
+            d_dev = plan.matvec(mh.cuda())
+            m_dev = plan.rmatvec(dvec.cuda())
+            n_dev = plan.normal(mh.cuda())
+            d_host = torch.empty_like(d_dev, device="cpu").pin_memory()
+            m_host = torch.empty_like(m_dev, device="cpu").pin_memory()
+            n_host = torch.empty_like(n_dev, device="cpu").pin_memory()
+            tt.tt_matvec_host(plan.handle, mh, d_host)
+            tt.tt_rmatvec_host(plan.handle, dvec, m_host)
+            tt.tt_normal_host(plan.handle, mh, n_host)
+            tt.tt_rmatvec_host(plan.handle, dvec, m_host)            # back to back: staging reuse is ordered
+            torch.cuda.synchronize()
+            assert torch.equal(d_host, d_dev.cpu()) and torch.equal(m_host, m_dev.cpu()) and torch.equal(n_host, n_dev.cpu())
+        for form in (tt.TT_MAP_PAPER, tt.TT_MAP_GAIN):
+            ref = mp.infer(dh.cuda(), form).cpu()
+            out = torch.empty_like(ref).pin_memory()
+            tt.tt_map_infer_host(mp.handle, form, dh, out)
+            torch.cuda.synchronize()
+            assert torch.equal(out, ref)
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close(); pC.close()
