@@ -135,3 +135,17 @@ def post_cov_apply(F, G, L, Gamma_s, v) -> np.ndarray:
     u = v * Gs[None, :] if Gs.ndim == 1 else v @ Gs          # Gamma_prior v (Gamma_s symmetric)
     c = chol_solve(L, tp.matvec(F, u).reshape(N_t * N_d)).reshape(N_t, N_d)
     return u - apply_gstar(G, c)
+
+
+def K_entry(F_s, G_s2, i: int, i2: int, noise: float = 0.0) -> float:
+    """One entry K[(i, s), (i2, s2)] of K = Gamma_noise + F G* (PAPER.md:306), for sampled parity at sizes where
+    assemble_K is out of reach: row (i, s) of F times column (i2, s2) of G*,
+
+        sum_{j=0..min(i, i2)} F_{i-j}[s, :] . G_{i2-j}[s2, :]     (+ noise if (i, s) == (i2, s2), passed by the caller).
+
+    F_s: [N_t, N_m] = F[:, s, :];  G_s2: [N_t, N_m] = G[:, s2, :].
+    """
+    acc = 0.0
+    for j in range(min(i, i2) + 1):
+        acc += float(np.dot(np.asarray(F_s[i - j], dtype=np.float64), np.asarray(G_s2[i2 - j], dtype=np.float64)))
+    return acc + noise

@@ -216,3 +216,46 @@ def test_online_p5_full_size_sampled(tt):
         ref = np.array([op.rmatvec_entry(cols[p], zr, j, 0) for j in range(0, w.N_t, 7)])
         err = np.linalg.norm(got[p][::7] - ref) / max(np.linalg.norm(ref), 1e-3 * scale * np.sqrt(len(ref)))
         assert err <= 1e-5, (p, err)
+
+
+def test_K_assembly_p5_full_size_sampled(tt):
+    """tt_assemble_K at the paper's shape in the configuration `bench.py --config P5 --online --k-batch 16` times
+    (fp32 plans, batches of 16 unit vectors through the batched FFTs and the complex64 GEMMs): 16 columns of K, sampled
+    entries against oracle/online_plain.K_entry computed from single sensor rows of the block columns."""
+    from oracle import online_plain as oo
+    w = synth.CONFIGS["P5"]
+    need_memory(160)
+    n = w.N_d * w.N_t
+    F = synth.block_column(w, device="cuda")
+    rows_F = {s: F[:, s, :].cpu().numpy() for s in (0, 17, 48)}
+    pF = tt.Plan(F, k_max=16)
+    synth.gstar_block_column(w, F, out=F)
+    cols = [(3, 5), (250, 17), (499, 48)]                      # (time step, sensor) of sampled columns of K
+    rows_G = {s2: F[:, s2, :].cpu().numpy() for _, s2 in cols}
+    pG = tt.Plan(F, k_max=16)
+    del F
+    torch.cuda.empty_cache()
+    nv = synth.noise_var(w, device="cuda")
+    try:
+        got = {}
+        K = torch.zeros((n, n), dtype=torch.float64, device="cuda")
+        for i2, s2 in cols:
+            c = i2 * w.N_d + s2
+            c0 = min(c - c % 16, n - 16)
+            tt.tt_assemble_K(pF.handle, pG.handle, nv, c0, 16, K, n)
+            got[(i2, s2)] = K[:, c].cpu().numpy()
+        del K
+    finally:
+        pF.close(); pG.close()
+    nvh = nv.cpu().numpy().astype(np.float64)
+    for (i2, s2), col in got.items():
+        scale = np.sqrt(np.mean(col ** 2))
+        for i, s in ((0, 0), (i2, 17), (min(i2 + 40, w.N_t - 1), 48), (w.N_t - 1, 0), (i2, s2)):
+            if (i, s) == (i2, s2):
+                rows = rows_F.get(s)
+                if rows is None:
+                    continue
+                ref = oo.K_entry(rows, rows_G[s2], i, i2, nvh[i, s])
+            else:
+                ref = oo.K_entry(rows_F[s], rows_G[s2], i, i2)
+            assert abs(col[i * w.N_d + s] - ref) <= 1e-5 * max(abs(ref), scale), ((i, s), (i2, s2), col[i * w.N_d + s], ref)

@@ -71,6 +71,20 @@ def test_K_dense(N_d, N_m, N_t):
     assert np.linalg.eigvalsh(0.5 * (K + K.T)).min() >= nv.min() * (1 - 1e-9)   # K - Gamma_noise is PSD
 
 
+def test_K_entry_equals_assembled_K():
+    N_d, N_m, N_t = 3, 5, 7
+    F, Gs, nv, A, Gp = setup(N_d, N_m, N_t)
+    G = oo.gstar_block_column(F, Gs)
+    K_ref = np.diag(nv.ravel()) + A @ Gp @ A.T
+    for i in range(N_t):
+        for s in range(N_d):
+            for i2 in (0, 3, N_t - 1):
+                for s2 in range(N_d):
+                    noise = nv[i, s] if (i, s) == (i2, s2) else 0.0
+                    got = oo.K_entry(F[:, s, :], G[:, s2, :], i, i2, noise)
+                    assert abs(got - K_ref[i * N_d + s, i2 * N_d + s2]) <= 1e-12 * np.abs(K_ref).max()
+
+
 # ------------------------------------------------------------------ triangular solves
 @pytest.mark.parametrize("n", [1, 2, 7, 64, 130])
 def test_substitution_against_lapack(n):
