@@ -154,7 +154,15 @@ trsv_fwd_kernel(const double* __restrict__ Lt, const double* __restrict__ bt, do
         }
     }
     const double tot = reduce8(acc, lane);
-    if ((lane & 3) == 0) st_publish(y + my_row, publishable(my_bt - tot));
+    // Publish the 64 values of the block row with ONE warp-wide store: when the eight warps publish their eight rows
+    // each, a consumer's poll usually lands in the middle and pays a second L2 round trip (~0.3 us) for the rest.
+    __shared__ __align__(16) double ys[NB];
+    if ((lane & 3) == 0) ys[warp * RW + my_r] = publishable(my_bt - tot);
+    __syncthreads();
+    if (warp == 0) {
+        const double2 v = *reinterpret_cast<const double2*>(ys + 2 * lane);
+        asm volatile("st.relaxed.gpu.global.v2.f64 [%0], {%1, %2};" ::"l"(y + (size_t)I * NB + 2 * lane), "d"(v.x), "d"(v.y) : "memory");
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -218,6 +226,7 @@ trsv_bwd_kernel(const double* __restrict__ Lt, const double* __restrict__ yin, d
     part[warp][2 * lane] = acc.x;
     part[warp][2 * lane + 1] = acc.y;
     __syncthreads();
+    // (two warps publish 256 bytes each; a single warp-wide store as in the forward kernel was measured slower here)
     if (threadIdx.x < NB) {
         double s = 0.0;
 #pragma unroll
@@ -390,9 +399,9 @@ cudaError_t trsv_fwd_launch(const TrsvGeom& g, cudaStream_t s) {
     return cudaGetLastError();
 }
 cudaError_t trsv_bwd_launch(const TrsvGeom& g, const double* yin, cudaStream_t s) {
-    if (g_trsv_U == 3) trsv_bwd_kernel<3><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
-    else if (g_trsv_U == 1) trsv_bwd_kernel<1><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
-    else trsv_bwd_kernel<2><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    if (g_trsv_U == 1) trsv_bwd_kernel<1><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    else if (g_trsv_U == 2) trsv_bwd_kernel<2><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);
+    else trsv_bwd_kernel<3><<<g.nblk, NTHREADS, 0, s>>>(g.Lt, yin, g.xt, g.ticket + 1, g.nblk);   // default: three blocks in flight
     return cudaGetLastError();
 }
 cudaError_t trsv_post_launch(const TrsvGeom& g, double* x, cudaStream_t s) {
