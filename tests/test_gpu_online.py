@@ -348,3 +348,25 @@ def test_pipelined_host_calls_equal_device_calls(tt, dtype, layout):
             assert torch.equal(out, ref)
     finally:
         mp.close(); chol.close(); pF.close(); pG.close(); pC.close()
+
+
+def test_trsv_repeated_launches_are_stable(tt):
+    """The chain kernels spin on self-flagging data: 300 back-to-back solves (no host synchronisation in between, the
+    flags are re-armed by the pre-step of every call) must all terminate and return the same bits."""
+    n = 2500
+    L = random_factor(n, 3)
+    chol = tt.Chol(torch.from_numpy(L).cuda())
+    try:
+        b = torch.from_numpy(np.random.default_rng(2).standard_normal(n)).cuda()
+        first = chol.solve(b).clone()
+        outs = [torch.empty_like(b) for _ in range(4)]
+        for it in range(300):
+            tt.tt_chol_solve(chol.handle, b, outs[it % 4])
+            if it % 3 == 0:
+                tt.tt_chol_trsv(chol.handle, bool(it % 2), b, outs[(it + 1) % 4])
+                tt.tt_chol_solve(chol.handle, b, outs[(it + 1) % 4])
+        torch.cuda.synchronize()
+        for o in outs:
+            assert torch.equal(o, first)
+    finally:
+        chol.close()
