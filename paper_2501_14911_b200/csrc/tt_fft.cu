@@ -186,7 +186,7 @@ template <typename R, int T, int NS = 0>
 __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int lane_s, int g, int G) {
     constexpr int MAXR = MaxRadix<R>::value;
     const Cx<R>* tw = reinterpret_cast<const Cx<R>*>(P.tw);
-    if constexpr (NS != 0) {
+    if constexpr (NS != 0 && NS != 500) {   // 500: only the load / post-processing loops are static (registers)
         using SP = StaticPlan<R, NS>;
         constexpr int R1 = SP::r1, R2 = SP::r2, R3 = SP::r3;
         static_assert(R1 * R2 * R3 == NS, "static FFT plan does not match its length");
@@ -427,14 +427,16 @@ FftChoice fft_choose(int N, size_t elem) {
 // The static variant for this plan, or 0: T = 16 / 256 threads only (the planner's choice for these lengths), and the
 // plan's radices must be the ones compiled in.
 template <typename Tc>
-static int static_length(const FftParams& P, const FftChoice& c, int nt) {
+static int static_length(const FftParams& P, const FftChoice& c, int nt, bool inverse) {
     if (g_no_static > 0 || c.T != 16 || nt != 256) return 0;
     auto is = [&](int n, int r1, int r2, int r3) {
         return P.N == n && P.n_stages == (r3 > 1 ? 3 : 2) && P.radix[0] == r1 && P.radix[1] == r2 &&
                (r3 == 1 || P.radix[2] == r3);
     };
-    // (the 500 = 25 x 20 variant needs ~130 registers - it spills under the three-CTA budget and was measured slower)
-    if (sizeof(Tc) == 4) return is(400, 25, 16, 1) ? 400 : g_no_static == -1 && is(500, 25, 20, 1) ? 500 : is(256, 16, 16, 1) ? 256 : 0;
+    // 500 = 25 x 20: fully static passes need ~130 registers (slower); only the load / post-processing loops are static
+    // there, and only in the forward kernel (A1 0.63 -> 0.585 ms; the inverse kernel spills and was measured slower)
+    if (sizeof(Tc) == 4)
+        return is(400, 25, 16, 1) ? 400 : (!inverse && is(500, 25, 20, 1)) ? 500 : is(256, 16, 16, 1) ? 256 : 0;
     return is(512, 8, 8, 8) ? 512 : is(256, 8, 8, 4) ? 256 : 0;
 }
 
@@ -452,7 +454,7 @@ static cudaError_t r2c_dispatch(const void* in, void* out, const FftParams& P, i
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Tin*>(in), static_cast<Cx<Tout>*>(out), P);             \
     }
-    const int ns = static_length<Tc>(P, c, nt);
+    const int ns = static_length<Tc>(P, c, nt, false);
     if (ns) {
         if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_R2C(16, 256, 400) else if (ns == 500) TT_R2C(16, 256, 500) else TT_R2C(16, 256, 256) }
         else                           { if (ns == 512) TT_R2C(16, 256, 512) else TT_R2C(16, 256, 256) }
@@ -484,7 +486,7 @@ static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, i
         if (e != cudaSuccess) return e;                                                                      \
         k<<<grid, NT, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P);                \
     }
-    const int ns = static_length<Tc>(P, c, nt);
+    const int ns = static_length<Tc>(P, c, nt, true);
     if (ns) {
         if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_C2R(16, 256, 400) else if (ns == 500) TT_C2R(16, 256, 500) else TT_C2R(16, 256, 256) }
         else                           { if (ns == 512) TT_C2R(16, 256, 512) else TT_C2R(16, 256, 256) }
