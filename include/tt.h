@@ -216,7 +216,10 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
  * register butterfly the planner may use (0 = no limit),
  * "gemv_chunk" = parameters per CTA of the forward matvec (multiple of 64; 0 = planner's choice),
  * "gemv_fwd_warps" = warps per CTA of the forward matvec (1..32; 0 = planner's choice),
- * "gemv_adj_threads" = threads per CTA of the adjoint matvec (multiple of 32, <= 512; 0 = default).
+ * "gemv_adj_threads" = threads per CTA of the adjoint matvec (multiple of 32, <= 512; 0 = default),
+ * "fft_no_static" = 1: never use the statically specialised FFT variants (N_t = 256, 400, 500),
+ * "trsv_U" = blocks of the factor in flight per warp of the triangular-solve chains (1, 2, 3; 0 = defaults),
+ * "gemm32_fwd" = tile variant of the fp32 k-RHS forward GEMM (1, 2; 0 = planner's choice).
  * Returns TT_ERR_SHAPE for an unknown key. */
 int tt_debug_set(const char* key, int value);
 

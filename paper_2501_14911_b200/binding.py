@@ -329,6 +329,14 @@ def tt_map_infer_host(m: int, form: int, d_obs_host, m_map_host, stream=None) ->
 _DT = {torch.float32: TT_F32, torch.float64: TT_F64}
 
 
+def _sync_quietly() -> None:
+    """Device synchronisation before a handle is destroyed; tolerant of interpreter shutdown (module globals gone)."""
+    try:
+        torch.cuda.synchronize()
+    except Exception:
+        pass
+
+
 class Plan:
     """RAII convenience over the calls above (tests and bench.py use it).
 
@@ -347,7 +355,7 @@ class Plan:
 
     def close(self):
         if getattr(self, "handle", None):
-            torch.cuda.synchronize()
+            _sync_quietly()
             tt_plan_destroy(self.handle)
             self.handle = None
 
@@ -411,7 +419,7 @@ class Chol:
 
     def close(self):
         if getattr(self, "handle", None):
-            torch.cuda.synchronize()
+            _sync_quietly()
             tt_chol_destroy(self.handle)
             self.handle = None
 
@@ -451,7 +459,7 @@ class MapInference:
 
     def close(self):
         if getattr(self, "handle", None):
-            torch.cuda.synchronize()
+            _sync_quietly()
             tt_map_destroy(self.handle)
             self.handle = None
 

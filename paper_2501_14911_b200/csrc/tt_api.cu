@@ -45,7 +45,6 @@ struct tt_plan {
     void* dwork = nullptr;    // [N_t][N_d] reals (tt_normal)
     void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
     void* d_stage = nullptr;
-    void* m_stage2 = nullptr;
     cudaStream_t copy_stream = nullptr;   // *_host calls: the PCIe copies of the parameter-sized vector run here, chunk by
     cudaEvent_t cev[kHostChunks + 2] = {};  // chunk over ranges of the parameter axis, overlapped with the kernels (lazily created)
     int chunk = 0, n_chunks = 0, fwd_warps = 0;
@@ -498,7 +497,7 @@ const char* tt_status_string(int status) {
 void tt_plan_destroy(tt_plan* p) {
     if (!p) return;
     void* bufs[] = {p->tw_d, p->tw_f, p->pos[0], p->pos[1], p->Fhat, p->xhat, p->dhat, p->partial,
-                    p->dwork, p->m_stage, p->m_stage2, p->d_stage};
+                    p->dwork, p->m_stage, p->d_stage};
     for (void* b : bufs)
         if (b) cudaFree(b);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
