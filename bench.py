@@ -248,6 +248,7 @@ def run_online(args, w):
     d_tmp = torch.empty_like(d_obs)
     ms_G = time_op(lambda: tt.tt_rmatvec(pG.handle, d_obs, m_tmp, stream), args.steps)
     ms_F = time_op(lambda: tt.tt_matvec(pF.handle, m_tmp, d_tmp, stream), args.steps)
+    ms_smw = time_op(lambda: tt.tt_smw_apply(mp.handle, m_tmp, m_map, stream), args.steps)   # (I - G* K^-1 F) u, eq (4.7)/(4.8)
     del m_tmp
 
     # end to end with HOST vectors: d_obs in (98 KB), m_map out (526 MB)
@@ -302,7 +303,9 @@ def run_online(args, w):
                      "forward_ms": ms_fwd, "backward_ms": ms_bwd, "chain_steps": (n + 63) // 64,
                      "note": "latency chain of n/64 block steps on top of the stream; see DESIGN.md section 11"},
         "ops": {"map_paper_form_ms": ms_paper, "map_gain_form_ms": ms_gain, "Gstar_ms": ms_G, "F_ms": ms_F,
-                "K_solve_ms": ms_solve,
+                "K_solve_ms": ms_solve, "smw_operator_ms": ms_smw,
+                "smw_context": "(I - G* K^-1 F) u = the posterior covariance action of eq (4.7) without the prior solve; "
+                               "PAPER.md:409: 11 + 11 + 20 ms on 24 A100 (+ 84 ms prior solve)",
                 "paper_form_GBs": (3 * (fhat_bytes + vec) + 2 * lt_bytes) / (ms_paper * 1e-3) / 1e9,
                 "gain_form_GBs": (fhat_bytes + vec + 2 * lt_bytes) / (ms_gain * 1e-3) / 1e9,
                 "paper_timing_context": "PAPER.md:436-438: ~53 ms on 24 A100 (11 ms per G*/F, 20 ms K-solve)"},

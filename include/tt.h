@@ -289,6 +289,13 @@ void tt_map_destroy(tt_map* m);
  * and layout).  Asynchronous on `stream`.  The K-solve runs in fp64 whatever the plans' dtype. */
 int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void* stream);
 
+/* out = (I - G* K^{-1} F) u : the Sherman-Morrison-Woodbury operator of eq (4.7) and eq (4.8), applied in
+ * the paper's order F, K-solve, G*, subtract.  With u = Gamma_prior(m) v (the prior action is the caller's: a sparse elliptic solve
+ * in the paper) it is the posterior covariance action Gamma_post(m) v, "exact up to rounding error"
+ * (PAPER.md:308); with u = m_prior it is the prior-mean term m_map^prior that eq (4.13) adds.
+ *   u, out  DEVICE, N_t*N_m reals (plans' dtype and layout); out == u returns TT_ERR_ALIAS.  Needs F (TT_ERR_NULL without). */
+int tt_smw_apply(const tt_map* m, const void* u, void* out, void* stream);
+
 /* eq (4.13) in two halves, split at the one exchange step of the N_m-sharded path (DESIGN.md section 6 / 11):
  *   tt_map_infer_partial:  y = Gamma_noise^{-1} d_obs (kept in the tt_map), a = G* y -> a_scratch (N_t*N_m reals),
  *                          b = F a -> b (N_t*N_d reals).  On a rank that holds a parameter slice, b is its PARTIAL

@@ -125,6 +125,16 @@ def map_point(F, G, noise_var, L, d_obs, conv=tp) -> np.ndarray:
     return a - conv.rmatvec(G, c)
 
 
+def smw_apply(F, G, L, u, conv=tp) -> np.ndarray:
+    """(I - G* K^{-1} F) u: the operator of eq (4.7) and eq (4.8), in the paper's order
+    F, K-solve, G*, subtract.  u: [N_t, N_m].  With u = Gamma_prior v it is Gamma_post(m) v; with u = m_prior it is
+    the prior-mean contribution m_map^prior of eq (4.8)."""
+    u = _f64(u)
+    N_t, N_d = F.shape[0], F.shape[1]
+    c = chol_solve(L, conv.matvec(F, u).reshape(N_t * N_d)).reshape(N_t, N_d)
+    return u - conv.rmatvec(G, c)
+
+
 def post_cov_apply(F, G, L, Gamma_s, v) -> np.ndarray:
     """Gamma_post(m) v = (I - G* K^{-1} F) Gamma_prior(m) v, eq (4.7) (PAPER.md:304).
 

@@ -86,6 +86,7 @@ def lib() -> ctypes.CDLL:
         "tt_map_destroy": (None, [vp]),
         "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
         "tt_map_infer_host": (ci, [vp, ci, vp, vp, vp]),
+        "tt_smw_apply": (ci, [vp, vp, vp, vp]),
         "tt_map_infer_partial": (ci, [vp, vp, vp, vp, vp]),
         "tt_map_infer_finish": (ci, [vp, vp, vp, vp]),
     }
@@ -104,7 +105,7 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
            "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
-           "tt_map_infer_partial", "tt_map_infer_finish"]
+           "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply"]
 
 
 def _stream(stream) -> int:
@@ -314,6 +315,10 @@ def tt_map_infer(m: int, form: int, d_obs, m_map, stream=None) -> None:
     _check("tt_map_infer", lib().tt_map_infer(m, form, _ptr(d_obs), _ptr(m_map), _stream(stream)))
 
 
+def tt_smw_apply(m: int, u, out, stream=None) -> None:
+    _check("tt_smw_apply", lib().tt_smw_apply(m, _ptr(u), _ptr(out), _stream(stream)))
+
+
 def tt_map_infer_partial(m: int, d_obs, a_scratch, b, stream=None) -> None:
     _check("tt_map_infer_partial", lib().tt_map_infer_partial(m, _ptr(d_obs), _ptr(a_scratch), _ptr(b), _stream(stream)))
 
@@ -468,6 +473,12 @@ class MapInference:
     def infer(self, d_obs, form: int = TT_MAP_PAPER, out=None, stream=None):
         out = self.G._out(self.G.N_m) if out is None else out
         tt_map_infer(self.handle, form, d_obs, out, stream)
+        return out
+
+    def smw_apply(self, u, out=None, stream=None):
+        """(I - G* K^-1 F) u: Gamma_post(m) v for u = Gamma_prior v (eq 4.7), m_map^prior for u = m_prior (eq 4.8)."""
+        out = torch.empty_like(u) if out is None else out
+        tt_smw_apply(self.handle, u, out, stream)
         return out
 
     def infer_partial(self, d_obs, stream=None):

@@ -132,6 +132,13 @@ __global__ void scatter_K_kernel(const T* __restrict__ D, const T* __restrict__ 
     K[(size_t)q * ldk + col0 + r] = v;
 }
 
+// out = u - out, element-wise over a parameter-sized vector (the subtraction of eq 4.7 / 4.8), grid-stride
+template <typename T>
+__global__ void __launch_bounds__(256) sub_from_kernel(const T* __restrict__ u, T* __restrict__ out, long long n) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) out[i] = u[i] - out[i];
+}
+
 inline unsigned nblocks(long long n, int t = 256) { return (unsigned)((n + t - 1) / t); }
 
 bool same_shape(const PlanInfo& a, const PlanInfo& b) {
@@ -197,6 +204,23 @@ int map_finish_typed(const tt_map* m, const T* y /* nullptr: gain form, z = K^{-
     TTO_CUDA(m, cudaGetLastError());
     if (m_host) return plan_rmatvec_to_host(m->G, dv, m_host, s);
     return tt_rmatvec(m->G, dv, m_map, s);                                                          // m_map = G* z
+}
+
+// out = (I - G* K^{-1} F) u  (eq 4.7 with u = Gamma_prior v; eq 4.8 with u = m_prior), in the paper's order
+template <typename T>
+int smw_typed(const tt_map* m, const T* u, T* out, cudaStream_t s) {
+    const PlanInfo& pi = m->pi;
+    const long long n = pi.N_d * pi.N_t, nm = pi.N_m * pi.N_t;
+    T* dv = static_cast<T*>(m->dv);
+    int rc;
+    if ((rc = tt_matvec(m->F, u, dv, s)) != TT_OK) return rc;                                       // b = F u
+    to_k_kernel<T><<<nblocks(n), 256, 0, s>>>(dv, m->k64, pi.N_d, pi.N_t, pi.layout);
+    if ((rc = tt_chol_solve(m->K, m->k64, m->k64, s)) != TT_OK) return rc;                          // c = K^{-1} b
+    from_k_kernel<T><<<nblocks(n), 256, 0, s>>>(static_cast<const T*>(nullptr), m->k64, dv, pi.N_d, pi.N_t, pi.layout);
+    if ((rc = tt_rmatvec(m->G, dv, out, s)) != TT_OK) return rc;                                    // e = G* c
+    sub_from_kernel<T><<<148 * 8, 256, 0, s>>>(u, out, nm);                                        // out = u - e
+    TTO_CUDA(m, cudaGetLastError());
+    return TT_OK;
 }
 
 template <typename T>
@@ -402,6 +426,14 @@ int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void
     if (m->pi.dtype == TT_F32)
         return map_infer_typed<float>(m, form, static_cast<const float*>(d_obs), static_cast<float*>(m_map), s);
     return map_infer_typed<double>(m, form, static_cast<const double*>(d_obs), static_cast<double*>(m_map), s);
+}
+
+int tt_smw_apply(const tt_map* m, const void* u, void* out, void* stream) {
+    if (!m || !u || !out || !m->F) return TT_ERR_NULL;
+    if (u == out) return TT_ERR_ALIAS;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (m->pi.dtype == TT_F32) return smw_typed<float>(m, static_cast<const float*>(u), static_cast<float*>(out), s);
+    return smw_typed<double>(m, static_cast<const double*>(u), static_cast<double*>(out), s);
 }
 
 int tt_map_infer_partial(const tt_map* m, const void* d_obs, void* a_scratch, void* b, void* stream) {

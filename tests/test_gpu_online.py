@@ -370,3 +370,35 @@ def test_trsv_repeated_launches_are_stable(tt):
             assert torch.equal(o, first)
     finally:
         chol.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_smw_operator(tt, dtype, layout):
+    """(I - G* K^{-1} F) u, eq (4.7) / (4.8): the posterior covariance action for u = Gamma_prior v, against the oracle
+    (which is pinned to the dense inverse Hessian)."""
+    N_d, N_m, N_t = 5, 1000, 35
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    Fn, Gn = F.numpy(), G.numpy()
+    K = oo.assemble_K(Fn, Gn, nv.numpy())
+    L = oo.cholesky(K)
+    ev = np.linalg.eigvalsh(K)
+    kappa = ev[-1] / ev[0]
+    v = synth.vector_m(w, k_rhs=1)
+    u = (v.double() * synth.prior_gamma(w)[None, :]).to(dtype)           # Gamma_prior v, rounded once: the input of both sides
+    ref = oo.smw_apply(Fn, Gn, L, u.numpy())
+    lay = (lambda t: t.t().contiguous()) if layout == 1 else (lambda t: t)
+    unlay = (lambda t: t.t()) if layout == 1 else (lambda t: t)
+    pF, pG = tt.Plan(F.cuda(), layout=layout), tt.Plan(G.cuda(), layout=layout)
+    chol = tt.Chol(torch.from_numpy(L).cuda())
+    mp = tt.MapInference(pF, pG, chol, lay(nv).cuda())
+    try:
+        ud = lay(u).cuda()
+        got = unlay(mp.smw_apply(ud)).cpu().numpy()
+        with pytest.raises(tt.TTError) as ei:
+            tt.tt_smw_apply(mp.handle, ud, ud)
+        assert ei.value.status == -7                                      # TT_ERR_ALIAS
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close()
+    # u - G* K^{-1} F u: the correction is O(1) of u here, both terms carry the matvec bar; the solve amplifies by kappa
+    assert rel(got, ref) <= BAR[dtype] + 8 * U[dtype] * kappa

@@ -158,6 +158,26 @@ def test_post_cov_is_inverse_hessian(N_d, N_m, N_t):
         assert rel(col, Hinv[:, c]) <= 1e-9
 
 
+@pytest.mark.parametrize("N_d,N_m,N_t", SHAPES[:3])
+def test_smw_operator(N_d, N_m, N_t):
+    # (I - G* K^{-1} F) u:  with u = Gamma_prior v it is H^{-1} v (eq 4.7 vs 2.13); with u = m_prior it is the prior-mean
+    # term of eq (4.8), Gamma_post Gamma_prior^{-1} m_prior, and together with eq (4.13) it solves eq (2.12) with m_prior != 0
+    F, Gs, nv, A, Gp = setup(N_d, N_m, N_t)
+    G = oo.gstar_block_column(F, Gs)
+    L = oo.cholesky(oo.assemble_K(F, G, nv))
+    Gn_inv = np.diag(1.0 / nv.ravel())
+    H = A.T @ Gn_inv @ A + np.linalg.inv(Gp)
+    v = RNG.standard_normal((N_t, N_m))
+    u = (Gp @ v.ravel()).reshape(N_t, N_m)
+    assert rel(oo.smw_apply(F, G, L, u), np.linalg.solve(H, v.ravel())) <= 1e-9
+    assert rel(oo.smw_apply(F, G, L, u), oo.post_cov_apply(F, G, L, Gs, v)) <= 1e-13
+    m_prior = RNG.standard_normal((N_t, N_m))
+    d_obs = RNG.standard_normal((N_t, N_d))
+    m_full = np.linalg.solve(H, A.T @ Gn_inv @ d_obs.ravel() + np.linalg.solve(Gp, m_prior.ravel()))   # eq (2.12)
+    got = oo.map_point(F, G, nv, L, d_obs) + oo.smw_apply(F, G, L, m_prior)                              # eq (4.13) + (4.8)
+    assert rel(got, m_full) <= 1e-9
+
+
 def test_zero_noise_limit_fits_the_data():
     # Gamma_noise -> 0: K -> F G*, so F m_map = F G* K^{-1} d_obs -> d_obs (N_m N_t >= N_d N_t, F full row rank)
     N_d, N_m, N_t = 2, 6, 5
