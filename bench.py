@@ -263,6 +263,32 @@ def run_online(args, w):
     stream.synchronize()
     ms_e2e = (time.perf_counter() - t0) * 1e3 / n_e2e
 
+    # Phase 3 actions (eq 4.10, 4.11) through the p2q plans of the paper's shape (N_q = 16, every 10th step), --phase3
+    phase3 = None
+    if args.phase3:
+        wq = synth.CONFIGS["Q5"]
+        r = 10
+        Fq = synth.block_column(wq, device=dev)
+        pFq = tt.Plan(Fq, out_every=r)
+        synth.gstar_block_column(wq, Fq, out=Fq)
+        pGq = tt.Plan(Fq, out_every=r)
+        del Fq
+        torch.cuda.empty_cache()
+        vq = synth.vector_d(wq.scaled(N_t=wq.N_t // r), device=dev, k_rhs=1)
+        qout = torch.empty_like(vq)
+        work = torch.empty((2, w.N_t, w.N_m), dtype=w.dtype, device=dev)
+        ms_pq = time_op(lambda: tt.tt_postcov_q_apply(mp.handle, pFq.handle, pGq.handle, vq, work, qout, stream), args.steps)
+        ms_q = time_op(lambda: tt.tt_d2q_apply(mp.handle, pFq.handle, tt.TT_MAP_PAPER, d_obs, work, qout, stream), args.steps)
+        ms_qg = time_op(lambda: tt.tt_d2q_apply(mp.handle, pFq.handle, tt.TT_MAP_GAIN, d_obs, work, qout, stream), args.steps)
+        nq = wq.N_d * (wq.N_t // r)
+        phase3 = {"postcov_q_action_ms": ms_pq, "all_columns_s": ms_pq * nq * 1e-3, "d2q_action_ms": ms_q,
+                  "d2q_action_gain_form_ms": ms_qg, "n_qoi": nq,
+                  "paper_timing_context": "PAPER.md:421-423: 48 ms per Gamma_post(q) action (38.4 s for 800), 56 ms per Q action, 24 A100"}
+        pFq.close(); pGq.close()
+        del work
+        torch.cuda.empty_cache()
+        args.k_cols = min(args.k_cols, 4)
+
     # K assembly: a bounded number of columns, extrapolated like the paper does (n x time per column)
     kcols = min(n, args.k_cols)
     c0 = min(n // 2, n - kcols)
@@ -312,6 +338,7 @@ def run_online(args, w):
         "K_assembly": {"columns_timed": kcols, "k_batch": kb, "s_per_column": s_cols / kcols,
                        "extrapolated_total_s": s_cols / kcols * n, "symmetry_defect_of_the_diagonal_block": sym,
                        "paper_timing_context": "PAPER.md:407: 24 500 x 0.022 s ~ 9 min on 24 A100"},
+        "phase3": phase3,
         "setup": {"seconds": t_setup, "plan_bytes": pF.device_bytes + pG.device_bytes, "chol_bytes": chol.device_bytes},
     }
     if not args.no_cpu_baseline:
@@ -349,6 +376,8 @@ def main() -> int:
     ap.add_argument("--online", action="store_true",
                     help="time the online phase (eq 4.13 MAP inference, K-solve, K assembly) instead of the matvec pair; "
                          "meant for --config P5, the paper's own shape")
+    ap.add_argument("--phase3", action="store_true",
+                    help="--online: also time the Phase 3 actions Gamma_post(q) v (eq 4.10) and Q d_obs (eq 4.11) with the p2q plans")
     ap.add_argument("--k-cols", type=int, default=64, help="--online: columns of K assembled and timed")
     ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
     ap.add_argument("--out-every", type=int, default=0,

@@ -296,6 +296,17 @@ int tt_map_infer(const tt_map* m, int form, const void* d_obs, void* m_map, void
  *   u, out  DEVICE, N_t*N_m reals (plans' dtype and layout); out == u returns TT_ERR_ALIAS.  Needs F (TT_ERR_NULL without). */
 int tt_smw_apply(const tt_map* m, const void* u, void* out, void* stream);
 
+/* Phase 3 with the p2q map: Fq and Gq are plans made by tt_plan_create_coarse from the block columns of
+ * F_q and of G_q* = Gamma_prior F_q* (N_q "sensors", the same N_m, N_t, dtype and layout as the plans of `m`; any out_every).
+ *   tt_postcov_q_apply:  out = Gamma_post(q) v = F_q (I - G* K^{-1} F) G_q* v            (eq 4.10)
+ *                        v, out: DEVICE, (N_t/out_every)*N_q reals;  work: DEVICE, 2*N_t*N_m reals
+ *   tt_d2q_apply:        q = Q d_obs = F_q m_map(d_obs), the QoI prediction of eq (4.11) / (4.14) without a stored Q;
+ *                        form as in tt_map_infer;  d_obs: N_t*N_d reals;  work: N_t*N_m reals (receives m_map);  q: as v
+ * Columns of Gamma_post(q) (800 x 800 in the paper) and rows of Q come from unit vectors, as in the paper. */
+int tt_postcov_q_apply(const tt_map* m, const tt_plan* Fq, const tt_plan* Gq, const void* v, void* work, void* out,
+                       void* stream);
+int tt_d2q_apply(const tt_map* m, const tt_plan* Fq, int form, const void* d_obs, void* work, void* q, void* stream);
+
 /* eq (4.13) in two halves, split at the one exchange step of the N_m-sharded path (DESIGN.md section 6 / 11):
  *   tt_map_infer_partial:  y = Gamma_noise^{-1} d_obs (kept in the tt_map), a = G* y -> a_scratch (N_t*N_m reals),
  *                          b = F a -> b (N_t*N_d reals).  On a rank that holds a parameter slice, b is its PARTIAL

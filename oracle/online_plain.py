@@ -159,3 +159,18 @@ def K_entry(F_s, G_s2, i: int, i2: int, noise: float = 0.0) -> float:
     for j in range(min(i, i2) + 1):
         acc += float(np.dot(np.asarray(F_s[i - j], dtype=np.float64), np.asarray(G_s2[i2 - j], dtype=np.float64)))
     return acc + noise
+
+
+# ---------------------------------------------------------------------------------------------
+# Phase 3: QoI posterior covariance and the data-to-QoI map, through the p2q map F_q on its
+# coarser output grid (oracle/toeplitz_plain.matvec_decimated, reading R19) and G_q* = Gamma_prior F_q*.
+# ---------------------------------------------------------------------------------------------
+def post_cov_q_apply(F, G, L, Fq, Gq, r: int, v) -> np.ndarray:
+    """Gamma_post(q) v = F_q (I - G* K^{-1} F) G_q* v, eq (4.10) (PAPER.md:323).  v: [N_t/r, N_q]."""
+    a = tp.rmatvec_decimated(Gq, v, r)                     # G_q* v
+    return tp.matvec_decimated(Fq, smw_apply(F, G, L, a), r)
+
+
+def d2q_apply(F, G, noise_var, L, Fq, r: int, d_obs) -> np.ndarray:
+    """q_map = Q d_obs with Q = F_q (I - G* K^{-1} F) G* Gamma_noise^{-1}, eq (4.11)/(4.14), m_prior = 0."""
+    return tp.matvec_decimated(Fq, map_point(F, G, noise_var, L, d_obs), r)

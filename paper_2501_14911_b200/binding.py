@@ -87,6 +87,8 @@ def lib() -> ctypes.CDLL:
         "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
         "tt_map_infer_host": (ci, [vp, ci, vp, vp, vp]),
         "tt_smw_apply": (ci, [vp, vp, vp, vp]),
+        "tt_postcov_q_apply": (ci, [vp, vp, vp, vp, vp, vp, vp]),
+        "tt_d2q_apply": (ci, [vp, vp, ci, vp, vp, vp, vp]),
         "tt_map_infer_partial": (ci, [vp, vp, vp, vp, vp]),
         "tt_map_infer_finish": (ci, [vp, vp, vp, vp]),
     }
@@ -105,7 +107,8 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
            "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
-           "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply"]
+           "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
+           "tt_postcov_q_apply", "tt_d2q_apply"]
 
 
 def _stream(stream) -> int:
@@ -317,6 +320,14 @@ def tt_map_infer(m: int, form: int, d_obs, m_map, stream=None) -> None:
 
 def tt_smw_apply(m: int, u, out, stream=None) -> None:
     _check("tt_smw_apply", lib().tt_smw_apply(m, _ptr(u), _ptr(out), _stream(stream)))
+
+
+def tt_postcov_q_apply(m: int, Fq: int, Gq: int, v, work, out, stream=None) -> None:
+    _check("tt_postcov_q_apply", lib().tt_postcov_q_apply(m, Fq, Gq, _ptr(v), _ptr(work), _ptr(out), _stream(stream)))
+
+
+def tt_d2q_apply(m: int, Fq: int, form: int, d_obs, work, q, stream=None) -> None:
+    _check("tt_d2q_apply", lib().tt_d2q_apply(m, Fq, form, _ptr(d_obs), _ptr(work), _ptr(q), _stream(stream)))
 
 
 def tt_map_infer_partial(m: int, d_obs, a_scratch, b, stream=None) -> None:

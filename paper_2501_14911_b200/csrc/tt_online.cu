@@ -436,6 +436,39 @@ int tt_smw_apply(const tt_map* m, const void* u, void* out, void* stream) {
     return smw_typed<double>(m, static_cast<const double*>(u), static_cast<double*>(out), s);
 }
 
+// Phase 3 as compositions of the calls above with the p2q plans (tt_plan_create_coarse):
+//   Gamma_post(q) v = F_q (I - G* K^{-1} F) G_q* v  (eq 4.10);   q_map = F_q m_map(d_obs) = Q d_obs  (eq 4.11, 4.14)
+namespace {
+bool q_plans_fit(const tt_map* m, const tt_plan* Fq, const tt_plan* Gq) {
+    const PlanInfo a = plan_info(Fq);
+    if (a.N_m != m->pi.N_m || a.N_t != m->pi.N_t || a.dtype != m->pi.dtype || a.layout != m->pi.layout) return false;
+    if (!Gq) return true;
+    const PlanInfo b = plan_info(Gq);
+    return b.N_d == a.N_d && b.N_m == a.N_m && b.N_t == a.N_t && b.dtype == a.dtype && b.layout == a.layout && b.dec == a.dec;
+}
+}  // namespace
+
+int tt_postcov_q_apply(const tt_map* m, const tt_plan* Fq, const tt_plan* Gq, const void* v, void* work, void* out,
+                       void* stream) {
+    if (!m || !Fq || !Gq || !v || !work || !out || !m->F) return TT_ERR_NULL;
+    if (!q_plans_fit(m, Fq, Gq)) return TT_ERR_MISMATCH;
+    const size_t nm = (size_t)m->pi.N_m * m->pi.N_t * esize(m->pi.dtype);
+    void* a = work;
+    void* u = static_cast<char*>(work) + nm;
+    int rc;
+    if ((rc = tt_rmatvec(Gq, v, a, stream)) != TT_OK) return rc;      // a = G_q* v
+    if ((rc = tt_smw_apply(m, a, u, stream)) != TT_OK) return rc;     // u = (I - G* K^{-1} F) a
+    return tt_matvec(Fq, u, out, stream);                             // F_q u
+}
+
+int tt_d2q_apply(const tt_map* m, const tt_plan* Fq, int form, const void* d_obs, void* work, void* q, void* stream) {
+    if (!m || !Fq || !d_obs || !work || !q) return TT_ERR_NULL;
+    if (!q_plans_fit(m, Fq, nullptr)) return TT_ERR_MISMATCH;
+    const int rc = tt_map_infer(m, form, d_obs, work, stream);        // m_map
+    if (rc != TT_OK) return rc;
+    return tt_matvec(Fq, work, q, stream);                            // q_map = F_q m_map
+}
+
 int tt_map_infer_partial(const tt_map* m, const void* d_obs, void* a_scratch, void* b, void* stream) {
     if (!m || !d_obs || !a_scratch || !b || !m->F) return TT_ERR_NULL;
     cudaStream_t s = static_cast<cudaStream_t>(stream);

@@ -402,3 +402,46 @@ def test_smw_operator(tt, dtype, layout):
         mp.close(); chol.close(); pF.close(); pG.close()
     # u - G* K^{-1} F u: the correction is O(1) of u here, both terms carry the matvec bar; the solve amplifies by kappa
     assert rel(got, ref) <= BAR[dtype] + 8 * U[dtype] * kappa
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_phase3_compositions(tt, dtype):
+    """eq (4.10) Gamma_post(q) v and eq (4.11)/(4.14) q_map = Q d_obs through the p2q plans on a coarser output grid."""
+    N_d, N_q, N_m, N_t, r = 4, 3, 600, 30, 5
+    w, F, G, nv, d_obs = online_inputs(N_d, N_m, N_t, dtype)
+    wq = synth.CONFIGS["Q5"].scaled(N_d=N_q, N_m=N_m, N_t=N_t, dtype=dtype)
+    Fq = synth.block_column(wq)
+    Gq = synth.gstar_block_column(wq, Fq)
+    v = synth.vector_d(wq.scaled(N_t=N_t // r), k_rhs=1)
+    Fn, Gn, nvn = F.numpy(), G.numpy(), nv.numpy()
+    K = oo.assemble_K(Fn, Gn, nvn)
+    L = oo.cholesky(K)
+    ev = np.linalg.eigvalsh(K)
+    kappa = ev[-1] / ev[0]
+    ref_pq = oo.post_cov_q_apply(Fn, Gn, L, Fq.numpy(), Gq.numpy(), r, v.numpy())
+    ref_q = oo.d2q_apply(Fn, Gn, nvn, L, Fq.numpy(), r, d_obs.numpy())
+    pF, pG = tt.Plan(F.cuda()), tt.Plan(G.cuda())
+    pFq, pGq = tt.Plan(Fq.cuda(), out_every=r), tt.Plan(Gq.cuda(), out_every=r)
+    chol = tt.Chol(torch.from_numpy(L).cuda())
+    mp = tt.MapInference(pF, pG, chol, nv.cuda())
+    try:
+        work = torch.empty((2, N_t, N_m), dtype=dtype, device="cuda")
+        out = torch.empty((N_t // r, N_q), dtype=dtype, device="cuda")
+        tt.tt_postcov_q_apply(mp.handle, pFq.handle, pGq.handle, v.cuda(), work, out)
+        got_pq = out.cpu().numpy()
+        got_q = {}
+        for form in (tt.TT_MAP_PAPER, tt.TT_MAP_GAIN):
+            tt.tt_d2q_apply(mp.handle, pFq.handle, form, d_obs.cuda(), work, out)
+            got_q[form] = out.cpu().numpy()
+        with pytest.raises(tt.TTError) as ei:                       # a p2q plan of another parameter dimension
+            bad = tt.Plan(Fq[:, :, :500].contiguous().cuda(), out_every=r)
+            try:
+                tt.tt_d2q_apply(mp.handle, bad.handle, tt.TT_MAP_GAIN, d_obs.cuda(), work, out)
+            finally:
+                bad.close()
+        assert ei.value.status == -12
+    finally:
+        mp.close(); chol.close(); pF.close(); pG.close(); pFq.close(); pGq.close()
+    tol = BAR[dtype] + 8 * U[dtype] * kappa
+    assert rel(got_pq, ref_pq) <= tol
+    assert rel(got_q[tt.TT_MAP_PAPER], ref_q) <= tol and rel(got_q[tt.TT_MAP_GAIN], ref_q) <= BAR[dtype] + 8 * U[torch.float64] * kappa

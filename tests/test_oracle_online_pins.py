@@ -178,6 +178,24 @@ def test_smw_operator(N_d, N_m, N_t):
     assert rel(got, m_full) <= 1e-9
 
 
+@pytest.mark.parametrize("N_d,N_m,N_t,N_q,r", [(3, 5, 6, 2, 2), (2, 4, 9, 1, 3), (1, 3, 4, 2, 1)])
+def test_phase3_against_dense(N_d, N_m, N_t, N_q, r):
+    # eq (4.9)/(2.18): Gamma_post(q) = F_q H^{-1} F_q^*;  eq (4.11): Q = F_q H^{-1} F^* Gamma_noise^{-1}, with F_q = S A_q
+    F, Gs, nv, A, Gp = setup(N_d, N_m, N_t)
+    Fq = RNG.standard_normal((N_t, N_q, N_m)) * np.exp(-np.arange(N_t) / 3.0)[:, None, None]
+    G, Gq = oo.gstar_block_column(F, Gs), oo.gstar_block_column(Fq, Gs)
+    L = oo.cholesky(oo.assemble_K(F, G, nv))
+    Aq_fine = dense_from_block_column(Fq)
+    keep = np.concatenate([np.arange(N_q) + (r * (I + 1) - 1) * N_q for I in range(N_t // r)])
+    Aq = Aq_fine[keep]
+    Gn_inv = np.diag(1.0 / nv.ravel())
+    Hinv = np.linalg.inv(A.T @ Gn_inv @ A + np.linalg.inv(Gp))
+    v = RNG.standard_normal((N_t // r, N_q))
+    d_obs = RNG.standard_normal((N_t, N_d))
+    assert rel(oo.post_cov_q_apply(F, G, L, Fq, Gq, r, v), Aq @ Hinv @ Aq.T @ v.ravel()) <= 1e-9
+    assert rel(oo.d2q_apply(F, G, nv, L, Fq, r, d_obs), Aq @ Hinv @ A.T @ Gn_inv @ d_obs.ravel()) <= 1e-9
+
+
 def test_zero_noise_limit_fits_the_data():
     # Gamma_noise -> 0: K -> F G*, so F m_map = F G* K^{-1} d_obs -> d_obs (N_m N_t >= N_d N_t, F full row rank)
     N_d, N_m, N_t = 2, 6, 5
