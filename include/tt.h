@@ -212,7 +212,7 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
 
 /* Tuning hook for experiments (process-wide, affects plans created / calls made afterwards):
  * "fft_T" = series per CTA of the FFT kernels (8, 16, 32; 0 = planner's choice),
- * "fft_threads" = threads per CTA of the FFT kernels (256, 512; 0 = default), "fft_max_radix" = largest
+ * "fft_threads" = threads per CTA of the FFT kernels (256, 320 (inverse kernel, T = 16), 512; 0 = default), "fft_max_radix" = largest
  * register butterfly the planner may use (0 = no limit),
  * "gemv_chunk" = parameters per CTA of the forward matvec (multiple of 64; 0 = planner's choice),
  * "gemv_fwd_warps" = warps per CTA of the forward matvec (1..32; 0 = planner's choice),

@@ -839,7 +839,7 @@ int tt_debug_set(const char* key, int value) {
     if (!key) return TT_ERR_NULL;
     if (!std::strcmp(key, "fft_T")) { fft_debug_force_T(value); return TT_OK; }
     if (!std::strcmp(key, "fft_threads")) {
-        if (value != 0 && value != 256 && value != 512) return TT_ERR_SHAPE;
+        if (value != 0 && value != 256 && value != 320 && value != 512) return TT_ERR_SHAPE;
         fft_debug_force_threads(value);
         return TT_OK;
     }

@@ -233,7 +233,7 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
 // The static 400 variant is held to 64 registers so that FOUR CTAs share an SM (its 51 KB tiles allow it): the phases of a
 // CTA are serial, resident neighbours are what overlaps loads with butterflies - A1 0.445 -> 0.380 ms, B3 0.551 -> 0.479 ms.
 template <typename Tin, typename Tc, typename Tout, int T, int NT, int NS = 0>
-__global__ void __launch_bounds__(NT, NS == 400 ? 4 : NS == 500 ? 3 : 0)
+__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320) ? 3 : 0)
 fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
@@ -296,7 +296,7 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
 // inverse: complex-to-real inverse FFT + truncate + scale                               (A3, B3)
 // ---------------------------------------------------------------------------------------
 template <typename Tc, int T, int NT, int NS = 0>
-__global__ void __launch_bounds__(NT, NS == 400 ? 4 : NS == 500 ? 3 : 0)
+__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320) ? 3 : 0)
 fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
@@ -477,7 +477,9 @@ template <typename Tc>
 static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {
     const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
     if (c.T == 0) return cudaErrorInvalidValue;
-    const int nt = g_force_NT ? g_force_NT : 256;
+    // N_t = 500 = 25 x 20: 320 butterflies per pass-1 round of 16 series - ten warps do it in one round and three such
+    // CTAs at 64 registers share an SM: B3 0.76 -> 0.69 ms (the forward kernel was measured slower that way)
+    const int nt = g_force_NT ? g_force_NT : (sizeof(Tc) == 4 && P.N == 500 && c.T == 16) ? 320 : 256;
     dim3 grid((unsigned)((P.B + c.T - 1) / c.T), (unsigned)ny);
 #define TT_C2R(TT, NT, ...)                                                                                  \
     {                                                                                                        \
@@ -491,6 +493,7 @@ static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, i
         if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_C2R(16, 256, 400) else if (ns == 500) TT_C2R(16, 256, 500) else TT_C2R(16, 256, 256) }
         else                           { if (ns == 512) TT_C2R(16, 256, 512) else TT_C2R(16, 256, 256) }
     }
+    else if (nt == 320 && c.T == 16) { if constexpr (sizeof(Tc) == 4) TT_C2R(16, 320) }
     else if (nt == 512) { if (c.T == 32) TT_C2R(32, 512) else if (c.T == 16) TT_C2R(16, 512) else TT_C2R(8, 512) }
     else                { if (c.T == 32) TT_C2R(32, 256) else if (c.T == 16) TT_C2R(16, 256) else TT_C2R(8, 256) }
 #undef TT_C2R
