@@ -193,9 +193,15 @@ def test_online_p5_full_size_sampled(tt):
     d_obs = synth.vector_d(w, device="cuda", k_rhs=1)
     d_np = d_obs.cpu().numpy().astype(np.float64)
     z_ref = oo.chol_solve(L_h, d_np.reshape(n))
-    del L_h
     z = chol.solve(torch.from_numpy(d_np.reshape(n)).cuda()).cpu().numpy()
     assert rel(z, z_ref) <= 1e-12
+    chol_h = tt.Chol(torch.from_numpy(L_h))       # the same factor from HOST memory: five 1 GiB slabs of block rows
+    try:
+        z_h = chol_h.solve(torch.from_numpy(d_np.reshape(n)).cuda()).cpu().numpy()
+    finally:
+        chol_h.close()
+    assert np.array_equal(z_h, z)
+    del L_h
     G = synth.block_column(w, device="cuda")
     synth.gstar_block_column(w, G, out=G)
     rng = np.random.default_rng(5)
