@@ -445,3 +445,18 @@ def test_phase3_compositions(tt, dtype):
     tol = BAR[dtype] + 8 * U[dtype] * kappa
     assert rel(got_pq, ref_pq) <= tol
     assert rel(got_q[tt.TT_MAP_PAPER], ref_q) <= tol and rel(got_q[tt.TT_MAP_GAIN], ref_q) <= BAR[dtype] + 8 * U[torch.float64] * kappa
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_assemble_K_space_major(tt, dtype):
+    """K's ordering is row = i*N_d + s whatever the plans' layout: unit vectors and results of TT_SPACE_MAJOR plans are permuted."""
+    N_d, N_m, N_t = 3, 200, 14
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    K_ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
+    for k_max in (1, 5):
+        pF, pG = tt.Plan(F.cuda(), layout=1, k_max=k_max), tt.Plan(G.cuda(), layout=1, k_max=k_max)
+        try:
+            K = tt.assemble_K(pF, pG, nv.t().contiguous().cuda()).cpu().numpy()
+        finally:
+            pF.close(); pG.close()
+        assert rel(K, K_ref) <= BAR[dtype]
