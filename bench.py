@@ -169,7 +169,8 @@ def config_dict(w, args):
                         + (f", k={w.k_rhs} right-hand sides" if w.k_rhs > 1 else ""),
             "baseline_config": args.config,
             "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)" if w.k_rhs == 1
-                    else f"one batched F.M + one batched F^T.D, k={w.k_rhs} (batched FFTs + per-frequency DMMA GEMMs)",
+                    else f"one batched F.M + one batched F^T.D, k={w.k_rhs} (batched FFTs + per-frequency "
+                         f"{'complex64 FMA' if w.dtype == torch.float32 else 'DMMA'} GEMMs)",
             "layout": "time-major",
             "out_every": getattr(args, "r_out", 1),
             "parallelism": ("single GPU" if args.gpus == 1 else "replicas only" if args.parallel == "replicas"
@@ -380,6 +381,9 @@ def main() -> int:
                     help="--online: also time the Phase 3 actions Gamma_post(q) v (eq 4.10) and Q d_obs (eq 4.11) with the p2q plans")
     ap.add_argument("--k-cols", type=int, default=64, help="--online: columns of K assembled and timed")
     ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
+    ap.add_argument("--k-rhs", type=int, default=0,
+                    help="run the k-RHS batched calls with k right-hand sides on any config (default: the config's own, "
+                         "32 for C4, else 1); fp32 configs then take the complex64 FMA GEMM path")
     ap.add_argument("--out-every", type=int, default=0,
                     help="data side on every r-th time step (tt_plan_create_coarse); default 10 for Q5 (the p2q map), else 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -387,6 +391,8 @@ def main() -> int:
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = synth.CONFIGS[args.config]
+    if args.k_rhs > 0:
+        w = w.scaled(k_rhs=args.k_rhs)
     if args.impl == "reference":
         return run_reference(args, w)
     if args.online:
@@ -588,6 +594,24 @@ def main() -> int:
             "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
                                "algorithmic_bytes_per_launch": bytes_adj_kernel, "ms_per_launch": adj[1],
                                "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
+        }
+    elif w.dtype == torch.float32:
+        # fp32 k-RHS: register-tiled complex64 FMA GEMMs (tt_gemm32.cu), bound by the FP32 FMA pipe.  Peak derived from the
+        # unit counts of the guide: 148 SMs x 128 FP32 FMA lanes x 2 flop x the SM clock sampled during this run.
+        clk = clocks.summary().get("sm_mhz") or 1965.0
+        peak32 = 148 * 128 * 2 * clk * 1e6 / 1e12
+        flops = 8.0 * n_f * w.N_d * w.N_m * K
+        ach_fwd = flops / (fwd[1] * 1e-3) / 1e12 if fwd[1] > 0 else 0.0
+        ach_adj = flops / (adj[1] * 1e-3) / 1e12 if adj[1] > 0 else 0.0
+        roofline = {
+            "bound": "alu", "kernel": "gemm32_fwd_kernel (k-RHS A2: per-frequency complex64 GEMM, FP32 FMA)",
+            "achieved": ach_fwd, "peak": peak32, "unit": "TFLOP/s", "frac": ach_fwd / peak32, "traffic": None,
+            "peak_kind": f"148 SMs x 128 FMA lanes x 2 flop x {clk:.0f} MHz (nominal FP32 FMA rate; three-register FFMA issues "
+                         "every other cycle per sub-partition on this part, so ~half of it is the practical ceiling)",
+            "algorithmic_flops_per_launch": flops, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
+            "hbm_bytes_per_launch": fhat_bytes + n_f * w.N_m * K * 8,
+            "adjoint_kernel": {"kernel": "gemm32_adj_kernel (k-RHS B2)", "achieved": ach_adj, "frac": ach_adj / peak32,
+                               "ms_per_launch": adj[1]},
         }
     else:
         # the k-RHS per-frequency GEMMs are a dense contraction on the FP64 tensor pipe (DMMA); its peak is

@@ -31,6 +31,12 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // Measured and rejected: packed fma.rn.f32x2 (SASS FFMA2) for the complex MACs - the register-pair shuffles
 // (a.re, a.re), (-a.im, a.im), (b.im, b.re) cost one MOV per FFMA2 and the kernels ran 1.2-1.3x slower on B200.
 
+// The 4 columns of column group tx: {2tx, 2tx+1} and {2 NCG + 2tx, 2 NCG + 2tx + 1}, so that the 8 (or 4) lanes of a
+// quarter-warp read 16-byte pieces of the Xhat / Dhat tile that are CONTIGUOUS (two pieces per lane at stride 32 B cost
+// twice the shared-memory wavefronts: ncu, 8 instead of 4 per LDS.128).
+template <int NCG>
+__device__ __forceinline__ int thread_col(int tx, int j) { return (j < 2 ? 0 : 2 * NCG) + 2 * tx + (j & 1); }
+
 constexpr int KP = 32;        // forward: parameters per pipeline stage
 constexpr int AP = KP + 2;    // A-tile pitch in complex elements (272 B: 16-byte aligned rows, skewed banks)
 constexpr int NC = 32;        // columns per launch: NCG = 8 column groups of 4 (NCG = 4 when only <= 16 are left)
@@ -38,7 +44,7 @@ constexpr int NC = 32;        // columns per launch: NCG = 8 column groups of 4 
 // ---------------------------------------------------------------------------------------
 // forward: partial[((w*nsplit + c)*N_d + s)*k + r0 + r] = sum_{p in split c} Fhat_w[s,p] Xhat_w[p, r0 + r]
 // grid (nsplit, n_f, ceil(N_d / (TY TS))), 8 TY threads = TY sensor rows x 8 column groups; a thread owns TS
-// sensors (ty, ty + TY, ...) x 4 columns.  Shared-memory bandwidth bounds this kernel (every thread re-reads its
+// sensors (ty, ty + TY, ...) x 4 columns (thread_col).  Shared-memory bandwidth bounds this kernel (every thread re-reads its
 // 4 columns of the Xhat tile per parameter), so the sensor tile per thread is made as tall as N_d allows.
 // ---------------------------------------------------------------------------------------
 template <int TS, int TY, int NCG>
@@ -91,10 +97,10 @@ gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c6
         if (it + 1 < n_it) load_stage((it + 1) & 1, it + 1);
         cp_async_commit();
         const c64* a = As + (it & 1) * ROWS * AP + ty * AP;
-        const float4* b = reinterpret_cast<const float4*>(Bs + (it & 1) * KP * NCW + 4 * tx);
+        const float4* b = reinterpret_cast<const float4*>(Bs + (it & 1) * KP * NCW) + tx;
 #pragma unroll 8
         for (int p = 0; p < KP; ++p) {
-            const float4 b01 = b[p * (NCW / 2)], b23 = b[p * (NCW / 2) + 1];
+            const float4 b01 = b[p * (NCW / 2)], b23 = b[p * (NCW / 2) + NCG];   // 8 lanes x 16 B contiguous: no bank conflict
             const c64 bv[4] = {mk<float>(b01.x, b01.y), mk<float>(b01.z, b01.w), mk<float>(b23.x, b23.y),
                                mk<float>(b23.z, b23.w)};
 #pragma unroll
@@ -109,10 +115,12 @@ gemm32_fwd_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Xhat, c6
     for (int i = 0; i < TS; ++i) {
         const int s = s0 + ty + TY * i;
         if (s >= g.N_d) continue;
-        c64* dst = partial + (((long long)w * g.split + c) * g.N_d + s) * g.k + r0 + 4 * tx;
+        c64* dst = partial + (((long long)w * g.split + c) * g.N_d + s) * g.k + r0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (4 * tx + j < kk) dst[j] = acc[i][j];
+        for (int j = 0; j < 4; ++j) {
+            const int col = thread_col<NCG>(tx, j);
+            if (col < kk) dst[col] = acc[i][j];
+        }
     }
 }
 
@@ -169,11 +177,11 @@ gemm32_adj_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Dhat, c6
         if (it + 1 < n_it) load_stage((it + 1) & 1, it + 1);
         cp_async_commit();
         const float4* a = reinterpret_cast<const float4*>(As + (it & 1) * KS * PT + ty * 8);
-        const float4* d = reinterpret_cast<const float4*>(Ds + (it * KS) * NCW + 4 * tx);
+        const float4* d = reinterpret_cast<const float4*>(Ds + (it * KS) * NCW) + tx;
 #pragma unroll
         for (int sl = 0; sl < KS; ++sl) {                  // rows beyond N_d are zero-filled tiles: they add nothing
             if (it * KS + sl >= g.N_d) break;
-            const float4 d01 = d[sl * (NCW / 2)], d23 = d[sl * (NCW / 2) + 1];
+            const float4 d01 = d[sl * (NCW / 2)], d23 = d[sl * (NCW / 2) + NCG];
             const c64 dv[4] = {mk<float>(d01.x, d01.y), mk<float>(d01.z, d01.w), mk<float>(d23.x, d23.y),
                                mk<float>(d23.z, d23.w)};
 #pragma unroll
@@ -192,10 +200,12 @@ gemm32_adj_kernel(const c64* __restrict__ Fhat, const c64* __restrict__ Dhat, c6
     for (int i = 0; i < 8; ++i) {
         const long long p = p0 + ty * 8 + i;
         if (p >= g.N_m) continue;
-        c64* dst = Xout + (long long)w * g.ldx + p * g.k + r0 + 4 * tx;
+        c64* dst = Xout + (long long)w * g.ldx + p * g.k + r0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (4 * tx + j < kk) dst[j] = acc[i][j];
+        for (int j = 0; j < 4; ++j) {
+            const int col = thread_col<NCG>(tx, j);
+            if (col < kk) dst[col] = acc[i][j];
+        }
     }
 }
 
