@@ -224,7 +224,8 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
 int tt_debug_set(const char* key, int value);
 
 /* ======================================================================================
- * Online phase: the data-space solve and the real-time MAP point.
+ * Online phase and what Phases 2-3 of the paper need around it: the data-space
+ * solve, the real-time MAP point, the SMW operator and the QoI actions.
  *
  *   G* := Gamma_prior F*  is block Toeplitz with the structure of F* when the prior is time
  *   invariant: it is the TRANSPOSE-structured operator of the block column
@@ -244,9 +245,9 @@ typedef struct tt_chol tt_chol;
  *   L       n x n doubles, row-major with row pitch ld (>= n) elements, HOST or DEVICE (detected);
  *           only the lower triangle is read; not retained
  *   stream  work is enqueued here and the call returns after it has completed
- * The factor is stored rescaled by the inverses of its 64 x 64 diagonal blocks (strictly lower
- * blocks packed by block row: n^2/2 doubles) so that neither solve has a diagonal solve on its
- * dependency chain (see tt_trsv.cu).  TT_ERR_NOT_SPD if a diagonal entry is <= 0 or not finite. */
+ * The factor is stored rescaled by the inverses of its 64 x 64 diagonal blocks (only the strictly
+ * lower blocks, each contiguous, block row after block row: n^2/2 doubles) so that neither solve
+ * has a diagonal solve on its dependency chain (see tt_trsv.cu).  TT_ERR_NOT_SPD if a diagonal entry is <= 0 or not finite. */
 int tt_chol_create(tt_chol** out, int64_t n, const void* L, int64_t ld, void* stream);
 void tt_chol_destroy(tt_chol* c);
 size_t tt_chol_device_bytes(const tt_chol* c);
@@ -317,7 +318,9 @@ int tt_d2q_apply(const tt_map* m, const tt_plan* Fq, int form, const void* d_obs
 int tt_map_infer_partial(const tt_map* m, const void* d_obs, void* a_scratch, void* b, void* stream);
 int tt_map_infer_finish(const tt_map* m, const void* b, void* m_map, void* stream);
 
-/* Same with HOST vectors (pinned memory recommended): d_obs is copied in and m_map copied out on `stream`. */
+/* Same with HOST vectors (pinned memory recommended): d_obs is copied in on `stream`; m_map is delivered range by range of the
+ * parameter axis on the copy stream of plan G while the final G* action still computes the next range (as tt_rmatvec_host);
+ * `stream` waits for the last copy. */
 int tt_map_infer_host(const tt_map* m, int form, const void* d_obs_host, void* m_map_host, void* stream);
 
 #ifdef __cplusplus
