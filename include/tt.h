@@ -152,6 +152,8 @@ int tt_normal(const tt_plan* plan, const void* m, void* out, void* stream);
  *   M  DEVICE, N_t*N_m*k reals;   D  DEVICE, N_t*N_d*k reals (layouts above). */
 int tt_matvec_batched(const tt_plan* plan, int k, const void* M, void* D, void* stream);
 int tt_rmatvec_batched(const tt_plan* plan, int k, const void* D, void* M, void* stream);
+/* Out = F^T (F M) for k columns at once; the intermediate data vectors live in plan scratch.  Out == M: TT_ERR_ALIAS. */
+int tt_normal_batched(const tt_plan* plan, int k, const void* M, void* Out, void* stream);
 
 /* The same calls with HOST vectors (pinned memory recommended; what bench.py's `e2e` times).  The parameter-sized
  * vector crosses PCIe in 8 ranges of the parameter axis on a copy stream owned by the plan, overlapped with the kernels

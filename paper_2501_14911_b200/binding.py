@@ -63,6 +63,7 @@ def lib() -> ctypes.CDLL:
         "tt_normal": (ci, [vp, vp, vp, vp]),
         "tt_matvec_batched": (ci, [vp, ci, vp, vp, vp]),
         "tt_rmatvec_batched": (ci, [vp, ci, vp, vp, vp]),
+        "tt_normal_batched": (ci, [vp, ci, vp, vp, vp]),
         "tt_matvec_host": (ci, [vp, vp, vp, vp]),
         "tt_rmatvec_host": (ci, [vp, vp, vp, vp]),
         "tt_normal_host": (ci, [vp, vp, vp, vp]),
@@ -102,7 +103,7 @@ def lib() -> ctypes.CDLL:
 
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_coarse", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
-           "tt_matvec_batched", "tt_rmatvec_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
+           "tt_matvec_batched", "tt_rmatvec_batched", "tt_normal_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
@@ -192,6 +193,10 @@ def tt_matvec_batched(plan: int, k: int, M, D, stream=None) -> None:
 
 def tt_rmatvec_batched(plan: int, k: int, D, M, stream=None) -> None:
     _check("tt_rmatvec_batched", lib().tt_rmatvec_batched(plan, k, _ptr(D), _ptr(M), _stream(stream)), plan)
+
+
+def tt_normal_batched(plan: int, k: int, M, Out, stream=None) -> None:
+    _check("tt_normal_batched", lib().tt_normal_batched(plan, k, _ptr(M), _ptr(Out), _stream(stream)), plan)
 
 
 def tt_matvec_host(plan: int, m_host, d_host, stream=None) -> None:

@@ -724,6 +724,16 @@ int tt_rmatvec_batched(const tt_plan* p, int k, const void* D, void* M, void* st
     return TT_OK;
 }
 
+int tt_normal_batched(const tt_plan* p, int k, const void* M, void* Out, void* stream) {
+    int r = check_apply(p, M, Out);
+    if (r) return r;
+    if (M == Out) return TT_ERR_ALIAS;
+    if (k < 1 || k > p->k_max) return TT_ERR_K;
+    r = tt_matvec_batched(p, k, M, p->dwork, stream);      // D = F M stays in plan scratch ([N_t][N_d][k_max] reals)
+    if (r) return r;
+    return tt_rmatvec_batched(p, k, p->dwork, Out, stream);
+}
+
 int tt_matvec_host(const tt_plan* p, const void* m_host, void* d_host, void* stream) {
     int r = check_apply(p, m_host, d_host);
     if (r) return r;

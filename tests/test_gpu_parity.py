@@ -344,3 +344,29 @@ def test_error_codes(tt):
     finally:
         plan.close()
     L.tt_plan_destroy(None)  # NULL-safe
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("layout", [0, 1])
+def test_normal_batched(tt, dtype, layout):
+    """tt_normal_batched: F^T (F M) for k columns, each column equal to the single-vector normal operator of the oracle."""
+    N_d, N_m, N_t, k = 5, 700, 24, 6
+    w = workload("C4", N_d, N_m, N_t, dtype)
+    F = synth.block_column(w)
+    M = synth.vector_m(w, k_rhs=k)
+    lay = (lambda t: t.permute(2, 1, 0).contiguous()) if layout == 1 else (lambda t: t)
+    unlay = (lambda t: t.permute(2, 1, 0)) if layout == 1 else (lambda t: t)
+    plan = tt.Plan(F.cuda(), layout=layout, k_max=8)
+    try:
+        Md = lay(M).cuda()
+        out = torch.empty_like(Md)
+        tt.tt_normal_batched(plan.handle, k, Md, out)
+        got = unlay(out).cpu().numpy()
+        with pytest.raises(tt.TTError):
+            tt.tt_normal_batched(plan.handle, k, Md, Md)
+        with pytest.raises(tt.TTError):
+            tt.tt_normal_batched(plan.handle, 9, Md, out)
+    finally:
+        plan.close()
+    for r in range(k):
+        assert rel(got[..., r], ob.rmatvec(F.numpy(), ob.matvec(F.numpy(), M[..., r].contiguous().numpy()))) <= 2 * TOL[dtype]
