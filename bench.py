@@ -526,8 +526,22 @@ def main() -> int:
         torch.cuda.synchronize()
         return a.elapsed_time(b) / n
 
+    def time_each(fn, n):
+        """Per-call device times (one CUDA event pair per call): median and min over n calls (SURVEY.md 8(d) protocol)."""
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        torch.cuda.synchronize()
+        for a, b in evs:
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        t = sorted(a.elapsed_time(b) for a, b in evs)
+        return {"median": t[len(t) // 2], "min": t[0], "calls": n}
+
     ms_fwd = max_over_ranks(time_op(op_fwd, args.steps))
     ms_adj = max_over_ranks(time_op(op_adj, args.steps))
+    n_each = max(20, args.steps) if K == 1 else max(5, args.steps)
+    each_fwd, each_adj = time_each(op_fwd, n_each), time_each(op_adj, n_each)
     ms_normal = None
     if K == 1:  # F^T F m (one solver iteration, configs[4]); the intermediate d never leaves the device
         n_out = torch.empty_like(m)
@@ -695,6 +709,7 @@ def main() -> int:
         "roofline": roofline,
         "ops": {
             "matvec_ms": ms_fwd, "rmatvec_ms": ms_adj, "normal_ms": ms_normal, "k_rhs": K,
+            "matvec_ms_per_call": each_fwd, "rmatvec_ms_per_call": each_adj,
             "normal_GBs": (2 * fhat_bytes + 2 * w.N_t * w.N_m * es) / (ms_normal * 1e-3) / 1e9 if ms_normal else None,
             "matvec_GBs": bytes_op / (ms_fwd * 1e-3) / 1e9, "rmatvec_GBs": bytes_op / (ms_adj * 1e-3) / 1e9,
             "roofline_bytes_per_op": bytes_op,
