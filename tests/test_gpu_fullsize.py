@@ -265,3 +265,40 @@ def test_K_assembly_p5_full_size_sampled(tt):
             else:
                 ref = oo.K_entry(rows_F[s], rows_G[s2], i, i2)
             assert abs(col[i * w.N_d + s] - ref) <= 1e-5 * max(abs(ref), scale), ((i, s), (i2, s2), col[i * w.N_d + s], ref)
+
+
+def test_online_fp64_full_parameter_dimension(tt):
+    """The fp64 path (complex128 spectrum) at the paper's full parameter and time dimensions (N_m = 263169, N_t = 500) with
+    8 sensors - the configuration of `bench.py --config P5 --online --f64` with fewer sensors, block column handed over as a
+    HOST pointer: m_map = G* K^{-1} d_obs on sampled outputs against the oracle, bar 1e-12 of the rms."""
+    from oracle import online_plain as oo
+    from oracle import toeplitz_plain as op
+    w = synth.CONFIGS["P5"].scaled(N_d=8, dtype=torch.float64)
+    need_memory(40)
+    n = w.N_d * w.N_t
+    G_h = torch.empty((w.N_t, w.N_d, w.N_m), dtype=torch.float64)
+    for s0 in range(0, w.N_d, 4):
+        slab = synth.block_column(w, device="cuda", s_range=(s0, s0 + 4))
+        synth.gstar_block_column(w, slab, out=slab)
+        G_h[:, s0:s0 + 4, :] = slab.cpu()
+        del slab
+    pG = tt.Plan(G_h)                                              # host pointer: streamed through 1 GiB slabs
+    ps = (0, 131072, w.N_m - 1)
+    cols = {p: G_h[:, :, p:p + 1].numpy().copy() for p in ps}
+    del G_h
+    L = synth.factor_standin(n, w.seed, device="cuda")
+    chol = tt.Chol(L)
+    L_h = L.cpu().numpy()
+    del L
+    d_obs = synth.vector_d(w, device="cuda", k_rhs=1)
+    mp = tt.MapInference(None, pG, chol, synth.noise_var(w, device="cuda"))
+    try:
+        m_map = mp.infer(d_obs, tt.TT_MAP_GAIN)
+        scale = float(m_map.pow(2).mean().sqrt())
+        got = {p: m_map[::25, p].cpu().numpy() for p in ps}
+    finally:
+        mp.close(); chol.close(); pG.close()
+    z = oo.chol_solve(L_h, d_obs.cpu().numpy().reshape(n)).reshape(w.N_t, w.N_d)
+    for p in ps:
+        ref = np.array([op.rmatvec_entry(cols[p], z, j, 0) for j in range(0, w.N_t, 25)])
+        assert np.abs(got[p] - ref).max() <= 1e-12 * scale, p
