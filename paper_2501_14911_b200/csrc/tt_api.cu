@@ -119,6 +119,13 @@ void build_pos(int N, const int* radix, int n_stages, std::vector<unsigned short
         pos[k] = (unsigned short)slot;
     }
 }
+// the device table: pos followed by its inverse (slot -> bin), which the inverse kernel's last pass stores through
+static std::vector<unsigned short> with_inverse(const std::vector<unsigned short>& pos) {
+    const size_t N = pos.size();
+    std::vector<unsigned short> t(2 * N);
+    for (size_t k = 0; k < N; ++k) { t[k] = pos[k]; t[N + pos[k]] = (unsigned short)k; }
+    return t;
+}
 
 // tw[k] = exp(-2 pi i k / L), k < L, exact on the axes and symmetric by construction.
 void build_twiddles(int L, std::vector<double>& tw) {
@@ -591,7 +598,10 @@ int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, 
         std::vector<double> tw;
         build_twiddles(L, tw);
         std::vector<unsigned short> pos[2];
-        for (int wch = 0; wch < 2; ++wch) build_pos((int)N_t, radix[wch], n_stages[wch], pos[wch]);
+        for (int wch = 0; wch < 2; ++wch) {
+            build_pos((int)N_t, radix[wch], n_stages[wch], pos[wch]);
+            pos[wch] = with_inverse(pos[wch]);
+        }
         TT_TRY(dev_alloc(p, &p->tw_d, tw.size() * sizeof(double)));
         TT_TRYC(cudaMemcpyAsync(p->tw_d, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         std::vector<float> twf(tw.size());
@@ -858,6 +868,7 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }
+    if (!std::strcmp(key, "gemm_adj_mt")) { gemm_debug_set_adj(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_fwd_warps")) {
         if (value < 0 || value > 32) return TT_ERR_SHAPE;
         gemv_debug_set(value, -1);

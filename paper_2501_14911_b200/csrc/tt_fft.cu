@@ -227,6 +227,116 @@ __device__ __forceinline__ void fft_inplace(Cx<R>* sm, const FftParams& P, int l
     __syncthreads();
 }
 
+// The last pass of the inverse kernel (M == 1, Ns == RAD): like fft_stage, but the outputs go straight to global memory
+// through io(n, value), n = the bin held by the slot - slot blk*RAD + q holds bin ipos[blk*RAD] + q*(N/RAD), q being the
+// most significant digit of the bin index (tt_api.cu build_pos).  No store to shared memory, no barrier, no gather
+// through `pos`; and for even RAD the truncation keeps exactly the outputs q < RAD/2, so the other half of the
+// butterfly is dead code.  (The mirror image - the forward kernel's first pass reading global memory, with or without
+// the zero half of its inputs folded away - was measured slower in both precisions: A1 0.38 -> 0.40 ms at N_t = 400,
+// 0.585 -> 0.61 ms at 500, 7.64 -> 7.73 ms for C4's fp64 batch.  The forward path is therefore left exactly as it was.)
+template <typename R, int T, int RAD, typename IO>
+__device__ __forceinline__ void fft_stage_out(const Cx<R>* __restrict__ sm, int N, int lane_s, int g, int G, const IO& make_io) {
+    const int nb = N / RAD;
+    const auto io = make_io();
+#pragma unroll 1
+    for (int u = g; u < nb; u += G) {
+        const Cx<R>* p = sm + u * RAD * T + lane_s;
+        Cx<R> x[RAD];
+#pragma unroll
+        for (int a = 0; a < RAD; ++a) x[a] = p[a * T];
+        butterfly<R, RAD>(x);
+        const int n0 = (int)io.ipos[u * RAD];
+#pragma unroll
+        for (int q = 0; q < (RAD % 2 == 0 ? RAD / 2 : RAD); ++q) io(n0 + q * nb, x[q]);
+    }
+}
+
+// fft_inplace for the inverse kernel: every pass but the last as above, the last one through fft_stage_out; there is
+// no barrier after it.  N == 1 (no pass): the caller handles it.
+template <typename R, int T, int NS, typename IO>
+__device__ __forceinline__ void fft_inplace_out(Cx<R>* sm, const FftParams& P, int lane_s, int g, int G, const IO& io) {
+    constexpr int MAXR = MaxRadix<R>::value;
+    const Cx<R>* tw = reinterpret_cast<const Cx<R>*>(P.tw);
+    if constexpr (NS != 0 && NS != 500) {
+        using SP = StaticPlan<R, NS>;
+        constexpr int R1 = SP::r1, R2 = SP::r2, R3 = SP::r3;
+        static_assert(R1 * R2 * R3 == NS, "static FFT plan does not match its length");
+        __syncthreads();
+        fft_stage<R, T, R1, true>(sm, tw, NS, NS, NS / R1, 0u, lane_s, g, G);
+        __syncthreads();
+        if constexpr (R3 > 1) {
+            fft_stage<R, T, R2, true>(sm, tw, NS, NS / R1, NS / (R1 * R2), 0u, lane_s, g, G);
+            __syncthreads();
+            fft_stage_out<R, T, R3>(sm, NS, lane_s, g, G, io);
+        } else {
+            fft_stage_out<R, T, R2>(sm, NS, lane_s, g, G, io);
+        }
+        return;
+    }
+    int Ns = P.N;
+    for (int st = 0; st + 1 < P.n_stages; ++st) {
+        __syncthreads();
+        const int r = P.radix[st];
+        const int M = Ns / r;
+        const unsigned mg = P.magic[st];
+        switch (r) {
+            case 2: fft_stage<R, T, 2>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 3: fft_stage<R, T, 3>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 4: fft_stage<R, T, 4>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 5: fft_stage<R, T, 5>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 7: fft_stage<R, T, 7>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            case 8: fft_stage<R, T, 8>(sm, tw, P.N, Ns, M, mg, lane_s, g, G); break;
+            default:
+                if constexpr (MAXR >= 25) {
+                    if (r == 16) fft_stage<R, T, 16>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                    else if (r == 20) fft_stage<R, T, 20>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                    else fft_stage<R, T, 25>(sm, tw, P.N, Ns, M, mg, lane_s, g, G);
+                }
+                break;
+        }
+        Ns = M;
+    }
+    if (P.n_stages == 0) return;
+    __syncthreads();
+    switch (Ns) {  // the last radix
+        case 2: fft_stage_out<R, T, 2>(sm, P.N, lane_s, g, G, io); break;
+        case 3: fft_stage_out<R, T, 3>(sm, P.N, lane_s, g, G, io); break;
+        case 4: fft_stage_out<R, T, 4>(sm, P.N, lane_s, g, G, io); break;
+        case 5: fft_stage_out<R, T, 5>(sm, P.N, lane_s, g, G, io); break;
+        case 7: fft_stage_out<R, T, 7>(sm, P.N, lane_s, g, G, io); break;
+        case 8: fft_stage_out<R, T, 8>(sm, P.N, lane_s, g, G, io); break;
+        default:
+            if constexpr (MAXR >= 25) {
+                if (Ns == 16) fft_stage_out<R, T, 16>(sm, P.N, lane_s, g, G, io);
+                else if (Ns == 20) fft_stage_out<R, T, 20>(sm, P.N, lane_s, g, G, io);
+                else fft_stage_out<R, T, 25>(sm, P.N, lane_s, g, G, io);
+            }
+            break;
+    }
+}
+
+// What the inverse kernel's last pass writes: conj(result)_n = z_n * N, x_{2n} = Re z_n, x_{2n+1} = Im z_n, scaled;
+// only j < N_t is kept (the truncation)
+template <typename Tc>
+struct RealStorer {
+    Tc* dst;
+    long long r_ts;
+    const unsigned short* ipos;  // ipos[slot] = bin held by that slot of the in-place DIF output
+    int N, dec;
+    Tc sc;
+    bool live;
+    __device__ __forceinline__ void st_real(int j, Tc val) const {  // on a coarser grid only every dec-th time step is kept
+        if (dec == 1) dst[(long long)j * r_ts] = val;
+        else if ((j + 1) % dec == 0) dst[(long long)((j + 1) / dec - 1) * r_ts] = val;
+    }
+    __device__ __forceinline__ void operator()(int n, Cx<Tc> v) const {
+        if (live && 2 * n < N) {
+            st_real(2 * n, v.re * sc);
+            if (2 * n + 1 < N) st_real(2 * n + 1, -v.im * sc);
+        }
+    }
+};
+
 // ---------------------------------------------------------------------------------------
 // forward: zero-pad + real-to-complex FFT + frequency-major store          (P0, A1, B1)
 // ---------------------------------------------------------------------------------------
@@ -296,7 +406,7 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
 // inverse: complex-to-real inverse FFT + truncate + scale                               (A3, B3)
 // ---------------------------------------------------------------------------------------
 template <typename Tc, int T, int NT, int NS = 0>
-__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320) ? 3 : 0)
+__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320 || (NS == 0 && NT == 256 && sizeof(Tc) == 4)) ? 3 : 0)
 fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
@@ -307,58 +417,51 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
     const int N = NS ? NS : P.N;
     const Cx<Tc>* src = in + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
 
-    constexpr int UB = 8;
-    for (int k0 = g; k0 <= N; k0 += G * UB) {
-        Cx<Tc> v[UB];
-#pragma unroll
-        for (int u = 0; u < UB; ++u) {
-            const int k = k0 + u * G;
-            v[u] = mk<Tc>(Tc(0), Tc(0));
-            if (live && k <= N) v[u] = src[(long long)k * P.c_fs];
-        }
-#pragma unroll
-        for (int u = 0; u < UB; ++u) {
-            const int k = k0 + u * G;
-            if (k <= N) sm[k * T + lane_s] = v[u];
-        }
-    }
-    __syncthreads();
-
     // Z_k = (X_k + conj X_{N-k}) + i conj(w^k) (X_k - conj X_{N-k});  store conj(Z_k) so that the
-    // forward FFT below yields conj of the inverse transform.  Pairs (k, N-k) are disjoint.
+    // forward FFT below yields conj of the inverse transform.  Pairs (k, N-k) are disjoint; both members are read
+    // from global memory by the thread that needs them, in batches of 2*UB independent requests.
     const Cx<Tc>* tw = reinterpret_cast<const Cx<Tc>*>(P.tw);
-    for (int k = g; k <= N / 2; k += G) {
-        if (k == 0) {
-            const Tc x0 = sm[lane_s].re, xn = sm[N * T + lane_s].re;  // DC, Nyquist: real parts only
-            sm[lane_s] = mk<Tc>(x0 + xn, -(x0 - xn));
-        } else {
-            const int kk = N - k;
-            const Cx<Tc> Xk = sm[k * T + lane_s], Xn = sm[kk * T + lane_s];
-            const Cx<Tc> Zk = (Xk + conj(Xn)) + mul_pi((Xk - conj(Xn)) * conj(tw[k]));
-            if (kk != k) {
-                const Cx<Tc> Zkk = (Xn + conj(Xk)) + mul_pi((Xn - conj(Xk)) * conj(tw[kk]));
-                sm[kk * T + lane_s] = conj(Zkk);
+    constexpr int UB = 4;
+    const int nh = N / 2;
+    for (int k0 = g; k0 <= nh; k0 += G * UB) {
+        Cx<Tc> va[UB], vb[UB];
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int k = k0 + u * G;
+            va[u] = mk<Tc>(Tc(0), Tc(0)); vb[u] = va[u];
+            if (live && k <= nh) {
+                va[u] = src[(long long)k * P.c_fs];
+                vb[u] = src[(long long)(N - k) * P.c_fs];
             }
-            sm[k * T + lane_s] = conj(Zk);
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+            const int k = k0 + u * G;
+            if (k > nh) continue;
+            if (k == 0) {
+                const Tc x0 = va[u].re, xn = vb[u].re;  // DC, Nyquist: real parts only
+                sm[lane_s] = mk<Tc>(x0 + xn, -(x0 - xn));
+            } else {
+                const int kk = N - k;
+                const Cx<Tc> Xk = va[u], Xn = vb[u];
+                const Cx<Tc> Zk = (Xk + conj(Xn)) + mul_pi((Xk - conj(Xn)) * conj(tw[k]));
+                if (kk != k) {
+                    const Cx<Tc> Zkk = (Xn + conj(Xk)) + mul_pi((Xn - conj(Xk)) * conj(tw[kk]));
+                    sm[kk * T + lane_s] = conj(Zkk);
+                }
+                sm[k * T + lane_s] = conj(Zk);
+            }
         }
     }
-    fft_inplace<Tc, T, NS>(sm, P, lane_s, g, G);
-
-    // conj(result)_n = z_n * N:  x_{2n} = Re z_n, x_{2n+1} = Im z_n; keep j < N_t (truncation)
-    if (live) {
-        Tc* dst = out + (long long)blockIdx.y * P.r_ys + b * P.r_bs;
-        const Tc sc = Tc(P.scale);
-        const int dec = P.dec;
-        auto st_real = [&](int j, Tc val) {   // on a coarser grid only every dec-th time step is kept
-            if (dec == 1) dst[(long long)j * P.r_ts] = val;
-            else if ((j + 1) % dec == 0) dst[(long long)((j + 1) / dec - 1) * P.r_ts] = val;
-        };
-        for (int n = g; 2 * n < N; n += G) {
-            const Cx<Tc> v = sm[(int)P.pos[n] * T + lane_s];
-            st_real(2 * n, v.re * sc);
-            if (2 * n + 1 < N) st_real(2 * n + 1, -v.im * sc);
-        }
+    // built where it is used (after the passes over shared memory), so that its fields are not live across them
+    auto stz = [&]() {
+        return RealStorer<Tc>{out + (long long)blockIdx.y * P.r_ys + b * P.r_bs, P.r_ts, P.pos + N, N, P.dec, Tc(P.scale), live};
+    };
+    if (N == 1) {  // no pass
+        __syncthreads();
+        if (g == 0) stz()(0, sm[lane_s]);
     }
+    fft_inplace_out<Tc, T, NS>(sm, P, lane_s, g, G, stz);
 }
 
 // ---------------------------------------------------------------------------------------

@@ -134,11 +134,13 @@ gemm_fwd_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Xhat, c1
 constexpr int kAdjSB = 64;    // sensors per shared-memory block of Dhat
 constexpr int kAdjPT = 256;   // parameters per CTA (4 rounds of 8 warps x 8)
 
-template <int NN>
-__global__ void __launch_bounds__(256, 2)
+// MT = m-tiles (8 parameters each) per warp.  MT = 2 (four warps, like the forward kernel: a B fragment read from shared
+// memory feeds two DMMA groups) or MT = 1 (eight warps).  Either way a round covers 64 parameters of the CTA's 256.
+template <int NN, int MT>
+__global__ void __launch_bounds__(256 / MT, MT == 2 ? 3 : 2)
 gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c128* __restrict__ Xout,
                 const GemmGeom g, const int r0, const int kk) {
-    constexpr int BP = 8 * NN + 2;
+    constexpr int BP = 8 * NN + 2, NTH = 256 / MT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     c128* Ds = reinterpret_cast<c128*>(smem_raw);  // [kAdjSB][BP]
 
@@ -149,7 +151,7 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
     const c128* Dw = Dhat + (long long)w * g.N_d * g.k + r0;
 
     auto stage_d = [&](int sb) {
-        for (int e = tid; e < kAdjSB * 8 * NN; e += 256) {
+        for (int e = tid; e < kAdjSB * 8 * NN; e += NTH) {
             const int row = e / (8 * NN), col = e % (8 * NN);
             c128 v = mk<double>(0.0, 0.0);
             if (sb + row < g.N_d && col < kk) v = Dw[(long long)(sb + row) * g.k + col];
@@ -159,64 +161,80 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
     const bool single = g.N_d <= kAdjSB;  // Dhat_w fits one shared-memory block: stage it once
     if (single) { stage_d(0); __syncthreads(); }
 
-    for (int rd = 0; rd < kAdjPT / 64; ++rd) {  // rounds of 8 warps x 8 parameters
-        const long long p = pblk + rd * 64 + warp * 8 + (lane >> 2);
-        const bool pok = p < g.N_m;
-        double cr[NN][2], ci[NN][2];
+    for (int rd = 0; rd < kAdjPT / 64; ++rd) {  // rounds of 64 parameters: (8 / MT) warps x MT m-tiles x 8
+        long long p[MT];
+        bool pok[MT];
 #pragma unroll
-        for (int nt = 0; nt < NN; ++nt) { cr[nt][0] = cr[nt][1] = ci[nt][0] = ci[nt][1] = 0.0; }
+        for (int mt = 0; mt < MT; ++mt) {
+            p[mt] = pblk + rd * 64 + (warp * MT + mt) * 8 + (lane >> 2);
+            pok[mt] = p[mt] < g.N_m;
+        }
+        double cr[MT][NN][2], ci[MT][NN][2];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < NN; ++nt) { cr[mt][nt][0] = cr[mt][nt][1] = ci[mt][nt][0] = ci[mt][nt][1] = 0.0; }
 
         for (int sb = 0; sb < g.N_d; sb += kAdjSB) {
             if (!single) { __syncthreads(); stage_d(sb); __syncthreads(); }
             const int ns = g.N_d - sb < kAdjSB ? g.N_d - sb : kAdjSB;
             const int nsteps = (ns + 3) / 4;
-            const c128* col = Fw + (long long)(sb + (lane & 3)) * g.ldp + (pok ? p : 0);
-            // software pipeline over batches of 4 k-steps: the A fragments of batch b+1 are in flight
+            const c128* row = Fw + (long long)(sb + (lane & 3)) * g.ldp;
+            // software pipeline over batches of BK k-steps: the A fragments of batch b+1 are in flight
             // while the DMMAs of batch b issue
-            auto load_batch = [&](c128 (&af)[4], int t0) {
+            constexpr int BK = MT == 1 ? 4 : 2;
+            auto load_batch = [&](c128 (&af)[MT][BK], int t0) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < BK; ++u) {
                     const int t = t0 + u;
-                    af[u] = mk<double>(0.0, 0.0);
-                    if (pok && t < nsteps && sb + 4 * t + (lane & 3) < g.N_d) {
-                        const double2 v = ldg_stream(reinterpret_cast<const double2*>(col + (long long)(4 * t) * g.ldp));
-                        af[u] = mk<double>(v.x, v.y);
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        af[mt][u] = mk<double>(0.0, 0.0);
+                        if (pok[mt] && t < nsteps && sb + 4 * t + (lane & 3) < g.N_d) {
+                            const double2 v = ldg_stream(reinterpret_cast<const double2*>(row + (long long)(4 * t) * g.ldp + p[mt]));
+                            af[mt][u] = mk<double>(v.x, v.y);
+                        }
                     }
                 }
             };
-            auto mma_batch = [&](const c128 (&af)[4], int t0) {
+            auto mma_batch = [&](const c128 (&af)[MT][BK], int t0) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < BK; ++u) {
                     const int t = t0 + u;
                     if (t < nsteps) {
                         const c128* b = Ds + (4 * t + (lane & 3)) * BP + (lane >> 2);
 #pragma unroll
                         for (int nt = 0; nt < NN; ++nt) {
                             const c128 bf = b[nt * 8];
-                            dmma(cr[nt][0], cr[nt][1], af[u].re, bf.re);
-                            dmma(cr[nt][0], cr[nt][1], af[u].im, bf.im);
-                            dmma(ci[nt][0], ci[nt][1], af[u].re, bf.im);
-                            dmma(ci[nt][0], ci[nt][1], -af[u].im, bf.re);
+#pragma unroll
+                            for (int mt = 0; mt < MT; ++mt) {
+                                dmma(cr[mt][nt][0], cr[mt][nt][1], af[mt][u].re, bf.re);
+                                dmma(cr[mt][nt][0], cr[mt][nt][1], af[mt][u].im, bf.im);
+                                dmma(ci[mt][nt][0], ci[mt][nt][1], af[mt][u].re, bf.im);
+                                dmma(ci[mt][nt][0], ci[mt][nt][1], -af[mt][u].im, bf.re);
+                            }
                         }
                     }
                 }
             };
-            c128 a0[4], a1[4];
+            c128 a0[MT][BK], a1[MT][BK];
             load_batch(a0, 0);
-            for (int t0 = 0; t0 < nsteps; t0 += 8) {
-                load_batch(a1, t0 + 4);
+            for (int t0 = 0; t0 < nsteps; t0 += 2 * BK) {
+                load_batch(a1, t0 + BK);
                 mma_batch(a0, t0);
-                load_batch(a0, t0 + 8);
-                mma_batch(a1, t0 + 4);
+                load_batch(a0, t0 + 2 * BK);
+                mma_batch(a1, t0 + BK);
             }
         }
-        if (pok) {
-            c128* dst = Xout + (long long)w * g.ldx + p * g.k + r0;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) {
+            if (!pok[mt]) continue;
+            c128* dst = Xout + (long long)w * g.ldx + p[mt] * g.k + r0;
 #pragma unroll
             for (int nt = 0; nt < NN; ++nt) {
                 const int r = nt * 8 + (lane & 3) * 2;
-                if (r < kk) dst[r] = mk<double>(cr[nt][0], ci[nt][0]);
-                if (r + 1 < kk) dst[r + 1] = mk<double>(cr[nt][1], ci[nt][1]);
+                if (r < kk) dst[r] = mk<double>(cr[mt][nt][0], ci[mt][nt][0]);
+                if (r + 1 < kk) dst[r + 1] = mk<double>(cr[mt][nt][1], ci[mt][nt][1]);
             }
         }
     }
@@ -262,15 +280,25 @@ static cudaError_t fwd_launch_nn(const c128* F, const c128* X, c128* P, const Ge
     return cudaGetLastError();
 }
 
+static int g_adj_mt = 2;   // m-tiles per warp of the adjoint kernel (debug key "gemm_adj_mt"; 2 measured 2.3% faster on C4)
+void gemm_debug_set_adj(int mt) { g_adj_mt = mt == 1 ? 1 : 2; }
+
 template <int NN>
 static cudaError_t adj_launch_nn(const c128* F, const c128* D, c128* X, const GemmGeom& g, int r0, int kk,
                                  cudaStream_t s) {
-    auto k = gemm_adj_kernel<NN>;
     const size_t smem = (size_t)kAdjSB * (8 * NN + 2) * sizeof(c128);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((g.N_m + kAdjPT - 1) / kAdjPT), (unsigned)g.n_f);
-    k<<<grid, 256, smem, s>>>(F, D, X, g, r0, kk);
+    if (g_adj_mt == 2) {
+        auto k = gemm_adj_kernel<NN, 2>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, 128, smem, s>>>(F, D, X, g, r0, kk);
+    } else {
+        auto k = gemm_adj_kernel<NN, 1>;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k<<<grid, 256, smem, s>>>(F, D, X, g, r0, kk);
+    }
     return cudaGetLastError();
 }
 

@@ -36,7 +36,8 @@ struct FftParams {
                             // each from {2,3,4,5,7,8,16,20,25}
     unsigned magic[kMaxStages];  // ceil(2^32 / M_st), M_st = block length after pass st (exact u / M_st for u < 2^16)
     const void* tw;         // Cx<Tc>[2N]: tw[k] = exp(-2 pi i k / (2N))
-    const unsigned short* pos;  // pos[k] = slot of the in-place DIF output that holds bin k
+    const unsigned short* pos;  // pos[k] = slot of the in-place DIF output that holds bin k, k < N; followed by the
+                                // inverse table: pos[N + slot] = bin held by that slot
     long long B;            // series per y-row
     long long B_store;      // forward only: series in [B, B_store) are stored as zeros (row padding)
     long long r_ys, r_bs, r_ts;
@@ -99,6 +100,8 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
                             cudaStream_t s);
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s);
+
+void gemm_debug_set_adj(int m_tiles_per_warp);  // 1 or 2 (default)
 
 // complex64 FMA GEMMs of TT_F32 plans (tt_gemm32.cu); N_d <= kGemm32MaxNd for the adjoint (Dhat_w lives in shared memory)
 constexpr int kGemm32MaxNd = 768;
