@@ -160,6 +160,26 @@ def test_impulse_returns_block_column(tt, dtype):
         plan.close()
 
 
+# Transform lengths that walk every kind of pass sequence of the FFT kernels: no pass (1), a single pass (first = last:
+# 2, 3, 4, 8, 25), an odd last radix (9, 27, 125, 343, 625), an even one whose upper output half is dead code
+# (686 = 7*7*7*2, 1000, 1024), and three- and four-pass plans; 37 series leave a ragged last tile of 5.
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("N_t", [2, 3, 4, 8, 9, 25, 27, 125, 343, 625, 686, 1000, 1024])
+def test_fft_pass_sequences_vs_oracle(tt, N_t, dtype):
+    w = workload("C2", 2, 37, N_t, dtype)
+    F, m, d = inputs(w)
+    plan = tt.Plan(F.cuda())
+    try:
+        got_d = plan.matvec(m.cuda()).cpu().numpy()
+        got_m = plan.rmatvec(d.cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    orc = op if N_t * N_t * 2 * 37 < 2e6 else ob
+    tol = TOL[dtype]
+    assert rel(got_d, orc.matvec(F.numpy(), m.numpy())) <= tol
+    assert rel(got_m, orc.rmatvec(F.numpy(), d.numpy())) <= tol
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
 def test_adjoint_identity_linearity_shift_on_gpu(tt, dtype):
     w = workload("C5", 6, 777, 60, dtype)
