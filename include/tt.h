@@ -273,6 +273,21 @@ int tt_chol_trsv(const tt_chol* c, int transposed, const void* b, void* x, void*
 int tt_assemble_K(const tt_plan* F, const tt_plan* G, const void* noise_var, int64_t col0, int64_t ncols,
                   void* K, int64_t ldk, void* stream);
 
+/* The same K = Gamma_noise + F G*, all of it, straight from the two block columns and without any matvec.  F is block
+ * lower-triangular Toeplitz and G* = Gamma_prior F* block upper-triangular Toeplitz, so entry ((i,r),(t,s)) of
+ * F G* is  sum_{j=0..min(i,t)} F_{i-j}[r,:] . G_{t-j}[s,:] : with W = Fcol Gcol^T (one real n x n x N_m GEMM of the block columns
+ * seen as n x N_m matrices) it is W[(i,r),(t,s)] plus the entry one block up the block diagonal.  The paper's column-by-column
+ * recipe (what tt_assemble_K does) costs 2 n FFT matvecs; this costs n^2 N_m multiply-adds (K is symmetric: the
+ * lower triangle is computed, the upper one mirrored).
+ *   Fcol, Gcol  DEVICE, [N_t][N_d][N_m] reals of `dtype`, N_m fastest: the first block columns F_k and G_k = F_k Gamma_prior
+ *               (the arrays tt_plan_create takes with TT_TIME_MAJOR); no alignment requirement
+ *   noise_var   DEVICE, [N_t][N_d] reals of `dtype`: the diagonal of Gamma_noise
+ *   K           DEVICE, n x n doubles, row-major, pitch ldk (>= n), n = N_t*N_d, row = i*N_d + s; overwritten entirely
+ * TT_F32: products and sums over runs of 8192 parameters in fp32, everything above that in fp64; TT_F64: fp64 throughout.
+ * Asynchronous on `stream`, no allocation. */
+int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m, int64_t N_t,
+                         int dtype, void* K, int64_t ldk, void* stream);
+
 typedef struct tt_map tt_map;
 typedef enum tt_map_form {
     TT_MAP_PAPER = 0,  /* eq (4.13) as written: G*, F, K-solve, G* (footnote 14); by linearity the

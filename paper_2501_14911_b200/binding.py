@@ -83,6 +83,7 @@ def lib() -> ctypes.CDLL:
         "tt_chol_solve": (ci, [vp, vp, vp, vp]),
         "tt_chol_trsv": (ci, [vp, ci, vp, vp, vp]),
         "tt_assemble_K": (ci, [vp, vp, vp, i64, i64, vp, i64, vp]),
+        "tt_assemble_K_direct": (ci, [vp, vp, vp, i64, i64, i64, ci, vp, i64, vp]),
         "tt_map_create": (ci, [pp, vp, vp, vp, vp, vp]),
         "tt_map_destroy": (None, [vp]),
         "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
@@ -107,7 +108,7 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
-           "tt_chol_trsv", "tt_assemble_K", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
+           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
            "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
            "tt_postcov_q_apply", "tt_d2q_apply"]
 
@@ -309,6 +310,11 @@ def tt_assemble_K(F: int, G: int, noise_var, col0: int, ncols: int, K, ldk: int,
     _check("tt_assemble_K", lib().tt_assemble_K(F, G, _ptr(noise_var), col0, ncols, _ptr(K), ldk, _stream(stream)), F)
 
 
+def tt_assemble_K_direct(Fcol, Gcol, noise_var, N_d: int, N_m: int, N_t: int, dtype: int, K, ldk: int, stream=None) -> None:
+    _check("tt_assemble_K_direct", lib().tt_assemble_K_direct(_ptr(Fcol), _ptr(Gcol), _ptr(noise_var), N_d, N_m, N_t, dtype,
+                                                                _ptr(K), ldk, _stream(stream)))
+
+
 def tt_map_create(F: int | None, G: int, chol: int, noise_var, stream=None) -> int:
     out = ctypes.c_void_p()
     _check("tt_map_create", lib().tt_map_create(ctypes.byref(out), F, G, chol, _ptr(noise_var), _stream(stream)))
@@ -468,6 +474,18 @@ def assemble_K(F: Plan, G: Plan, noise_var: torch.Tensor, cols: tuple[int, int] 
     K = torch.zeros((n, n), dtype=torch.float64, device="cuda") if out is None else out
     col0, ncols = cols if cols is not None else (0, n)
     tt_assemble_K(F.handle, G.handle, noise_var, col0, ncols, K, K.stride(0), stream)
+    return K
+
+
+def assemble_K_direct(Fcol: torch.Tensor, Gcol: torch.Tensor, noise_var: torch.Tensor, out: torch.Tensor | None = None,
+                      stream=None) -> torch.Tensor:
+    """K = Gamma_noise + F G* from the [N_t, N_d, N_m] block columns F_k and G_k = F_k Gamma_prior (no plans, no matvecs)."""
+    N_t, N_d, N_m = Fcol.shape
+    assert Gcol.shape == Fcol.shape and Gcol.dtype == Fcol.dtype and Fcol.is_contiguous() and Gcol.is_contiguous()
+    n = N_t * N_d
+    K = torch.empty((n, n), dtype=torch.float64, device="cuda") if out is None else out
+    tt_assemble_K_direct(Fcol, Gcol, noise_var, N_d, N_m, N_t, TT_F32 if Fcol.dtype == torch.float32 else TT_F64,
+                         K, K.stride(0), stream)
     return K
 
 

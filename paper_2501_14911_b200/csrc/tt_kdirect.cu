@@ -1,0 +1,217 @@
+// tt_kdirect.cu - tt_assemble_K_direct: K = Gamma_noise + F G* straight from the two block columns, without a single matvec.
+//
+// F is block lower-triangular Toeplitz with blocks F_k, G* = Gamma_prior F* block upper-triangular Toeplitz with
+// blocks G_k^T, G_k = F_k Gamma_prior, so that row (i, r) of F times column (t, s) of G* is
+//
+//     (F G*)[(i,r),(t,s)] = sum_{j = 0 .. min(i,t)}  F_{i-j}[r,:] . G_{t-j}[s,:] .
+//
+// With  W[(i,r),(t,s)] = F_i[r,:] . G_t[s,:]  - ONE real GEMM  W = Fcol Gcol^T  of the block columns viewed as n x N_m matrices,
+// n = N_t N_d - the sum telescopes down every block diagonal:
+//
+//     (F G*)[(i,r),(t,s)] = W[(i,r),(t,s)] + (F G*)[(i-1,r),(t-1,s)] .
+//
+// The paper forms K "column by column", one G* action and one F action per unit data vector (24 500 x 22 ms
+// on 24 A100); tt_assemble_K does that with batched FFT matvecs (4.1 ms per column on one B200).  The same matrix costs
+// 2 n^2 N_m flop this way (half of it: K is symmetric, only the lower triangle is computed and then mirrored) and no FFT at all.
+//
+//   1. kd_gemm_kernel     W (lower tiles) = Fcol Gcol^T, fp32 or fp64 FMA, register-tiled, into K (fp64)
+//   2. kd_diag_kernel     in-place running sums down the block diagonals of the lower triangle, + Gamma_noise on the diagonal
+//   3. kd_mirror_kernel   upper triangle := transpose of the lower one
+//
+// Precision: TT_F32 multiplies and accumulates in fp32 over chunks of 8192 parameters and adds the chunk sums, and the running
+// sums of step 2, in fp64; TT_F64 is fp64 throughout.
+#include "../../include/tt.h"
+#include "tt_common.cuh"
+#include "tt_internal.h"
+
+namespace tt {
+namespace {
+
+constexpr int kKdBM = 128;     // rows of Fcol per CTA tile
+constexpr int kKdBK = 32;      // parameters per shared-memory stage
+constexpr int kKdThreads = 256;  // 16 x 16 threads, a thread owns 8 x TN entries (rows ty + 16 i, columns tx + 16 j)
+constexpr int kKdChunkTiles = 256;  // TT_F32: flush the fp32 accumulators into the fp64 result every 256 stages = 8192 parameters
+
+template <typename R> struct KdVec;
+template <> struct KdVec<float> { using type = float4; static constexpr int n = 4; };
+template <> struct KdVec<double> { using type = double2; static constexpr int n = 2; };
+__device__ __forceinline__ float kd_get(const float4& v, int i) { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
+__device__ __forceinline__ double kd_get(const double2& v, int i) { return i == 0 ? v.x : v.y; }
+
+// C[a][b] (+)= sum_k A[a][k] B[b][k] for the tiles that touch the lower triangle; A, B: n x Kdim row-major (pitch Kdim, any
+// alignment: scalar loads, a warp reads 32 consecutive k of one row).  Shared memory holds [row][k] with a pitch of
+// 32 + 16 bytes, so that the 16-byte fragment loads of 8 consecutive rows fall into 8 different bank groups.
+template <typename R, int TN>
+__global__ void __launch_bounds__(kKdThreads, 1)
+kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restrict__ C, const long long n,
+               const long long Kdim, const long long ldc, const int chunk_tiles) {
+    using V = typename KdVec<R>::type;
+    constexpr int KV = KdVec<R>::n, P = kKdBK + KV, BN = 16 * TN, ROWS = kKdBM + BN;
+    constexpr int LA = kKdBM / 8, LB = BN / 8;   // rows of the A / B tile loaded per thread and stage
+    const int tn = blockIdx.x, tm = blockIdx.y;
+    if ((long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;   // tile entirely above the diagonal
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    R* sm = reinterpret_cast<R*>(smem_raw);   // [2][ROWS][P]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, tx = tid & 15, ty = tid >> 4;
+    const long long rowA0 = (long long)tm * kKdBM, rowB0 = (long long)tn * BN;
+    const R* pa = A + (rowA0 + warp) * Kdim + lane;
+    const R* pb = B + (rowB0 + warp) * Kdim + lane;
+    unsigned okA = 0, okB = 0;
+#pragma unroll
+    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < n ? 1u : 0u) << i;
+#pragma unroll
+    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < n ? 1u : 0u) << i;
+
+    R pre[LA + LB];
+    auto gload = [&](long long k0) {
+        const bool kok = k0 + lane < Kdim;
+#pragma unroll
+        for (int i = 0; i < LA; ++i) pre[i] = (kok && ((okA >> i) & 1u)) ? __ldg(pa + k0 + (long long)(8 * i) * Kdim) : R(0);
+#pragma unroll
+        for (int i = 0; i < LB; ++i) pre[LA + i] = (kok && ((okB >> i) & 1u)) ? __ldg(pb + k0 + (long long)(8 * i) * Kdim) : R(0);
+    };
+    auto sstore = [&](int stage) {
+        R* s = sm + stage * (ROWS * P);
+#pragma unroll
+        for (int i = 0; i < LA; ++i) s[(warp + 8 * i) * P + lane] = pre[i];
+#pragma unroll
+        for (int i = 0; i < LB; ++i) s[(kKdBM + warp + 8 * i) * P + lane] = pre[LA + i];
+    };
+
+    R acc[8][TN];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) acc[i][j] = R(0);
+
+    const long long nk = (Kdim + kKdBK - 1) / kKdBK;
+    bool first = true;
+    gload(0);
+    sstore(0);
+    __syncthreads();
+    for (long long t = 0; t < nk; ++t) {
+        if (t + 1 < nk) gload((t + 1) * kKdBK);
+        const R* s = sm + (int)(t & 1) * (ROWS * P);
+#pragma unroll
+        for (int g = 0; g < kKdBK / KV; ++g) {
+            V a[8], b[TN];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const V*>(s + (ty + 16 * i) * P + g * KV);
+#pragma unroll
+            for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const V*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
+#pragma unroll
+            for (int kk = 0; kk < KV; ++kk)
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) acc[i][j] = fma(kd_get(a[i], kk), kd_get(b[j], kk), acc[i][j]);
+        }
+        if (t + 1 < nk) sstore((int)((t + 1) & 1));
+        __syncthreads();
+        if ((t + 1) % chunk_tiles == 0 || t + 1 == nk) {   // chunk sums meet in fp64, in a fixed order
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const long long row = rowA0 + ty + 16 * i;
+#pragma unroll
+                for (int j = 0; j < TN; ++j) {
+                    const long long col = rowB0 + tx + 16 * j;
+                    if (row < n && col < n) {
+                        double* c = C + row * ldc + col;
+                        *c = (first ? 0.0 : *c) + (double)acc[i][j];
+                    }
+                    acc[i][j] = R(0);
+                }
+            }
+            first = false;
+        }
+    }
+}
+
+// Lower triangle, in place: K[a][b] := sum_{j >= 0} W[a - j N_d][b - j N_d]  (+ noise_var[a] if a == b).  One thread per
+// chain = per start (a0, b0) in the first block column (b0 < N_d, a0 >= b0); consecutive threads are consecutive b0.
+template <typename R>
+__global__ void __launch_bounds__(256)
+kd_diag_kernel(double* __restrict__ K, const R* __restrict__ noise_var, const long long n, const int N_d,
+               const long long ldk) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long a0 = idx / N_d;
+    const int b0 = (int)(idx - a0 * N_d);
+    if (a0 >= n || b0 > a0) return;
+    double run = 0.0;
+    long long a = a0, b = b0;
+    for (; a < n; a += N_d, b += N_d) {
+        double* p = K + a * ldk + b;
+        run += *p;
+        *p = a == b ? run + (double)noise_var[a] : run;
+    }
+}
+
+// K[b][a] := K[a][b] for a > b, through 32 x 32 shared-memory tiles
+__global__ void __launch_bounds__(256)
+kd_mirror_kernel(double* __restrict__ K, const long long n, const long long ldk) {
+    __shared__ double tile[32][33];
+    const int tj = blockIdx.x, ti = blockIdx.y;
+    if (tj > ti) return;
+    const int x = threadIdx.x & 31, y0 = threadIdx.x >> 5;
+    for (int y = y0; y < 32; y += 8) {
+        const long long a = (long long)ti * 32 + y, b = (long long)tj * 32 + x;
+        tile[y][x] = (a < n && b < n) ? K[a * ldk + b] : 0.0;
+    }
+    __syncthreads();
+    for (int y = y0; y < 32; y += 8) {
+        const long long b = (long long)tj * 32 + y, a = (long long)ti * 32 + x;   // writes K[b][a], a fastest
+        if (a < n && b < n && a > b) K[b * ldk + a] = tile[x][y];
+    }
+}
+
+template <typename R, int TN>
+cudaError_t kd_run(const R* Fcol, const R* Gcol, const R* noise_var, long long N_d, long long N_m, long long N_t, double* K,
+                   long long ldk, cudaStream_t s) {
+    constexpr int P = kKdBK + KdVec<R>::n, BN = 16 * TN;
+    const long long n = N_t * N_d;
+    auto k = kd_gemm_kernel<R, TN>;
+    const size_t smem = (size_t)2 * (kKdBM + BN) * P * sizeof(R);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((unsigned)((n + BN - 1) / BN), (unsigned)((n + kKdBM - 1) / kKdBM));
+    const int chunk = sizeof(R) == 4 ? kKdChunkTiles : 0x7fffffff;
+    k<<<grid, kKdThreads, smem, s>>>(Fcol, Gcol, K, n, N_m, ldk, chunk);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    const long long chains = n * N_d;
+    kd_diag_kernel<R><<<(unsigned)((chains + 255) / 256), 256, 0, s>>>(K, noise_var, n, (int)N_d, ldk);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    const unsigned nt = (unsigned)((n + 31) / 32);
+    kd_mirror_kernel<<<dim3(nt, nt), 256, 0, s>>>(K, n, ldk);
+    return cudaGetLastError();
+}
+
+}  // namespace
+}  // namespace tt
+
+extern "C" int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m,
+                                    int64_t N_t, int dtype, void* K, int64_t ldk, void* stream) {
+    using namespace tt;
+    if (!Fcol || !Gcol || !noise_var || !K) return TT_ERR_NULL;
+    if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
+    if (N_d < 1 || N_m < 1 || N_t < 1 || N_d > 65535) return TT_ERR_SHAPE;
+    const long long n = N_d * N_t;
+    if (ldk < n || n > (1LL << 24)) return TT_ERR_SHAPE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return TT_ERR_NO_DEVICE; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return TT_ERR_NO_DEVICE;
+    }
+    if (prop.major != 10) return TT_ERR_NO_DEVICE;   // built for sm_100a only
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e = dtype == TT_F32
+        ? kd_run<float, 8>(static_cast<const float*>(Fcol), static_cast<const float*>(Gcol), static_cast<const float*>(noise_var),
+                           N_d, N_m, N_t, static_cast<double*>(K), ldk, s)
+        : kd_run<double, 4>(static_cast<const double*>(Fcol), static_cast<const double*>(Gcol),
+                            static_cast<const double*>(noise_var), N_d, N_m, N_t, static_cast<double*>(K), ldk, s);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TT_ERR_OOM : TT_ERR_CUDA; }
+    return TT_OK;
+}

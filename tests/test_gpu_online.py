@@ -148,6 +148,59 @@ def test_assemble_K(tt, N_d, N_m, N_t, dtype, k_max):
     assert (part[:, :c0] == -1.0).all() and (part[:, c0 + nc:] == -1.0).all()
 
 
+# n = N_t N_d spans one tile (36), ragged second tiles (300, 350), the order of a diagonal block larger than a tile (N_d = 150);
+# N_m spans less than one shared-memory stage (5), ragged stages (1000, 2100) and more than one fp32 chunk of 8192 (9000).
+DIRECT_SHAPES = ONLINE_SHAPES + [(7, 9000, 30), (3, 33, 100), (150, 70, 2), (2, 5, 3), (1, 1, 1), (10, 257, 35)]
+
+
+@pytest.mark.parametrize("N_d,N_m,N_t", DIRECT_SHAPES)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_assemble_K_direct(tt, N_d, N_m, N_t, dtype):
+    """tt_assemble_K_direct (one GEMM of the block columns + running sums down the block diagonals) against the oracle's
+    column-by-column K = Gamma_noise + F G* (PAPER.md:296, 306)."""
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    K_ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
+    n = N_d * N_t
+    buf = torch.full((n, n + 3), -1.0, dtype=torch.float64, device="cuda")             # pitched output
+    tt.tt_assemble_K_direct(F.cuda(), G.cuda(), nv.cuda(), N_d, N_m, N_t, tt.TT_F32 if dtype == torch.float32 else tt.TT_F64,
+                            buf, n + 3)
+    buf = buf.cpu().numpy()
+    K = buf[:, :n]
+    assert (buf[:, n:] == -1.0).all()
+    assert rel(K, K_ref) <= BAR[dtype]
+    assert np.array_equal(K, K.T)                                                      # the upper triangle is a copy
+    # the noise sits on the diagonal only: the same call with twice the noise moves exactly the diagonal
+    K2 = tt.assemble_K_direct(F.cuda(), G.cuda(), (2 * nv).cuda()).cpu().numpy()
+    off = ~np.eye(n, dtype=bool)
+    assert np.array_equal(K2[off], K[off])
+    assert np.allclose(np.diag(K2) - np.diag(K), nv.numpy().reshape(n).astype(np.float64), rtol=1e-6, atol=0)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_assemble_K_direct_agrees_with_column_by_column(tt, dtype):
+    N_d, N_m, N_t = 6, 700, 40
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    pF, pG = tt.Plan(F.cuda(), k_max=8), tt.Plan(G.cuda(), k_max=8)
+    try:
+        K_cols = tt.assemble_K(pF, pG, nv.cuda()).cpu().numpy()
+    finally:
+        pF.close(); pG.close()
+    K_dir = tt.assemble_K_direct(F.cuda(), G.cuda(), nv.cuda()).cpu().numpy()
+    assert rel(K_dir, K_cols) <= 2 * BAR[dtype]
+
+
+def test_assemble_K_direct_validation(tt):
+    F = torch.zeros((4, 2, 8), dtype=torch.float32, device="cuda")
+    nv = torch.ones((4, 2), dtype=torch.float32, device="cuda")
+    K = torch.zeros((8, 8), dtype=torch.float64, device="cuda")
+    L = tt.lib()
+    st = torch.cuda.current_stream().cuda_stream
+    assert L.tt_assemble_K_direct(None, F.data_ptr(), nv.data_ptr(), 2, 8, 4, tt.TT_F32, K.data_ptr(), 8, st) == -1      # TT_ERR_NULL
+    assert L.tt_assemble_K_direct(F.data_ptr(), F.data_ptr(), nv.data_ptr(), 2, 8, 4, 7, K.data_ptr(), 8, st) == -3   # TT_ERR_DTYPE
+    assert L.tt_assemble_K_direct(F.data_ptr(), F.data_ptr(), nv.data_ptr(), 2, 8, 4, tt.TT_F32, K.data_ptr(), 7, st) == -2   # TT_ERR_SHAPE (ldk < n)
+    assert L.tt_assemble_K_direct(F.data_ptr(), F.data_ptr(), nv.data_ptr(), 0, 8, 4, tt.TT_F32, K.data_ptr(), 8, st) == -2   # TT_ERR_SHAPE
+
+
 @pytest.mark.parametrize("N_d,N_m,N_t", ONLINE_SHAPES)
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("layout", [0, 1])
