@@ -85,15 +85,16 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
 #pragma unroll
         for (int j = 0; j < TN; ++j) acc[i][j] = R(0);
 
-    const long long nk = (Kdim + kKdBK - 1) / kKdBK;
+    const int nk = (int)((Kdim + kKdBK - 1) / kKdBK);
     bool first = true;
+    int until_flush = chunk_tiles;
     gload(0);
     sstore(0);
     __syncthreads();
-    for (long long t = 0; t < nk; ++t) {
-        if (t + 1 < nk) gload((t + 1) * kKdBK);
+    for (int t = 0; t < nk; ++t) {
+        if (t + 1 < nk) gload((long long)(t + 1) * kKdBK);
         const R* s = sm + (int)(t & 1) * (ROWS * P);
-#pragma unroll
+#pragma unroll 2
         for (int g = 0; g < kKdBK / KV; ++g) {
             V a[8], b[TN];
 #pragma unroll
@@ -109,7 +110,8 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
         }
         if (t + 1 < nk) sstore((int)((t + 1) & 1));
         __syncthreads();
-        if ((t + 1) % chunk_tiles == 0 || t + 1 == nk) {   // chunk sums meet in fp64, in a fixed order
+        if (--until_flush == 0 || t + 1 == nk) {   // chunk sums meet in fp64, in a fixed order
+            until_flush = chunk_tiles;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const long long row = rowA0 + ty + 16 * i;

@@ -267,6 +267,37 @@ def test_K_assembly_p5_full_size_sampled(tt):
             assert abs(col[i * w.N_d + s] - ref) <= 1e-5 * max(abs(ref), scale), ((i, s), (i2, s2), col[i * w.N_d + s], ref)
 
 
+def test_K_direct_p5_full_size_sampled(tt):
+    """tt_assemble_K_direct at the paper's shape (fp32 block columns of 25.8 GB each, n = 24 500): the whole K in one call, as
+    `bench.py --config P5 --online` times it; sampled entries against oracle/online_plain.K_entry, exact symmetry, and
+    the noise on the diagonal."""
+    from oracle import online_plain as oo
+    w = synth.CONFIGS["P5"]
+    need_memory(70)
+    n = w.N_d * w.N_t
+    F = synth.block_column(w, device="cuda")
+    G = synth.gstar_block_column(w, F)
+    nv = synth.noise_var(w, device="cuda")
+    K = torch.full((n, n), float("nan"), dtype=torch.float64, device="cuda")
+    tt.tt_assemble_K_direct(F, G, nv, w.N_d, w.N_m, w.N_t, tt.TT_F32, K, n)
+    torch.cuda.synchronize()
+    rows_F = {s: F[:, s, :].cpu().numpy() for s in (0, 17, 48)}
+    rows_G = {s: G[:, s, :].cpu().numpy() for s in (5, 17, 48)}
+    del F, G
+    assert bool(torch.isfinite(K).all())
+    for r0 in range(0, n, 4900):                                   # K == K^T bit for bit, slab by slab
+        assert bool((K[r0:r0 + 4900, :] == K[:, r0:r0 + 4900].t()).all())
+    nvh = nv.cpu().numpy().astype(np.float64)
+    scale = float(K[:: 97, :: 89].pow(2).mean().sqrt())
+    pairs = [((0, 0), (3, 5)), ((3, 17), (3, 5)), ((43, 48), (3, 5)), ((499, 0), (3, 5)),
+             ((250, 17), (250, 17)), ((290, 48), (250, 17)), ((0, 0), (250, 17)), ((499, 0), (250, 17)),
+             ((499, 48), (499, 48)), ((499, 17), (499, 48)), ((127, 0), (499, 48)), ((2, 48), (1, 48)), ((261, 17), (262, 5))]
+    for (i, s), (i2, s2) in pairs:
+        ref = oo.K_entry(rows_F[s], rows_G[s2], i, i2, nvh[i, s] if (i, s) == (i2, s2) else 0.0)
+        got = float(K[i * w.N_d + s, i2 * w.N_d + s2])
+        assert abs(got - ref) <= 1e-5 * max(abs(ref), scale), ((i, s), (i2, s2), got, ref)
+
+
 def test_online_fp64_full_parameter_dimension(tt):
     """The fp64 path (complex128 spectrum) at the paper's full parameter and time dimensions (N_m = 263169, N_t = 500) with
     8 sensors - the configuration of `bench.py --config P5 --online --f64` with fewer sensors, block column handed over as a
