@@ -18,8 +18,10 @@
 //   2. kd_diag_kernel     in-place running sums down the block diagonals of the lower triangle, + Gamma_noise on the diagonal
 //   3. kd_mirror_kernel   upper triangle := transpose of the lower one
 //
-// Precision: TT_F32 multiplies and accumulates in fp32 over chunks of 8192 parameters and adds the chunk sums, and the running
-// sums of step 2, in fp64; TT_F64 is fp64 throughout.
+// Precision: TT_F32 multiplies and accumulates in fp32 over chunks of 8192 parameters (even and odd parameters in separate
+// accumulators) and adds the chunk sums, and the running sums of step 2, in fp64; TT_F64 is fp64 throughout.
+#include <type_traits>
+
 #include "../../include/tt.h"
 #include "tt_common.cuh"
 #include "tt_internal.h"
@@ -37,6 +39,15 @@ template <> struct KdVec<float> { using type = float4; static constexpr int n = 
 template <> struct KdVec<double> { using type = double2; static constexpr int n = 2; };
 __device__ __forceinline__ float kd_get(const float4& v, int i) { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
 __device__ __forceinline__ double kd_get(const double2& v, int i) { return i == 0 ? v.x : v.y; }
+// c.lo += a.lo * b.lo,  c.hi += a.hi * b.hi  on packed pairs of floats
+__device__ __forceinline__ void kd_fma2(unsigned long long& c, unsigned long long a, unsigned long long b) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ double kd_total(unsigned long long c) {
+    return (double)__uint_as_float((unsigned)(c & 0xffffffffull)) + (double)__uint_as_float((unsigned)(c >> 32));
+}
+__device__ __forceinline__ double kd_total(double c) { return c; }
+__device__ __forceinline__ double kd_total(float c) { return (double)c; }
 
 // C[a][b] (+)= sum_k A[a][k] B[b][k] for the tiles that touch the lower triangle; A, B: n x Kdim row-major (pitch Kdim, any
 // alignment: scalar loads, a warp reads 32 consecutive k of one row).  Shared memory holds [row][k] with a pitch of
@@ -79,11 +90,16 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
         for (int i = 0; i < LB; ++i) s[(kKdBM + warp + 8 * i) * P + lane] = pre[LA + i];
     };
 
-    R acc[8][TN];
+    // fp32: packed accumulators {sum over even k, sum over odd k} driven by fma.rn.f32x2 (SASS FFMA2) - both operands are
+    // k-adjacent pairs exactly as they lie in shared memory, so no packing moves are needed; a three-register scalar FFMA issues
+    // every other cycle per sub-partition on this part, FFMA2 does two of them in that slot.  fp64: scalar DFMA.
+    constexpr bool PACKED = sizeof(R) == 4;
+    using Acc = typename std::conditional<PACKED, unsigned long long, R>::type;
+    Acc acc[8][TN];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j] = R(0);
+        for (int j = 0; j < TN; ++j) acc[i][j] = Acc(0);
 
     const int nk = (int)((Kdim + kKdBK - 1) / kKdBK);
     bool first = true;
@@ -96,17 +112,33 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
         const R* s = sm + (int)(t & 1) * (ROWS * P);
 #pragma unroll 2
         for (int g = 0; g < kKdBK / KV; ++g) {
-            V a[8], b[TN];
+            if constexpr (PACKED) {
+                ulonglong2 a[8], b[TN];   // .x = (k, k+1), .y = (k+2, k+3) of one row
 #pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const V*>(s + (ty + 16 * i) * P + g * KV);
+                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const ulonglong2*>(s + (ty + 16 * i) * P + g * KV);
 #pragma unroll
-            for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const V*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
-#pragma unroll
-            for (int kk = 0; kk < KV; ++kk)
+                for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const ulonglong2*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
 #pragma unroll
                 for (int i = 0; i < 8; ++i)
 #pragma unroll
-                    for (int j = 0; j < TN; ++j) acc[i][j] = fma(kd_get(a[i], kk), kd_get(b[j], kk), acc[i][j]);
+                    for (int j = 0; j < TN; ++j) kd_fma2(acc[i][j], a[i].x, b[j].x);
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) kd_fma2(acc[i][j], a[i].y, b[j].y);
+            } else {
+                V a[8], b[TN];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const V*>(s + (ty + 16 * i) * P + g * KV);
+#pragma unroll
+                for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const V*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
+#pragma unroll
+                for (int kk = 0; kk < KV; ++kk)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+#pragma unroll
+                        for (int j = 0; j < TN; ++j) acc[i][j] = fma(kd_get(a[i], kk), kd_get(b[j], kk), acc[i][j]);
+            }
         }
         if (t + 1 < nk) sstore((int)((t + 1) & 1));
         __syncthreads();
@@ -120,9 +152,9 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
                     const long long col = rowB0 + tx + 16 * j;
                     if (row < n && col < n) {
                         double* c = C + row * ldc + col;
-                        *c = (first ? 0.0 : *c) + (double)acc[i][j];
+                        *c = (first ? 0.0 : *c) + kd_total(acc[i][j]);
                     }
-                    acc[i][j] = R(0);
+                    acc[i][j] = Acc(0);
                 }
             }
             first = false;
