@@ -410,6 +410,23 @@ def run_online_f64(args, w):
     torch.cuda.set_device(dev)
     w = w.scaled(dtype=torch.float64)
     n = w.N_d * w.N_t
+    # all of K in fp64 from the two fp64 block columns (2 x 51.6 GB at P5), before the 103 GB spectrum is built
+    F = synth.block_column(w, device=dev)
+    G = synth.gstar_block_column(w, F)
+    nv0 = synth.noise_var(w, device=dev)
+    Kd = torch.empty((n, n), dtype=torch.float64, device=dev)
+    tiny = (slice(0, 2), slice(0, min(w.N_d, 2)), slice(0, 64))
+    tt.assemble_K_direct(F[tiny].contiguous(), G[tiny].contiguous(), nv0[:2, : min(w.N_d, 2)].contiguous())   # first-launch costs
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    tt.tt_assemble_K_direct(F, G, nv0, w.N_d, w.N_m, w.N_t, tt.TT_F64, Kd, n)
+    e1.record()
+    torch.cuda.synchronize()
+    s_direct = e0.elapsed_time(e1) * 1e-3
+    kd_sym = bool((Kd[: min(n, 4096)] == Kd[:, : min(n, 4096)].t()).all())
+    del F, G, Kd, nv0
+    torch.cuda.empty_cache()
     t0 = time.perf_counter()
     G_h = torch.empty((w.N_t, w.N_d, w.N_m), dtype=torch.float64).pin_memory()
     for s0 in range(0, w.N_d, 4):
@@ -472,6 +489,12 @@ def run_online_f64(args, w):
         "ops": {"map_gain_form_ms": ms_gain, "Gstar_ms": ms_G, "K_solve_ms": ms_solve,
                 "parity": "tests/test_gpu_fullsize.py::test_online_fp64_full_parameter_dimension (sampled outputs vs the oracle)",
                 "paper_timing_context": "PAPER.md:436-438: ~53 ms on 24 A100 for eq (4.13) as written, fp64 storage"},
+        "K_assembly_direct": {"seconds": s_direct, "what": "tt_assemble_K_direct, TT_F64: all of K from the two fp64 block columns "
+                              "(DMMA GEMM of the lower triangle + running sums down the block diagonals + mirror)",
+                              "multiply_adds": n * (n + 1) // 2 * w.N_m, "TFLOPs": n * (n + 1) * w.N_m / s_direct * 1e-12,
+                              "upper_equals_lower_transposed": kd_sym,
+                              "parity": "tests/test_gpu_online.py::test_assemble_K_direct (fp64: 1e-12 against the oracle)",
+                              "paper_timing_context": "PAPER.md:407: 24 500 x 0.022 s ~ 9 min on 24 A100 (column by column, fp64)"},
         "setup": {"block_column_generation_s": t_gen, "plan_create_from_host_s": t_plan,
                   "device_bytes": pG.device_bytes + chol.device_bytes},
     }
