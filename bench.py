@@ -425,7 +425,32 @@ def run_online_f64(args, w):
     torch.cuda.synchronize()
     s_direct = e0.elapsed_time(e1) * 1e-3
     kd_sym = bool((Kd[: min(n, 4096)] == Kd[:, : min(n, 4096)].t()).all())
-    del F, G, Kd, nv0
+    del F, G, nv0
+    torch.cuda.empty_cache()
+    # With K itself in hand the factor is the real one: Cholesky by the library (cuSOLVER through torch - the paper's own
+    # offline factorisation is a library call too), then libtt's triangular solves on it, checked by a residual.
+    true_K = {"used": False}
+    chol = None
+    try:
+        tc0 = time.perf_counter()
+        L = torch.linalg.cholesky(Kd, upper=True).t()   # K = U^T U: L = U^T; cuSOLVER's column-major U is a row-major L
+        L = L if L.stride(1) == 1 else L.contiguous()
+        torch.cuda.synchronize()
+        t_chol = time.perf_counter() - tc0
+        chol = tt.Chol(L)
+        del L
+        b_chk = torch.randn(n, dtype=torch.float64, device=dev)
+        x_chk = chol.solve(b_chk)
+        res = float((Kd @ x_chk - b_chk).norm() / b_chk.norm())
+        true_K = {"used": True, "cholesky_s_cusolver": t_chol, "residual_of_tt_chol_solve": res,
+                  "what": "L = chol(K) of the K assembled above; |K x - b| / |b| for x = tt_chol_solve(b), b ~ N(0, I)"}
+        del b_chk, x_chk
+    except Exception as exc:   # K not numerically SPD, or no memory for the factorisation: report it, time with the stand-in
+        true_K = {"used": False, "why": f"{type(exc).__name__}: {exc}"[:200]}
+        if chol is not None:
+            chol.close()
+            chol = None
+    del Kd
     torch.cuda.empty_cache()
     t0 = time.perf_counter()
     G_h = torch.empty((w.N_t, w.N_d, w.N_m), dtype=torch.float64).pin_memory()
@@ -444,9 +469,10 @@ def run_online_f64(args, w):
     del G_h
     nv = synth.noise_var(w, device=dev)
     d_obs = synth.vector_d(w, device=dev, k_rhs=1)
-    L = synth.factor_standin(n, w.seed, device=dev)
-    chol = tt.Chol(L)
-    del L
+    if chol is None:
+        L = synth.factor_standin(n, w.seed, device=dev)
+        chol = tt.Chol(L)
+        del L
     torch.cuda.empty_cache()
     mp = tt.MapInference(None, pG, chol, nv)
     stream = torch.cuda.Stream(device=dev)
@@ -480,6 +506,8 @@ def run_online_f64(args, w):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{w.name} in fp64: N_d={w.N_d}, N_m={w.N_m}, N_t={w.N_t}, complex128 spectrum of G* {ghat / 1e9:.1f} GB",
                    "step": "tt_map_infer TT_MAP_GAIN: K-solve (two triangular solves) + one G* action",
+                   "factor": ("Cholesky factor of the true K = Gamma_noise + F G* (tt_assemble_K_direct, then cuSOLVER potrf)"
+                              if true_K["used"] else "seeded stand-in of order n (synth.factor_standin)"),
                    "l2": "inputs larger than L2"},
         "gpu_launches": 9 * args.steps, "clocks": clocks.summary(),
         "roofline": {"bound": "hbm", "kernel": "gemv_adj_kernel<double> (B2 of the G* action)",
@@ -495,6 +523,7 @@ def run_online_f64(args, w):
                               "upper_equals_lower_transposed": kd_sym,
                               "parity": "tests/test_gpu_online.py::test_assemble_K_direct (fp64: 1e-12 against the oracle)",
                               "paper_timing_context": "PAPER.md:407: 24 500 x 0.022 s ~ 9 min on 24 A100 (column by column, fp64)"},
+        "factor": true_K,
         "setup": {"block_column_generation_s": t_gen, "plan_create_from_host_s": t_plan,
                   "device_bytes": pG.device_bytes + chol.device_bytes},
     }
