@@ -217,6 +217,37 @@ def run_online(args, w):
     kd_c0 = min(n // 2, n - min(n, args.k_cols))
     Kd_cols = Kd[:, kd_c0:kd_c0 + min(n, args.k_cols)].clone()       # compared below with the column-by-column route
     kd_sym = bool((Kd[: min(n, 4096)] == Kd[:, : min(n, 4096)].t()).all())
+    # With all of K in hand the factor can be the real one: Cholesky by the library (cuSOLVER through torch; the paper's offline
+    # factorisation is a library call too), libtt's triangular solves on it, checked by a residual.  If this K
+    # (fp32 products) is not numerically SPD the seeded stand-in below is used and the line says so.
+    true_K, chol, L_h = {"used": False}, None, None
+    try:
+        tc0 = time.perf_counter()
+        L = torch.linalg.cholesky(Kd, upper=True).t()   # K = U^T U: cuSOLVER's column-major U is a row-major L
+        L = L if L.stride(1) == 1 else L.contiguous()
+        torch.cuda.synchronize()
+        t_chol = time.perf_counter() - tc0
+        chol = tt.Chol(L)
+        L_h = L.cpu().numpy() if not args.no_cpu_baseline else None
+        del L
+        b_chk = torch.randn(n, dtype=torch.float64, device=dev)
+        x_chk = chol.solve(b_chk)
+        true_K = {"used": True, "cholesky_s_cusolver": t_chol,
+                  "residual_of_tt_chol_solve": float((Kd @ x_chk - b_chk).norm() / b_chk.norm()),
+                  "what": "L = chol(K) of the K assembled by tt_assemble_K_direct; |K x - b| / |b| for x = tt_chol_solve(b), b ~ N(0, I)"}
+        v = torch.randn(n, dtype=torch.float64, device=dev)
+        for _ in range(30):                              # power iteration: lambda_max(K); lambda_min(K) >= min(Gamma_noise)
+            v = Kd @ v
+            lam = float(v.norm())
+            v /= lam
+        true_K["cond_estimate"] = lam / float(nv0.min())
+        true_K["cond_what"] = "lambda_max(K) by power iteration / min diag(Gamma_noise) (a lower bound of lambda_min: F G* is PSD)"
+        del b_chk, x_chk, v
+    except Exception as exc:
+        true_K = {"used": False, "why": f"{type(exc).__name__}: {exc}"[:200]}
+        if chol is not None:
+            chol.close()
+        chol, L_h = None, None
     del Kd, nv0
     torch.cuda.empty_cache()                         # libtt allocates with cudaMalloc: hand torch's cached blocks back first
     pF = tt.Plan(F, k_max=kb)
@@ -230,10 +261,11 @@ def run_online(args, w):
     torch.cuda.empty_cache()
     nv = synth.noise_var(w, device=dev)
     d_obs = synth.vector_d(w, device=dev, k_rhs=1)
-    L = synth.factor_standin(n, w.seed, device=dev)
-    chol = tt.Chol(L)
-    L_h = L.cpu().numpy() if not args.no_cpu_baseline else None
-    del L
+    if chol is None:
+        L = synth.factor_standin(n, w.seed, device=dev)
+        chol = tt.Chol(L)
+        L_h = L.cpu().numpy() if not args.no_cpu_baseline else None
+        del L
     torch.cuda.empty_cache()
     mp = tt.MapInference(pF, pG, chol, nv)
     torch.cuda.synchronize()
@@ -258,6 +290,18 @@ def run_online(args, w):
     gain = lambda: tt.tt_map_infer(mp.handle, tt.TT_MAP_GAIN, d_obs, m_map, stream)
     for _ in range(args.warmup):
         paper(); gain()
+    if true_K["used"]:   # with the factor of the true K the two forms of eq (4.13) are the same vector (reading R16)
+        paper()
+        stream.synchronize()          # the calls run on `stream`, the clone and the norms on torch's current stream
+        m_p = m_map.clone()
+        torch.cuda.synchronize()
+        gain()
+        stream.synchronize()
+        true_K["paper_form_vs_gain_form_rel_l2"] = float((m_p - m_map).norm() / m_map.norm())
+        true_K["paper_form_note"] = ("eq (4.13) as written forms z = y - K^-1 (F G* y): the roundings of the two matvecs (relative u of "
+                                     "the plan dtype) are amplified by cond(K) before the subtraction, the gain form G* K^-1 d has no "
+                                     "such cancellation (DESIGN.md section 11, tolerances: bar + 8 u cond(K))")
+        del m_p
     with ClockSampler(0) as clocks:
         ms_paper = time_op(paper, args.steps)
     ms_gain = time_op(gain, args.steps)
@@ -340,7 +384,9 @@ def run_online(args, w):
                                f"{n} data), online phase of PAPER.md:343-350",
                    "step": "tt_map_infer TT_MAP_PAPER: y = Gn^-1 d, a = G* y, b = F a, c = K^-1 b (two triangular solves), "
                            "m_map = G* (y - c)",
-                   "factor": "seeded stand-in of order n (synth.factor_standin); timing is value independent",
+                   "factor": ("Cholesky factor of the true K = Gamma_noise + F G* (tt_assemble_K_direct, then cuSOLVER potrf)"
+                              if true_K["used"] else
+                              "seeded stand-in of order n (synth.factor_standin); timing is value independent"),
                    "l2": "inputs larger than L2 (two 52 GB spectra + 2.4 GB factor streamed per step)"},
         "e2e": {"value": ms_e2e, "unit": "ms", "h2d_bytes_per_step": n * es, "d2h_bytes_per_step": w.N_t * w.N_m * es,
                 "steps": n_e2e, "api": "tt_map_infer_host, pinned host vectors"},
@@ -360,6 +406,7 @@ def run_online(args, w):
                 "paper_form_GBs": (3 * (fhat_bytes + vec) + 2 * lt_bytes) / (ms_paper * 1e-3) / 1e9,
                 "gain_form_GBs": (fhat_bytes + vec + 2 * lt_bytes) / (ms_gain * 1e-3) / 1e9,
                 "paper_timing_context": "PAPER.md:436-438: ~53 ms on 24 A100 (11 ms per G*/F, 20 ms K-solve)"},
+        "factor": true_K,
         "K_assembly_direct": {"seconds": s_direct, "what": "tt_assemble_K_direct: all of K from the two block columns, one real GEMM "
                               "(lower triangle) + running sums down the block diagonals + mirror; no matvecs",
                               "multiply_adds": n * (n + 1) // 2 * w.N_m,
