@@ -84,6 +84,7 @@ def lib() -> ctypes.CDLL:
         "tt_chol_trsv": (ci, [vp, ci, vp, vp, vp]),
         "tt_assemble_K": (ci, [vp, vp, vp, i64, i64, vp, i64, vp]),
         "tt_assemble_K_direct": (ci, [vp, vp, vp, i64, i64, i64, ci, vp, i64, vp]),
+        "tt_qoi_direct": (ci, [vp, vp, vp, i64, i64, i64, i64, i64, ci, vp, vp, i64, vp, i64, vp]),
         "tt_map_create": (ci, [pp, vp, vp, vp, vp, vp]),
         "tt_map_destroy": (None, [vp]),
         "tt_map_infer": (ci, [vp, ci, vp, vp, vp]),
@@ -108,7 +109,7 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
-           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
+           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
            "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
            "tt_postcov_q_apply", "tt_d2q_apply"]
 
@@ -315,6 +316,12 @@ def tt_assemble_K_direct(Fcol, Gcol, noise_var, N_d: int, N_m: int, N_t: int, dt
                                                                 _ptr(K), ldk, _stream(stream)))
 
 
+def tt_qoi_direct(Fqcol, Gqcol, Gcol, N_q: int, N_d: int, N_m: int, N_t: int, out_every: int, dtype: int, chol: int,
+                  Q, ldq: int, post_cov_q, ldc: int, stream=None) -> None:
+    _check_chol("tt_qoi_direct", lib().tt_qoi_direct(_ptr(Fqcol), _ptr(Gqcol), _ptr(Gcol), N_q, N_d, N_m, N_t, out_every, dtype,
+                                                      chol, _ptr(Q), ldq, _ptr(post_cov_q), ldc, _stream(stream)), chol)
+
+
 def tt_map_create(F: int | None, G: int, chol: int, noise_var, stream=None) -> int:
     out = ctypes.c_void_p()
     _check("tt_map_create", lib().tt_map_create(ctypes.byref(out), F, G, chol, _ptr(noise_var), _stream(stream)))
@@ -487,6 +494,20 @@ def assemble_K_direct(Fcol: torch.Tensor, Gcol: torch.Tensor, noise_var: torch.T
     tt_assemble_K_direct(Fcol, Gcol, noise_var, N_d, N_m, N_t, TT_F32 if Fcol.dtype == torch.float32 else TT_F64,
                          K, K.stride(0), stream)
     return K
+
+
+def qoi_direct(Fqcol: torch.Tensor, Gqcol: torch.Tensor, Gcol: torch.Tensor, out_every: int, chol: "Chol", stream=None):
+    """(Q, Gamma_post(q)) as dense float64 CUDA tensors [n_q, n] and [n_q, n_q] from the block columns (tt_qoi_direct)."""
+    N_t, N_q, N_m = Fqcol.shape
+    N_d = Gcol.shape[1]
+    assert Gqcol.shape == Fqcol.shape and Gcol.shape == (N_t, N_d, N_m) and Fqcol.dtype == Gqcol.dtype == Gcol.dtype
+    assert Fqcol.is_contiguous() and Gqcol.is_contiguous() and Gcol.is_contiguous()
+    nq, n = (N_t // out_every) * N_q, N_t * N_d
+    Q = torch.empty((nq, n), dtype=torch.float64, device="cuda")
+    C = torch.empty((nq, nq), dtype=torch.float64, device="cuda")
+    tt_qoi_direct(Fqcol, Gqcol, Gcol, N_q, N_d, N_m, N_t, out_every, TT_F32 if Fqcol.dtype == torch.float32 else TT_F64,
+                  chol.handle, Q, n, C, nq, stream)
+    return Q, C
 
 
 class MapInference:

@@ -5,6 +5,7 @@
 #include <stdint.h>
 
 struct tt_plan;
+struct tt_chol;
 
 namespace tt {
 
@@ -15,6 +16,7 @@ struct PlanInfo {
     long long dec;  // data vectors on every dec-th time step (tt_plan_create_coarse)
 };
 PlanInfo plan_info(const ::tt_plan* p);
+long long chol_order(const ::tt_chol* c);  // order n of the factor (tt_online.cu)
 // m_host = F^T d_dev, delivered to HOST memory with the D2H copies pipelined behind the kernels (tt_api.cu); returns a tt_status
 int plan_rmatvec_to_host(const ::tt_plan* p, const void* d_dev, void* m_host, cudaStream_t s);
 

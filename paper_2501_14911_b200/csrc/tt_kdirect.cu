@@ -55,13 +55,13 @@ __device__ __forceinline__ double kd_total(float c) { return (double)c; }
 // 32 + 16 bytes, so that the 16-byte fragment loads of 8 consecutive rows fall into 8 different bank groups.
 template <typename R, int TN>
 __global__ void __launch_bounds__(kKdThreads, 1)
-kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restrict__ C, const long long n,
-               const long long Kdim, const long long ldc, const int chunk_tiles) {
+kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restrict__ C, const long long nA,
+               const long long nB, const long long Kdim, const long long ldc, const int chunk_tiles, const int lower_only) {
     using V = typename KdVec<R>::type;
     constexpr int KV = KdVec<R>::n, P = kKdBK + KV, BN = 16 * TN, ROWS = kKdBM + BN;
     constexpr int LA = kKdBM / 8, LB = BN / 8;   // rows of the A / B tile loaded per thread and stage
     const int tn = blockIdx.x, tm = blockIdx.y;
-    if ((long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;   // tile entirely above the diagonal
+    if (lower_only && (long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;   // tile entirely above the diagonal
     extern __shared__ __align__(16) unsigned char smem_raw[];
     R* sm = reinterpret_cast<R*>(smem_raw);   // [2][ROWS][P]
 
@@ -71,9 +71,9 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
     const R* pb = B + (rowB0 + warp) * Kdim + lane;
     unsigned okA = 0, okB = 0;
 #pragma unroll
-    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < n ? 1u : 0u) << i;
+    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < nA ? 1u : 0u) << i;
 #pragma unroll
-    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < n ? 1u : 0u) << i;
+    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < nB ? 1u : 0u) << i;
 
     R pre[LA + LB];
     auto gload = [&](long long k0) {
@@ -151,7 +151,7 @@ kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restr
 #pragma unroll
                 for (int j = 0; j < TN; ++j) {
                     const long long col = rowB0 + tx + 16 * j;
-                    if (row < n && col < n) {
+                    if (row < nA && col < nB) {
                         double* c = C + row * ldc + col;
                         *c = (first ? 0.0 : *c) + kd_total(acc[i][j]);
                     }
@@ -173,11 +173,11 @@ __device__ __forceinline__ void kd_dmma(double& c0, double& c1, double a, double
 }
 constexpr int kKdDmmaBN = 64, kKdDmmaP = kKdBK + 4;
 __global__ void __launch_bounds__(kKdThreads, 1)
-kd_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B, double* __restrict__ C, const long long n,
-                    const long long Kdim, const long long ldc) {
+kd_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B, double* __restrict__ C, const long long nA,
+                    const long long nB, const long long Kdim, const long long ldc, const int lower_only) {
     constexpr int P = kKdDmmaP, BN = kKdDmmaBN, ROWS = kKdBM + BN, LA = kKdBM / 8, LB = BN / 8;
     const int tn = blockIdx.x, tm = blockIdx.y;
-    if ((long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;
+    if (lower_only && (long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* sm = reinterpret_cast<double*>(smem_raw);   // [2][ROWS][P]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, tq = lane & 3;
@@ -187,9 +187,9 @@ kd_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B, 
     const double* pb = B + (rowB0 + warp) * Kdim + lane;
     unsigned okA = 0, okB = 0;
 #pragma unroll
-    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < n ? 1u : 0u) << i;
+    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < nA ? 1u : 0u) << i;
 #pragma unroll
-    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < n ? 1u : 0u) << i;
+    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < nB ? 1u : 0u) << i;
     double pre[LA + LB];
     auto gload = [&](long long k0) {
         const bool kok = k0 + lane < Kdim;
@@ -241,7 +241,7 @@ kd_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B, 
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
                 const long long row = rowA0 + wm * 32 + mt * 8 + g, col = rowB0 + wn * 32 + nt * 8 + 2 * tq + r;
-                if (row < n && col < n) C[row * ldc + col] = acc[mt][nt][r];
+                if (row < nA && col < nB) C[row * ldc + col] = acc[mt][nt][r];
             }
 }
 
@@ -282,35 +282,141 @@ kd_mirror_kernel(double* __restrict__ K, const long long n, const long long ldk)
     }
 }
 
-template <typename R, int TN>
-cudaError_t kd_run(const R* Fcol, const R* Gcol, const R* noise_var, long long N_d, long long N_m, long long N_t, double* K,
-                   long long ldk, cudaStream_t s) {
-    constexpr int P = kKdBK + KdVec<R>::n, BN = 16 * TN;
-    const long long n = N_t * N_d;
-    auto k = kd_gemm_kernel<R, TN>;
-    const size_t smem = (size_t)2 * (kKdBM + BN) * P * sizeof(R);
+// C (nA x nB, fp64, pitch ldc) = A B^T for row-major A (nA x Kdim) and B (nB x Kdim) of type R; lower_only: only the tiles that
+// touch the lower triangle (nA == nB)
+template <typename R>
+cudaError_t kd_launch_gemm(const R* A, const R* B, double* C, long long nA, long long nB, long long Kdim, long long ldc,
+                           int lower_only, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
-    if constexpr (sizeof(R) == 4) {
+    if constexpr (sizeof(R) == 8) {   // DMMA: 0.585 s against 0.864 s for the DFMA form of kd_gemm_kernel at N_m = 26 316
+        const size_t smem = (size_t)2 * (kKdBM + kKdDmmaBN) * kKdDmmaP * sizeof(double);
+        e = cudaFuncSetAttribute(kd_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const dim3 grid((unsigned)((nB + kKdDmmaBN - 1) / kKdDmmaBN), (unsigned)((nA + kKdBM - 1) / kKdBM));
+        kd_gemm_dmma_kernel<<<grid, kKdThreads, smem, s>>>(A, B, C, nA, nB, Kdim, ldc, lower_only);
+    } else {
+        constexpr int TN = 8, BN = 16 * TN, P = kKdBK + KdVec<R>::n;
+        auto k = kd_gemm_kernel<R, TN>;
+        const size_t smem = (size_t)2 * (kKdBM + BN) * P * sizeof(R);
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
+        const dim3 grid((unsigned)((nB + BN - 1) / BN), (unsigned)((nA + kKdBM - 1) / kKdBM));
+        k<<<grid, kKdThreads, smem, s>>>(A, B, C, nA, nB, Kdim, ldc, kKdChunkTiles, lower_only);
     }
-    const dim3 grid((unsigned)((n + BN - 1) / BN), (unsigned)((n + kKdBM - 1) / kKdBM));
-    const int chunk = sizeof(R) == 4 ? kKdChunkTiles : 0x7fffffff;
-    if constexpr (sizeof(R) == 8) {   // DMMA: 0.585 s against 0.864 s for the DFMA form of kd_gemm_kernel at N_m = 26 316
-        const size_t smem2 = (size_t)2 * (kKdBM + kKdDmmaBN) * kKdDmmaP * sizeof(double);
-        e = cudaFuncSetAttribute(kd_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
-        if (e != cudaSuccess) return e;
-        kd_gemm_dmma_kernel<<<grid, kKdThreads, smem2, s>>>(Fcol, Gcol, K, n, N_m, ldk);
-    } else {
-        k<<<grid, kKdThreads, smem, s>>>(Fcol, Gcol, K, n, N_m, ldk, chunk);
-    }
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    return cudaGetLastError();
+}
+
+template <typename R>
+cudaError_t kd_run(const R* Fcol, const R* Gcol, const R* noise_var, long long N_d, long long N_m, long long N_t, double* K,
+                   long long ldk, cudaStream_t s) {
+    const long long n = N_t * N_d;
+    cudaError_t e = kd_launch_gemm<R>(Fcol, Gcol, K, n, n, N_m, ldk, 1, s);
+    if (e != cudaSuccess) return e;
     const long long chains = n * N_d;
     kd_diag_kernel<R><<<(unsigned)((chains + 255) / 256), 256, 0, s>>>(K, noise_var, n, (int)N_d, ldk);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     const unsigned nt = (unsigned)((n + 31) / 32);
     kd_mirror_kernel<<<dim3(nt, nt), 256, 0, s>>>(K, n, ldk);
     return cudaGetLastError();
+}
+
+// Whole matrix, in place: M[a][b] := sum_{j >= 0} W[a - j sa][b - j sb] (the block rows of the two operands may differ in
+// height).  One thread per chain; a chain starts in the first block column (b0 < sb) or in the first block row (a0 < sa).
+__global__ void __launch_bounds__(256)
+kd_diag_rect_kernel(double* __restrict__ M, const long long nA, const long long nB, const int sa, const int sb,
+                    const long long ld) {
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long first = nA * sb;
+    long long a0, b0;
+    if (idx < first) {
+        a0 = idx / sb;
+        b0 = idx - a0 * sb;
+    } else {
+        idx -= first;
+        const long long wb = nB - sb;
+        if (wb <= 0) return;
+        a0 = idx / wb;
+        if (a0 >= sa) return;
+        b0 = sb + (idx - a0 * wb);
+    }
+    if (a0 >= nA || b0 >= nB) return;
+    double run = 0.0;
+    for (long long a = a0, b = b0; a < nA && b < nB; a += sa, b += sb) {
+        double* p = M + a * ld + b;
+        run += *p;
+        *p = run;
+    }
+}
+
+// dst[ro][co] = src[rmap(ro)][cmap(co)]: rows / columns (I, q) of a coarse time grid are the fine-grid rows (r (I + 1) - 1, q)
+// (reading R19); r == 1: identity
+__global__ void __launch_bounds__(256)
+kd_pick_kernel(const double* __restrict__ src, const long long lds, double* __restrict__ dst, const long long ldd,
+               const long long nro, const long long nco, const int Nr, const int rr, const int Nc, const int rc) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nro * nco) return;
+    const long long ro = idx / nco, co = idx - ro * nco;
+    const long long rs = rr > 1 ? ((long long)rr * (ro / Nr + 1) - 1) * Nr + ro % Nr : ro;
+    const long long cs = rc > 1 ? ((long long)rc * (co / Nc + 1) - 1) * Nc + co % Nc : co;
+    dst[ro * ldd + co] = src[rs * lds + cs];
+}
+
+// out[i][j] -= c[i][j]
+__global__ void __launch_bounds__(256)
+kd_sub_kernel(double* __restrict__ out, const long long ldo, const double* __restrict__ c, const long long ldc,
+              const long long nr, const long long nc) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nr * nc) return;
+    const long long i = idx / nc, j = idx - i * nc;
+    out[i * ldo + j] -= c[i * ldc + j];
+}
+
+struct KdScratch {   // frees on every exit path
+    void* p[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    ~KdScratch() { for (void* q : p) if (q) cudaFree(q); }
+};
+
+template <typename R>
+int kd_qoi_run(const R* Fq, const R* Gq, const R* G, long long N_q, long long N_d, long long N_m, long long N_t, long long r,
+               const ::tt_chol* K, double* Q, long long ldq, double* pcq, long long ldc, cudaStream_t s) {
+    const long long nqf = N_t * N_q, n = N_t * N_d, nq = (N_t / r) * N_q;
+    KdScratch ws;
+    double *Bfull, *Afull, *Bdec, *Qc, *Cq;
+    cudaError_t e = cudaMalloc(&ws.p[0], (size_t)nqf * n * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ws.p[1], (size_t)nqf * nqf * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ws.p[2], (size_t)nq * n * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ws.p[3], (size_t)nq * n * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ws.p[4], (size_t)nq * nq * 8);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_OOM; }
+    Bfull = static_cast<double*>(ws.p[0]); Afull = static_cast<double*>(ws.p[1]); Bdec = static_cast<double*>(ws.p[2]);
+    Qc = static_cast<double*>(ws.p[3]); Cq = static_cast<double*>(ws.p[4]);
+#define KD_TRY(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; } } while (0)
+    auto blocks = [](long long work) { return (unsigned)((work + 255) / 256); };
+    // B = F_q G* on the fine grid, then its coarse rows
+    KD_TRY(kd_launch_gemm<R>(Fq, G, Bfull, nqf, n, N_m, n, 0, s));
+    kd_diag_rect_kernel<<<blocks(nqf * N_d + N_q * (n - N_d)), 256, 0, s>>>(Bfull, nqf, n, (int)N_q, (int)N_d, n);
+    KD_TRY(cudaGetLastError());
+    kd_pick_kernel<<<blocks(nq * n), 256, 0, s>>>(Bfull, n, Bdec, n, nq, n, (int)N_q, (int)r, (int)N_d, 1);
+    KD_TRY(cudaGetLastError());
+    // A = F_q G_q* on the fine grid, then its coarse rows and columns, straight into the output
+    KD_TRY(kd_launch_gemm<R>(Fq, Gq, Afull, nqf, nqf, N_m, nqf, 0, s));
+    kd_diag_rect_kernel<<<blocks(nqf * N_q + N_q * (nqf - N_q)), 256, 0, s>>>(Afull, nqf, nqf, (int)N_q, (int)N_q, nqf);
+    KD_TRY(cudaGetLastError());
+    kd_pick_kernel<<<blocks(nq * nq), 256, 0, s>>>(Afull, nqf, pcq, ldc, nq, nq, (int)N_q, (int)r, (int)N_q, (int)r);
+    KD_TRY(cudaGetLastError());
+    // Q = B K^{-1}: K is symmetric, so row i of Q is K^{-1} (row i of B)
+    for (long long i = 0; i < nq; ++i) {
+        const int st = tt_chol_solve(K, Bdec + i * n, Qc + i * n, s);
+        if (st != TT_OK) return st;
+    }
+    KD_TRY(cudaMemcpy2DAsync(Q, (size_t)ldq * 8, Qc, (size_t)n * 8, (size_t)n * 8, (size_t)nq, cudaMemcpyDeviceToDevice, s));
+    // Gamma_post(q) = A - Q B^T
+    KD_TRY(kd_launch_gemm<double>(Qc, Bdec, Cq, nq, nq, n, nq, 0, s));
+    kd_sub_kernel<<<blocks(nq * nq), 256, 0, s>>>(pcq, ldc, Cq, nq, nq, nq);
+    KD_TRY(cudaGetLastError());
+    KD_TRY(cudaStreamSynchronize(s));   // the scratch is freed on return
+#undef KD_TRY
+    return TT_OK;
 }
 
 }  // namespace
@@ -335,10 +441,38 @@ extern "C" int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const vo
     if (prop.major != 10) return TT_ERR_NO_DEVICE;   // built for sm_100a only
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     cudaError_t e = dtype == TT_F32
-        ? kd_run<float, 8>(static_cast<const float*>(Fcol), static_cast<const float*>(Gcol), static_cast<const float*>(noise_var),
+        ? kd_run<float>(static_cast<const float*>(Fcol), static_cast<const float*>(Gcol), static_cast<const float*>(noise_var),
                            N_d, N_m, N_t, static_cast<double*>(K), ldk, s)
-        : kd_run<double, 4>(static_cast<const double*>(Fcol), static_cast<const double*>(Gcol),
+        : kd_run<double>(static_cast<const double*>(Fcol), static_cast<const double*>(Gcol),
                             static_cast<const double*>(noise_var), N_d, N_m, N_t, static_cast<double*>(K), ldk, s);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TT_ERR_OOM : TT_ERR_CUDA; }
     return TT_OK;
+}
+
+extern "C" int tt_qoi_direct(const void* Fqcol, const void* Gqcol, const void* Gcol, int64_t N_q, int64_t N_d, int64_t N_m,
+                             int64_t N_t, int64_t out_every, int dtype, const tt_chol* K, void* Q, int64_t ldq,
+                             void* post_cov_q, int64_t ldc, void* stream) {
+    using namespace tt;
+    if (!Fqcol || !Gqcol || !Gcol || !K || !Q || !post_cov_q) return TT_ERR_NULL;
+    if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
+    if (N_q < 1 || N_d < 1 || N_m < 1 || N_t < 1 || out_every < 1 || N_t % out_every != 0 || N_q > 65535 || N_d > 65535)
+        return TT_ERR_SHAPE;
+    const long long n = N_d * N_t, nq = (N_t / out_every) * N_q;
+    if (ldq < n || ldc < nq || n > (1LL << 24) || N_t * N_q > (1LL << 24)) return TT_ERR_SHAPE;
+    if (chol_order(K) != n) return TT_ERR_MISMATCH;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return TT_ERR_NO_DEVICE; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return TT_ERR_NO_DEVICE;
+    }
+    if (prop.major != 10) return TT_ERR_NO_DEVICE;   // built for sm_100a only
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (dtype == TT_F32)
+        return kd_qoi_run<float>(static_cast<const float*>(Fqcol), static_cast<const float*>(Gqcol), static_cast<const float*>(Gcol),
+                                 N_q, N_d, N_m, N_t, out_every, K, static_cast<double*>(Q), ldq, static_cast<double*>(post_cov_q), ldc, s);
+    return kd_qoi_run<double>(static_cast<const double*>(Fqcol), static_cast<const double*>(Gqcol), static_cast<const double*>(Gcol),
+                              N_q, N_d, N_m, N_t, out_every, K, static_cast<double*>(Q), ldq, static_cast<double*>(post_cov_q), ldc, s);
 }

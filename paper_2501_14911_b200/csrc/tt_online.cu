@@ -38,6 +38,10 @@ struct tt_map {
     mutable int last_cuda = 0;
 };
 
+namespace tt {
+long long chol_order(const ::tt_chol* c) { return c ? c->n : 0; }
+}  // namespace tt
+
 namespace {
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }

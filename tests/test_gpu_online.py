@@ -500,6 +500,48 @@ def test_phase3_compositions(tt, dtype):
     assert rel(got_q[tt.TT_MAP_PAPER], ref_q) <= tol and rel(got_q[tt.TT_MAP_GAIN], ref_q) <= BAR[dtype] + 8 * U[torch.float64] * kappa
 
 
+@pytest.mark.parametrize("N_d,N_q,N_m,N_t,r", [(4, 3, 600, 30, 5), (2, 5, 130, 12, 1), (3, 2, 70, 40, 10), (1, 1, 9, 6, 3)])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_qoi_direct(tt, N_d, N_q, N_m, N_t, r, dtype):
+    """tt_qoi_direct: the dense data-to-QoI map Q (eq 4.11) and the dense QoI posterior covariance (eq 4.10) from block columns,
+    against the oracle's operator forms applied to every unit vector."""
+    w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
+    wq = synth.CONFIGS["Q5"].scaled(N_d=N_q, N_m=N_m, N_t=N_t, dtype=dtype)
+    Fq = synth.block_column(wq)
+    Gq = synth.gstar_block_column(wq, Fq)
+    Fn, Gn, nvn, Fqn, Gqn = F.numpy(), G.numpy(), nv.numpy(), Fq.numpy(), Gq.numpy()
+    K = oo.assemble_K(Fn, Gn, nvn)
+    L = oo.cholesky(K)
+    ev = np.linalg.eigvalsh(K)
+    kappa = ev[-1] / ev[0]
+    n, nq = N_t * N_d, (N_t // r) * N_q
+    Q_ref = np.empty((nq, n))
+    for c in range(n):
+        e = np.zeros(n); e[c] = 1.0
+        Q_ref[:, c] = oo.d2q_apply(Fn, Gn, nvn, L, Fqn, r, e.reshape(N_t, N_d)).reshape(nq)
+    C_ref = np.empty((nq, nq))
+    for c in range(nq):
+        e = np.zeros(nq); e[c] = 1.0
+        C_ref[:, c] = oo.post_cov_q_apply(Fn, Gn, L, Fqn, Gqn, r, e.reshape(N_t // r, N_q)).reshape(nq)
+    chol = tt.Chol(torch.from_numpy(L).cuda())
+    try:
+        Q, C = tt.qoi_direct(Fq.cuda(), Gq.cuda(), G.cuda(), r, chol)
+        Q, C = Q.cpu().numpy(), C.cpu().numpy()
+        bad = tt.Chol(torch.eye(n + 1, dtype=torch.float64).cuda())
+        try:
+            with pytest.raises(tt.TTError) as ei:
+                tt.qoi_direct(Fq.cuda(), Gq.cuda(), G.cuda(), r, bad)
+            assert ei.value.status == -12                               # TT_ERR_MISMATCH: factor of another order
+        finally:
+            bad.close()
+    finally:
+        chol.close()
+    tol = BAR[dtype] + 8 * U[dtype] * kappa
+    assert rel(Q, Q_ref) <= tol
+    assert rel(C, C_ref) <= tol
+    assert rel(C, C.T) <= tol
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 def test_assemble_K_space_major(tt, dtype):
     """K's ordering is row = i*N_d + s whatever the plans' layout: unit vectors and results of TT_SPACE_MAJOR plans are permuted."""
