@@ -250,6 +250,20 @@ def run_online(args, w):
         chol, L_h = None, None
     del Kd, nv0
     torch.cuda.empty_cache()                         # libtt allocates with cudaMalloc: hand torch's cached blocks back first
+    # --phase3: the dense Q and Gamma_post(q) from block columns (tt_qoi_direct), while G's block column is resident
+    qoi_direct = None
+    if args.phase3 and true_K["used"]:
+        wq0 = synth.CONFIGS["Q5"]
+        Fq0 = synth.block_column(wq0, device=dev)
+        Gq0 = synth.gstar_block_column(wq0, Fq0)
+        torch.cuda.empty_cache()
+        torch.cuda.synchronize()
+        tq0 = time.perf_counter()
+        Q_dense, C_dense = tt.qoi_direct(Fq0, Gq0, G, 10, chol)
+        torch.cuda.synchronize()
+        qoi_direct = {"seconds": time.perf_counter() - tq0}
+        del Fq0, Gq0
+        torch.cuda.empty_cache()
     pF = tt.Plan(F, k_max=kb)
     del F
     torch.cuda.empty_cache()
@@ -348,6 +362,24 @@ def run_online(args, w):
         phase3 = {"postcov_q_action_ms": ms_pq, "all_columns_s": ms_pq * nq * 1e-3, "d2q_action_ms": ms_q,
                   "d2q_action_gain_form_ms": ms_qg, "n_qoi": nq,
                   "paper_timing_context": "PAPER.md:421-423: 48 ms per Gamma_post(q) action (38.4 s for 800), 56 ms per Q action, 24 A100"}
+        if qoi_direct is not None:   # the dense matrices against the operator actions of the same run
+            stream.synchronize()
+            q_act = qout.double().reshape(-1).clone()                                 # tt_d2q_apply, gain form, of d_obs
+            q_mat = Q_dense @ d_obs.double().reshape(-1)
+            tt.tt_postcov_q_apply(mp.handle, pFq.handle, pGq.handle, vq, work, qout, stream)
+            stream.synchronize()
+            c_act = qout.double().reshape(-1)
+            c_mat = C_dense @ vq.double().reshape(-1)
+            qoi_direct.update({
+                "what": "tt_qoi_direct: dense Q (800 x 24 500) and Gamma_post(q) (800 x 800) from the block columns of F_q, G_q and G "
+                        "and the factor of K: two rectangular direct Toeplitz products, 800 K-solves, one GEMM; no matvecs",
+                "Q_times_d_obs_vs_tt_d2q_apply_rel_l2": float((q_mat - q_act).norm() / q_act.norm()),
+                "postcov_times_v_vs_tt_postcov_q_apply_rel_l2": float((c_mat - c_act).norm() / c_act.norm()),
+                "postcov_symmetry_defect": float((C_dense - C_dense.t()).norm() / C_dense.norm()),
+                "by_actions_s": (ms_pq + ms_qg) * nq * 1e-3,
+                "paper_timing_context": "PAPER.md:421-423: 800 actions each: 38.4 s (Gamma_post(q)) + ~45 s (Q), 24 A100"})
+            phase3["qoi_direct"] = qoi_direct
+            del Q_dense, C_dense
         pFq.close(); pGq.close()
         del work
         torch.cuda.empty_cache()
