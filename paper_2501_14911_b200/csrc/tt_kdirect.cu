@@ -245,7 +245,7 @@ kd_gemm_dmma_kernel(const double* __restrict__ A, const double* __restrict__ B, 
             }
 }
 
-// Lower triangle, in place: K[a][b] := sum_{j >= 0} W[a - j N_d][b - j N_d]  (+ noise_var[a] if a == b).  One thread per
+// Lower triangle, in place: K[a][b] := sum_{j >= 0} W[a - j N_d][b - j N_d]  (+ noise_var[a] if a == b; noise_var may be null).  One thread per
 // chain = per start (a0, b0) in the first block column (b0 < N_d, a0 >= b0); consecutive threads are consecutive b0.
 template <typename R>
 __global__ void __launch_bounds__(256)
@@ -260,7 +260,7 @@ kd_diag_kernel(double* __restrict__ K, const R* __restrict__ noise_var, const lo
     for (; a < n; a += N_d, b += N_d) {
         double* p = K + a * ldk + b;
         run += *p;
-        *p = a == b ? run + (double)noise_var[a] : run;
+        *p = (a == b && noise_var) ? run + (double)noise_var[a] : run;
     }
 }
 
@@ -399,8 +399,11 @@ int kd_qoi_run(const R* Fq, const R* Gq, const R* G, long long N_q, long long N_
     kd_pick_kernel<<<blocks(nq * n), 256, 0, s>>>(Bfull, n, Bdec, n, nq, n, (int)N_q, (int)r, (int)N_d, 1);
     KD_TRY(cudaGetLastError());
     // A = F_q G_q* on the fine grid, then its coarse rows and columns, straight into the output
-    KD_TRY(kd_launch_gemm<R>(Fq, Gq, Afull, nqf, nqf, N_m, nqf, 0, s));
-    kd_diag_rect_kernel<<<blocks(nqf * N_q + N_q * (nqf - N_q)), 256, 0, s>>>(Afull, nqf, nqf, (int)N_q, (int)N_q, nqf);
+    // (symmetric like K: lower tiles, running sums on the lower triangle, mirror)
+    KD_TRY(kd_launch_gemm<R>(Fq, Gq, Afull, nqf, nqf, N_m, nqf, 1, s));
+    kd_diag_kernel<R><<<blocks(nqf * N_q), 256, 0, s>>>(Afull, static_cast<const R*>(nullptr), nqf, (int)N_q, nqf);
+    KD_TRY(cudaGetLastError());
+    kd_mirror_kernel<<<dim3((unsigned)((nqf + 31) / 32), (unsigned)((nqf + 31) / 32)), 256, 0, s>>>(Afull, nqf, nqf);
     KD_TRY(cudaGetLastError());
     kd_pick_kernel<<<blocks(nq * nq), 256, 0, s>>>(Afull, nqf, pcq, ldc, nq, nq, (int)N_q, (int)r, (int)N_q, (int)r);
     KD_TRY(cudaGetLastError());

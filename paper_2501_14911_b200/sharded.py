@@ -100,3 +100,17 @@ def map_from_binding(mp, group=None) -> ShardedMapInference:
         return mp.infer_finish(b, state.pop("a"))
 
     return ShardedMapInference(partial, finish, lambda d: mp.infer(d, tt.TT_MAP_GAIN), group)
+
+
+def assemble_K_sharded(local_assemble, noise_var: torch.Tensor, group=None) -> torch.Tensor:
+    """K = Gamma_noise + F G* with the parameter axis sharded: F G* = sum_g F[:, :, P_g] G[:, :, P_g]^* is a sum over the ranks'
+    parameter slices, so every rank assembles the product of its own slices WITHOUT noise (`local_assemble(noise_var)` is called
+    with zeros: binding.assemble_K_direct on the rank's block-column slices on a GPU, the oracle in the gloo test), ONE
+    all-reduce (sum) of the n x n matrix follows (4.8 GB at the paper's shape), and the noise is added once, after it."""
+    K = local_assemble(torch.zeros_like(noise_var))
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(K, op=dist.ReduceOp.SUM, group=group)
+    n = K.shape[0]
+    K.view(-1)[:: n + 1] += noise_var.reshape(-1).to(K.dtype)
+    return K
+

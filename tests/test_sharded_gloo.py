@@ -69,6 +69,10 @@ def _worker(rank, world, port, out_dir):
         for gain in (False, True):
             got = smap.infer(torch.from_numpy(dob), gain_form=gain).numpy()
             ok = ok and np.allclose(got, m_ref[:, p0:p1], rtol=0, atol=1e-10 * np.abs(m_ref).max())
+        # K = Gamma_noise + F G* assembled from the ranks' parameter slices: one all-reduce, the noise added once
+        K_ref = oo.assemble_K(Fo, Go, nv)
+        K_sh = sharded.assemble_K_sharded(lambda z: torch.from_numpy(oo.assemble_K(Fl2, Gl2, z.numpy())), torch.from_numpy(nv)).numpy()
+        ok = ok and np.allclose(K_sh, K_ref, rtol=0, atol=1e-12 * np.abs(K_ref).max())
         with open(os.path.join(out_dir, f"rank{rank}.ok"), "w") as f:
             f.write("1" if ok else "0")
     finally:
