@@ -222,3 +222,48 @@ def test_infinite_noise_limit_returns_prior_mean():
     m_map = oo.map_point(F, G, nv, L, d_obs)
     # first order in 1/noise: m_map -> Gamma_prior F* Gamma_noise^{-1} d_obs
     assert rel(m_map, Gp @ A.T @ (d_obs.ravel() / nv.ravel())) <= 1e-8
+
+
+# ------------------------------------------------------------------ reading R20: the algebra behind tt_assemble_K_direct / tt_qoi_direct
+def _toeplitz_product(Acol, Bcol):
+    """[(i,q),(t,s)] -> sum_{j <= min(i,t)} A_{i-j}[q,:] . B_{t-j}[s,:], written as the GPU path forms it: one product of the
+    block columns seen as matrices, then running sums down the block diagonals.  Plain numpy, no oracle code."""
+    N_t, Na, N_m = Acol.shape
+    Nb = Bcol.shape[1]
+    W = Acol.reshape(N_t * Na, N_m) @ Bcol.reshape(N_t * Nb, N_m).T
+    P = W.copy()
+    for i in range(1, N_t):
+        for t in range(1, N_t):
+            P[i * Na:(i + 1) * Na, t * Nb:(t + 1) * Nb] += P[(i - 1) * Na:i * Na, (t - 1) * Nb:t * Nb]
+    return P
+
+
+@pytest.mark.parametrize("N_d,N_m,N_t", SHAPES)
+def test_K_is_one_product_of_the_block_columns_plus_running_sums(N_d, N_m, N_t):
+    F, Gs, nv, A, Gp = setup(N_d, N_m, N_t)
+    G = oo.gstar_block_column(F, Gs)
+    K_direct = _toeplitz_product(F, G) + np.diag(nv.ravel())
+    assert rel(K_direct, oo.assemble_K(F, G, nv)) <= 1e-13
+    assert rel(K_direct, np.diag(nv.ravel()) + A @ Gp @ A.T) <= 1e-13
+
+
+@pytest.mark.parametrize("r", [1, 2, 3])
+def test_dense_Q_and_post_cov_q_from_toeplitz_products(r):
+    """Q = B K^{-1} and Gamma_post(q) = A - Q B^T with B = F_q G*, A = F_q G_q* on the coarse rows (R19), against the operator
+    forms of eq (4.11) and eq (4.10) applied to every unit vector."""
+    N_d, N_q, N_m, N_t = 2, 3, 7, 6
+    F, Gs, nv, _, _ = setup(N_d, N_m, N_t)
+    Fq = RNG.standard_normal((N_t, N_q, N_m)) * np.exp(-np.arange(N_t) / 2.0)[:, None, None]
+    G, Gq = oo.gstar_block_column(F, Gs), oo.gstar_block_column(Fq, Gs)
+    K = oo.assemble_K(F, G, nv)
+    L = oo.cholesky(K)
+    rows = np.array([(r * (I + 1) - 1) * N_q + q for I in range(N_t // r) for q in range(N_q)])
+    B = _toeplitz_product(Fq, G)[rows]
+    Amat = _toeplitz_product(Fq, Gq)[np.ix_(rows, rows)]
+    Q = np.linalg.solve(K, B.T).T
+    C = Amat - Q @ B.T
+    n, nq = N_t * N_d, len(rows)
+    Q_ref = np.stack([oo.d2q_apply(F, G, nv, L, Fq, r, e.reshape(N_t, N_d)).ravel() for e in np.eye(n)], axis=1)
+    C_ref = np.stack([oo.post_cov_q_apply(F, G, L, Fq, Gq, r, e.reshape(N_t // r, N_q)).ravel() for e in np.eye(nq)], axis=1)
+    assert rel(Q, Q_ref) <= 1e-11
+    assert rel(C, C_ref) <= 1e-11
