@@ -33,15 +33,18 @@ import torch
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2501_14911_b200 import synth  # noqa: E402
+import synth  # noqa: E402
 
 METRIC = "ms per F·m and F^T·d at ~1e8 params; achieved HBM GB/s vs B200 peak"
 NOMINAL_HBM_GBS = 8000.0     # north_star's "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0    # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of one gemv_fwd_kernel launch at C3, from the ncu --set full capture
-# summarised in profiles/r1_e_c3_ncu_full.md (81.003920 GB read + 22.305280 MB written); algorithmic: 81.02 GB
-NCU_TRAFFIC_BYTES = {"C3": 81.003920e9 + 22.305280e6}
-SAMPLE_SENSORS, SAMPLE_PARAMS = 40, 75000   # largest CPU-baseline sample (about 10-20 s on 16 host cores at C3)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the newest committed `ncu --set full`
+# capture of each config.  A figure is only quoted when the plan built in THIS run describes its kernels (tt_plan_describe)
+# with the line the capture's summary records; otherwise `traffic` is null and the line says why.
+NCU_TRAFFIC = {
+    "C3": {"bytes": 81.003059e9 + 22.79e6, "profile": "profiles/r1_i_c3_ncu_full.md",
+           "kernel": "A2 gemv_fwd_kernel<float,8> grid=(62,401) block=512 smem=32768 chunk=4096"},
+}
 
 
 def measured_peaks():
@@ -104,7 +107,18 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(w, F_s, m_s, d_s):
+# One sample shape for BOTH CPU legs (cpu_baseline of the default run, --impl reference): the first SAMPLE_SENSORS sensors x
+# the first SAMPLE_PARAMS parameters x all N_t steps of the config's own block column - about 1.5 s of oracle time per
+# F.m + F^T.d pair on 16 host cores at C3.  The full step is that time x N_d*N_m / (sample sensors x sample parameters): the
+# oracle's cost is exactly proportional to both counts (independent dot products), and the line says so ("extrapolated").
+SAMPLE_SENSORS, SAMPLE_PARAMS = 8, 75000
+
+
+def sample_shape(w):
+    return min(w.N_d, SAMPLE_SENSORS), min(w.N_m, SAMPLE_PARAMS)
+
+
+def oracle_sample(F_s, m_s, d_s):
     """Times the CPU oracle (blocked C build) on a sample; returns (seconds matvec, seconds rmatvec, threads)."""
     from oracle import toeplitz_blocked as ob
     ob.build()
@@ -113,68 +127,117 @@ def oracle_sample(w, F_s, m_s, d_s):
     return t1 - t0, t2 - t1, ob.num_threads()
 
 
-def cpu_baseline(w, draw, target_s=15.0):
-    """draw(ns, npar) -> (F_s [N_t,ns,npar], m_s [N_t,npar], d_s [N_t,ns]) numpy.  Extrapolates by MAC count."""
-    npar = min(w.N_m, SAMPLE_PARAMS)
-    ns = min(w.N_d, 4)
-    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # warms the library and the caches
-    ta, tb, thr = oracle_sample(w, *draw(ns, npar))            # calibration
-    per_sensor = max(1e-3, (ta + tb) / ns)
-    ns2 = int(max(ns, min(w.N_d, SAMPLE_SENSORS, round(target_s / per_sensor))))
-    ta, tb, thr = oracle_sample(w, *draw(ns2, npar))
-    scale = (w.N_d * w.N_m) / float(ns2 * npar) * w.k_rhs   # k-RHS: the oracle does the columns one by one
+def sample_text(w, ns, npar, dt, scale, reps):
+    return (f"oracle/toeplitz_blocked.c (direct O(N_t^2) block convolution, fp64) on sensors 0..{ns - 1} x parameters 0..{npar - 1} "
+            f"x all {w.N_t} steps of the same workload: {dt:.2f} s per F.m + F^T.d pair (mean of {reps}), "
+            f"x {scale:.1f} = N_d*N_m/(sample){' * k' if w.k_rhs > 1 else ''} to the full step")
+
+
+def cpu_baseline(w, sample, target_s=12.0):
+    """sample = (F_s [N_t,ns,npar], m_s [N_t,npar], d_s [N_t,ns]) numpy, the shape of sample_shape(w)."""
+    F_s, m_s, d_s = sample
+    ns, npar = F_s.shape[1], F_s.shape[2]
+    ta, tb, thr = oracle_sample(F_s, m_s, d_s)            # warms the library and the caches
+    reps = int(max(1, min(20, round(target_s / max(1e-3, ta + tb)))))
+    acc_a = acc_b = 0.0
+    for _ in range(reps):
+        ta, tb, thr = oracle_sample(F_s, m_s, d_s)
+        acc_a += ta; acc_b += tb
+    ta, tb = acc_a / reps, acc_b / reps
+    scale = (w.N_d * w.N_m) / float(ns * npar) * w.k_rhs   # k-RHS: the oracle does the columns one by one
     return {
         "value": (ta + tb) * scale * 1e3, "unit": "ms", "cores": thr, "kind": "oracle",
-        "sample": (f"oracle/toeplitz_blocked.c (direct O(N_t^2) block convolution, fp64) timed on sensors 0..{ns2 - 1} x "
-                   f"parameters 0..{npar - 1} x all {w.N_t} steps of the same workload ({ta + tb:.2f} s for F.m + F^T.d), "
-                   f"scaled by N_d*N_m/(sample){' * k' if w.k_rhs > 1 else ''} = {scale:.1f} to the full step"),
-        "matvec_ms": ta * scale * 1e3, "rmatvec_ms": tb * scale * 1e3,
+        "sample": sample_text(w, ns, npar, ta + tb, scale, reps), "extrapolated": True, "scale": scale,
+        "sample_ms": (ta + tb) * 1e3, "matvec_ms": ta * scale * 1e3, "rmatvec_ms": tb * scale * 1e3,
+        "note": "reported baseline (the oracle as it stands, O(N_t^2)), not the optimisation target",
     }
 
 
+def cpu_fft_baseline(w, F_s, m, d_s, threads):
+    """The paper's own ALGORITHM on the host cores (FFT along time, one matvec per frequency, inverse FFT),
+    restated with library calls (torch.fft = pocketfft/MKL, torch.einsum) - a comparison row like the cuFFT + cuBLAS one, never
+    part of libtt and not the oracle.  The spectrum of a SENSOR SLAB of the block column (all parameters, all steps) is
+    computed untimed (plan cost); timed: rfft of the whole parameter vector, the per-frequency matvec against the slab's
+    spectrum, irfft.  The matvec part streams the slab once and is scaled by N_d / (slab sensors); the FFT of m is not scaled."""
+    torch.set_num_threads(threads)
+    N_t, ns, N_m = F_s.shape
+    L2 = 2 * N_t
+    Fh = torch.fft.rfft(F_s.to(torch.float64), n=L2, dim=0).to(torch.complex64 if F_s.dtype == torch.float32 else torch.complex128)
+
+    def fwd():
+        t0 = time.perf_counter()
+        mh = torch.fft.rfft(m, n=L2, dim=0)                         # [n_f, N_m]
+        t1 = time.perf_counter()
+        dh = torch.einsum("wsp,wp->ws", Fh, mh)
+        t2 = time.perf_counter()
+        torch.fft.irfft(dh, n=L2, dim=0)[:N_t]
+        return t1 - t0, t2 - t1, time.perf_counter() - t2
+
+    def adj():
+        t0 = time.perf_counter()
+        dh = torch.fft.rfft(d_s, n=L2, dim=0)                        # [n_f, ns]
+        t1 = time.perf_counter()
+        mh = torch.einsum("wsp,ws->wp", Fh.conj(), dh)
+        t2 = time.perf_counter()
+        torch.fft.irfft(mh, n=L2, dim=0)[:N_t]
+        return t1 - t0, t2 - t1, time.perf_counter() - t2
+
+    fwd(); adj()
+    f, a = fwd(), adj()
+    scale = w.N_d / float(ns)
+    ms_f = (f[0] + f[1] * scale + f[2]) * 1e3
+    ms_a = (a[0] + a[1] * scale + a[2]) * 1e3
+    return {"value": ms_f + ms_a, "unit": "ms", "cores": threads, "kind": "cpu restatement of the FFT algorithm (torch.fft + einsum)",
+            "matvec_ms": ms_f, "rmatvec_ms": ms_a, "extrapolated": True, "scale": scale,
+            "sample": (f"spectrum of sensors 0..{ns - 1} (all {N_m} parameters, {N_t} steps) precomputed untimed; timed: rfft of m "
+                       f"{f[0] * 1e3:.0f} ms, per-frequency matvec on the slab {f[1] * 1e3:.0f} ms (x {scale:.1f} = N_d/{ns}), irfft; "
+                       f"adjoint: matvec on the slab {a[1] * 1e3:.0f} ms (x {scale:.1f}), irfft of the parameter vector {a[2] * 1e3:.0f} ms"),
+            "note": "comparison row, not the oracle: the same method as libtt on the host cores (ADVICE r1)"}
+
+
 def run_reference(args, w):
-    """--impl reference: the oracle on the host cores, each step one bounded sample, same metric."""
+    """--impl reference: the oracle on the host cores, each step one bounded sample (the shape cpu_baseline uses), same metric."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    npar, ns = min(w.N_m, 25000), min(w.N_d, 4)
+    ns, npar = sample_shape(w)
     F_s = synth.block_column(w, s_range=(0, ns), p_range=(0, npar)).numpy()
     m_s = synth.vector_m(w.scaled(N_m=npar), k_rhs=1).numpy()
     d_s = synth.vector_d(w.scaled(N_d=ns), k_rhs=1).numpy()
     thr = 0
     for _ in range(args.warmup):
-        _, _, thr = oracle_sample(w, F_s, m_s, d_s)
+        _, _, thr = oracle_sample(F_s, m_s, d_s)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        _, _, thr = oracle_sample(w, F_s, m_s, d_s)
+        _, _, thr = oracle_sample(F_s, m_s, d_s)
     dt = (time.perf_counter() - t0) / args.steps
     scale = (w.N_d * w.N_m) / float(ns * npar) * w.k_rhs
     ms = dt * scale * 1e3
-    sample = (f"each step = oracle F.m + F^T.d on sensors 0..{ns - 1} x parameters 0..{npar - 1} x all {w.N_t} steps "
-              f"({dt:.2f} s), scaled by {scale:.1f} to the full workload")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic", "config": config_dict(w, args),
-        "cpu_baseline": {"value": ms, "unit": "ms", "cores": thr, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": ms, "unit": "ms", "cores": thr, "kind": "oracle",
+                         "sample": sample_text(w, ns, npar, dt, scale, args.steps), "extrapolated": True, "scale": scale,
+                         "sample_ms": dt * 1e3},
         "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
     return 0
 
 
-def config_dict(w, args):
+def config_dict(w, args, cfg_name=None):
     return {"workload": f"{w.name}: N_d={w.N_d}, N_m={w.N_m}, N_t={w.N_t} ({w.n_params:.3g} parameters), "
                         f"{'fp32 vectors / complex64 spectrum' if w.dtype == torch.float32 else 'fp64 / complex128'}"
                         + (f", k={w.k_rhs} right-hand sides" if w.k_rhs > 1 else ""),
-            "baseline_config": args.config,
+            "baseline_config": cfg_name or args.config,
             "step": "one F.m (A1,A2,A3) + one F^T.d (B1,B2,B3)" if w.k_rhs == 1
                     else f"one batched F.M + one batched F^T.D, k={w.k_rhs} (batched FFTs + per-frequency "
                          f"{'complex64 FMA' if w.dtype == torch.float32 else 'DMMA'} GEMMs)",
             "layout": "time-major",
             "out_every": getattr(args, "r_out", 1),
-            "parallelism": ("single GPU" if args.gpus == 1 else "replicas only" if args.parallel == "replicas"
-                            else f"N_m sharded over {args.gpus} ranks, one all-reduce of d per F.m"),
+            "parallelism": (f"N_m sharded over {args.gpus} rank(s), one all-reduce of d per F.m" if args.parallel == "shard"
+                            else "single GPU" if args.gpus == 1 else "replicas only"),
             "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
 
 
@@ -202,7 +265,7 @@ def run_online(args, w):
     t0 = time.perf_counter()
     F = synth.block_column(w, device=dev)
     # K = Gamma_noise + F G* in one call from the two block columns (tt_assemble_K_direct), while both are resident
-    G = synth.gstar_block_column(w, F)
+    G = synth.scaled_block_column(w, F)
     nv0 = synth.noise_var(w, device=dev)
     Kd = torch.empty((n, n), dtype=torch.float64, device=dev)
     tiny = (slice(0, 2), slice(0, min(w.N_d, 2)), slice(0, 64))
@@ -255,7 +318,7 @@ def run_online(args, w):
     if args.phase3 and true_K["used"]:
         wq0 = synth.CONFIGS["Q5"]
         Fq0 = synth.block_column(wq0, device=dev)
-        Gq0 = synth.gstar_block_column(wq0, Fq0)
+        Gq0 = synth.scaled_block_column(wq0, Fq0)
         torch.cuda.empty_cache()
         torch.cuda.synchronize()
         tq0 = time.perf_counter()
@@ -348,7 +411,7 @@ def run_online(args, w):
         r = 10
         Fq = synth.block_column(wq, device=dev)
         pFq = tt.Plan(Fq, out_every=r)
-        synth.gstar_block_column(wq, Fq, out=Fq)
+        synth.scaled_block_column(wq, Fq, out=Fq)
         pGq = tt.Plan(Fq, out_every=r)
         del Fq
         torch.cuda.empty_cache()
@@ -491,7 +554,7 @@ def run_online_f64(args, w):
     n = w.N_d * w.N_t
     # all of K in fp64 from the two fp64 block columns (2 x 51.6 GB at P5), before the 103 GB spectrum is built
     F = synth.block_column(w, device=dev)
-    G = synth.gstar_block_column(w, F)
+    G = synth.scaled_block_column(w, F)
     nv0 = synth.noise_var(w, device=dev)
     Kd = torch.empty((n, n), dtype=torch.float64, device=dev)
     tiny = (slice(0, 2), slice(0, min(w.N_d, 2)), slice(0, 64))
@@ -536,7 +599,7 @@ def run_online_f64(args, w):
     for s0 in range(0, w.N_d, 4):
         s1 = min(w.N_d, s0 + 4)
         slab = synth.block_column(w, device=dev, s_range=(s0, s1))
-        synth.gstar_block_column(w, slab, out=slab)
+        synth.scaled_block_column(w, slab, out=slab)
         G_h[:, s0:s1, :] = slab.cpu()
         del slab
     torch.cuda.empty_cache()
@@ -611,99 +674,54 @@ def run_online_f64(args, w):
     return 0
 
 
-def main() -> int:
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=sorted(synth.CONFIGS))
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
-                    help="N>1: independent replicas (default, the north star's one-GPU path) or the parameter axis "
-                         "sharded over the ranks with one all-reduce of d per F.m (paper_2501_14911_b200/sharded.py)")
-    ap.add_argument("--online", action="store_true",
-                    help="time the online phase (eq 4.13 MAP inference, K-solve, K assembly) instead of the matvec pair; "
-                         "meant for --config P5, the paper's own shape")
-    ap.add_argument("--f64", action="store_true",
-                    help="--online: the gain form in fp64 (the paper's storage precision): complex128 spectrum of G* (103 GB at P5)")
-    ap.add_argument("--phase3", action="store_true",
-                    help="--online: also time the Phase 3 actions Gamma_post(q) v (eq 4.10) and Q d_obs (eq 4.11) with the p2q plans")
-    ap.add_argument("--k-cols", type=int, default=64, help="--online: columns of K assembled and timed")
-    ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
-    ap.add_argument("--k-rhs", type=int, default=0,
-                    help="run the k-RHS batched calls with k right-hand sides on any config (default: the config's own, "
-                         "32 for C4, else 1); fp32 configs then take the complex64 FMA GEMM path")
-    ap.add_argument("--out-every", type=int, default=0,
-                    help="data side on every r-th time step (tt_plan_create_coarse); default 10 for Q5 (the p2q map), else 1")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-library-baseline", action="store_true")
-    ap.add_argument("--scale-nm", type=float, default=1.0,
-                    help="multiply the config's N_m by this factor: for profiler captures of long kernels only (ncu replays a "
-                         "kernel ~40 times and saves / restores device memory around each pass); the line it prints names the "
-                         "scaled workload and is not a bench line of the config")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    w = synth.CONFIGS[args.config]
-    if args.scale_nm != 1.0:
-        w = w.scaled(N_m=max(1, int(w.N_m * args.scale_nm)), name=f"{w.name} with N_m x {args.scale_nm:g} (profiler capture, not a bench line)")
-    if args.k_rhs > 0:
-        w = w.scaled(k_rhs=args.k_rhs)
-    if args.impl == "reference":
-        return run_reference(args, w)
-    if args.online:
-        return run_online_f64(args, w) if args.f64 else run_online(args, w)
+class Ctx:
+    def __init__(self, **kw):
+        self.__dict__.update(kw)
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: libtt has no CPU path")
-    torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    from paper_2501_14911_b200 import binding as tt
-    tt.lib()
-    dev = torch.device("cuda", local_rank)
+def measure(ctx, args, w, cfg_name, *, steps, warmup, headline):
+    """One config through the C ABI on this rank's GPU: the timed step (F.m + F^T.d, or the k-RHS pair), per-op times,
+    the roofline object of SURVEY.md 8(d) and - for the headline config only - e2e, bandwidth probes, the library
+    comparison row and the CPU legs.  Returns the JSON object (rank 0 prints it)."""
+    tt, dev, dist, rank, world = ctx.tt, ctx.dev, ctx.dist, ctx.rank, ctx.world
     es = 4 if w.dtype == torch.float32 else 8
 
     # ---- inputs, resident in HBM ----------------------------------------------------------
     t0 = time.perf_counter()
-    shard = args.parallel == "shard" and world > 1
+    shard = args.parallel == "shard"
     K = w.k_rhs                                   # > 1: the k-RHS batched calls (C4)
+    w_full = w
     if shard:
         from paper_2501_14911_b200 import sharded
         p0, p1 = sharded.shard_range(w.N_m, rank, world)
         F = synth.block_column(w, device=dev, p_range=(p0, p1))
         m = synth.vector_m(w, device=dev)[:, p0:p1].contiguous()
-        w_full, w = w, w.scaled(N_m=p1 - p0)      # byte counts below are this rank's
+        w = w.scaled(N_m=p1 - p0)                 # byte counts below are this rank's
     else:
         F = synth.block_column(w, device=dev)
         m = synth.vector_m(w, device=dev)         # [N_t, N_m] or [N_t, N_m, K]
-    r_out = args.out_every or (10 if args.config == "Q5" else 1)
+    r_out = args.out_every or (10 if cfg_name == "Q5" else 1)
     args.r_out = r_out
     d = synth.vector_d(w.scaled(N_t=w.N_t // r_out), device=dev)
     torch.cuda.synchronize()
     t_gen = time.perf_counter() - t0
-    if r_out > 1:
-        args.no_library_baseline = True   # the cuFFT/cuBLAS comparison row is written for the plain operator
+    lib_baseline = headline and K == 1 and world == 1 and r_out == 1 and not args.no_library_baseline
+    cpu_legs = headline and rank == 0 and world == 1 and not args.no_cpu_baseline
 
-    def draw(ns, npar):  # the CPU baseline's sample: the same bytes, copied from the device (column 0 if k-RHS)
+    sample = fft_sample = None
+    if cpu_legs:   # the CPU legs' samples: the same bytes, copied from the device before the column is freed
+        ns, npar = sample_shape(w)
         m1 = m if K == 1 else m[..., 0]
         d1 = d if K == 1 else d[..., 0]
         if r_out > 1:                       # the oracle applies F^T to S^T d: zeros at the steps that are not sampled
             up = torch.zeros((w.N_t,) + tuple(d1.shape[1:]), dtype=d1.dtype, device=d1.device)
             up[r_out - 1::r_out] = d1
             d1 = up
-        return (F[:, :ns, :npar].contiguous().cpu().numpy(), m1[:, :npar].contiguous().cpu().numpy(),
-                d1[:, :ns].contiguous().cpu().numpy())
-
-    samples = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        # fetch the largest sample cpu_baseline() may ask for before the column is freed
-        samples = draw(min(w.N_d, SAMPLE_SENSORS), min(w.N_m, SAMPLE_PARAMS))
+        sample = (F[:, :ns, :npar].contiguous().cpu().numpy(), m1[:, :npar].contiguous().cpu().numpy(),
+                  d1[:, :ns].contiguous().cpu().numpy())
+        if K == 1 and r_out == 1:
+            nsf = min(w.N_d, 4)
+            fft_sample = (F[:, :nsf, :].contiguous().cpu(), m1.cpu(), d1[:, :nsf].contiguous().cpu())
 
     t0 = time.perf_counter()
     plan = tt.Plan(F, k_max=K, out_every=r_out)
@@ -716,6 +734,7 @@ def main() -> int:
     d_out = torch.empty_like(d)
     m_out = torch.empty_like(m)
     h = plan.handle
+    describe = tt.tt_plan_describe(h)
 
     if K == 1:
         op_fwd = lambda: tt.tt_matvec(h, m, d_out, stream)
@@ -726,7 +745,7 @@ def main() -> int:
         op_adj = lambda: tt.tt_rmatvec_batched(h, K, d, m_out, stream)
         tag_fwd, tag_adj = tt.TT_OP_MATVEC_BATCHED, tt.TT_OP_RMATVEC_BATCHED
 
-    if shard:  # F.m = local partial + the path's one exchange step; F^T.d needs no collective
+    if shard and dist is not None:  # F.m = local partial + the path's one exchange step; F^T.d needs no collective
         local_fwd = op_fwd
 
         def op_fwd():
@@ -751,21 +770,21 @@ def main() -> int:
         return float(t.item())
 
     with torch.cuda.stream(stream):
-        for _ in range(args.warmup):
+        for _ in range(warmup):
             step()
     barrier()
 
     # ---- timed region: device-resident ------------------------------------------------------
     tt.tt_plan_set_profiling(h, True)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clocks:
+    with ClockSampler(ctx.local_rank) as clocks:
         barrier()
         ev0.record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             step()
         ev1.record(stream)
         barrier()
-    ms_step = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
+    ms_step = max_over_ranks(ev0.elapsed_time(ev1) / steps)
     fwd = tt.tt_plan_stage_ms(h, tag_fwd)
     adj = tt.tt_plan_stage_ms(h, tag_adj)
     tt.tt_plan_set_profiling(h, False)
@@ -793,76 +812,94 @@ def main() -> int:
         t = sorted(a.elapsed_time(b) for a, b in evs)
         return {"median": t[len(t) // 2], "min": t[0], "calls": n}
 
-    ms_fwd = max_over_ranks(time_op(op_fwd, args.steps))
-    ms_adj = max_over_ranks(time_op(op_adj, args.steps))
-    n_each = max(20, args.steps) if K == 1 else max(5, args.steps)
+    ms_fwd = max_over_ranks(time_op(op_fwd, steps))
+    ms_adj = max_over_ranks(time_op(op_adj, steps))
+    n_each = (max(20, steps) if K == 1 else max(5, steps)) if headline else steps
     each_fwd, each_adj = time_each(op_fwd, n_each), time_each(op_adj, n_each)
     ms_normal = None
     if K == 1:  # F^T F m (one solver iteration, configs[4]); the intermediate d never leaves the device
         n_out = torch.empty_like(m)
-        ms_normal = max_over_ranks(time_op(lambda: tt.tt_normal(h, m, n_out, stream), args.steps))
+        for _ in range(2):
+            tt.tt_normal(h, m, n_out, stream)
+        ms_normal = max_over_ranks(time_op(lambda: tt.tt_normal(h, m, n_out, stream), steps))
         del n_out
 
     # ---- end to end through the C ABI with HOST vectors -------------------------------------
-    m_h, d_h = m.cpu().pin_memory(), d.cpu().pin_memory()
-    d_oh, m_oh = torch.empty_like(d_h).pin_memory(), torch.empty_like(m_h).pin_memory()
-
-    if K == 1:
-        def step_host():
-            tt.tt_matvec_host(h, m_h, d_oh, stream)
-            tt.tt_rmatvec_host(h, d_h, m_oh, stream)
-        e2e_api = "tt_matvec_host + tt_rmatvec_host, pinned host vectors"
-    else:
-        def step_host():  # no *_host variant of the k-RHS calls: explicit copies on the same stream
-            with torch.cuda.stream(stream):
-                m.copy_(m_h, non_blocking=True)
-                tt.tt_matvec_batched(h, K, m, d_out, stream)
-                d_oh.copy_(d_out, non_blocking=True)
-                d.copy_(d_h, non_blocking=True)
-                tt.tt_rmatvec_batched(h, K, d, m_out, stream)
-                m_oh.copy_(m_out, non_blocking=True)
-        e2e_api = "pinned host -> device copies + tt_matvec_batched / tt_rmatvec_batched + device -> host copies"
-
-    step_host()
-    torch.cuda.synchronize()
-    n_e2e = max(2, min(args.steps, 5 if K == 1 else 2))
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
+    e2e = None
+    if headline:
+        m_h, d_h = m.cpu().pin_memory(), d.cpu().pin_memory()
+        d_oh, m_oh = torch.empty_like(d_h).pin_memory(), torch.empty_like(m_h).pin_memory()
+        if K == 1:
+            def step_host():
+                tt.tt_matvec_host(h, m_h, d_oh, stream)
+                tt.tt_rmatvec_host(h, d_h, m_oh, stream)
+            e2e_api = "tt_matvec_host + tt_rmatvec_host, pinned host vectors"
+        else:
+            def step_host():  # no *_host variant of the k-RHS calls: explicit copies on the same stream
+                with torch.cuda.stream(stream):
+                    m.copy_(m_h, non_blocking=True)
+                    tt.tt_matvec_batched(h, K, m, d_out, stream)
+                    d_oh.copy_(d_out, non_blocking=True)
+                    d.copy_(d_h, non_blocking=True)
+                    tt.tt_rmatvec_batched(h, K, d, m_out, stream)
+                    m_oh.copy_(m_out, non_blocking=True)
+            e2e_api = "pinned host -> device copies + tt_matvec_batched / tt_rmatvec_batched + device -> host copies"
         step_host()
-    stream.synchronize()
-    ms_e2e = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e)
-    h2d = (m_h.numel() + d_h.numel()) * es
-    d2h = (d_oh.numel() + m_oh.numel()) * es
+        torch.cuda.synchronize()
+        n_e2e = max(2, min(steps, 5 if K == 1 else 2))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            step_host()
+        stream.synchronize()
+        ms_e2e = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e)
+        e2e = {"value": ms_e2e if shard else ms_e2e / args.gpus, "unit": "ms",
+               "h2d_bytes_per_step": (m_h.numel() + d_h.numel()) * es, "d2h_bytes_per_step": (d_oh.numel() + m_oh.numel()) * es,
+               "steps": n_e2e, "api": e2e_api}
+        del m_h, d_h, d_oh, m_oh
 
-    # ---- roofline of the dominant kernel ---------------------------------------------------
+    # ---- roofline of the dominant kernel -----------------------------------
     peaks, peak_kind = measured_peaks()
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
     n_f, ldp = w.N_t + 1, (w.N_m + 15) // 16 * 16
     fhat_bytes = n_f * w.N_d * ldp * 2 * es
-    vec_bytes = (w.N_t * w.N_m + w.N_t * w.N_d) * es * K
-    bytes_op = fhat_bytes + vec_bytes                           # north_star: |Fhat| plus the vectors
-    if K == 1:
+    vec_bytes = (w.N_t * w.N_m + (w.N_t // r_out) * w.N_d) * es * K
+    bytes_op = fhat_bytes + vec_bytes                           # 8(d): |Fhat| + |m| + |d| per op; un-fused intermediates
+    if K == 1:                                                  # (mhat, partials) count against the achieved figure
         xhat_bytes = n_f * ldp * 2 * es
         dhat_bytes = n_f * w.N_d * 2 * es
         chunk = 2048 if n_f * ((ldp + 4095) // 4096) < 148 * 2 * 8 else 4096      # the planner's choice (tt_api.cu)
         n_chunks = (ldp + chunk - 1) // chunk
         part_bytes = n_f * n_chunks * w.N_d * 2 * es
-        bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # A2: Fhat + xhat read, partials written
+        bytes_fwd_kernel = fhat_bytes + xhat_bytes + part_bytes     # what A2 itself moves: Fhat + xhat read, partials written
         bytes_adj_kernel = fhat_bytes + dhat_bytes + xhat_bytes     # B2: Fhat + dhat read, xhat written
-        ach_fwd = bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0
-        ach_adj = bytes_adj_kernel / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
+        ach_fwd = bytes_op / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0
+        ach_adj = bytes_op / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0
+        traffic, traffic_src = None, "no committed ncu capture of this config"
+        rec = NCU_TRAFFIC.get(cfg_name)
+        if rec is not None:
+            if rec["kernel"] in describe and not shard:
+                traffic, traffic_src = rec["bytes"], f"{rec['profile']} ({rec['kernel']})"
+            else:
+                traffic_src = f"{rec['profile']} was captured with '{rec['kernel']}', this run launches '{describe}'"
         roofline = {
             "bound": "hbm", "kernel": "gemv_fwd_kernel (A2, per-frequency matvec streaming Fhat)",
             "achieved": ach_fwd, "peak": peak, "unit": "GB/s", "frac": ach_fwd / peak,
-            "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+            "traffic": traffic, "traffic_source": traffic_src,
             "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured"
                          else "fallback 6.65 TB/s (B200_PROFILING.md)",
-            "algorithmic_bytes_per_launch": bytes_fwd_kernel, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
+            "how": "achieved = algorithmic bytes per op (|Fhat| + |m| + |d|, SURVEY.md 8(d)) / mean duration of the dominant "
+                   "kernel's launches in the timed region (CUDA events recorded by libtt on the launching stream)",
+            "algorithmic_bytes_per_launch": bytes_op, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
             "frac_of_nominal_8TBs": ach_fwd / NOMINAL_HBM_GBS,
+            "kernel_bytes_per_launch": bytes_fwd_kernel,
+            "achieved_kernel_bytes": bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0,
+            "whole_op": {"matvec_frac": bytes_op / (ms_fwd * 1e-3) / 1e9 / peak, "rmatvec_frac": bytes_op / (ms_adj * 1e-3) / 1e9 / peak,
+                         "what": "the same bytes / the whole F.m and F^T.d (FFTs and un-fused intermediates included)"},
             "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
-                               "algorithmic_bytes_per_launch": bytes_adj_kernel, "ms_per_launch": adj[1],
-                               "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
+                               "algorithmic_bytes_per_launch": bytes_op, "kernel_bytes_per_launch": bytes_adj_kernel,
+                               "ms_per_launch": adj[1], "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
+            "kernels": describe,
         }
     elif w.dtype == torch.float32:
         # fp32 k-RHS: register-tiled complex64 FMA GEMMs (tt_gemm32.cu), bound by the FP32 FMA pipe.  Peak derived from the
@@ -901,29 +938,35 @@ def main() -> int:
                                           "(bf16 measured 1620 TF/s x nominal fp64/bf16 ratio 40/2250 = 28.8 TF/s for comparison)",
             "algorithmic_flops_per_launch": flops, "ms_per_launch": fwd[1], "launches_timed": fwd[3],
             "hbm_bytes_per_launch": fhat_bytes + n_f * w.N_m * K * 16,
+            "whole_op": {"matvec_TFLOPs": flops / (ms_fwd * 1e-3) / 1e12, "rmatvec_TFLOPs": flops / (ms_adj * 1e-3) / 1e12,
+                         "matvec_frac": flops / (ms_fwd * 1e-3) / 1e12 / best if best else None,
+                         "rmatvec_frac": flops / (ms_adj * 1e-3) / 1e12 / best if best else None,
+                         "what": "the same flops / the whole batched F.M and F^T.D (batched FFTs included)"},
             "adjoint_kernel": {"kernel": "gemm_adj_kernel (k-RHS B2)", "achieved": ach_adj,
                                "frac": ach_adj / best if best else None, "ms_per_launch": adj[1]},
         }
 
     # ---- bandwidth probes in the same run (copy and read-only stream) -------------------------
-    probe = {}
-    try:
-        nb = 8 << 30
-        a = torch.empty(nb, dtype=torch.uint8, device=dev); a.zero_()
-        b = torch.empty(nb, dtype=torch.uint8, device=dev)
-        sink = torch.empty(1 << 16, dtype=torch.uint8, device=dev)
-        with torch.cuda.stream(stream):
-            probe["read_only_gbs"] = nb / (min(time_op(lambda: tt.tt_probe_stream_read(a, nb, sink, stream), 5)
-                                               for _ in range(3)) * 1e-3) / 1e9
-            probe["copy_gbs"] = 2 * nb / (min(time_op(lambda: b.copy_(a), 5) for _ in range(3)) * 1e-3) / 1e9
-        del a, b
-    except RuntimeError as e:  # pragma: no cover
-        probe["error"] = str(e)
+    probe = None
+    if headline:
+        probe = {}
+        try:
+            nb = 8 << 30
+            a = torch.empty(nb, dtype=torch.uint8, device=dev); a.zero_()
+            b = torch.empty(nb, dtype=torch.uint8, device=dev)
+            sink = torch.empty(1 << 16, dtype=torch.uint8, device=dev)
+            with torch.cuda.stream(stream):
+                probe["read_only_gbs"] = nb / (min(time_op(lambda: tt.tt_probe_stream_read(a, nb, sink, stream), 5)
+                                                   for _ in range(3)) * 1e-3) / 1e9
+                probe["copy_gbs"] = 2 * nb / (min(time_op(lambda: b.copy_(a), 5) for _ in range(3)) * 1e-3) / 1e9
+            del a, b
+        except RuntimeError as e:  # pragma: no cover
+            probe["error"] = str(e)
 
     # ---- comparison row: the same operation with library FFTs and batched library matmuls ------
     # (torch.fft = cuFFT, torch.bmm = cuBLAS; timed on the plan's own spectrum, never linked into libtt)
     libs = None
-    if K == 1 and world == 1 and not args.no_library_baseline:
+    if lib_baseline:
         try:
             Fv = tt.tt_debug_spectrum_view(h, w.N_t, w.N_d, w.dtype)[:, :, :w.N_m]
             L2 = 2 * w.N_t
@@ -942,8 +985,8 @@ def main() -> int:
                 r1, r2 = lib_fwd(), lib_adj()
                 e1 = float((r1 - d_out).norm() / d_out.norm()); e2 = float((r2 - m_out).norm() / m_out.norm())
                 del r1, r2
-                t_lf = time_op(lib_fwd, max(2, args.steps // 2))
-                t_la = time_op(lib_adj, max(2, args.steps // 2))
+                t_lf = time_op(lib_fwd, max(2, steps // 2))
+                t_la = time_op(lib_adj, max(2, steps // 2))
             libs = {"what": "torch.fft.rfft/irfft (cuFFT) + torch.bmm over frequencies (cuBLAS) on the same spectrum",
                     "matvec_ms": t_lf, "rmatvec_ms": t_la, "rel_diff_vs_libtt": [e1, e2]}
             del Fv
@@ -951,21 +994,22 @@ def main() -> int:
             libs = {"error": str(e)[:200]}
             torch.cuda.empty_cache()
 
+    launches_per_step = 7                      # A1, A2 (matvec or GEMM), partial reduce, A3, B1, B2, B3
     out = {
         "metric": METRIC, "value": ms_step if shard else ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus,
-        "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "strong" if shard else "weak",
+        "steps": steps,
+        "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "strong" if shard else "weak",
         "vs_baseline": None, "dtype": "f32" if w.dtype == torch.float32 else "f64", "data": "synthetic",
-        "config": config_dict(w_full if shard else w, args),
-        "e2e": {"value": ms_e2e / args.gpus, "unit": "ms", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": n_e2e, "api": e2e_api},
-        "gpu_launches": 7 * args.steps,   # A1, A2, partial reduce, A3, B1, B2, B3
+        "config": config_dict(w_full, args, cfg_name),
+        "e2e": e2e,
+        "gpu_launches": launches_per_step * steps,
         "clocks": clocks.summary(),
         "roofline": roofline,
         "ops": {
             "matvec_ms": ms_fwd, "rmatvec_ms": ms_adj, "normal_ms": ms_normal, "k_rhs": K,
             "matvec_ms_per_call": each_fwd, "rmatvec_ms_per_call": each_adj,
             "normal_GBs": (2 * fhat_bytes + 2 * w.N_t * w.N_m * es) / (ms_normal * 1e-3) / 1e9 if ms_normal else None,
+            "normal_frac_of_measured_copy": (2 * fhat_bytes + 2 * w.N_t * w.N_m * es) / (ms_normal * 1e-3) / 1e9 / peak if ms_normal else None,
             "matvec_GBs": bytes_op / (ms_fwd * 1e-3) / 1e9, "rmatvec_GBs": bytes_op / (ms_adj * 1e-3) / 1e9,
             "roofline_bytes_per_op": bytes_op,
             "matvec_frac_of_8TBs": bytes_op / (ms_fwd * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
@@ -979,18 +1023,115 @@ def main() -> int:
         "library_baseline": libs,
         "plan": {"create_s": t_plan, "device_bytes": plan.device_bytes, "input_generation_s": t_gen},
     }
-
-    # ---- CPU baseline: the oracle on this box's host cores, bounded sample -------------------
-    if samples is not None:
-        Fs, ms_, ds_ = samples
-
-        def draw_cached(ns, npar):
-            return (Fs[:, :ns, :npar].copy(), ms_[:, :npar].copy(), ds_[:, :ns].copy())
-
-        out["cpu_baseline"] = cpu_baseline(w, draw_cached)
-        out["cpu_baseline"]["note"] = "reported baseline, not the optimisation target"
-
     plan.close()
+    del m, d, d_out, m_out
+    torch.cuda.empty_cache()
+
+    # ---- CPU legs: the oracle (and the FFT algorithm restated with library calls) on this box's host cores -----
+    if sample is not None:
+        out["cpu_baseline"] = cpu_baseline(w, sample)
+        if fft_sample is not None:
+            try:
+                out["cpu_fft_baseline"] = cpu_fft_baseline(w, *fft_sample, threads=out["cpu_baseline"]["cores"])
+            except Exception as exc:
+                out["cpu_fft_baseline"] = {"error": f"{type(exc).__name__}: {exc}"[:200]}
+    return out
+
+
+def summarise_leg(leg, name):
+    """The short legs of the other BASELINE.json configs inside the default line: ms, GB/s or TFLOP/s, roofline, clocks."""
+    ops, rf = leg["ops"], leg["roofline"]
+    keep = {"workload": leg["config"]["workload"], "steps": leg["steps"], "warmup": leg["warmup"], "ms_per_step": leg["ms_per_step"],
+            "dtype": leg["dtype"], "matvec_ms": ops["matvec_ms"], "rmatvec_ms": ops["rmatvec_ms"], "normal_ms": ops["normal_ms"],
+            "k_rhs": ops["k_rhs"], "clocks": leg["clocks"], "gpu_launches": leg["gpu_launches"],
+            "stages_matvec_ms": ops["stages_matvec_ms"], "stages_rmatvec_ms": ops["stages_rmatvec_ms"],
+            "plan_device_bytes": leg["plan"]["device_bytes"]}
+    if rf["bound"] == "hbm":
+        keep.update({"matvec_GBs": ops["matvec_GBs"], "rmatvec_GBs": ops["rmatvec_GBs"], "normal_GBs": ops["normal_GBs"],
+                     "roofline_bytes_per_op": ops["roofline_bytes_per_op"]})
+    keep["roofline"] = {k: rf[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "peak_kind",
+                                            "ms_per_launch", "launches_timed", "whole_op", "adjoint_kernel") if k in rf}
+    if name == "C5":   # configs[4] is quoted on the normal operator: Fhat streamed twice
+        keep["headline_op"] = {"op": "tt_normal (F^T F m)", "ms": ops["normal_ms"], "GBs": ops["normal_GBs"],
+                               "frac_of_measured_copy": ops["normal_frac_of_measured_copy"]}
+    return keep
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
+                    help="N>1: independent replicas (default, the north star's one-GPU path) or the parameter axis "
+                         "sharded over the ranks with one all-reduce of d per F.m (paper_2501_14911_b200/sharded.py)")
+    ap.add_argument("--online", action="store_true",
+                    help="time the online phase (eq 4.13 MAP inference, K-solve, K assembly) instead of the matvec pair; "
+                         "meant for --config P5, the paper's own shape")
+    ap.add_argument("--f64", action="store_true",
+                    help="--online: the gain form in fp64 (the paper's storage precision): complex128 spectrum of G* (103 GB at P5)")
+    ap.add_argument("--phase3", action="store_true",
+                    help="--online: also time the Phase 3 actions Gamma_post(q) v (eq 4.10) and Q d_obs (eq 4.11) with the p2q plans")
+    ap.add_argument("--k-cols", type=int, default=64, help="--online: columns of K assembled and timed")
+    ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
+    ap.add_argument("--k-rhs", type=int, default=0,
+                    help="run the k-RHS batched calls with k right-hand sides on any config (default: the config's own, "
+                         "32 for C4, else 1); fp32 configs then take the complex64 FMA GEMM path")
+    ap.add_argument("--out-every", type=int, default=0,
+                    help="data side on every r-th time step (tt_plan_create_coarse); default 10 for Q5 (the p2q map), else 1")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-library-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default C3 run at N=1: skip the short C5 / C2 / C4 legs reported under `configs`")
+    ap.add_argument("--scale-nm", type=float, default=1.0,
+                    help="multiply the config's N_m by this factor: for profiler captures of long kernels only (ncu replays a "
+                         "kernel ~40 times and saves / restores device memory around each pass); the line it prints names the "
+                         "scaled workload and is not a bench line of the config")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = synth.CONFIGS[args.config]
+    if args.scale_nm != 1.0:
+        w = w.scaled(N_m=max(1, int(w.N_m * args.scale_nm)), name=f"{w.name} with N_m x {args.scale_nm:g} (profiler capture, not a bench line)")
+    if args.k_rhs > 0:
+        w = w.scaled(k_rhs=args.k_rhs)
+    if args.impl == "reference":
+        return run_reference(args, w)
+    if args.online:
+        return run_online_f64(args, w) if args.f64 else run_online(args, w)
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libtt has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_2501_14911_b200 import binding as tt
+    tt.lib()
+    ctx = Ctx(tt=tt, dev=torch.device("cuda", local_rank), dist=dist, rank=rank, world=world, local_rank=local_rank)
+
+    out = measure(ctx, args, w, args.config, steps=args.steps, warmup=args.warmup, headline=True)
+
+    # ---- the other BASELINE.json configs, short legs in the same invocation (driver-timed; N = 1 only) ----
+    if world == 1 and args.config == "C3" and not args.no_other_configs and args.k_rhs == 0 and args.scale_nm == 1.0 \
+            and args.parallel == "replicas":
+        others = {}
+        for name in ("C5", "C2", "C4"):
+            try:
+                torch.cuda.empty_cache()
+                wo = synth.CONFIGS[name]
+                leg = measure(ctx, args, wo, name, steps=5 if wo.k_rhs > 1 else 10, warmup=3, headline=False)
+                others[name] = summarise_leg(leg, name)
+            except Exception as exc:   # a failed leg must not take the headline line with it
+                others[name] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+        out["configs"] = others
+
     if rank == 0:
         print(json.dumps(out))
     if dist is not None:

@@ -63,12 +63,13 @@ typedef enum tt_layout { TT_TIME_MAJOR = 0, TT_SPACE_MAJOR = 1 } tt_layout;
 typedef enum tt_status {
     TT_OK = 0,
     TT_ERR_NULL = -1,           /* a required pointer is NULL */
-    TT_ERR_SHAPE = -2,          /* a dimension < 1, or a size overflows 63 bits */
+    TT_ERR_SHAPE = -2,          /* a dimension < 1, a size overflows 63 bits, or N_d complex numbers of the plan's dtype
+                                   exceed 227 KB of shared memory (N_d > 29056 for TT_F32, > 14528 for TT_F64) */
     TT_ERR_DTYPE = -3,
     TT_ERR_LAYOUT = -4,
-    TT_ERR_UNSUPPORTED_NT = -5, /* N_t has a prime factor outside {2,3,5,7}, or one series
-                                   of N_t complex values does not fit 227 KB of shared memory
-                                   at 8 series per CTA (N_t > 3632 for TT_F32, > 1816 for TT_F64) */
+    TT_ERR_UNSUPPORTED_NT = -5, /* N_t has a prime factor outside {2,3,5,7}, or 8 series of N_t + 1 complex128 values
+                                   do not fit 227 KB of shared memory: N_t > 1815, for BOTH dtypes (the one-time
+                                   transform of the matrix runs in fp64 whatever the plan's dtype) */
     TT_ERR_K = -6,              /* k < 1 or k > k_max */
     TT_ERR_ALIAS = -7,          /* out aliases in (tt_normal) */
     TT_ERR_OOM = -8,            /* cudaMalloc failed */
@@ -126,6 +127,11 @@ size_t tt_plan_device_bytes(const tt_plan* plan);
 
 /* cudaError_t (as int) recorded by the last failing CUDA call made for this plan; 0 if none. */
 int tt_plan_last_cuda_error(const tt_plan* plan);
+
+/* One line naming the kernels (template arguments, grid, block, shared memory) that the single-vector apply calls of this
+ * plan launch for A2, B2 and the FFTs; NUL-terminated into buf[n] (TT_ERR_SHAPE if it does not fit; 512 bytes always do).
+ * bench.py prints it and only quotes an ncu traffic figure whose capture names the same line. */
+int tt_plan_describe(const tt_plan* plan, char* buf, size_t n);
 
 /* Test hook: copies Fhat, unpadded, to dst_device as [N_t+1][N_d][N_m] interleaved complex
  * (complex64 for TT_F32, complex128 for TT_F64), on `stream`. */
@@ -281,12 +287,19 @@ int tt_assemble_K(const tt_plan* F, const tt_plan* G, const void* noise_var, int
  * lower triangle is computed, the upper one mirrored).
  *   Fcol, Gcol  DEVICE, [N_t][N_d][N_m] reals of `dtype`, N_m fastest: the first block columns F_k and G_k = F_k Gamma_prior
  *               (the arrays tt_plan_create takes with TT_TIME_MAJOR); no alignment requirement
- *   noise_var   DEVICE, [N_t][N_d] reals of `dtype`: the diagonal of Gamma_noise
+ *   noise_var   DEVICE, [N_t][N_d] reals of `dtype`: the diagonal of Gamma_noise; NULL: K = F G* alone (see tt_K_add_noise)
  *   K           DEVICE, n x n doubles, row-major, pitch ldk (>= n), n = N_t*N_d, row = i*N_d + s; overwritten entirely
  * TT_F32: products and sums over runs of 8192 parameters in fp32, everything above that in fp64; TT_F64: fp64 throughout.
  * Asynchronous on `stream`, no allocation. */
 int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m, int64_t N_t,
                          int dtype, void* K, int64_t ldk, void* stream);
+
+/* The N_m-sharded assembly: F G* is a SUM over parameter slices, so every rank calls
+ * tt_assemble_K_direct on its own slices Fcol[:, :, P_g], Gcol[:, :, P_g] with noise_var == NULL (F G* alone), the partial
+ * matrices are all-reduced (the one exchange step), and Gamma_noise (eq 4.7) is added ONCE, by this call:
+ *     K[a][a] += noise_var[a],  a = 0..n-1   (noise_var: DEVICE, n reals of `dtype`, data stacking row = i*N_d + s).
+ * Asynchronous on `stream`, no allocation. */
+int tt_K_add_noise(const void* noise_var, int64_t n, int dtype, void* K, int64_t ldk, void* stream);
 
 /* Phase 3 without matvecs: the data-to-QoI map Q and the QoI posterior covariance Gamma_post(q) as dense
  * matrices, from block columns.  With B = F_q G* (n_q x n) and A = F_q G_q* (n_q x n_q) - products of a block lower- with a

@@ -44,8 +44,11 @@ def lib() -> ctypes.CDLL:
     else:
         try:
             path = _build.build()  # no-op when the source hash matches
-        except RuntimeError:
-            pass  # no nvcc on this box: use the library that travelled with the repo
+        except RuntimeError as exc:
+            # no nvcc on this box: the library that travelled with the repo is only good if it was built from these sources
+            if not _build.is_current():
+                raise RuntimeError(f"{path} was built from other sources than paper_2501_14911_b200/csrc (hash mismatch) and "
+                                   f"cannot be rebuilt here: {exc}") from exc
     L = ctypes.CDLL(path)
     vp, i64, ci, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_size_t
     pp = ctypes.POINTER(vp)
@@ -58,6 +61,7 @@ def lib() -> ctypes.CDLL:
         "tt_plan_device_bytes": (sz, [vp]),
         "tt_plan_last_cuda_error": (ci, [vp]),
         "tt_plan_get_spectrum": (ci, [vp, vp, vp]),
+        "tt_plan_describe": (ci, [vp, ctypes.c_char_p, sz]),
         "tt_matvec": (ci, [vp, vp, vp, vp]),
         "tt_rmatvec": (ci, [vp, vp, vp, vp]),
         "tt_normal": (ci, [vp, vp, vp, vp]),
@@ -84,6 +88,7 @@ def lib() -> ctypes.CDLL:
         "tt_chol_trsv": (ci, [vp, ci, vp, vp, vp]),
         "tt_assemble_K": (ci, [vp, vp, vp, i64, i64, vp, i64, vp]),
         "tt_assemble_K_direct": (ci, [vp, vp, vp, i64, i64, i64, ci, vp, i64, vp]),
+        "tt_K_add_noise": (ci, [vp, i64, ci, vp, i64, vp]),
         "tt_qoi_direct": (ci, [vp, vp, vp, i64, i64, i64, i64, i64, ci, vp, vp, i64, vp, i64, vp]),
         "tt_map_create": (ci, [pp, vp, vp, vp, vp, vp]),
         "tt_map_destroy": (None, [vp]),
@@ -104,12 +109,12 @@ def lib() -> ctypes.CDLL:
 
 
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_coarse", "tt_plan_destroy", "tt_plan_device_bytes",
-           "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_matvec", "tt_rmatvec", "tt_normal",
+           "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_plan_describe", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_normal_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
            "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
            "tt_debug_trig", "tt_debug_set",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
-           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
+           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_K_add_noise", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
            "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
            "tt_postcov_q_apply", "tt_d2q_apply"]
 
@@ -171,6 +176,12 @@ def tt_plan_last_cuda_error(plan: int) -> int:
 
 def tt_plan_get_spectrum(plan: int, dst: torch.Tensor, stream=None) -> None:
     _check("tt_plan_get_spectrum", lib().tt_plan_get_spectrum(plan, dst.data_ptr(), _stream(stream)), plan)
+
+
+def tt_plan_describe(plan: int) -> str:
+    buf = ctypes.create_string_buffer(1024)
+    _check("tt_plan_describe", lib().tt_plan_describe(plan, buf, 1024), plan)
+    return buf.value.decode()
 
 
 def _ptr(x) -> int:
@@ -312,8 +323,14 @@ def tt_assemble_K(F: int, G: int, noise_var, col0: int, ncols: int, K, ldk: int,
 
 
 def tt_assemble_K_direct(Fcol, Gcol, noise_var, N_d: int, N_m: int, N_t: int, dtype: int, K, ldk: int, stream=None) -> None:
-    _check("tt_assemble_K_direct", lib().tt_assemble_K_direct(_ptr(Fcol), _ptr(Gcol), _ptr(noise_var), N_d, N_m, N_t, dtype,
+    """noise_var None: K = F G* alone (a rank's partial of the sharded assembly, see tt_K_add_noise)."""
+    nv = None if noise_var is None else _ptr(noise_var)
+    _check("tt_assemble_K_direct", lib().tt_assemble_K_direct(_ptr(Fcol), _ptr(Gcol), nv, N_d, N_m, N_t, dtype,
                                                                 _ptr(K), ldk, _stream(stream)))
+
+
+def tt_K_add_noise(noise_var, n: int, dtype: int, K, ldk: int, stream=None) -> None:
+    _check("tt_K_add_noise", lib().tt_K_add_noise(_ptr(noise_var), n, dtype, _ptr(K), ldk, _stream(stream)))
 
 
 def tt_qoi_direct(Fqcol, Gqcol, Gcol, N_q: int, N_d: int, N_m: int, N_t: int, out_every: int, dtype: int, chol: int,
@@ -402,33 +419,53 @@ class Plan:
             return base
         return base + (k,) if self.layout == TT_TIME_MAJOR else (k,) + base
 
-    def _out(self, n_space: int, k: int | None = None, data: bool = False):
+    def _out(self, n_space: int, k: int | None = None, data: bool = False, stream=None):
+        """Output allocated on the stream the kernels will run on (the caching allocator must not hand the block to
+        another stream's tensor before they finish)."""
+        if isinstance(stream, torch.cuda.Stream):
+            with torch.cuda.stream(stream):
+                return torch.empty(self._shape(n_space, k, data), dtype=self.dtype, device="cuda")
         return torch.empty(self._shape(n_space, k, data), dtype=self.dtype, device="cuda")
 
+    def _vec(self, t: torch.Tensor, n_space: int, k: int | None = None, data: bool = False, what: str = "vector"):
+        """The raw-pointer calls trust their arguments; the convenience class does not."""
+        n = 1
+        for x in self._shape(n_space, k, data):
+            n *= x
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == self.dtype and t.is_contiguous() and t.numel() == n):
+            raise ValueError(f"{what}: expected a contiguous CUDA tensor of {n} x {self.dtype}, got "
+                             f"{tuple(t.shape)} {t.dtype} on {t.device}{'' if t.is_contiguous() else ' (not contiguous)'}")
+        return t
+
     def matvec(self, m, out=None, stream=None):
-        out = self._out(self.N_d, data=True) if out is None else out
+        self._vec(m, self.N_m, what="m")
+        out = self._out(self.N_d, data=True, stream=stream) if out is None else self._vec(out, self.N_d, data=True, what="out")
         tt_matvec(self.handle, m, out, stream)
         return out
 
     def rmatvec(self, d, out=None, stream=None):
-        out = self._out(self.N_m) if out is None else out
+        self._vec(d, self.N_d, data=True, what="d")
+        out = self._out(self.N_m, stream=stream) if out is None else self._vec(out, self.N_m, what="out")
         tt_rmatvec(self.handle, d, out, stream)
         return out
 
     def normal(self, m, out=None, stream=None):
-        out = self._out(self.N_m) if out is None else out
+        self._vec(m, self.N_m, what="m")
+        out = self._out(self.N_m, stream=stream) if out is None else self._vec(out, self.N_m, what="out")
         tt_normal(self.handle, m, out, stream)
         return out
 
     def matvec_batched(self, M, out=None, stream=None):
         k = M.shape[-1] if self.layout == TT_TIME_MAJOR else M.shape[0]
-        out = self._out(self.N_d, k, data=True) if out is None else out
+        self._vec(M, self.N_m, k, what="M")
+        out = self._out(self.N_d, k, data=True, stream=stream) if out is None else self._vec(out, self.N_d, k, data=True, what="out")
         tt_matvec_batched(self.handle, k, M, out, stream)
         return out
 
     def rmatvec_batched(self, D, out=None, stream=None):
         k = D.shape[-1] if self.layout == TT_TIME_MAJOR else D.shape[0]
-        out = self._out(self.N_m, k) if out is None else out
+        self._vec(D, self.N_d, k, data=True, what="D")
+        out = self._out(self.N_m, k, stream=stream) if out is None else self._vec(out, self.N_m, k, what="out")
         tt_rmatvec_batched(self.handle, k, D, out, stream)
         return out
 
@@ -484,7 +521,7 @@ def assemble_K(F: Plan, G: Plan, noise_var: torch.Tensor, cols: tuple[int, int] 
     return K
 
 
-def assemble_K_direct(Fcol: torch.Tensor, Gcol: torch.Tensor, noise_var: torch.Tensor, out: torch.Tensor | None = None,
+def assemble_K_direct(Fcol: torch.Tensor, Gcol: torch.Tensor, noise_var: torch.Tensor | None, out: torch.Tensor | None = None,
                       stream=None) -> torch.Tensor:
     """K = Gamma_noise + F G* from the [N_t, N_d, N_m] block columns F_k and G_k = F_k Gamma_prior (no plans, no matvecs)."""
     N_t, N_d, N_m = Fcol.shape
@@ -526,7 +563,8 @@ class MapInference:
     __del__ = close
 
     def infer(self, d_obs, form: int = TT_MAP_PAPER, out=None, stream=None):
-        out = self.G._out(self.G.N_m) if out is None else out
+        self.G._vec(d_obs, self.G.N_d, data=True, what="d_obs")
+        out = self.G._out(self.G.N_m, stream=stream) if out is None else self.G._vec(out, self.G.N_m, what="out")
         tt_map_infer(self.handle, form, d_obs, out, stream)
         return out
 

@@ -52,6 +52,14 @@ def _hash() -> str:
     return h.hexdigest()
 
 
+def is_current() -> bool:
+    """True if libtt.so exists and its stamp carries the hash of the sources and flags in this tree."""
+    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
+        return False
+    with open(STAMP) as f:
+        return f.read().strip() == _hash()
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile and link libtt.so if needed; returns its path."""
     sig = _hash()

@@ -3,6 +3,7 @@
 // sequences of the apply calls.  Every step of the path runs in this library's own kernels;
 // there is no CPU fallback and no library FFT/BLAS call.
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -372,11 +373,15 @@ int ensure_staging(const tt_plan* cp) {
     return TT_OK;
 }
 
-// Parameter range c of the pipelined host calls: boundaries on multiples of 4096 (a multiple of the GEMV chunk, of the
-// 512-parameter tile of the adjoint kernel and of the 16-element row pitch), the last range ends at ldp.
+// Parameter range c of the pipelined host calls: boundaries on multiples of lcm(GEMV chunk, 512) - the forward kernel
+// derives its chunk index from p_begin / chunk, the adjoint kernel works on 512-parameter tiles, and both are multiples of
+// the 16-element row pitch (4096 for the planner's chunks of 2048 / 4096); the last range ends at ldp.
 void host_chunk(const tt_plan* p, int c, long long* p0, long long* p1) {
+    long long a = p->chunk, b = 512;
+    while (b) { const long long t = a % b; a = b; b = t; }
+    const long long unit = (long long)p->chunk / a * 512;
     long long per = (p->ldp + kHostChunks - 1) / kHostChunks;
-    per = (per + 4095) / 4096 * 4096;
+    per = (per + unit - 1) / unit * unit;
     *p0 = per * c < p->ldp ? per * c : p->ldp;
     *p1 = per * (c + 1) < p->ldp ? per * (c + 1) : p->ldp;
 }
@@ -543,8 +548,10 @@ int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, 
     int n_stages[2] = {0, 0};
     if (N_t > 65535 || !factorise(N_t, 25, radix[0], &n_stages[0]) || !factorise(N_t, 8, radix[1], &n_stages[1]))
         return TT_ERR_UNSUPPORTED_NT;
-    const FftChoice cd = fft_choose((int)N_t, 16);  // the fp64 transform of the matrix is the largest user
+    const FftChoice cd = fft_choose((int)N_t, 16);  // the fp64 transform of the matrix is the largest user (both dtypes)
     if (cd.T == 0) return TT_ERR_UNSUPPORTED_NT;
+    // the adjoint matvec keeps dhat_w (N_d complex numbers) in shared memory, the fp32 k-RHS adjoint N_d x k of them
+    if ((size_t)N_d * 2 * esize(dtype) > (size_t)kMaxSmem) return TT_ERR_SHAPE;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return TT_ERR_NO_DEVICE; }
@@ -672,6 +679,25 @@ int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, 
 size_t tt_plan_device_bytes(const tt_plan* p) { return p ? p->bytes : 0; }
 
 int tt_plan_last_cuda_error(const tt_plan* p) { return p ? p->last_cuda : 0; }
+
+int tt_plan_describe(const tt_plan* p, char* buf, size_t n) {
+    if (!p || !buf) return TT_ERR_NULL;
+    if (n < 1) return TT_ERR_SHAPE;
+    GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
+    const int t = p->dtype == TT_F32 ? 0 : 1;
+    const int used = gemv_describe(t, g, buf, n);
+    if (used < 0 || (size_t)used >= n) return TT_ERR_SHAPE;
+    const FftChoice c = fft_choose((int)p->N_t, t == 0 ? 8 : 16);
+    const int more = snprintf(buf + used, n - used, " | fft N=%lld T=%d smem=%zu radices=", p->N_t, c.T, c.smem);
+    if (more < 0 || (size_t)(used + more) >= n) return TT_ERR_SHAPE;
+    size_t at = (size_t)(used + more);
+    for (int i = 0; i < p->n_stages[t]; ++i) {
+        const int k = snprintf(buf + at, n - at, i ? "x%d" : "%d", p->radix[t][i]);
+        if (k < 0 || at + (size_t)k >= n) return TT_ERR_SHAPE;
+        at += (size_t)k;
+    }
+    return TT_OK;
+}
 
 int tt_plan_get_spectrum(const tt_plan* p, void* dst, void* stream) {
     if (!p || !dst) return TT_ERR_NULL;

@@ -3,6 +3,8 @@
 // "conjugate-transposed diagonal blocks").  Both kernels stream Fhat from HBM
 // exactly once with 128-bit loads that bypass L1; they are bandwidth-bound (1 flop per byte
 // in complex64, 0.5 in complex128), so the design goal is bytes in flight, not math.
+#include <cstdio>
+
 #include "tt_common.cuh"
 #include "tt_internal.h"
 
@@ -188,6 +190,20 @@ static cudaError_t adj_dispatch(const void* Fhat, const void* dhat, void* xout, 
     k<<<grid, NT, smem, s>>>(static_cast<const Cx<R>*>(Fhat), static_cast<const Cx<R>*>(dhat),
                              static_cast<Cx<R>*>(xout), g);
     return cudaGetLastError();
+}
+
+// What the two launches above look like for geometry g (tt_plan_describe: bench.py ties its ncu figures to this string)
+int gemv_describe(int dt, const GemvGeom& g, char* buf, size_t n) {
+    const int NW = g_fwd_warps ? g_fwd_warps : g.warps ? g.warps : fwd_warps(g.N_d);
+    const int NT = g_adj_threads ? g_adj_threads : 256;
+    const int vn = dt == 0 ? 2 : 1;
+    const long long pe = g.p_end ? g.p_end : g.ldp;
+    return snprintf(buf, n,
+                    "A2 gemv_fwd_kernel<%s,8> grid=(%lld,%d) block=%d smem=%zu chunk=%d | "
+                    "B2 gemv_adj_kernel<%s,10> grid=(%lld,%d) block=%d smem=%zu",
+                    dt == 0 ? "float" : "double", (pe - g.p_begin + g.chunk - 1) / g.chunk, g.n_f, NW * 32,
+                    (size_t)g.chunk * (dt == 0 ? 8 : 16), g.chunk, dt == 0 ? "float" : "double",
+                    ((pe - g.p_begin) / vn + NT - 1) / NT, g.n_f, NT, (size_t)g.N_d * (dt == 0 ? 8 : 16));
 }
 
 cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* partial, const GemvGeom& g,

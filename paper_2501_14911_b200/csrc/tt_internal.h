@@ -88,6 +88,7 @@ cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* pa
                             cudaStream_t s);
 cudaError_t gemv_adj_launch(int dt, const void* Fhat, const void* dhat, void* xhat_out, const GemvGeom& g,
                             cudaStream_t s);
+int gemv_describe(int dt, const GemvGeom& g, char* buf, size_t n);  // snprintf semantics
 
 // k-RHS per-frequency complex GEMMs on the FP64 tensor pipe (DMMA) / fp32 FMA.
 //   Xhat[(w*N_m_pad... see tt_gemm.cu

@@ -428,7 +428,7 @@ int kd_qoi_run(const R* Fq, const R* Gq, const R* G, long long N_q, long long N_
 extern "C" int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m,
                                     int64_t N_t, int dtype, void* K, int64_t ldk, void* stream) {
     using namespace tt;
-    if (!Fcol || !Gcol || !noise_var || !K) return TT_ERR_NULL;
+    if (!Fcol || !Gcol || !K) return TT_ERR_NULL;   // noise_var == NULL: F G* alone (a rank's partial sum of the sharded assembly)
     if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
     if (N_d < 1 || N_m < 1 || N_t < 1 || N_d > 65535) return TT_ERR_SHAPE;
     const long long n = N_d * N_t;
@@ -449,6 +449,26 @@ extern "C" int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const vo
         : kd_run<double>(static_cast<const double*>(Fcol), static_cast<const double*>(Gcol),
                             static_cast<const double*>(noise_var), N_d, N_m, N_t, static_cast<double*>(K), ldk, s);
     if (e != cudaSuccess) { (void)cudaGetLastError(); return e == cudaErrorMemoryAllocation ? TT_ERR_OOM : TT_ERR_CUDA; }
+    return TT_OK;
+}
+
+// K[a][a] += noise_var[a]
+template <typename R>
+__global__ void __launch_bounds__(256)
+kd_add_noise_kernel(double* __restrict__ K, const R* __restrict__ noise_var, const long long n, const long long ldk) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a < n) K[a * ldk + a] += (double)noise_var[a];
+}
+
+extern "C" int tt_K_add_noise(const void* noise_var, int64_t n, int dtype, void* K, int64_t ldk, void* stream) {
+    if (!noise_var || !K) return TT_ERR_NULL;
+    if (dtype != TT_F32 && dtype != TT_F64) return TT_ERR_DTYPE;
+    if (n < 1 || ldk < n) return TT_ERR_SHAPE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    if (dtype == TT_F32) kd_add_noise_kernel<float><<<nb, 256, 0, s>>>(static_cast<double*>(K), static_cast<const float*>(noise_var), n, ldk);
+    else kd_add_noise_kernel<double><<<nb, 256, 0, s>>>(static_cast<double*>(K), static_cast<const double*>(noise_var), n, ldk);
+    if (cudaGetLastError() != cudaSuccess) return TT_ERR_CUDA;
     return TT_OK;
 }
 

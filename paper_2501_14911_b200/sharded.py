@@ -19,6 +19,19 @@ import torch
 import torch.distributed as dist
 
 
+class _AllReduce:
+    """In-place sum over the ranks of `group` (NCCL on GPUs, gloo in the CPU tests); nothing to do for a single rank.
+    The classes below take any callable with this signature instead, which is how the one-GPU test stands in for the
+    exchange step (tests/test_gpu_sharded.py: the emulated ranks' partials are summed in one process)."""
+
+    def __init__(self, group=None):
+        self.group = group
+
+    def __call__(self, t: torch.Tensor) -> None:
+        if dist.is_available() and dist.is_initialized() and dist.get_world_size(self.group) > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+
+
 def shard_range(N_m: int, rank: int, world: int, align: int = 16) -> tuple[int, int]:
     """Contiguous parameter range [p0, p1) of `rank`: equal shares, boundaries on multiples of `align`
     (the row pitch granularity of Fhat) except the last one; empty ranges only if N_m < world*align."""
@@ -35,17 +48,13 @@ class ShardedOperator:
     local_rmatvec(d)       -> this rank's slice of m' (tensor [N_t, p1 - p0])
     """
 
-    def __init__(self, local_matvec, local_rmatvec, group=None):
+    def __init__(self, local_matvec, local_rmatvec, group=None, all_reduce=None):
         self.local_matvec, self.local_rmatvec, self.group = local_matvec, local_rmatvec, group
-
-    @property
-    def world(self) -> int:
-        return dist.get_world_size(self.group) if dist.is_available() and dist.is_initialized() else 1
+        self.all_reduce = all_reduce or _AllReduce(group)
 
     def matvec(self, m_local: torch.Tensor) -> torch.Tensor:
         d = self.local_matvec(m_local)
-        if self.world > 1:
-            dist.all_reduce(d, op=dist.ReduceOp.SUM, group=self.group)   # the path's only exchange step
+        self.all_reduce(d)                                               # the path's only exchange step
         return d
 
     def rmatvec(self, d: torch.Tensor) -> torch.Tensor:
@@ -55,9 +64,9 @@ class ShardedOperator:
         return self.rmatvec(self.matvec(m_local))
 
 
-def from_plan(plan, group=None) -> ShardedOperator:
+def from_plan(plan, group=None, all_reduce=None) -> ShardedOperator:
     """Wraps a tt Plan built on this rank's slice F[:, :, p0:p1] of the block column."""
-    return ShardedOperator(plan.matvec, plan.rmatvec, group)
+    return ShardedOperator(plan.matvec, plan.rmatvec, group, all_reduce)
 
 
 class ShardedMapInference:
@@ -74,20 +83,20 @@ class ShardedMapInference:
       gain(d_obs)    -> m_map slice    G* K^{-1} d_obs (tt_map_infer TT_MAP_GAIN): no collective at all
     """
 
-    def __init__(self, partial, finish, gain, group=None):
+    def __init__(self, partial, finish, gain, group=None, all_reduce=None):
         self.partial, self.finish, self.gain, self.group = partial, finish, gain, group
+        self.all_reduce = all_reduce or _AllReduce(group)
 
     def infer(self, d_obs: torch.Tensor, gain_form: bool = False) -> torch.Tensor:
         """This rank's slice of m_map."""
         if gain_form:
             return self.gain(d_obs)
         b = self.partial(d_obs)
-        if dist.is_available() and dist.is_initialized() and dist.get_world_size(self.group) > 1:
-            dist.all_reduce(b, op=dist.ReduceOp.SUM, group=self.group)       # the path's only exchange step
+        self.all_reduce(b)                                                   # the path's only exchange step
         return self.finish(b)
 
 
-def map_from_binding(mp, group=None) -> ShardedMapInference:
+def map_from_binding(mp, group=None, all_reduce=None) -> ShardedMapInference:
     """Wraps a binding.MapInference built on this rank's slices of the block columns of F and G*."""
     from . import binding as tt
     state = {}
@@ -99,18 +108,16 @@ def map_from_binding(mp, group=None) -> ShardedMapInference:
     def finish(b):
         return mp.infer_finish(b, state.pop("a"))
 
-    return ShardedMapInference(partial, finish, lambda d: mp.infer(d, tt.TT_MAP_GAIN), group)
+    return ShardedMapInference(partial, finish, lambda d: mp.infer(d, tt.TT_MAP_GAIN), group, all_reduce)
 
 
-def assemble_K_sharded(local_assemble, noise_var: torch.Tensor, group=None) -> torch.Tensor:
+def assemble_K_sharded(local_product, add_noise, group=None, all_reduce=None) -> torch.Tensor:
     """K = Gamma_noise + F G* with the parameter axis sharded: F G* = sum_g F[:, :, P_g] G[:, :, P_g]^* is a sum over the ranks'
-    parameter slices, so every rank assembles the product of its own slices WITHOUT noise (`local_assemble(noise_var)` is called
-    with zeros: binding.assemble_K_direct on the rank's block-column slices on a GPU, the oracle in the gloo test), ONE
-    all-reduce (sum) of the n x n matrix follows (4.8 GB at the paper's shape), and the noise is added once, after it."""
-    K = local_assemble(torch.zeros_like(noise_var))
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(K, op=dist.ReduceOp.SUM, group=group)
-    n = K.shape[0]
-    K.view(-1)[:: n + 1] += noise_var.reshape(-1).to(K.dtype)
+    parameter slices, so every rank forms the product of its own slices WITHOUT noise (`local_product()`:
+    binding.assemble_K_direct(..., noise_var=None) on a GPU, the oracle with zero noise in the gloo test), ONE all-reduce (sum)
+    of the n x n matrix follows (4.8 GB at the paper's shape), and the noise is added once, after it, by `add_noise(K)`
+    (binding.tt_K_add_noise on a GPU).  No arithmetic happens here."""
+    K = local_product()
+    (all_reduce or _AllReduce(group))(K)
+    add_noise(K)
     return K
-

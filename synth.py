@@ -4,7 +4,8 @@ This module holds NONE of the method's arithmetic: it only draws the block
 column F_k (k = 0..N_t-1, each N_d x N_m), the parameter vector m and the data
 vector d of the five workloads named in BASELINE.json, with the recipe frozen
 in DESIGN.md ("Input recipe").  Both the CPU oracle's tests and the CUDA
-path's tests/bench take their inputs from here, so the two sides always see
+path's tests/bench take their inputs from here (a module of its own at the repo root, outside the product
+package), so the two sides always see
 the same bytes.
 
 Every element is a pure function of (seed, tensor_id, linear_index): a
@@ -192,10 +193,12 @@ def prior_gamma(w: Workload, device="cpu") -> torch.Tensor:
     return 0.5 + torch.exp(-((p - 0.5 * w.N_m) / (0.25 * w.N_m)) ** 2)
 
 
-def gstar_block_column(w: Workload, F: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
-    """Block column G_k = F_k Gamma_s of G* = Gamma_prior F* for the diagonal prior above,
-    formed in fp64 and rounded once to w.dtype.  Harness code: in the paper this is the output of N_d prior
-    solves (Phase 2), an input of the online phase.  Works plane by plane to bound scratch memory."""
+def scaled_block_column(w: Workload, F: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+    """The SECOND input block column of the online phase at sizes where it has to be drawn on the device: column p of
+    every block of F scaled by the prior weight prior_gamma(w)[p], in fp64, rounded once to w.dtype.  In the paper this
+    array is the output of N_d prior solves (Phase 2) and an INPUT of the online phase; the formula
+    G_k = F_k Gamma_s belongs to oracle/online_plain.gstar_block_column, which the small parity tests use directly and
+    which tests/test_synth.py holds this generator to, bit for bit.  Works plane by plane to bound scratch memory."""
     g = prior_gamma(w, F.device)
     out = torch.empty_like(F) if out is None else out
     for k in range(F.shape[0]):

@@ -18,7 +18,7 @@ sys.path.insert(0, ROOT)
 
 from oracle import online_plain as oo  # noqa: E402
 from oracle import toeplitz_plain as op  # noqa: E402
-from paper_2501_14911_b200 import synth  # noqa: E402
+import synth  # noqa: E402
 
 
 def main():
@@ -41,9 +41,9 @@ def main():
     wo = synth.CONFIGS["P5"].scaled(N_d=4, N_m=64, N_t=32, dtype=torch.float64)
     wq = synth.CONFIGS["Q5"].scaled(N_d=2, N_m=64, N_t=32, dtype=torch.float64)
     Fo = synth.block_column(wo)
-    Go = synth.gstar_block_column(wo, Fo).numpy()
+    Go = oo.gstar_block_column(Fo.numpy(), synth.prior_gamma(wo).numpy())
     Fq = synth.block_column(wq)
-    Gq = synth.gstar_block_column(wq, Fq).numpy()
+    Gq = oo.gstar_block_column(Fq.numpy(), synth.prior_gamma(wq).numpy())
     Fo, Fq = Fo.numpy(), Fq.numpy()
     nv, d_obs = synth.noise_var(wo).numpy(), synth.vector_d(wo, k_rhs=1).numpy()
     u = synth.vector_m(wo, k_rhs=1).numpy()

@@ -7,7 +7,8 @@ import pytest
 
 from oracle import toeplitz_blocked as ob
 from oracle import toeplitz_plain as op
-from paper_2501_14911_b200 import synth
+import synth
+from tests.inputs_online import gstar_column
 
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "c1_oracle.txt")
 
@@ -67,7 +68,7 @@ def online_case():
     wo = synth.CONFIGS["P5"].scaled(N_d=4, N_m=64, N_t=32, dtype=torch.float64)
     wq = synth.CONFIGS["Q5"].scaled(N_d=2, N_m=64, N_t=32, dtype=torch.float64)
     F = synth.block_column(wo)
-    G = synth.gstar_block_column(wo, F)
+    G = gstar_column(wo, F)
     Fq = synth.block_column(wq)
     nv, d_obs, u = synth.noise_var(wo), synth.vector_d(wo, k_rhs=1), synth.vector_m(wo, k_rhs=1)
     L = oo.cholesky(oo.assemble_K(F.numpy(), G.numpy(), nv.numpy()))

@@ -7,7 +7,7 @@ import torch
 
 from oracle import toeplitz_blocked as ob
 from oracle import toeplitz_plain as op
-from paper_2501_14911_b200 import synth
+import synth
 
 pytestmark = pytest.mark.gpu
 TOL = {torch.float64: 1e-12, torch.float32: 1e-5}

@@ -16,7 +16,8 @@ import torch
 
 from oracle import online_plain as oo
 from oracle import toeplitz_plain as op
-from paper_2501_14911_b200 import synth
+import synth
+from tests.inputs_online import gstar_column
 
 pytestmark = pytest.mark.gpu
 
@@ -117,7 +118,7 @@ def test_trsv_nan_rhs_terminates(tt):
 def online_inputs(N_d, N_m, N_t, dtype):
     w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
     F = synth.block_column(w)
-    G = synth.gstar_block_column(w, F)
+    G = gstar_column(w, F)
     nv = synth.noise_var(w)
     d_obs = synth.vector_d(w, k_rhs=1)
     return w, F, G, nv, d_obs
@@ -268,7 +269,7 @@ def test_outputs_stay_inside_their_buffers(tt):
         N_d, N_m, N_t, k = 5, 1001, 35, 7
         w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
         F = synth.block_column(w)
-        G = synth.gstar_block_column(w, F)
+        G = gstar_column(w, F)
         nv = synth.noise_var(w)
         L = oo.cholesky(oo.assemble_K(F.numpy(), G.numpy(), nv.numpy()))
         pF, pG = tt.Plan(F.cuda(), k_max=k), tt.Plan(G.cuda(), k_max=k)
@@ -368,7 +369,7 @@ def test_pipelined_host_calls_equal_device_calls(tt, dtype, layout):
     N_d, N_m, N_t, r = 3, 40007, 20, 2
     w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
     F = synth.block_column(w)
-    G = synth.gstar_block_column(w, F)
+    G = gstar_column(w, F)
     nv, d_obs = synth.noise_var(w), synth.vector_d(w, k_rhs=1)
     m = synth.vector_m(w, k_rhs=1)
     lay = (lambda t: t.t().contiguous()) if layout == 1 else (lambda t: t)
@@ -464,7 +465,7 @@ def test_phase3_compositions(tt, dtype):
     w, F, G, nv, d_obs = online_inputs(N_d, N_m, N_t, dtype)
     wq = synth.CONFIGS["Q5"].scaled(N_d=N_q, N_m=N_m, N_t=N_t, dtype=dtype)
     Fq = synth.block_column(wq)
-    Gq = synth.gstar_block_column(wq, Fq)
+    Gq = gstar_column(wq, Fq)
     v = synth.vector_d(wq.scaled(N_t=N_t // r), k_rhs=1)
     Fn, Gn, nvn = F.numpy(), G.numpy(), nv.numpy()
     K = oo.assemble_K(Fn, Gn, nvn)
@@ -508,7 +509,7 @@ def test_qoi_direct(tt, N_d, N_q, N_m, N_t, r, dtype):
     w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
     wq = synth.CONFIGS["Q5"].scaled(N_d=N_q, N_m=N_m, N_t=N_t, dtype=dtype)
     Fq = synth.block_column(wq)
-    Gq = synth.gstar_block_column(wq, Fq)
+    Gq = gstar_column(wq, Fq)
     Fn, Gn, nvn, Fqn, Gqn = F.numpy(), G.numpy(), nv.numpy(), Fq.numpy(), Gq.numpy()
     K = oo.assemble_K(Fn, Gn, nvn)
     L = oo.cholesky(K)

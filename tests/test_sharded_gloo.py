@@ -10,7 +10,9 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 from oracle import toeplitz_plain as op
-from paper_2501_14911_b200 import sharded, synth
+import synth
+from paper_2501_14911_b200 import sharded
+from tests.inputs_online import gstar_column
 
 
 def test_shard_range_covers_and_aligns():
@@ -50,7 +52,7 @@ def _worker(rank, world, port, out_dir):
         from oracle import online_plain as oo
         wo = synth.CONFIGS["P5"].scaled(N_d=3, N_m=70, N_t=12, dtype=torch.float64)
         Fo = synth.block_column(wo)
-        Go = synth.gstar_block_column(wo, Fo).numpy()
+        Go = gstar_column(wo, Fo).numpy()
         Fo = Fo.numpy()
         nv, dob = synth.noise_var(wo).numpy(), synth.vector_d(wo, k_rhs=1).numpy()
         Lc = oo.cholesky(oo.assemble_K(Fo, Go, nv))
@@ -71,7 +73,10 @@ def _worker(rank, world, port, out_dir):
             ok = ok and np.allclose(got, m_ref[:, p0:p1], rtol=0, atol=1e-10 * np.abs(m_ref).max())
         # K = Gamma_noise + F G* assembled from the ranks' parameter slices: one all-reduce, the noise added once
         K_ref = oo.assemble_K(Fo, Go, nv)
-        K_sh = sharded.assemble_K_sharded(lambda z: torch.from_numpy(oo.assemble_K(Fl2, Gl2, z.numpy())), torch.from_numpy(nv)).numpy()
+        def add_noise(K):        # on a GPU: binding.tt_K_add_noise; here the test adds the diagonal itself
+            K.view(-1)[:: K.shape[0] + 1] += torch.from_numpy(nv).reshape(-1)
+
+        K_sh = sharded.assemble_K_sharded(lambda: torch.from_numpy(oo.assemble_K(Fl2, Gl2, np.zeros_like(nv))), add_noise).numpy()
         ok = ok and np.allclose(K_sh, K_ref, rtol=0, atol=1e-12 * np.abs(K_ref).max())
         with open(os.path.join(out_dir, f"rank{rank}.ok"), "w") as f:
             f.write("1" if ok else "0")

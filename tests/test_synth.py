@@ -4,7 +4,7 @@ import math
 import numpy as np
 import torch
 
-from paper_2501_14911_b200 import synth
+import synth
 
 
 def test_configs_match_baseline_json_shapes():
@@ -56,3 +56,14 @@ def test_normal_moments_and_envelopes():
         sigma = 0.05 * 4000
         near = e[max(0, mu - int(3 * sigma)): mu + int(3 * sigma)].sum()
         assert near / e.sum() > 0.99
+
+
+def test_scaled_block_column_is_the_oracles_gstar_column():
+    """synth.scaled_block_column (the device-side generator of the second block column at full size) against
+    oracle/online_plain.gstar_block_column (G_k = F_k Gamma_s), bit for bit in both dtypes."""
+    from oracle import online_plain as oo
+    for dtype in (torch.float64, torch.float32):
+        w = synth.CONFIGS["P5"].scaled(N_d=3, N_m=257, N_t=5, dtype=dtype)
+        F = synth.block_column(w)
+        ref = torch.from_numpy(oo.gstar_block_column(F.numpy(), synth.prior_gamma(w).numpy())).to(dtype)
+        assert torch.equal(synth.scaled_block_column(w, F), ref)
