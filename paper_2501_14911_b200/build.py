@@ -22,7 +22,7 @@ BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtt.so")
 STAMP = os.path.join(BUILD, "libtt.stamp")
 
-SOURCES = ["tt_api.cu", "tt_fft.cu", "tt_gemv.cu", "tt_gemm.cu", "tt_gemm32.cu", "tt_trsv.cu", "tt_online.cu", "tt_kdirect.cu"]
+SOURCES = ["tt_api.cu", "tt_fft.cu", "tt_gemv.cu", "tt_gemm.cu", "tt_gemm32.cu", "tt_trsv.cu", "tt_online.cu", "tt_kdirect.cu", "tt_kdirect_umma.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",

@@ -892,6 +892,7 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "fft_max_radix")) { g_fft_max_radix = value; return TT_OK; }
     if (!std::strcmp(key, "fft_no_static")) { fft_debug_no_static(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
+    if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }
     if (!std::strcmp(key, "gemm_adj_mt")) { gemm_debug_set_adj(value); return TT_OK; }

@@ -135,6 +135,11 @@ cudaError_t trsv_post_launch(const TrsvGeom& g, double* x, cudaStream_t s);     
 void trsv_debug_set_U(int U);  // blocks in flight per warp: 1, 2 (default), 3
 cudaError_t trsv_copy_launch(const double* src, double* dst, long long n, cudaStream_t s);
 
+// fp32 C (fp64) = A B^T on tcgen05 (3 x tf32 split, TMA-fed, accumulators in tensor memory): tt_kdirect_umma.cu
+cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA, long long nB, long long Kdim, long long ldc,
+                         int lower_only, cudaStream_t s);
+void kd_umma_debug_set_slab(int ks);  // parameters accumulated in tensor memory between fp64 flushes (0 = default)
+
 // sink: >= 148*8*256 doubles
 cudaError_t probe_dmma_launch(int iters, void* sink, double* flops, cudaStream_t s);
 cudaError_t probe_stream_read_launch(const void* src, size_t bytes, void* sink, cudaStream_t s);

@@ -14,13 +14,15 @@
 // on 24 A100); tt_assemble_K does that with batched FFT matvecs (4.1 ms per column on one B200).  The same matrix costs
 // 2 n^2 N_m flop this way (half of it: K is symmetric, only the lower triangle is computed and then mirrored) and no FFT at all.
 //
-//   1. kd_gemm_kernel     W (lower tiles) = Fcol Gcol^T into K (fp64): fp32 FMA, register-tiled (kd_gemm_dmma_kernel for fp64
-//                         block columns: the FP64 tensor pipe)
+//   1. W (lower tiles) = Fcol Gcol^T into K (fp64).  fp32 block columns: kd_umma_kernel (tt_kdirect_umma.cu) - tcgen05.mma
+//                         kind::tf32 with the 3-product hi/lo split, TMA-fed, accumulators in tensor memory.  fp64 block
+//                         columns: kd_gemm_dmma_kernel, the FP64 tensor instruction (tcgen05 has no f64 kind)
 //   2. kd_diag_kernel     in-place running sums down the block diagonals of the lower triangle, + Gamma_noise on the diagonal
 //   3. kd_mirror_kernel   upper triangle := transpose of the lower one
 //
-// Precision: TT_F32 multiplies and accumulates in fp32 over chunks of 8192 parameters (even and odd parameters in separate
-// accumulators) and adds the chunk sums, and the running sums of step 2, in fp64; TT_F64 is fp64 throughout (DMMA).
+// Precision: TT_F32 forms every product from the tf32 hi/lo parts of its factors (error <= 2^-21 per product), sums 128
+// parameters in the tensor core's fp32 accumulator, the 128-parameter sums of a slab of 8192 in fp32 registers, and the slab
+// sums and the running sums of step 2 in fp64; TT_F64 is fp64 throughout (DMMA).
 #include <type_traits>
 
 #include "../../include/tt.h"
@@ -30,141 +32,12 @@
 namespace tt {
 namespace {
 
-constexpr int kKdBM = 128;     // rows of Fcol per CTA tile
+constexpr int kKdBM = 128;     // rows of Fcol per CTA tile (fp64 DMMA kernel)
 constexpr int kKdBK = 32;      // parameters per shared-memory stage
-constexpr int kKdThreads = 256;  // 16 x 16 threads, a thread owns 8 x TN entries (rows ty + 16 i, columns tx + 16 j)
-constexpr int kKdChunkTiles = 256;  // TT_F32: flush the fp32 accumulators into the fp64 result every 256 stages = 8192 parameters
-
-template <typename R> struct KdVec;
-template <> struct KdVec<float> { using type = float4; static constexpr int n = 4; };
-template <> struct KdVec<double> { using type = double2; static constexpr int n = 2; };
-__device__ __forceinline__ float kd_get(const float4& v, int i) { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
-__device__ __forceinline__ double kd_get(const double2& v, int i) { return i == 0 ? v.x : v.y; }
-// c.lo += a.lo * b.lo,  c.hi += a.hi * b.hi  on packed pairs of floats
-__device__ __forceinline__ void kd_fma2(unsigned long long& c, unsigned long long a, unsigned long long b) {
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
-}
-__device__ __forceinline__ double kd_total(unsigned long long c) {
-    return (double)__uint_as_float((unsigned)(c & 0xffffffffull)) + (double)__uint_as_float((unsigned)(c >> 32));
-}
-__device__ __forceinline__ double kd_total(double c) { return c; }
-__device__ __forceinline__ double kd_total(float c) { return (double)c; }
-
-// C[a][b] (+)= sum_k A[a][k] B[b][k] for the tiles that touch the lower triangle; A, B: n x Kdim row-major (pitch Kdim, any
-// alignment: scalar loads, a warp reads 32 consecutive k of one row).  Shared memory holds [row][k] with a pitch of
-// 32 + 16 bytes, so that the 16-byte fragment loads of 8 consecutive rows fall into 8 different bank groups.
-template <typename R, int TN>
-__global__ void __launch_bounds__(kKdThreads, 1)
-kd_gemm_kernel(const R* __restrict__ A, const R* __restrict__ B, double* __restrict__ C, const long long nA,
-               const long long nB, const long long Kdim, const long long ldc, const int chunk_tiles, const int lower_only) {
-    using V = typename KdVec<R>::type;
-    constexpr int KV = KdVec<R>::n, P = kKdBK + KV, BN = 16 * TN, ROWS = kKdBM + BN;
-    constexpr int LA = kKdBM / 8, LB = BN / 8;   // rows of the A / B tile loaded per thread and stage
-    const int tn = blockIdx.x, tm = blockIdx.y;
-    if (lower_only && (long long)tn * BN >= (long long)(tm + 1) * kKdBM) return;   // tile entirely above the diagonal
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    R* sm = reinterpret_cast<R*>(smem_raw);   // [2][ROWS][P]
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, tx = tid & 15, ty = tid >> 4;
-    const long long rowA0 = (long long)tm * kKdBM, rowB0 = (long long)tn * BN;
-    const R* pa = A + (rowA0 + warp) * Kdim + lane;
-    const R* pb = B + (rowB0 + warp) * Kdim + lane;
-    unsigned okA = 0, okB = 0;
-#pragma unroll
-    for (int i = 0; i < LA; ++i) okA |= (rowA0 + warp + 8 * i < nA ? 1u : 0u) << i;
-#pragma unroll
-    for (int i = 0; i < LB; ++i) okB |= (rowB0 + warp + 8 * i < nB ? 1u : 0u) << i;
-
-    R pre[LA + LB];
-    auto gload = [&](long long k0) {
-        const bool kok = k0 + lane < Kdim;
-#pragma unroll
-        for (int i = 0; i < LA; ++i) pre[i] = (kok && ((okA >> i) & 1u)) ? __ldg(pa + k0 + (long long)(8 * i) * Kdim) : R(0);
-#pragma unroll
-        for (int i = 0; i < LB; ++i) pre[LA + i] = (kok && ((okB >> i) & 1u)) ? __ldg(pb + k0 + (long long)(8 * i) * Kdim) : R(0);
-    };
-    auto sstore = [&](int stage) {
-        R* s = sm + stage * (ROWS * P);
-#pragma unroll
-        for (int i = 0; i < LA; ++i) s[(warp + 8 * i) * P + lane] = pre[i];
-#pragma unroll
-        for (int i = 0; i < LB; ++i) s[(kKdBM + warp + 8 * i) * P + lane] = pre[LA + i];
-    };
-
-    // fp32: packed accumulators {sum over even k, sum over odd k} driven by fma.rn.f32x2 (SASS FFMA2) - both operands are
-    // k-adjacent pairs exactly as they lie in shared memory, so no packing moves are needed; a three-register scalar FFMA issues
-    // every other cycle per sub-partition on this part, FFMA2 does two of them in that slot.  fp64: scalar DFMA.
-    constexpr bool PACKED = sizeof(R) == 4;
-    using Acc = typename std::conditional<PACKED, unsigned long long, R>::type;
-    Acc acc[8][TN];
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-#pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j] = Acc(0);
-
-    const int nk = (int)((Kdim + kKdBK - 1) / kKdBK);
-    bool first = true;
-    int until_flush = chunk_tiles;
-    gload(0);
-    sstore(0);
-    __syncthreads();
-    for (int t = 0; t < nk; ++t) {
-        if (t + 1 < nk) gload((long long)(t + 1) * kKdBK);
-        const R* s = sm + (int)(t & 1) * (ROWS * P);
-#pragma unroll 2
-        for (int g = 0; g < kKdBK / KV; ++g) {
-            if constexpr (PACKED) {
-                ulonglong2 a[8], b[TN];   // .x = (k, k+1), .y = (k+2, k+3) of one row
-#pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const ulonglong2*>(s + (ty + 16 * i) * P + g * KV);
-#pragma unroll
-                for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const ulonglong2*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-#pragma unroll
-                    for (int j = 0; j < TN; ++j) kd_fma2(acc[i][j], a[i].x, b[j].x);
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-#pragma unroll
-                    for (int j = 0; j < TN; ++j) kd_fma2(acc[i][j], a[i].y, b[j].y);
-            } else {
-                V a[8], b[TN];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = *reinterpret_cast<const V*>(s + (ty + 16 * i) * P + g * KV);
-#pragma unroll
-                for (int j = 0; j < TN; ++j) b[j] = *reinterpret_cast<const V*>(s + (kKdBM + tx + 16 * j) * P + g * KV);
-#pragma unroll
-                for (int kk = 0; kk < KV; ++kk)
-#pragma unroll
-                    for (int i = 0; i < 8; ++i)
-#pragma unroll
-                        for (int j = 0; j < TN; ++j) acc[i][j] = fma(kd_get(a[i], kk), kd_get(b[j], kk), acc[i][j]);
-            }
-        }
-        if (t + 1 < nk) sstore((int)((t + 1) & 1));
-        __syncthreads();
-        if (--until_flush == 0 || t + 1 == nk) {   // chunk sums meet in fp64, in a fixed order
-            until_flush = chunk_tiles;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const long long row = rowA0 + ty + 16 * i;
-#pragma unroll
-                for (int j = 0; j < TN; ++j) {
-                    const long long col = rowB0 + tx + 16 * j;
-                    if (row < nA && col < nB) {
-                        double* c = C + row * ldc + col;
-                        *c = (first ? 0.0 : *c) + kd_total(acc[i][j]);
-                    }
-                    acc[i][j] = Acc(0);
-                }
-            }
-            first = false;
-        }
-    }
-}
+constexpr int kKdThreads = 256;
 
 // fp64 on the FP64 tensor pipe: mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4), the same instruction as the k-RHS GEMMs of tt_gemm.cu.
-// CTA tile 128 x 64, 8 warps as 4 x 2, warp tile 32 x 32 = 4 x 4 DMMA tiles; same staging as kd_gemm_kernel; the [row][k] tile has
+// CTA tile 128 x 64, 8 warps as 4 x 2, warp tile 32 x 32 = 4 x 4 DMMA tiles; stages of 32 parameters read with scalar loads (rows have no alignment); the [row][k] tile has
 // a pitch of 36 doubles, so the fragment loads (row lane/4, k lane%4) of each half-warp fall into 16 different 8-byte bank pairs.
 // A fragment: A[row = lane/4][k = lane%4]; B fragment: B[n = lane/4][k = lane%4]; C: [lane/4][2 (lane%4) + {0, 1}].
 __device__ __forceinline__ void kd_dmma(double& c0, double& c1, double a, double b) {
@@ -288,20 +161,14 @@ template <typename R>
 cudaError_t kd_launch_gemm(const R* A, const R* B, double* C, long long nA, long long nB, long long Kdim, long long ldc,
                            int lower_only, cudaStream_t s) {
     cudaError_t e = cudaSuccess;
-    if constexpr (sizeof(R) == 8) {   // DMMA: 0.585 s against 0.864 s for the DFMA form of kd_gemm_kernel at N_m = 26 316
+    if constexpr (sizeof(R) == 8) {   // DMMA: 0.585 s against 0.864 s for a register-tiled DFMA form at N_m = 26 316
         const size_t smem = (size_t)2 * (kKdBM + kKdDmmaBN) * kKdDmmaP * sizeof(double);
         e = cudaFuncSetAttribute(kd_gemm_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         const dim3 grid((unsigned)((nB + kKdDmmaBN - 1) / kKdDmmaBN), (unsigned)((nA + kKdBM - 1) / kKdBM));
         kd_gemm_dmma_kernel<<<grid, kKdThreads, smem, s>>>(A, B, C, nA, nB, Kdim, ldc, lower_only);
-    } else {
-        constexpr int TN = 8, BN = 16 * TN, P = kKdBK + KdVec<R>::n;
-        auto k = kd_gemm_kernel<R, TN>;
-        const size_t smem = (size_t)2 * (kKdBM + BN) * P * sizeof(R);
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        const dim3 grid((unsigned)((nB + BN - 1) / BN), (unsigned)((nA + kKdBM - 1) / kKdBM));
-        k<<<grid, kKdThreads, smem, s>>>(A, B, C, nA, nB, Kdim, ldc, kKdChunkTiles, lower_only);
+    } else {   // fp32: 3 x tf32 split on tcgen05 (tt_kdirect_umma.cu)
+        return kd_umma_gemm(A, B, C, nA, nB, Kdim, ldc, lower_only, s);
     }
     return cudaGetLastError();
 }
