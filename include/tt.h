@@ -293,7 +293,7 @@ int tt_assemble_K(const tt_plan* F, const tt_plan* G, const void* noise_var, int
  * MMAs, error <= 2^-21 per product), 128-parameter sums in tensor memory, their sums over 8192 parameters in fp32, everything
  * above that in fp64; TT_F64: fp64 throughout (FP64 tensor instruction).
  * Asynchronous on `stream`.  TT_F32 takes its scratch (the hi/lo parts of one slab of 8192 parameters of both block columns,
- * 32 n * 8192 bytes = 6.4 GB at n = 24 500) from the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync on `stream`):
+ * 16 n * 8192 bytes = 3.2 GB at n = 24 500) from the stream-ordered allocator (cudaMallocAsync / cudaFreeAsync on `stream`):
  * no synchronisation, TT_ERR_OOM if the device cannot provide it. */
 int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m, int64_t N_t,
                          int dtype, void* K, int64_t ldk, void* stream);

@@ -302,6 +302,28 @@ def test_outputs_stay_inside_their_buffers(tt):
             assert torch.isfinite(buf[4096:4096 + n]).all()
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_K_direct_stays_inside_its_matrix(tt, dtype):
+    """tt_assemble_K_direct (fp32: the tcgen05 kernel, whose 128 x 256 tiles overhang a ragged n on both sides; fp64: DMMA)
+    into a matrix with a row pitch larger than n, canary zones before and after: the pad columns of every row and the zones
+    keep their values, every entry of K is written."""
+    N_d, N_m, N_t = 7, 333, 41                       # n = 287: two tile rows, two tile columns, both ragged
+    w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
+    F = synth.block_column(w)
+    G = gstar_column(w, F)
+    nv = synth.noise_var(w)
+    n, ldk = N_d * N_t, N_d * N_t + 37
+    buf, K = _guarded((n, ldk), torch.float64)
+    K[:, :n] = float("nan")
+    tt.tt_assemble_K_direct(F.cuda(), G.cuda(), nv.cuda(), N_d, N_m, N_t, tt.TT_F32 if dtype == torch.float32 else tt.TT_F64, K, ldk)
+    torch.cuda.synchronize()
+    assert (buf[:4096] == -7.0).all() and (buf[4096 + n * ldk:] == -7.0).all()
+    assert (K[:, n:] == -7.0).all()
+    assert torch.isfinite(K[:, :n]).all()
+    ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
+    assert rel(K[:, :n].cpu().numpy(), ref) <= (1e-12 if dtype == torch.float64 else 1e-5)
+
+
 def test_map_two_halves_equal_the_whole(tt):
     """tt_map_infer_partial + tt_map_infer_finish (the split at the sharded path's all-reduce) == tt_map_infer."""
     from paper_2501_14911_b200 import sharded
