@@ -42,7 +42,7 @@ FALLBACK_HBM_GBS = 6650.0    # B200_PROFILING.md fallback
 # capture of each config.  A figure is only quoted when the plan built in THIS run describes its kernels (tt_plan_describe)
 # with the line the capture's summary records; otherwise `traffic` is null and the line says why.
 NCU_TRAFFIC = {
-    "C3": {"bytes": 81.003059e9 + 22.79e6, "profile": "profiles/r1_i_c3_ncu_full.md",
+    "C3": {"bytes": 81.003854e9 + 23.052e6, "profile": "profiles/r2_c3_ncu_full.md",
            "kernel": "A2 gemv_fwd_kernel<float,8> grid=(62,401) block=512 smem=32768 chunk=4096"},
 }
 

@@ -34,16 +34,21 @@ namespace {
 
 using namespace umma;
 
-constexpr int kBM = 128, kBN = 256, kBK = 32;       // C tile, K-block (32 floats = one 128-byte swizzle row)
-constexpr int kStages = 2;
-constexpr int kABytes = kBM * kBK * 4, kBBytes = kBN * kBK * 4;
-constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // 96 KB: A hi, A lo, B hi, B lo
+constexpr int kBM = 128, kBN = 256;                 // C tile
+// K-block BK = floats of K per shared-memory stage and operand row = one swizzle span: 32 (128-byte swizzle, 96 KB per stage,
+// two stages).  BK = 16 (64-byte swizzle, four stages of 48 KB) was measured slower at the paper's shape: 1.09 s against 0.80 - 0.91 s.
+template <int BK> struct Geo {
+    static constexpr int kStages = BK == 32 ? 2 : 4;
+    static constexpr int kABytes = kBM * BK * 4, kBBytes = kBN * BK * 4;
+    static constexpr int kStageBytes = 2 * kABytes + 2 * kBBytes;   // A hi, A lo, B hi, B lo
+    static constexpr int kChunkBlocks = 128 / BK;   // K-blocks accumulated in tensor memory between register flushes (128 parameters)
+    static constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers, tmem address */;
+};
+constexpr int kMaxBK = 32;                          // slabs are padded to a multiple of this
 constexpr int kCtrlWarps = 4, kEpiWarps = 8;        // warpgroup 0: TMA / MMA / tensor-memory allocation; warpgroups 1-2: epilogue
 constexpr int kThreads = 32 * (kCtrlWarps + kEpiWarps);
 constexpr int kAccCols = kBN;                       // fp32 accumulator: one tensor-memory column per C column
-constexpr int kChunkBlocks = 4;                     // K-blocks accumulated in tensor memory between register flushes (128 parameters)
 constexpr int kPanel = 8;                           // tile columns per panel of the tile order
-constexpr int kSmemBytes = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers, tmem address */;
 
 // hi / lo split of one slab: dst_hi/dst_lo[row][0..kpad) for src[row][k0 .. k0 + ks), zero beyond ks (kpad = ks rounded
 // up to the K-block).  One warp per (row, 1024-parameter segment): lanes read consecutive parameters.
@@ -103,11 +108,14 @@ struct UmmaArgs {
     int first;             // 1: C = acc (first slab), 0: C += acc
 };
 
+template <int BK>
 __global__ void __launch_bounds__(kThreads, 1)
 kd_umma_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant__ CUtensorMap tmA_lo,
                const __grid_constant__ CUtensorMap tmB_hi, const __grid_constant__ CUtensorMap tmB_lo, const UmmaArgs g) {
+    constexpr int kBK = BK, kStages = Geo<BK>::kStages, kABytes = Geo<BK>::kABytes, kBBytes = Geo<BK>::kBBytes,
+                  kStageBytes = Geo<BK>::kStageBytes, kChunkBlocks = Geo<BK>::kChunkBlocks;
     extern __shared__ unsigned char smem_raw[];
-    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;       // 128-byte swizzle atoms want 1024-byte alignment
+    const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;       // swizzle atoms want 1024-byte alignment
     const uint32_t bars = base + kStages * kStageBytes;                // full[S], empty[S], tmem_full[2], tmem_empty[2]
     auto full_bar = [&](int s) { return bars + 8u * s; };
     auto empty_bar = [&](int s) { return bars + 8u * (kStages + s); };
@@ -170,9 +178,9 @@ kd_umma_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                         mbar_wait(full_bar(stage), phase);              // the four tiles of this stage have landed
                         tc_fence_after();
                         const uint32_t sa = base + stage * kStageBytes;
-                        const uint64_t a_hi = smem_desc_kmajor<128>(sa), a_lo = smem_desc_kmajor<128>(sa + kABytes);
-                        const uint64_t b_hi = smem_desc_kmajor<128>(sa + 2 * kABytes),
-                                       b_lo = smem_desc_kmajor<128>(sa + 2 * kABytes + kBBytes);
+                        const uint64_t a_hi = smem_desc_kmajor<4 * BK>(sa), a_lo = smem_desc_kmajor<4 * BK>(sa + kABytes);
+                        const uint64_t b_hi = smem_desc_kmajor<4 * BK>(sa + 2 * kABytes),
+                                       b_lo = smem_desc_kmajor<4 * BK>(sa + 2 * kABytes + kBBytes);
 #pragma unroll
                         for (int k = 0; k < kBK / 8; ++k) {             // 8 tf32 = 32 bytes along K: + 2 in the address field
                             const uint64_t o = (uint64_t)(k * 2);
@@ -259,15 +267,15 @@ EncodeTiledFn encode_fn() {
 
 // rows x kpad floats, row pitch `pitch` floats (a multiple of 4), boxes of box_rows x 32 floats, 128-byte swizzle; rows
 // beyond `rows` read as zeros
-bool make_map(CUtensorMap* m, float* ptr, long long rows, int kpad, long long pitch, int box_rows) {
+bool make_map(CUtensorMap* m, float* ptr, long long rows, int kpad, long long pitch, int box_rows, int bk) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t gdim[2] = {(cuuint64_t)kpad, (cuuint64_t)rows};
     const cuuint64_t gstride[1] = {(cuuint64_t)pitch * 4};
-    const cuuint32_t box[2] = {(cuuint32_t)kBK, (cuuint32_t)box_rows};
+    const cuuint32_t box[2] = {(cuuint32_t)bk, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, ptr, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+              bk == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 int g_slab = 0;   // tt_debug_set("kd_slab"): parameters per slab (0 = default)
@@ -283,8 +291,9 @@ cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA
                          int lower_only, cudaStream_t s) {
     // slab: parameters per pass of the split + GEMM pair; its sums meet the earlier slabs' in fp64 in C
     long long ks_max = g_slab > 0 ? g_slab : 8192;
-    ks_max = (ks_max + kBK - 1) / kBK * kBK;
-    if (ks_max > Kdim) ks_max = (Kdim + kBK - 1) / kBK * kBK;
+    constexpr int bk = 32;
+    ks_max = (ks_max + kMaxBK - 1) / kMaxBK * kMaxBK;
+    if (ks_max > Kdim) ks_max = (Kdim + kMaxBK - 1) / kMaxBK * kMaxBK;
     const long long pitch = ks_max;                                     // floats; a multiple of 32
     const int tm_n = (int)((nA + kBM - 1) / kBM), tn_n = (int)((nB + kBN - 1) / kBN);
     const long long n_tiles_ll = kd_tile_order(nullptr, tm_n, tn_n, lower_only);
@@ -302,22 +311,23 @@ cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA
     float *a_hi = scratch, *a_lo = scratch + plane_a, *b_hi = scratch + 2 * plane_a, *b_lo = b_hi + plane_b;
 
     CUtensorMap mA_hi, mA_lo, mB_hi, mB_lo;
-    if (!(make_map(&mA_hi, a_hi, nA, (int)ks_max, pitch, kBM) && make_map(&mA_lo, a_lo, nA, (int)ks_max, pitch, kBM) &&
-                              make_map(&mB_hi, b_hi, nB, (int)ks_max, pitch, kBN) && make_map(&mB_lo, b_lo, nB, (int)ks_max, pitch, kBN)))
+    if (!(make_map(&mA_hi, a_hi, nA, (int)ks_max, pitch, kBM, bk) && make_map(&mA_lo, a_lo, nA, (int)ks_max, pitch, kBM, bk) &&
+          make_map(&mB_hi, b_hi, nB, (int)ks_max, pitch, kBN, bk) && make_map(&mB_lo, b_lo, nB, (int)ks_max, pitch, kBN, bk)))
         e = cudaErrorInvalidValue;
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(kd_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+    constexpr int smem = Geo<bk>::kSmemBytes;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kd_umma_kernel<bk>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     int dev = 0, sms = 148;
     if (e == cudaSuccess) e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int grid = n_tiles < sms ? n_tiles : sms;
     for (long long k0 = 0; e == cudaSuccess && k0 < Kdim; k0 += ks_max) {
         const int ks = (int)(Kdim - k0 < ks_max ? Kdim - k0 : ks_max);
-        const int kpad = (ks + kBK - 1) / kBK * kBK;
+        const int kpad = (ks + kMaxBK - 1) / kMaxBK * kMaxBK;
         const dim3 ga((unsigned)((nA + 7) / 8), (unsigned)((kpad + 1023) / 1024)), gb((unsigned)((nB + 7) / 8), ga.y);
         kd_split_kernel<<<ga, 256, 0, s>>>(A, nA, Kdim, k0, ks, kpad, a_hi, a_lo, pitch);
         kd_split_kernel<<<gb, 256, 0, s>>>(B, nB, Kdim, k0, ks, kpad, b_hi, b_lo, pitch);
-        UmmaArgs g{d_tiles, n_tiles, kpad / kBK, C, nA, nB, ldc, k0 == 0 ? 1 : 0};
-        kd_umma_kernel<<<grid, kThreads, kSmemBytes, s>>>(mA_hi, mA_lo, mB_hi, mB_lo, g);
+        UmmaArgs g{d_tiles, n_tiles, kpad / bk, C, nA, nB, ldc, k0 == 0 ? 1 : 0};
+        kd_umma_kernel<bk><<<grid, kThreads, smem, s>>>(mA_hi, mA_lo, mB_hi, mB_lo, g);
         e = cudaGetLastError();
     }
     cudaFreeAsync(d_tiles, s);
