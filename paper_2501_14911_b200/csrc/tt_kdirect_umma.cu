@@ -51,7 +51,9 @@ constexpr int kAccCols = kBN;                       // fp32 accumulator: one ten
 constexpr int kPanel = 8;                           // tile columns per panel of the tile order
 
 // hi / lo split of one slab: dst_hi/dst_lo[row][0..kpad) for src[row][k0 .. k0 + ks), zero beyond ks (kpad = ks rounded
-// up to the K-block).  One warp per (row, 1024-parameter segment): lanes read consecutive parameters.
+// up to the K-block).  One warp per (row, 1024-parameter segment); a lane owns four consecutive parameters: four scalar
+// loads (the rows of a block column have no alignment; the warp's four load instructions share their cache lines) and one
+// 16-byte store per output (the scratch rows are 128-byte aligned).
 __global__ void __launch_bounds__(256)
 kd_split_kernel(const float* __restrict__ src, const long long rows, const long long ld, const long long k0, const int ks,
                 const int kpad, float* __restrict__ dst_hi, float* __restrict__ dst_lo, const long long pitch) {
@@ -62,14 +64,17 @@ kd_split_kernel(const float* __restrict__ src, const long long rows, const long 
     float* h = dst_hi + row * pitch;
     float* l = dst_lo + row * pitch;
     const int seg0 = blockIdx.y * 1024;
-#pragma unroll 4
-    for (int i = 0; i < 32; ++i) {
-        const int k = seg0 + i * 32 + lane;
-        if (k >= kpad) break;
-        const float a = k < ks ? __ldg(s + k) : 0.f;
-        const float hi = to_tf32(a);
-        h[k] = hi;
-        l[k] = to_tf32(a - hi);
+#pragma unroll 2
+    for (int i = 0; i < 8; ++i) {
+        const int k = seg0 + i * 128 + lane * 4;
+        if (k >= kpad) break;                      // kpad is a multiple of 32: a lane's four parameters are in or out together
+        float a[4], hi[4], lo[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) a[j] = k + j < ks ? __ldg(s + k + j) : 0.f;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { hi[j] = to_tf32(a[j]); lo[j] = to_tf32(a[j] - hi[j]); }
+        *reinterpret_cast<float4*>(h + k) = make_float4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<float4*>(l + k) = make_float4(lo[0], lo[1], lo[2], lo[3]);
     }
 }
 
