@@ -73,11 +73,9 @@ def lib() -> ctypes.CDLL:
         "tt_normal_host": (ci, [vp, vp, vp, vp]),
         "tt_plan_set_profiling": (ci, [vp, ci]),
         "tt_plan_stage_ms": (ci, [vp, ci, ctypes.POINTER(ctypes.c_float), ci]),
-        "tt_probe_stream_read": (ci, [vp, sz, vp, vp]),
         "tt_debug_fft_tables": (ci, [i64, ci, ctypes.POINTER(ci), ctypes.POINTER(ci),
                                      ctypes.POINTER(ctypes.c_ushort), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_spectrum_view": (ci, [vp, pp, ctypes.POINTER(i64)]),
-        "tt_probe_dmma": (ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]),
         "tt_debug_trig": (ci, [i64, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
         "tt_debug_set": (ci, [ctypes.c_char_p, ci]),
         "tt_chol_create": (ci, [pp, i64, vp, i64, vp]),
@@ -111,12 +109,30 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_coarse", "tt_plan_destroy", "tt_plan_device_bytes",
            "tt_plan_last_cuda_error", "tt_plan_get_spectrum", "tt_plan_describe", "tt_matvec", "tt_rmatvec", "tt_normal",
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_normal_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
-           "tt_plan_set_profiling", "tt_plan_stage_ms", "tt_probe_stream_read", "tt_probe_dmma", "tt_debug_spectrum_view", "tt_debug_fft_tables",
-           "tt_debug_trig", "tt_debug_set",
+           "tt_plan_set_profiling", "tt_plan_stage_ms",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
            "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_K_add_noise", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
            "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
            "tt_postcov_q_apply", "tt_d2q_apply"]
+
+
+# developer hooks (include/tt_dev.h: exported by libtt.so, not part of the product ABI) and the probe library (include/tt_probe.h)
+DEV_EXPORTS = ["tt_debug_spectrum_view", "tt_debug_fft_tables", "tt_debug_trig", "tt_debug_set"]
+PROBE_EXPORTS = ["tt_probe_stream_read", "tt_probe_dmma"]
+_probe = None
+
+
+def probe_lib() -> ctypes.CDLL:
+    """Loads paper_2501_14911_b200/libttprobe.so (built together with libtt.so)."""
+    global _probe
+    if _probe is None:
+        lib()
+        P = ctypes.CDLL(_build.PROBE_LIB)
+        vp, ci, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+        P.tt_probe_stream_read.restype, P.tt_probe_stream_read.argtypes = ci, [vp, sz, vp, vp]
+        P.tt_probe_dmma.restype, P.tt_probe_dmma.argtypes = ci, [ci, vp, ctypes.POINTER(ctypes.c_double), vp]
+        _probe = P
+    return _probe
 
 
 def _stream(stream) -> int:
@@ -236,7 +252,9 @@ def tt_plan_stage_ms(plan: int, op: int) -> tuple[float, float, float, int]:
 
 
 def tt_probe_stream_read(src, nbytes: int, sink, stream=None) -> None:
-    _check("tt_probe_stream_read", lib().tt_probe_stream_read(_ptr(src), nbytes, _ptr(sink), _stream(stream)))
+    st = probe_lib().tt_probe_stream_read(_ptr(src), nbytes, _ptr(sink), _stream(stream))
+    if st != 0:
+        raise RuntimeError(f"tt_probe_stream_read failed: {st}")
 
 
 class _CudaView:
@@ -258,7 +276,9 @@ def tt_debug_spectrum_view(plan: int, N_t: int, N_d: int, dtype) -> torch.Tensor
 def tt_probe_dmma(iters: int, sink, stream=None) -> float:
     """Enqueues the DMMA probe; returns the flop count of the launch."""
     fl = ctypes.c_double()
-    _check("tt_probe_dmma", lib().tt_probe_dmma(iters, _ptr(sink), ctypes.byref(fl), _stream(stream)))
+    st = probe_lib().tt_probe_dmma(iters, _ptr(sink), ctypes.byref(fl), _stream(stream))
+    if st != 0:
+        raise RuntimeError(f"tt_probe_dmma failed: {st}")
     return fl.value
 
 

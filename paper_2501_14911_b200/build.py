@@ -20,9 +20,11 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtt.so")
+PROBE_LIB = os.path.join(HERE, "libttprobe.so")     # include/tt_probe.h: bench.py's hardware probes, not part of libtt
 STAMP = os.path.join(BUILD, "libtt.stamp")
 
 SOURCES = ["tt_api.cu", "tt_fft.cu", "tt_gemv.cu", "tt_gemm.cu", "tt_gemm32.cu", "tt_trsv.cu", "tt_online.cu", "tt_kdirect.cu", "tt_kdirect_umma.cu"]
+PROBE_SOURCE = "tt_probe.cu"
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
@@ -42,7 +44,7 @@ def _nvcc() -> str:
 def _hash() -> str:
     h = hashlib.sha256()
     h.update(" ".join(NVCC_FLAGS).encode())
-    names = sorted(os.listdir(CSRC)) + ["../../include/tt.h"]
+    names = sorted(os.listdir(CSRC)) + ["../../include/tt.h", "../../include/tt_dev.h", "../../include/tt_probe.h"]
     for name in names:
         path = os.path.join(CSRC, name)
         if os.path.isfile(path):
@@ -54,7 +56,7 @@ def _hash() -> str:
 
 def is_current() -> bool:
     """True if libtt.so exists and its stamp carries the hash of the sources and flags in this tree."""
-    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
+    if not (os.path.exists(LIB) and os.path.exists(PROBE_LIB) and os.path.exists(STAMP)):
         return False
     with open(STAMP) as f:
         return f.read().strip() == _hash()
@@ -63,7 +65,7 @@ def is_current() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile and link libtt.so if needed; returns its path."""
     sig = _hash()
-    if not force and os.path.exists(LIB) and os.path.exists(STAMP):
+    if not force and os.path.exists(LIB) and os.path.exists(PROBE_LIB) and os.path.exists(STAMP):
         with open(STAMP) as f:
             if f.read().strip() == sig:
                 return LIB
@@ -82,14 +84,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(res.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(compile_one, SOURCES))
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc, "-shared", "-o", tmp, *objs, "-cudart", "shared"]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        raise RuntimeError(f"link failed:\n{res.stdout}\n{res.stderr}")
-    os.replace(tmp, LIB)
+    with ThreadPoolExecutor(max_workers=len(SOURCES) + 1) as ex:
+        objs = list(ex.map(compile_one, SOURCES + [PROBE_SOURCE]))
+    for lib, lib_objs in ((LIB, objs[:-1]), (PROBE_LIB, objs[-1:])):
+        tmp = lib + f".tmp{os.getpid()}"
+        cmd = [nvcc, "-shared", "-o", tmp, *lib_objs, "-cudart", "shared"]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError(f"link failed:\n{res.stdout}\n{res.stderr}")
+        os.replace(tmp, lib)
     with open(STAMP, "w") as f:
         f.write(sig)
     return LIB

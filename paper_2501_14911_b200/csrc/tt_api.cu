@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/tt.h"
+#include "../../include/tt_dev.h"
 #include "tt_internal.h"
 
 using namespace tt;
@@ -865,14 +866,6 @@ int tt_debug_spectrum_view(const tt_plan* p, void** ptr, int64_t* row_pitch) {
     return TT_OK;
 }
 
-int tt_probe_dmma(int iters, void* sink, double* flops, void* stream) {
-    if (!sink) return TT_ERR_NULL;
-    if (iters < 1) return TT_ERR_SHAPE;
-    cudaError_t e = probe_dmma_launch(iters, sink, flops, static_cast<cudaStream_t>(stream));
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
-    return TT_OK;
-}
-
 int tt_debug_trig(int64_t k, int64_t n, double* c, double* s) {
     if (!c || !s) return TT_ERR_NULL;
     if (n < 1) return TT_ERR_SHAPE;
@@ -907,14 +900,6 @@ int tt_debug_set(const char* key, int value) {
         return TT_OK;
     }
     return TT_ERR_SHAPE;
-}
-
-int tt_probe_stream_read(const void* src, size_t bytes, void* sink, void* stream) {
-    if (!src || !sink) return TT_ERR_NULL;
-    if (bytes % 16) return TT_ERR_SHAPE;
-    cudaError_t e = probe_stream_read_launch(src, bytes, sink, static_cast<cudaStream_t>(stream));
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
-    return TT_OK;
 }
 
 }  // extern "C"

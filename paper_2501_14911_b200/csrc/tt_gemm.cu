@@ -232,31 +232,6 @@ gemm_adj_kernel(const c128* __restrict__ Fhat, const c128* __restrict__ Dhat, c1
 }
 
 // ---------------------------------------------------------------------------------------
-// FP64 tensor-pipe probe (bench: the measured DMMA peak the k-RHS roofline is quoted against)
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) probe_dmma_kernel(double* __restrict__ sink, int iters) {
-    const double a = threadIdx.x * 1e-3, b = threadIdx.x * 2e-3;
-    double c[16][2];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) c[i][0] = c[i][1] = 0.0;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) dmma(c[i][0], c[i][1], a, b);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
-    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
-cudaError_t probe_dmma_launch(int iters, void* sink, double* flops, cudaStream_t s) {
-    const int grid = 148 * 8, block = 256;
-    probe_dmma_kernel<<<grid, block, 0, s>>>(static_cast<double*>(sink), iters);
-    if (flops) *flops = (double)grid * (block / 32) * (double)iters * 16.0 * 512.0;  // m8n8k4 = 512 flop
-    return cudaGetLastError();
-}
-
-// ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
 template <int NN>

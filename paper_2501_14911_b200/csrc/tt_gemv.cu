@@ -123,30 +123,6 @@ gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, 
 }
 
 // ---------------------------------------------------------------------------------------
-// read-only streaming probe (bench: measured read bandwidth next to the copy figure)
-// ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512) probe_read_kernel(const float4* __restrict__ src, size_t nvec,
-                                                         float4* __restrict__ sink) {
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; i + 7 * stride < nvec; i += 8 * stride) {
-        float4 f[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) f[u] = ldg_stream(src + i + u * stride);
-#pragma unroll
-        for (int u = 0; u < 8; ++u) { acc.x += f[u].x; acc.y += f[u].y; acc.z += f[u].z; acc.w += f[u].w; }
-    }
-    for (; i < nvec; i += stride) {
-        const float4 f = ldg_stream(src + i);
-        acc.x += f.x; acc.y += f.y; acc.z += f.z; acc.w += f.w;
-    }
-    // keep the loads alive: one (practically never taken) store per thread, one real store per CTA
-    if (acc.x == 1.2345678e-30f) sink[blockIdx.x] = acc;
-    if (threadIdx.x == 0) sink[blockIdx.x] = acc;
-}
-
-// ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
 static int g_fwd_warps = 0, g_adj_threads = 0;
@@ -213,12 +189,6 @@ cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* pa
 cudaError_t gemv_adj_launch(int dt, const void* Fhat, const void* dhat, void* xout, const GemvGeom& g,
                             cudaStream_t s) {
     return dt == 0 ? adj_dispatch<float>(Fhat, dhat, xout, g, s) : adj_dispatch<double>(Fhat, dhat, xout, g, s);
-}
-
-cudaError_t probe_stream_read_launch(const void* src, size_t bytes, void* sink, cudaStream_t s) {
-    probe_read_kernel<<<148 * 4, 512, 0, s>>>(static_cast<const float4*>(src), bytes / 16,
-                                              static_cast<float4*>(sink));
-    return cudaGetLastError();
 }
 
 }  // namespace tt

@@ -140,8 +140,5 @@ cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA
                          int lower_only, cudaStream_t s);
 void kd_umma_debug_set_slab(int ks);  // parameters accumulated in tensor memory between fp64 flushes (0 = default)
 
-// sink: >= 148*8*256 doubles
-cudaError_t probe_dmma_launch(int iters, void* sink, double* flops, cudaStream_t s);
-cudaError_t probe_stream_read_launch(const void* src, size_t bytes, void* sink, cudaStream_t s);
 
 }  // namespace tt

@@ -18,8 +18,8 @@ def tt():
     return binding
 
 
-def declared_symbols():
-    with open(os.path.join(ROOT, "include", "tt.h")) as f:
+def declared_symbols(header="tt.h"):
+    with open(os.path.join(ROOT, "include", header)) as f:
         src = re.sub(r"/\*.*?\*/", "", f.read(), flags=re.S)
     return sorted(set(re.findall(r"\b(tt_[A-Za-z_0-9]+)\s*\(", src)))
 
@@ -28,12 +28,23 @@ def test_library_exports_every_declared_symbol(tt):
     names = declared_symbols()
     assert "tt_plan_create" in names and "tt_matvec" in names and "tt_rmatvec" in names
     assert "tt_normal" in names and "tt_matvec_batched" in names and len(names) >= 18
+    assert not any(n.startswith(("tt_probe", "tt_debug")) for n in names)   # the product ABI carries no probes or tuning knobs
     L = tt.lib()
     for n in names:
         assert hasattr(L, n), f"libtt.so does not export {n}"
     assert sorted(tt.EXPORTS) == names        # the binding wraps exactly the declared calls
     for n in names:
         assert hasattr(tt, n)
+    # developer hooks (include/tt_dev.h, same library) and bench.py's probes (include/tt_probe.h, libttprobe.so)
+    dev = declared_symbols("tt_dev.h")
+    assert sorted(tt.DEV_EXPORTS) == dev
+    for n in dev:
+        assert hasattr(L, n) and hasattr(tt, n)
+    probes = declared_symbols("tt_probe.h")
+    assert sorted(tt.PROBE_EXPORTS) == probes
+    P = tt.probe_lib()
+    for n in probes:
+        assert hasattr(P, n) and hasattr(tt, n) and not hasattr(L, n)
 
 
 def test_version_and_status_strings(tt):

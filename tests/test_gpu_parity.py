@@ -191,21 +191,21 @@ def test_adjoint_identity_linearity_shift_on_gpu(tt, dtype):
         Fm = plan.matvec(mc).double()
         Ftd = plan.rmatvec(dc).double()
         lhs = float((Fm * dc.double()).sum()); rhs = float((mc.double() * Ftd).sum())
-        assert abs(lhs - rhs) <= 10 * tol * float(Fm.norm() * dc.double().norm())
+        assert abs(lhs - rhs) <= tol * float(Fm.norm() * dc.double().norm())
         # linearity
         m2 = synth.vector_m(w.scaled(seed=w.seed + 100), k_rhs=1).cuda()
         comb = plan.matvec((2.0 * mc - 3.0 * m2)).double()
         sep = 2.0 * Fm - 3.0 * plan.matvec(m2).double()
-        assert float((comb - sep).norm()) <= 10 * tol * float(sep.norm())
+        assert float((comb - sep).norm()) <= tol * float(sep.norm())
         # shift equivariance (block Toeplitz): delaying m by tau delays d by tau
         tau = 7
         ms = torch.zeros_like(mc); ms[tau:] = mc[:-tau]
         ds = plan.matvec(ms).double()
-        assert float((ds[tau:] - Fm[:-tau]).norm()) <= 10 * tol * float(Fm.norm())
-        assert float(ds[:tau].abs().max()) <= 10 * tol * float(Fm.abs().max())
+        assert float((ds[tau:] - Fm[:-tau]).norm()) <= tol * float(Fm.norm())
+        assert float(ds[:tau].abs().max()) <= tol * float(Fm.abs().max())
         # normal operator: <m, F^T F m> = |F m|^2
         n = plan.normal(mc).double()
-        assert abs(float((mc.double() * n).sum()) - float(Fm.norm() ** 2)) <= 10 * tol * float(Fm.norm() ** 2)
+        assert abs(float((mc.double() * n).sum()) - float(Fm.norm() ** 2)) <= tol * float(Fm.norm() ** 2)
     finally:
         plan.close()
 
@@ -389,4 +389,4 @@ def test_normal_batched(tt, dtype, layout):
     finally:
         plan.close()
     for r in range(k):
-        assert rel(got[..., r], ob.rmatvec(F.numpy(), ob.matvec(F.numpy(), M[..., r].contiguous().numpy()))) <= 2 * TOL[dtype]
+        assert rel(got[..., r], ob.rmatvec(F.numpy(), ob.matvec(F.numpy(), M[..., r].contiguous().numpy()))) <= TOL[dtype]
