@@ -85,10 +85,12 @@ def test_coarse_errors(tt):
         assert ei.value.status == -2  # TT_ERR_SHAPE
 
 
-def test_p2q_full_size_sampled(tt):
+def test_p2q_full_size_whole_vector(tt):
     """The paper's p2q shape (N_q = 16, N_m = 263169, N_t = 500, N_t^q = 50), in the launch
-    configuration bench.py --config Q5 times: whole coarse series of single QoIs, and whole fine series of parameter
-    ranges of the transpose, against the blocked oracle on slices of the block column."""
+    configuration bench.py --config Q5 times: q = S F_q m over all 800 QoIs and m' = F_q^T S^T q over all 131 584 500
+    parameters against the blocked oracle (reading R19: fine-grid result sampled at the end of every r-th step; exact
+    transpose with zeros at the unsampled steps), the block column streamed to the host in sensor slabs."""
+    import time
     w = synth.CONFIGS["Q5"]
     free, _ = torch.cuda.mem_get_info()
     if free < 40 * (1 << 30):
@@ -100,17 +102,25 @@ def test_p2q_full_size_sampled(tt):
     plan = tt.Plan(F, out_every=r)
     try:
         got_q, got_m = plan.matvec(m), plan.rmatvec(q)
-        mh, qh = m.cpu().numpy(), q.cpu().numpy()
-        for s in (0, 7, 15):
-            ref = ob.matvec(F[:, s:s + 1, :].contiguous().cpu().numpy(), mh)[r - 1::r]
-            assert rel(got_q[:, s].cpu().numpy(), ref[:, 0]) <= 1e-5
-        zq = np.zeros((w.N_t, w.N_d), dtype=np.float32)
-        zq[r - 1::r] = qh                                           # S^T q
-        for p0 in (0, 131072, w.N_m - 64):
-            ref = ob.rmatvec(F[:, :, p0:p0 + 64].contiguous().cpu().numpy(), zq)
-            assert rel(got_m[:, p0:p0 + 64].cpu().numpy(), ref) <= 1e-5
-        lhs = float((got_q.double() * q.double()).sum())
-        rhs = float((m.double() * got_m.double()).sum())
-        assert abs(lhs - rhs) <= 1e-5 * float(got_q.double().norm() * q.double().norm())
+        torch.cuda.synchronize()
     finally:
         plan.close()
+    lhs = float((got_q.double() * q.double()).sum())
+    rhs = float((m.double() * got_m.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * float(got_q.double().norm() * q.double().norm())
+    mh, qh = m.cpu().numpy(), q.cpu().numpy()
+    zq = np.zeros((w.N_t, w.N_d), dtype=np.float32)
+    zq[r - 1::r] = qh                                               # S^T q
+    ref_q = np.empty((w.N_t // r, w.N_d))
+    ref_m = np.zeros((w.N_t, w.N_m))
+    t0 = time.perf_counter()
+    for s0 in range(0, w.N_d, 4):
+        slab = F[:, s0:s0 + 4, :].contiguous().cpu().numpy()
+        ref_q[:, s0:s0 + 4] = ob.matvec(slab, mh)[r - 1::r]         # S (F m)
+        ref_m += ob.rmatvec(slab, np.ascontiguousarray(zq[:, s0:s0 + 4]))
+    e_q, e_m = rel(got_q.cpu().numpy(), ref_q), rel(got_m.cpu().numpy(), ref_m)
+    print(f"Q5 whole-vector rel-L2 vs the oracle (oracle {time.perf_counter() - t0:.0f} s): S F_q m {e_q:.2e}  F_q^T S^T q {e_m:.2e} (tol 1e-05)")
+    assert e_q <= 1e-5 and e_m <= 1e-5
+    gm = got_m.cpu().numpy()
+    for p0 in range(0, w.N_m, 8192):
+        assert rel(gm[:, p0:p0 + 8192], ref_m[:, p0:p0 + 8192]) <= 1e-5, f"parameters {p0}.."

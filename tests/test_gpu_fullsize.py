@@ -230,13 +230,14 @@ def test_online_medium_true_K(tt):
         assert rel(m_paper, m_ref) <= TOL[dtype] + 8 * u * kappa
 
 
-def test_online_p5_full_size_sampled(tt):
+def test_online_p5_full_size_whole_vector(tt):
     """The paper's own shape (N_d=49, N_m=263169, N_t=500: 131 584 500 parameters, 24 500 data), in the launch
     configuration `bench.py --config P5 --online` times: the K-solve against the oracle over the whole vector, and
-    m_map = G* K^{-1} d_obs (gain form) on sampled outputs the oracle computes one by one from single columns
-    G[:, :, p] of the block column.  The factor is the seeded stand-in the bench uses."""
+    m_map = G* K^{-1} d_obs (gain form, eq 4.13 by reading R16) over ALL 131 584 500 parameters against the oracle's
+    G* z = rmatvec(G, z), the block column of G* streamed to the host in sensor slabs.  The factor is the seeded
+    stand-in the tests use at this order."""
+    import time
     from oracle import online_plain as oo
-    from oracle import toeplitz_plain as op
     w = synth.CONFIGS["P5"]
     need_memory(120)
     n = w.N_d * w.N_t
@@ -258,24 +259,28 @@ def test_online_p5_full_size_sampled(tt):
     del L_h
     G = synth.block_column(w, device="cuda")
     synth.scaled_block_column(w, G, out=G)
-    rng = np.random.default_rng(5)
-    ps = sorted(set(int(p) for p in rng.integers(0, w.N_m, 12)) | {0, w.N_m - 1})
-    cols = {p: G[:, :, p:p + 1].cpu().numpy() for p in ps}
     pG = tt.Plan(G)
-    del G
-    torch.cuda.empty_cache()
     mp = tt.MapInference(None, pG, chol, synth.noise_var(w, device="cuda"))
     try:
         m_map = mp.infer(d_obs, tt.TT_MAP_GAIN)
-        got = {p: m_map[:, p].cpu().numpy() for p in ps}
-        scale = float(m_map.double().pow(2).mean().sqrt())
+        got = m_map.cpu().numpy()
     finally:
         mp.close(); pG.close(); chol.close()
+    del m_map
+    torch.cuda.empty_cache()
     zr = z_ref.reshape(w.N_t, w.N_d)
-    for p in ps:
-        ref = np.array([op.rmatvec_entry(cols[p], zr, j, 0) for j in range(0, w.N_t, 7)])
-        err = np.linalg.norm(got[p][::7] - ref) / max(np.linalg.norm(ref), 1e-3 * scale * np.sqrt(len(ref)))
-        assert err <= 1e-5, (p, err)
+    ref = np.zeros((w.N_t, w.N_m))
+    t0 = time.perf_counter()
+    for s0 in range(0, w.N_d, 4):
+        s1 = min(w.N_d, s0 + 4)
+        slab = G[:, s0:s1, :].contiguous().cpu().numpy()
+        ref += ob.rmatvec(slab.astype(np.float64), np.ascontiguousarray(zr[:, s0:s1]))
+        del slab
+    err = rel(got, ref)
+    print(f"P5 online, gain form, whole m_map ({w.N_t * w.N_m} parameters) rel-L2 vs the oracle (oracle {time.perf_counter() - t0:.0f} s): {err:.2e} (tol 1e-05)")
+    assert err <= 1e-5
+    for p0 in range(0, w.N_m, 8192):
+        assert rel(got[:, p0:p0 + 8192], ref[:, p0:p0 + 8192]) <= 1e-5, f"parameters {p0}.."
 
 
 def test_K_assembly_p5_full_size_sampled(tt):
