@@ -241,6 +241,25 @@ def config_dict(w, args, cfg_name=None):
             "l2": "inputs larger than L2 (Fhat streamed once per op; no flush needed)"}
 
 
+def kd_roofline(w, n, seconds, peaks):
+    """tt_assemble_K_direct is a dense contraction: bound "tensor".  fp32 block columns run on tcgen05 kind::tf32 with three MMAs
+    per product (hi/lo split), so the tensor work is 3 x the algorithmic flops; the tf32 peak is the measured bf16 figure of
+    MEASURED_PEAKS.json x the guide's nominal tf32/bf16 ratio (1.1 / 2.25 PFLOP/s) - the sustained one: the call runs ~0.8 s under
+    the power cap."""
+    flops = float(n) * (n + 1) * w.N_m                 # lower triangle incl. diagonal, 2 flop per multiply-add
+    if w.dtype != torch.float32:
+        return {"bound": "tensor", "kernel": "kd_gemm_dmma_kernel (mma.sync m8n8k4 f64)", "achieved": flops / seconds * 1e-12,
+                "unit": "TFLOP/s", "peak": None, "frac": None, "peak_kind": "FP64 DMMA: see the C4 leg of the default run (tt_probe_dmma)"}
+    bf16 = peaks.get("bf16_tflops_sustained") or peaks.get("bf16_tflops")
+    peak = bf16 * (1.1 / 2.25) if bf16 else None
+    ach = 3.0 * flops / seconds * 1e-12
+    return {"bound": "tensor", "kernel": "kd_umma_kernel (tcgen05.mma kind::tf32, 3 MMAs per fp32 product)", "achieved": ach,
+            "unit": "TFLOP/s", "peak": peak, "frac": ach / peak if peak else None, "effective_fp32_TFLOPs": flops / seconds * 1e-12,
+            "peak_kind": "MEASURED_PEAKS.json bf16_tflops_sustained x nominal tf32/bf16 ratio 1.1/2.25" if bf16 else "no measured peak",
+            "tensor_flops_per_call": 3.0 * flops, "traffic": None,
+            "ncu": "profiles/r2_kdirect_ncu_full.md: tensor pipe active 73.6 % of the cycles at N_m x 0.02"}
+
+
 ONLINE_METRIC = "ms per online MAP inference, eq (4.13): m_map from d_obs (G*, F, K-solve, G*)"
 
 
@@ -506,8 +525,7 @@ def run_online(args, w):
                               "(lower triangle) + running sums down the block diagonals + mirror; no matvecs",
                               "multiply_adds": n * (n + 1) // 2 * w.N_m,
                               "TFLOPs": n * (n + 1) * w.N_m / s_direct * 1e-12,
-                              "peak_TFLOPs": 148 * (128 if w.dtype == torch.float32 else 64) * 2 * (clocks.summary().get("sm_mhz") or 1965.0) * 1e-6,
-                              "peak_kind": "148 SMs x 128 FP32 (64 FP64) FMA lanes x 2 flop x the SM clock sampled in this run",
+                              "roofline": kd_roofline(w, n, s_direct, peaks),
                               "upper_equals_lower_transposed": kd_sym,
                               "rel_diff_vs_column_by_column": direct_vs_cols,
                               "paper_timing_context": "PAPER.md:407: 24 500 x 0.022 s ~ 9 min on 24 A100 (column by column)"},
