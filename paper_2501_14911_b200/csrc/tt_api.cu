@@ -20,7 +20,8 @@ namespace {
 constexpr int kVersion = 100;  // 0.1.0
 constexpr int kRing = 64;       // profiled apply calls remembered
 constexpr int kSlotEvents = 8;  // two kernel triples (tt_normal) x 4 marks
-constexpr int kHostChunks = 8;  // parameter ranges of the pipelined *_host calls
+constexpr int kMaxHostChunks = 32;  // most parameter ranges the pipelined *_host calls can use
+int g_host_chunks = 16;             // ranges in use (tt_debug_set("host_chunks"))
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
 int g_gemv_chunk = 0;  // tt_debug_set("gemv_chunk"): 0 = planner's choice
@@ -48,7 +49,7 @@ struct tt_plan {
     void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
     void* d_stage = nullptr;
     cudaStream_t copy_stream = nullptr;   // *_host calls: the PCIe copies of the parameter-sized vector run here, chunk by
-    cudaEvent_t cev[kHostChunks + 2] = {};  // chunk over ranges of the parameter axis, overlapped with the kernels (lazily created)
+    cudaEvent_t cev[kMaxHostChunks + 2] = {};  // chunk over ranges of the parameter axis, overlapped with the kernels (lazily created)
     int chunk = 0, n_chunks = 0, fwd_warps = 0;
     size_t bytes = 0;
     mutable int last_cuda = 0;
@@ -381,7 +382,7 @@ void host_chunk(const tt_plan* p, int c, long long* p0, long long* p1) {
     long long a = p->chunk, b = 512;
     while (b) { const long long t = a % b; a = b; b = t; }
     const long long unit = (long long)p->chunk / a * 512;
-    long long per = (p->ldp + kHostChunks - 1) / kHostChunks;
+    long long per = (p->ldp + g_host_chunks - 1) / g_host_chunks;
     per = (per + unit - 1) / unit * unit;
     *p0 = per * c < p->ldp ? per * c : p->ldp;
     *p1 = per * (c + 1) < p->ldp ? per * (c + 1) : p->ldp;
@@ -408,9 +409,9 @@ int run_matvec_from_host(const tt_plan* p, const void* m_host, void* d_dev, cuda
     const int t = f32 ? 0 : 1;
     const size_t es = esize(p->dtype);
     const VecView vm = view(p, p->N_m, p->N_t, 1, 0), vd = view(p, p->N_d, p->N_td, 1, 0);
-    TT_CUDA(p, cudaEventRecord(p->cev[kHostChunks], s));                 // the staging buffer is free once s gets here
-    TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[kHostChunks], 0));
-    for (int c = 0; c < kHostChunks; ++c) {
+    TT_CUDA(p, cudaEventRecord(p->cev[kMaxHostChunks], s));                 // the staging buffer is free once s gets here
+    TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[kMaxHostChunks], 0));
+    for (int c = 0; c < g_host_chunks; ++c) {
         long long p0, p1;
         host_chunk(p, c, &p0, &p1);
         if (p1 <= p0) continue;
@@ -451,7 +452,7 @@ int run_rmatvec_to_host(const tt_plan* p, const void* d_dev, void* m_host, cudaS
     P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
     TT_CUDA(p, fft_r2c_launch(t, t, t, d_dev, p->dhat, P, 1, s));
-    for (int c = 0; c < kHostChunks; ++c) {
+    for (int c = 0; c < g_host_chunks; ++c) {
         long long p0, p1;
         host_chunk(p, c, &p0, &p1);
         if (p1 <= p0) continue;
@@ -470,8 +471,8 @@ int run_rmatvec_to_host(const tt_plan* p, const void* d_dev, void* m_host, cudaS
         TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[c], 0));
         TT_CUDA(p, copy_m_range(p, m_host, p->m_stage, p0, p1, cudaMemcpyDeviceToHost, p->copy_stream));
     }
-    TT_CUDA(p, cudaEventRecord(p->cev[kHostChunks + 1], p->copy_stream));
-    TT_CUDA(p, cudaStreamWaitEvent(s, p->cev[kHostChunks + 1], 0));
+    TT_CUDA(p, cudaEventRecord(p->cev[kMaxHostChunks + 1], p->copy_stream));
+    TT_CUDA(p, cudaStreamWaitEvent(s, p->cev[kMaxHostChunks + 1], 0));
     return TT_OK;
 }
 
@@ -885,6 +886,11 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "fft_max_radix")) { g_fft_max_radix = value; return TT_OK; }
     if (!std::strcmp(key, "fft_no_static")) { fft_debug_no_static(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
+    if (!std::strcmp(key, "host_chunks")) {
+        if (value < 1 || value > kMaxHostChunks) return TT_ERR_SHAPE;
+        g_host_chunks = value;
+        return TT_OK;
+    }
     if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }

@@ -385,9 +385,9 @@ def test_apply_calls_are_cuda_graph_capturable(tt):
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("layout", [0, 1])
 def test_pipelined_host_calls_equal_device_calls(tt, dtype, layout):
-    """The *_host calls move the parameter-sized vector range by range (8 ranges of the parameter axis) on a copy stream
+    """The *_host calls move the parameter-sized vector range by range (16 ranges of the parameter axis) on a copy stream
     while the kernels of the neighbouring range run; the result must be bit-identical to the device-pointer calls.
-    N_m = 40007 gives five non-empty ranges with a ragged last one."""
+    N_m = 40007 gives ten non-empty ranges (4096 parameters each) with a ragged last one."""
     N_d, N_m, N_t, r = 3, 40007, 20, 2
     w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=dtype)
     F = synth.block_column(w)
