@@ -5,6 +5,8 @@ import os
 import subprocess
 import sys
 
+import pytest
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
@@ -39,3 +41,27 @@ def test_clock_sampler_summary():
               ["garbage"]]
     s = c.summary()
     assert s["sm_mhz"] == 1950.0 and s["sm_max_mhz"] == 1965.0 and s["reasons"] == ["sw_power_cap"] and s["samples"] == 3
+
+
+@pytest.mark.gpu
+def test_default_arm_line_is_reproducible_by_hand():
+    """bench.py on the GPU (configs[0], a few steps): one JSON line with the contract's keys, and a roofline object whose
+    numbers follow from each other the way DESIGN.md section 7 says (achieved = algorithmic bytes / kernel time, frac = achieved / peak)."""
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "C1", "--steps", "3", "--warmup", "3",
+                          "--no-library-baseline"], capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0, res.stderr[-2000:]
+    line = json.loads(res.stdout.strip().splitlines()[-1])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+                "dtype", "data", "config", "e2e", "gpu_launches", "clocks", "roofline", "cpu_baseline"):
+        assert key in line, key
+    assert line["config"]["workload"].startswith("C1") and line["higher_is_better"] is False and line["vs_baseline"] is None
+    rf = line["roofline"]
+    assert rf["bound"] == "hbm" and rf["unit"] == "GB/s"
+    assert abs(rf["achieved"] - rf["algorithmic_bytes_per_launch"] / (rf["ms_per_launch"] * 1e-3) / 1e9) <= 1e-6 * rf["achieved"]
+    assert abs(rf["frac"] - rf["achieved"] / rf["peak"]) <= 1e-9
+    w_bytes = 33 * 4 * 64 * 16 + (32 * 64 + 32 * 4) * 8          # |Fhat| (N_t + 1 frequencies, complex128) + |m| + |d|
+    assert rf["algorithmic_bytes_per_launch"] == w_bytes
+    assert line["gpu_launches"] == 7 * line["steps"]
+    assert line["e2e"]["h2d_bytes_per_step"] == (32 * 64 + 32 * 4) * 8
+    cb = line["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and "sample" in cb
