@@ -1041,6 +1041,9 @@ def measure(ctx, args, w, cfg_name, *, steps, warmup, headline):
         "library_baseline": libs,
         "plan": {"create_s": t_plan, "device_bytes": plan.device_bytes, "input_generation_s": t_gen},
     }
+    if shard:
+        out["exchange"] = {"collective": "NCCL all-reduce (sum) of d, N_d*N_t reals, once per F.m" if dist is not None else "none (single process)",
+                           "world_size": world, "bytes": d_out.numel() * es}
     plan.close()
     del m, d, d_out, m_out
     torch.cuda.empty_cache()
@@ -1126,7 +1129,9 @@ def main() -> int:
         raise SystemExit("bench.py needs a CUDA device: libtt has no CPU path")
     torch.cuda.set_device(local_rank)
     dist = None
-    if world > 1:
+    # one process per GPU under torchrun; a single rank launched by torchrun (RANK set, WORLD_SIZE = 1) with --parallel shard
+    # also brings NCCL up, so that the exchange step of the sharded path runs through the real collective on one GPU
+    if world > 1 or (args.parallel == "shard" and "RANK" in os.environ and "MASTER_ADDR" in os.environ):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 

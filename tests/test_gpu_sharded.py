@@ -128,3 +128,28 @@ def test_sharded_online_phase_equals_oracle(tt, dtype):
     assert rel(K, K_ref) <= TOL[dtype]
     assert rel(gain, m_ref) <= TOL[dtype] + 8 * 1.1e-16 * kappa
     assert rel(paper, m_ref) <= TOL[dtype] + 8 * u * kappa
+
+
+def test_bench_shard_branch_runs_nccl_on_one_gpu(tmp_path):
+    """bench.py --parallel shard as the driver launches it (torch.distributed.run, one rank per GPU) with ONE rank: NCCL comes
+    up, the all-reduce of d runs on the launching stream inside the timed step, and the step takes what the unsharded step
+    takes.  configs[1] (C2, 4.3 GB spectrum) keeps it short."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "1", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", "1", "--parallel", "shard", "--config", "C2",
+           "--steps", "5", "--warmup", "3", "--no-cpu-baseline", "--no-library-baseline"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=root)
+    assert res.returncode == 0, res.stderr[-3000:]
+    line = json.loads([l for l in res.stdout.strip().splitlines() if l.startswith("{")][-1])
+    assert line["scaling"] == "strong" and line["n_gpus"] == 1
+    assert line["exchange"]["collective"].startswith("NCCL") and line["exchange"]["world_size"] == 1
+    assert line["exchange"]["bytes"] == 256 * 64 * 8
+    assert 0.5 < line["ms_per_step"] < 5.0                      # C2: ~1.4 ms unsharded
