@@ -302,6 +302,30 @@ def test_outputs_stay_inside_their_buffers(tt):
             assert torch.isfinite(buf[4096:4096 + n]).all()
 
 
+def test_K_direct_fp32_slab_sums_meet_in_fp64(tt):
+    """The fp32 path of tt_assemble_K_direct walks the parameter axis in slabs (8192 parameters by default) whose sums meet in fp64 in K:
+    with the developer knob `kd_slab` the same call takes 1, 3 and 32 slabs (the last one ragged: N_m = 2021 is not a multiple of the
+    32-parameter K-block, and the rows of the block columns are not 16-byte aligned) - every variant within the bar of the oracle, and
+    close to each other (the slab boundaries only change where fp32 running sums are handed to fp64)."""
+    N_d, N_m, N_t = 6, 2021, 30
+    w = synth.CONFIGS["P5"].scaled(N_d=N_d, N_m=N_m, N_t=N_t, dtype=torch.float32)
+    F = synth.block_column(w)
+    G = gstar_column(w, F)
+    nv = synth.noise_var(w)
+    ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
+    got = {}
+    try:
+        for slab in (0, 704, 64):
+            tt.tt_debug_set("kd_slab", slab)
+            got[slab] = tt.assemble_K_direct(F.cuda(), G.cuda(), nv.cuda()).cpu().numpy()
+    finally:
+        tt.tt_debug_set("kd_slab", 0)
+    for slab, K in got.items():
+        assert rel(K, ref) <= 1e-5, (slab, rel(K, ref))
+        assert np.array_equal(K, K.T)
+    assert rel(got[64], got[0]) <= 2e-6 and rel(got[704], got[0]) <= 2e-6
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 def test_K_direct_stays_inside_its_matrix(tt, dtype):
     """tt_assemble_K_direct (fp32: the tcgen05 kernel, whose 128 x 256 tiles overhang a ragged n on both sides; fp64: DMMA)
