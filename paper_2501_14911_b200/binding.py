@@ -516,13 +516,26 @@ class Chol:
 
     __del__ = close
 
+    def _vec(self, t, what):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == self.n):
+            raise ValueError(f"{what}: expected a contiguous CUDA tensor of {self.n} x float64, got {tuple(t.shape)} {t.dtype} on {t.device}")
+        return t
+
+    def _out(self, stream):
+        if isinstance(stream, torch.cuda.Stream):
+            with torch.cuda.stream(stream):
+                return torch.empty(self.n, dtype=torch.float64, device="cuda")
+        return torch.empty(self.n, dtype=torch.float64, device="cuda")
+
     def solve(self, b, out=None, stream=None):
-        out = torch.empty(self.n, dtype=torch.float64, device="cuda") if out is None else out
+        self._vec(b, "b")
+        out = self._out(stream) if out is None else self._vec(out, "out")
         tt_chol_solve(self.handle, b, out, stream)
         return out
 
     def trsv(self, b, transposed=False, out=None, stream=None):
-        out = torch.empty(self.n, dtype=torch.float64, device="cuda") if out is None else out
+        self._vec(b, "b")
+        out = self._out(stream) if out is None else self._vec(out, "out")
         tt_chol_trsv(self.handle, transposed, b, out, stream)
         return out
 
