@@ -23,7 +23,7 @@ LIB = os.path.join(HERE, "libtt.so")
 PROBE_LIB = os.path.join(HERE, "libttprobe.so")     # include/tt_probe.h: bench.py's hardware probes, not part of libtt
 STAMP = os.path.join(BUILD, "libtt.stamp")
 
-SOURCES = ["tt_api.cu", "tt_fft.cu", "tt_gemv.cu", "tt_gemm.cu", "tt_gemm32.cu", "tt_trsv.cu", "tt_online.cu", "tt_kdirect.cu", "tt_kdirect_umma.cu"]
+SOURCES = ["tt_api.cu", "tt_fft.cu", "tt_gemv.cu", "tt_gemm.cu", "tt_gemm32.cu", "tt_gemm32_umma.cu", "tt_trsv.cu", "tt_online.cu", "tt_kdirect.cu", "tt_kdirect_umma.cu"]
 PROBE_SOURCE = "tt_probe.cu"
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -894,6 +894,7 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }
+    if (!std::strcmp(key, "gemm32_umma")) { gemm32_umma_debug_set(value); return TT_OK; }
     if (!std::strcmp(key, "gemm_adj_mt")) { gemm_debug_set_adj(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_fwd_warps")) {
         if (value < 0 || value > 32) return TT_ERR_SHAPE;

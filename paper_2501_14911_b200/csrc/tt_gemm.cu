@@ -270,7 +270,9 @@ static cudaError_t adj_launch_nn(const c128* F, const c128* D, c128* X, const Ge
 
 cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g,
                             cudaStream_t s) {
-    if (dt == 0) return gemm32_fwd_launch(Fhat, Xhat, partial, g, s);
+    if (dt == 0)
+        return gemm32_umma_fwd_ok(g) ? gemm32_umma_fwd_launch(Fhat, Xhat, partial, g, s)
+                                     : gemm32_fwd_launch(Fhat, Xhat, partial, g, s);
     const c128* F = static_cast<const c128*>(Fhat);
     const c128* X = static_cast<const c128*>(Xhat);
     c128* P = static_cast<c128*>(partial);

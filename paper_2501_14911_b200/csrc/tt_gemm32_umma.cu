@@ -1,0 +1,274 @@
+// tt_gemm32_umma.cu - the per-frequency complex64 GEMMs of TT_F32 plans with 32 right-hand sides on the 5th-generation
+// tensor cores (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423).
+//
+// forward   Dhat_w [N_d x k] = Fhat_w [N_d x N_m] * Xhat_w [N_m x k],  k = 32, as ONE real product per CTA tile
+//
+//     P [128 x 64] = A [128 x K] * B [K x 64],   K = parameters,
+//     A rows   = 64 sensors x {Re Fhat_w[s, .], Im Fhat_w[s, .]}   (de-interleaved by the transform warps -> tensor memory)
+//     B rows   = Xhat_w[p, .] exactly as it lies in memory: 32 complex = 64 floats (Re, Im interleaved), MN-major
+//     Dhat_w[s, r] = (P[s.re, 2r] - P[s.im, 2r+1]) + i (P[s.re, 2r+1] + P[s.im, 2r])      (combined in the epilogue)
+//
+// so that all 128 x 64 accumulators carry useful terms and neither operand is transposed.  fp32 accuracy comes from the
+// 3xTF32 split (x = hi + lo, both tf32; lo*hi + hi*lo + hi*hi, PAPER.md's fp32 runs need ~1e-6): Fhat is far too large
+// to split ahead of time, so both operands are split on the fly by transform warps between TMA and the MMA:
+//
+//   warp 0      TMA producer: Fhat_w tile (64 sensors x 32 parameters, 16 KB) and Xhat_w tile (32 x 64 floats, 8 KB) per stage
+//   warps 4-7   A transform: thread = tensor-memory lane = (sensor, re|im); reads its row from shared memory, splits, writes
+//               hi and lo into tensor memory (tcgen05.st) - the MMA takes A from tensor memory, which halves the shared-memory
+//               operand traffic that bounds small-N tcgen05 products
+//   warps 8-11  B transform: element-wise hi / lo of the raw tile into two tiles of the same (swizzled) layout
+//   warp 1      MMA issuer: 4 k-steps x 3 tcgen05.mma (M 128, N 64, K 8) per stage, accumulators in tensor memory
+//   warps 12-15 epilogue: tensor-core fp32 accumulation truncates, so the accumulator is drained every kChunkKB stages
+//               (two accumulators alternate) into fp32 register sums (round-to-nearest), as in tt_kdirect_umma.cu
+//   warp 2      tensor-memory allocation
+//
+// grid (p-splits, n_f, sensor tiles); the partial sums go through reduce_partials_kernel like those of the FMA kernel
+// (tt_gemm32.cu), which stays the path for k != 32.
+#include "tt_common.cuh"
+#include "tt_internal.h"
+#include "tt_umma.cuh"
+
+namespace tt {
+
+namespace {
+
+using namespace umma;
+
+constexpr int kSens = 64;                      // sensors per CTA tile (128 tensor-memory lanes)
+constexpr int kKB = 32;                        // parameters per pipeline stage
+constexpr int kN = 64;                         // floats per Xhat row = 2 k
+constexpr int kStages = 4;
+constexpr int kChunkKB = 2;                    // stages per accumulation chunk (64 parameters)
+constexpr int kRawA = kSens * kKB * 8;         // 16 KB: two TMA boxes of [64 rows][16 parameters = 128 B]
+constexpr int kRawB = kKB * kN * 4;            //  8 KB: raw [32 parameters][64 floats]; hi / lo [2 column halves][32][32 floats]
+constexpr int kStageBytes = kRawA + 3 * kRawB; // raw A, raw B, B hi, B lo
+constexpr int kFwdSmem = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+constexpr int kThreads = 512;
+constexpr int kColD = 0;                       // two accumulators of 64 columns
+constexpr int kColA = 128;                     // per stage: hi [32 columns], lo [32 columns]
+constexpr int kTmemCols = 512;
+
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
+                       c64* __restrict__ partial, const GemmGeom g, const int r0) {
+    extern __shared__ unsigned char smem_dyn[];
+    const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
+    const uint32_t bars = smem0 + kStages * kStageBytes;
+    auto bar_full = [&](int s) { return bars + 8u * s; };                   // TMA -> transforms
+    auto bar_ready = [&](int s) { return bars + 8u * (kStages + s); };      // transforms -> MMA
+    auto bar_free = [&](int s) { return bars + 8u * (2 * kStages + s); };   // MMA -> TMA
+    auto bar_tfull = [&](int b) { return bars + 8u * (3 * kStages + b); };  // MMA -> epilogue
+    auto bar_tempty = [&](int b) { return bars + 8u * (3 * kStages + 2 + b); };
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int c = blockIdx.x, w = blockIdx.y, s0 = blockIdx.z * kSens;
+    const long long p_lo = (long long)c * g.p_per_split;
+    long long p_hi = p_lo + g.p_per_split;
+    if (p_hi > g.N_m) p_hi = g.N_m;
+    const int n_kb = p_hi > p_lo ? (int)((p_hi - p_lo + kKB - 1) / kKB) : 0;
+    const int n_chunks = (n_kb + kChunkKB - 1) / kChunkKB;
+
+    if (tid == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_ready(s), 8);
+            mbar_init(bar_free(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_tfull(b), 1);
+            mbar_init(bar_tempty(b), 4);
+        }
+        mbar_fence_init();
+        tma_prefetch_desc(&mapF);
+        tma_prefetch_desc(&mapX);
+    }
+    if (warp == 2) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = tmem_base_s;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            for (int kb = 0; kb < n_kb; ++kb) {
+                const int st = kb % kStages;
+                mbar_wait(bar_free(st), ((kb / kStages) & 1) ^ 1);
+                const uint32_t base = smem0 + st * kStageBytes;
+                mbar_arrive_expect_tx(bar_full(st), kRawA + kRawB);
+                const long long p = p_lo + (long long)kb * kKB;
+                tma_load_3d(base, &mapF, bar_full(st), (int)(2 * p), s0, w);
+                tma_load_3d(base + kRawA / 2, &mapF, bar_full(st), (int)(2 * p + 32), s0, w);
+                tma_load_3d(base + kRawA, &mapX, bar_full(st), 2 * r0, (int)p, w);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            constexpr uint32_t idesc = idesc_tf32(128, kN, /*b_mn_major=*/1);
+            for (int kb = 0; kb < n_kb; ++kb) {
+                const int st = kb % kStages, chunk = kb / kChunkKB, buf = chunk & 1;
+                const bool first = kb % kChunkKB == 0;
+                if (first) {
+                    mbar_wait(bar_tempty(buf), ((chunk >> 1) & 1) ^ 1);
+                    tc_fence_after();
+                }
+                mbar_wait(bar_ready(st), (kb / kStages) & 1);
+                tc_fence_after();
+                const uint32_t d = tmem_base + kColD + buf * kN;
+                const uint32_t a_hi = tmem_base + kColA + st * 64, a_lo = a_hi + 32;
+                const uint32_t b_hi = smem0 + st * kStageBytes + kRawA + kRawB, b_lo = b_hi + kRawB;
+#pragma unroll
+                for (int ks = 0; ks < kKB / 8; ++ks) {
+                    const uint64_t dh = smem_desc_mnmajor_tf32(b_hi + ks * 1024, kKB * 128, 512);
+                    const uint64_t dl = smem_desc_mnmajor_tf32(b_lo + ks * 1024, kKB * 128, 512);
+                    mma_tf32_ts(d, a_lo + ks * 8, dh, idesc, (first && ks == 0) ? 0u : 1u);
+                    mma_tf32_ts(d, a_hi + ks * 8, dl, idesc, 1u);
+                    mma_tf32_ts(d, a_hi + ks * 8, dh, idesc, 1u);
+                }
+                tc_commit(bar_free(st));
+                if (kb % kChunkKB == kChunkKB - 1 || kb == n_kb - 1) tc_commit(bar_tfull(buf));
+            }
+        }
+    } else if (warp >= 4 && warp < 8) {
+        // A transform: lane l of quadrant q is tensor-memory lane 32 q + l = sensor 16 q + (l & 15), part l >> 4
+        const int q = warp & 3, row = 16 * q + (lane & 15), part = lane >> 4;
+        const uint32_t row_off = row * 128, sw = row & 7;
+        for (int kb = 0; kb < n_kb; ++kb) {
+            const int st = kb % kStages;
+            mbar_wait(bar_full(st), (kb / kStages) & 1);
+            const uint32_t base = smem0 + st * kStageBytes + row_off;
+            uint32_t hi[32], lo[32];
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int ch = 0; ch < 8; ++ch) {
+                    const float4 v = lds128(base + b * (kRawA / 2) + ((ch ^ sw) << 4));
+                    const float x0 = part ? v.y : v.x, x1 = part ? v.w : v.z;
+                    const float h0 = to_tf32(x0), h1 = to_tf32(x1);
+                    hi[16 * b + 2 * ch] = __float_as_uint(h0);
+                    hi[16 * b + 2 * ch + 1] = __float_as_uint(h1);
+                    lo[16 * b + 2 * ch] = __float_as_uint(to_tf32(x0 - h0));
+                    lo[16 * b + 2 * ch + 1] = __float_as_uint(to_tf32(x1 - h1));
+                }
+            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColA + st * 64;
+            tmem_st_32x32(ta, hi);
+            tmem_st_32x32(ta + 32, lo);
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_ready(st));
+        }
+    } else if (warp >= 8 && warp < 12) {
+        const int t = tid - 256;
+        for (int kb = 0; kb < n_kb; ++kb) {
+            const int st = kb % kStages;
+            mbar_wait(bar_full(st), (kb / kStages) & 1);
+            // raw 16-byte piece ci = 16 row + c16 (row = parameter, 256-byte rows) -> column half c16 / 8, row, piece c16 % 8
+            // of the operand layout, whose 32-byte pieces are XORed with row % 4
+            const uint32_t raw = smem0 + st * kStageBytes + kRawA + t * 16;
+            const uint32_t c16 = t & 15, row0 = t >> 4;
+#pragma unroll
+            for (int i = 0; i < kRawB / 16 / 128; ++i) {
+                const float4 v = lds128(raw + i * 2048);
+                const uint32_t row = row0 + 8 * i;
+                const uint32_t dst = smem0 + st * kStageBytes + kRawA + kRawB + (c16 >> 3) * (kKB * 128) + row * 128 +
+                                     ((((c16 & 7) >> 1) ^ (row & 3)) << 5) + ((c16 & 1) << 4);
+                float4 h, l;
+                h.x = to_tf32(v.x); h.y = to_tf32(v.y); h.z = to_tf32(v.z); h.w = to_tf32(v.w);
+                l.x = to_tf32(v.x - h.x); l.y = to_tf32(v.y - h.y); l.z = to_tf32(v.z - h.z); l.w = to_tf32(v.w - h.w);
+                sts128(dst, h);
+                sts128(dst + kRawB, l);
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_ready(st));
+        }
+    } else if (warp >= 12) {
+        const int q = warp & 3, part = lane >> 4;
+        float acc[kN];
+#pragma unroll
+        for (int j = 0; j < kN; ++j) acc[j] = 0.f;
+        for (int ch = 0; ch < n_chunks; ++ch) {
+            const int buf = ch & 1;
+            mbar_wait(bar_tfull(buf), (ch >> 1) & 1);
+            tc_fence_after();
+            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColD + buf * kN;
+#pragma unroll
+            for (int j = 0; j < kN / 16; ++j) {
+                uint32_t v[16];
+                tmem_ld_32x16(ta + 16 * j, v);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) acc[16 * j + i] += __uint_as_float(v[i]);
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_tempty(buf));
+        }
+        // lanes l and l ^ 16 hold the Re-row and the Im-row products of one sensor: the Re lane finishes columns 0..15,
+        // the Im lane columns 16..31
+        float a[32], b[32];
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+            const float send = part ? acc[j] : acc[32 + j];
+            const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
+            a[j] = part ? recv : acc[j];         // Re-row products of my 16 columns
+            b[j] = part ? acc[32 + j] : recv;    // Im-row products
+        }
+        const int s = s0 + 16 * q + (lane & 15);
+        if (s < g.N_d) {
+            float4* dst = reinterpret_cast<float4*>(partial + (((long long)w * g.split + c) * g.N_d + s) * g.k + r0 + 16 * part);
+#pragma unroll
+            for (int r = 0; r < 16; r += 2)
+                dst[r / 2] = make_float4(a[2 * r] - b[2 * r + 1], a[2 * r + 1] + b[2 * r], a[2 * r + 2] - b[2 * r + 3],
+                                         a[2 * r + 3] + b[2 * r + 2]);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
+}
+
+int g_enable = 1;   // tt_debug_set("gemm32_umma", 0): keep to the FMA kernels
+
+}  // namespace
+
+void gemm32_umma_debug_set(int v) { g_enable = v; }
+
+// The shapes the tensor-core path takes: 32-column groups (k a multiple of 32), Fhat rows 16-byte aligned (always).
+bool gemm32_umma_fwd_ok(const GemmGeom& g) { return g_enable && g.k > 0 && g.k % 32 == 0 && 2 * g.ldp < (1LL << 31); }
+
+cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g, cudaStream_t s) {
+    CUtensorMap mapF, mapX;
+    {   // Fhat as floats: [n_f][N_d][2 ldp]; box = 16 parameters x 64 sensors
+        const unsigned long long dims[3] = {(unsigned long long)(2 * g.ldp), (unsigned long long)g.N_d, (unsigned long long)g.n_f};
+        const unsigned long long strides[2] = {(unsigned long long)g.ldp * 8, (unsigned long long)g.N_d * g.ldp * 8};
+        const unsigned box[3] = {32, kSens, 1};
+        if (!make_tensor_map_f32(&mapF, Fhat, 3, dims, strides, box)) return cudaErrorInvalidValue;
+    }
+    {   // Xhat as floats: [n_f][N_m][2 k]; box = 64 floats x 32 parameters, rows as they lie in memory
+        const unsigned long long dims[3] = {(unsigned long long)(2 * g.k), (unsigned long long)g.N_m, (unsigned long long)g.n_f};
+        const unsigned long long strides[2] = {(unsigned long long)g.k * 8, (unsigned long long)g.ldx * 8};
+        const unsigned box[3] = {kN, kKB, 1};
+        if (!make_tensor_map_f32(&mapX, Xhat, 3, dims, strides, box, /*swizzle128=*/false)) return cudaErrorInvalidValue;
+    }
+    cudaError_t e = cudaFuncSetAttribute(gemm32_umma_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFwdSmem);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + kSens - 1) / kSens));
+    for (int r0 = 0; r0 < g.k; r0 += 32) {
+        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace tt
