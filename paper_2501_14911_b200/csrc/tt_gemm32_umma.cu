@@ -13,14 +13,13 @@
 // to split ahead of time, so both operands are split on the fly by transform warps between TMA and the MMA:
 //
 //   warp 0      TMA producer: Fhat_w tile (64 sensors x 32 parameters, 16 KB) and Xhat_w tile (32 x 64 floats, 8 KB) per stage
-//   warps 4-7   A transform: thread = tensor-memory lane = (sensor, re|im); reads its row from shared memory, splits, writes
+//   warps 4-11  A transform: thread = tensor-memory lane = (sensor, re|im); reads its row from shared memory, splits, writes
 //               hi and lo into tensor memory (tcgen05.st) - the MMA takes A from tensor memory, which halves the shared-memory
-//               operand traffic that bounds small-N tcgen05 products
-//   warps 8-11  B transform: element-wise hi / lo of the raw tile into two tiles of the same (swizzled) layout
-//   warp 1      MMA issuer: 4 k-steps x 3 tcgen05.mma (M 128, N 64, K 8) per stage, accumulators in tensor memory
+//               operand traffic that bounds small-N tcgen05 products.  Two warps per lane quadrant, alternating stages.
+//   warps 2-3   B transform: element-wise hi / lo of the raw tile into two tiles in the MN-major operand layout
+//   warp 1      tensor-memory allocation; MMA issuer: 4 k-steps x 3 tcgen05.mma (M 128, N 64, K 8) per stage
 //   warps 12-15 epilogue: tensor-core fp32 accumulation truncates, so the accumulator is drained every kChunkKB stages
 //               (two accumulators alternate) into fp32 register sums (round-to-nearest), as in tt_kdirect_umma.cu
-//   warp 2      tensor-memory allocation
 //
 // grid (p-splits, n_f, sensor tiles); the partial sums go through reduce_partials_kernel like those of the FMA kernel
 // (tt_gemm32.cu), which stays the path for k != 32.
@@ -37,12 +36,13 @@ using namespace umma;
 constexpr int kSens = 64;                      // sensors per CTA tile (128 tensor-memory lanes)
 constexpr int kKB = 32;                        // parameters per pipeline stage
 constexpr int kN = 64;                         // floats per Xhat row = 2 k
-constexpr int kStages = 4;
+constexpr int kRaw = 6;                        // ring of raw tiles: filled by TMA, released by the transforms
+constexpr int kOps = 4;                        // ring of operands (B hi / lo in shared, A hi / lo in tensor memory): -> MMA
 constexpr int kChunkKB = 2;                    // stages per accumulation chunk (64 parameters)
 constexpr int kRawA = kSens * kKB * 8;         // 16 KB: two TMA boxes of [64 rows][16 parameters = 128 B]
 constexpr int kRawB = kKB * kN * 4;            //  8 KB: raw [32 parameters][64 floats]; hi / lo [2 column halves][32][32 floats]
-constexpr int kStageBytes = kRawA + 3 * kRawB; // raw A, raw B, B hi, B lo
-constexpr int kFwdSmem = kStages * kStageBytes + 1024 /* alignment slack */ + 256 /* barriers */;
+constexpr int kRawBytes = kRawA + kRawB, kOpBytes = 2 * kRawB;
+constexpr int kFwdSmem = kRaw * kRawBytes + kOps * kOpBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 constexpr int kThreads = 512;
 constexpr int kColD = 0;                       // two accumulators of 64 columns
 constexpr int kColA = 128;                     // per stage: hi [32 columns], lo [32 columns]
@@ -53,21 +53,31 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
-    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// x = hi + lo with hi = x rounded to tf32 (nearest, ties away: the bit pattern plus half a tf32 ulp, low 13 bits cleared -
+// what cvt.rna.tf32.f32 computes, in two integer operations instead of the five the conversion expands to) and lo = the
+// exact remainder cut to tf32 (its dropped bits are below 2^-21 |x|, the size of the lo*lo term 3xTF32 leaves out anyway)
+__device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
+    hi = (__float_as_uint(x) + 0x1000u) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi)) & 0xffffe000u;
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
 gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
-                       c64* __restrict__ partial, const GemmGeom g, const int r0) {
+                       c64* __restrict__ partial, const GemmGeom g, const int r0, const int mode) {
     extern __shared__ unsigned char smem_dyn[];
     const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
-    const uint32_t bars = smem0 + kStages * kStageBytes;
-    auto bar_full = [&](int s) { return bars + 8u * s; };                   // TMA -> transforms
-    auto bar_ready = [&](int s) { return bars + 8u * (kStages + s); };      // transforms -> MMA
-    auto bar_free = [&](int s) { return bars + 8u * (2 * kStages + s); };   // MMA -> TMA
-    auto bar_tfull = [&](int b) { return bars + 8u * (3 * kStages + b); };  // MMA -> epilogue
-    auto bar_tempty = [&](int b) { return bars + 8u * (3 * kStages + 2 + b); };
+    const uint32_t ops0 = smem0 + kRaw * kRawBytes;
+    const uint32_t bars = ops0 + kOps * kOpBytes;
+    auto bar_full = [&](int s) { return bars + 8u * s; };                        // TMA -> transforms (raw tile landed)
+    auto bar_rfree = [&](int s) { return bars + 8u * (kRaw + s); };              // transforms -> TMA (raw tile read)
+    auto bar_ready = [&](int s) { return bars + 8u * (2 * kRaw + s); };          // transforms -> MMA (operands written)
+    auto bar_free = [&](int s) { return bars + 8u * (2 * kRaw + kOps + s); };    // MMA -> transforms (operands consumed)
+    auto bar_tfull = [&](int b) { return bars + 8u * (2 * kRaw + 2 * kOps + b); };   // MMA -> epilogue
+    auto bar_tempty = [&](int b) { return bars + 8u * (2 * kRaw + 2 * kOps + 2 + b); };
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -79,9 +89,12 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
     const int n_chunks = (n_kb + kChunkKB - 1) / kChunkKB;
 
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) {
+        for (int s = 0; s < kRaw; ++s) {
             mbar_init(bar_full(s), 1);
-            mbar_init(bar_ready(s), 8);
+            mbar_init(bar_rfree(s), 6);   // 4 A-transform warps (one per lane quadrant) + 2 B-transform warps
+        }
+        for (int s = 0; s < kOps; ++s) {
+            mbar_init(bar_ready(s), 6);
             mbar_init(bar_free(s), 1);
         }
         for (int b = 0; b < 2; ++b) {
@@ -92,18 +105,18 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
         tma_prefetch_desc(&mapF);
         tma_prefetch_desc(&mapX);
     }
-    if (warp == 2) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
+    if (warp == 1) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = tmem_base_s;
 
     if (warp == 0) {
-        if (lane == 0) {
+        if (elect_one()) {
             for (int kb = 0; kb < n_kb; ++kb) {
-                const int st = kb % kStages;
-                mbar_wait(bar_free(st), ((kb / kStages) & 1) ^ 1);
-                const uint32_t base = smem0 + st * kStageBytes;
+                const int st = kb % kRaw;
+                mbar_wait(bar_rfree(st), ((kb / kRaw) & 1) ^ 1);
+                const uint32_t base = smem0 + st * kRawBytes;
                 mbar_arrive_expect_tx(bar_full(st), kRawA + kRawB);
                 const long long p = p_lo + (long long)kb * kKB;
                 tma_load_3d(base, &mapF, bar_full(st), (int)(2 * p), s0, w);
@@ -112,20 +125,21 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
+        if (elect_one()) {
             constexpr uint32_t idesc = idesc_tf32(128, kN, /*b_mn_major=*/1);
             for (int kb = 0; kb < n_kb; ++kb) {
-                const int st = kb % kStages, chunk = kb / kChunkKB, buf = chunk & 1;
+                const int st = kb % kOps, chunk = kb / kChunkKB, buf = chunk & 1;
                 const bool first = kb % kChunkKB == 0;
                 if (first) {
                     mbar_wait(bar_tempty(buf), ((chunk >> 1) & 1) ^ 1);
                     tc_fence_after();
                 }
-                mbar_wait(bar_ready(st), (kb / kStages) & 1);
+                mbar_wait(bar_ready(st), (kb / kOps) & 1);
                 tc_fence_after();
                 const uint32_t d = tmem_base + kColD + buf * kN;
                 const uint32_t a_hi = tmem_base + kColA + st * 64, a_lo = a_hi + 32;
-                const uint32_t b_hi = smem0 + st * kStageBytes + kRawA + kRawB, b_lo = b_hi + kRawB;
+                const uint32_t b_hi = ops0 + st * kOpBytes, b_lo = b_hi + kRawB;
+                if (!(mode & 4))
 #pragma unroll
                 for (int ks = 0; ks < kKB / 8; ++ks) {
                     const uint64_t dh = smem_desc_mnmajor_tf32(b_hi + ks * 1024, kKB * 128, 512);
@@ -138,59 +152,72 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                 if (kb % kChunkKB == kChunkKB - 1 || kb == n_kb - 1) tc_commit(bar_tfull(buf));
             }
         }
-    } else if (warp >= 4 && warp < 8) {
-        // A transform: lane l of quadrant q is tensor-memory lane 32 q + l = sensor 16 q + (l & 15), part l >> 4
+    } else if (warp >= 4 && warp < 12) {
+        // A transform: lane l of quadrant q is tensor-memory lane 32 q + l = sensor 16 q + (l & 15), part l >> 4; two warps
+        // per quadrant take the stages in turn
         const int q = warp & 3, row = 16 * q + (lane & 15), part = lane >> 4;
         const uint32_t row_off = row * 128, sw = row & 7;
-        for (int kb = 0; kb < n_kb; ++kb) {
-            const int st = kb % kStages;
-            mbar_wait(bar_full(st), (kb / kStages) & 1);
-            const uint32_t base = smem0 + st * kStageBytes + row_off;
+        for (int kb = (warp - 4) >> 2; kb < n_kb; kb += 2) {
+            const int rs = kb % kRaw, st = kb % kOps;
+            mbar_wait(bar_full(rs), (kb / kRaw) & 1);
+            const uint32_t base = smem0 + rs * kRawBytes + row_off;
             uint32_t hi[32], lo[32];
+            if (mode & 1) {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) hi[j] = lo[j] = 0;
+            } else
 #pragma unroll
             for (int b = 0; b < 2; ++b)
 #pragma unroll
                 for (int ch = 0; ch < 8; ++ch) {
                     const float4 v = lds128(base + b * (kRawA / 2) + ((ch ^ sw) << 4));
-                    const float x0 = part ? v.y : v.x, x1 = part ? v.w : v.z;
-                    const float h0 = to_tf32(x0), h1 = to_tf32(x1);
-                    hi[16 * b + 2 * ch] = __float_as_uint(h0);
-                    hi[16 * b + 2 * ch + 1] = __float_as_uint(h1);
-                    lo[16 * b + 2 * ch] = __float_as_uint(to_tf32(x0 - h0));
-                    lo[16 * b + 2 * ch + 1] = __float_as_uint(to_tf32(x1 - h1));
+                    split_tf32(part ? v.y : v.x, hi[16 * b + 2 * ch], lo[16 * b + 2 * ch]);
+                    split_tf32(part ? v.w : v.z, hi[16 * b + 2 * ch + 1], lo[16 * b + 2 * ch + 1]);
                 }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_rfree(rs));
+            mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
+            tc_fence_after();
             const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColA + st * 64;
+            if (!(mode & 1)) {
             tmem_st_32x32(ta, hi);
             tmem_st_32x32(ta + 32, lo);
             tmem_st_wait();
+            }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_ready(st));
         }
-    } else if (warp >= 8 && warp < 12) {
-        const int t = tid - 256;
+    } else if (warp == 2 || warp == 3) {
+        const int t = tid - 64;
         for (int kb = 0; kb < n_kb; ++kb) {
-            const int st = kb % kStages;
-            mbar_wait(bar_full(st), (kb / kStages) & 1);
+            const int rs = kb % kRaw, st = kb % kOps;
+            mbar_wait(bar_full(rs), (kb / kRaw) & 1);
             // raw 16-byte piece ci = 16 row + c16 (row = parameter, 256-byte rows) -> column half c16 / 8, row, piece c16 % 8
             // of the operand layout, whose 32-byte pieces are XORed with row % 4
-            const uint32_t raw = smem0 + st * kStageBytes + kRawA + t * 16;
+            const uint32_t raw = smem0 + rs * kRawBytes + kRawA + t * 16;
             const uint32_t c16 = t & 15, row0 = t >> 4;
+            constexpr int kPieces = kRawB / 16 / 64;
+            float4 v[kPieces];
 #pragma unroll
-            for (int i = 0; i < kRawB / 16 / 128; ++i) {
-                const float4 v = lds128(raw + i * 2048);
-                const uint32_t row = row0 + 8 * i;
-                const uint32_t dst = smem0 + st * kStageBytes + kRawA + kRawB + (c16 >> 3) * (kKB * 128) + row * 128 +
-                                     ((((c16 & 7) >> 1) ^ (row & 3)) << 5) + ((c16 & 1) << 4);
-                float4 h, l;
-                h.x = to_tf32(v.x); h.y = to_tf32(v.y); h.z = to_tf32(v.z); h.w = to_tf32(v.w);
-                l.x = to_tf32(v.x - h.x); l.y = to_tf32(v.y - h.y); l.z = to_tf32(v.z - h.z); l.w = to_tf32(v.w - h.w);
-                sts128(dst, h);
-                sts128(dst + kRawB, l);
+            for (int i = 0; i < kPieces; ++i) v[i] = lds128(raw + i * 1024);     // all loads in flight before the first use
+            mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
+            const uint32_t dst0 = ops0 + st * kOpBytes + (c16 >> 3) * (kKB * 128) + row0 * 128 +
+                                  ((((c16 & 7) >> 1) ^ (row0 & 3)) << 5) + ((c16 & 1) << 4);   // (row0 + 4 i) % 4 == row0 % 4
+            if (!(mode & 2))
+#pragma unroll
+            for (int i = 0; i < kPieces; ++i) {
+                uint4 h, l;
+                split_tf32(v[i].x, h.x, l.x); split_tf32(v[i].y, h.y, l.y); split_tf32(v[i].z, h.z, l.z); split_tf32(v[i].w, h.w, l.w);
+                sts128(dst0 + i * 512, h);
+                sts128(dst0 + i * 512 + kRawB, l);
             }
             fence_proxy_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_ready(st));
+            if (lane == 0) {
+                mbar_arrive(bar_rfree(rs));
+                mbar_arrive(bar_ready(st));
+            }
         }
     } else if (warp >= 12) {
         const int q = warp & 3, part = lane >> 4;
@@ -234,7 +261,7 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 2) tmem_dealloc(tmem_base, kTmemCols);
+    if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
 }
 
 int g_enable = 1;   // tt_debug_set("gemm32_umma", 0): keep to the FMA kernels
@@ -264,7 +291,7 @@ cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* par
     if (e != cudaSuccess) return e;
     const dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + kSens - 1) / kSens));
     for (int r0 = 0; r0 < g.k; r0 += 32) {
-        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
+        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0, g_enable >> 1);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
