@@ -59,15 +59,17 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
 
 // x = hi + lo with hi = x rounded to tf32 (nearest, ties away: the bit pattern plus half a tf32 ulp, low 13 bits cleared -
 // what cvt.rna.tf32.f32 computes, in two integer operations instead of the five the conversion expands to) and lo = the
-// exact remainder cut to tf32 (its dropped bits are below 2^-21 |x|, the size of the lo*lo term 3xTF32 leaves out anyway)
+// exact remainder.  lo is handed over with all its bits: the tensor core reads the upper 19 bits of a tf32 operand
+// (measured: masking lo changes no bit of any result), and what it drops is below 2^-21 |x|, the size of the lo*lo term
+// 3xTF32 leaves out anyway.
 __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
     hi = (__float_as_uint(x) + 0x1000u) & 0xffffe000u;
-    lo = __float_as_uint(x - __uint_as_float(hi)) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
 gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
-                       c64* __restrict__ partial, const GemmGeom g, const int r0, const int mode) {
+                       c64* __restrict__ partial, const GemmGeom g, const int r0) {
     extern __shared__ unsigned char smem_dyn[];
     const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
     const uint32_t ops0 = smem0 + kRaw * kRawBytes;
@@ -139,7 +141,6 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                 const uint32_t d = tmem_base + kColD + buf * kN;
                 const uint32_t a_hi = tmem_base + kColA + st * 64, a_lo = a_hi + 32;
                 const uint32_t b_hi = ops0 + st * kOpBytes, b_lo = b_hi + kRawB;
-                if (!(mode & 4))
 #pragma unroll
                 for (int ks = 0; ks < kKB / 8; ++ks) {
                     const uint64_t dh = smem_desc_mnmajor_tf32(b_hi + ks * 1024, kKB * 128, 512);
@@ -162,10 +163,6 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             mbar_wait(bar_full(rs), (kb / kRaw) & 1);
             const uint32_t base = smem0 + rs * kRawBytes + row_off;
             uint32_t hi[32], lo[32];
-            if (mode & 1) {
-#pragma unroll
-                for (int j = 0; j < 32; ++j) hi[j] = lo[j] = 0;
-            } else
 #pragma unroll
             for (int b = 0; b < 2; ++b)
 #pragma unroll
@@ -179,11 +176,9 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
             tc_fence_after();
             const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColA + st * 64;
-            if (!(mode & 1)) {
             tmem_st_32x32(ta, hi);
             tmem_st_32x32(ta + 32, lo);
             tmem_st_wait();
-            }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_ready(st));
@@ -204,7 +199,6 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
             const uint32_t dst0 = ops0 + st * kOpBytes + (c16 >> 3) * (kKB * 128) + row0 * 128 +
                                   ((((c16 & 7) >> 1) ^ (row0 & 3)) << 5) + ((c16 & 1) << 4);   // (row0 + 4 i) % 4 == row0 % 4
-            if (!(mode & 2))
 #pragma unroll
             for (int i = 0; i < kPieces; ++i) {
                 uint4 h, l;
@@ -291,7 +285,7 @@ cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* par
     if (e != cudaSuccess) return e;
     const dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + kSens - 1) / kSens));
     for (int r0 = 0; r0 < g.k; r0 += 32) {
-        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0, g_enable >> 1);
+        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
