@@ -288,7 +288,9 @@ cudaError_t gemm_fwd_launch(int dt, const void* Fhat, const void* Xhat, void* pa
 
 cudaError_t gemm_adj_launch(int dt, const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g,
                             cudaStream_t s) {
-    if (dt == 0) return gemm32_adj_launch(Fhat, Dhat, Xhat_out, g, s);
+    if (dt == 0)
+        return gemm32_umma_adj_ok(g) ? gemm32_umma_adj_launch(Fhat, Dhat, Xhat_out, g, s)
+                                     : gemm32_adj_launch(Fhat, Dhat, Xhat_out, g, s);
     const c128* F = static_cast<const c128*>(Fhat);
     const c128* D = static_cast<const c128*>(Dhat);
     c128* X = static_cast<c128*>(Xhat_out);

@@ -67,6 +67,17 @@ __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) 
     lo = __float_as_uint(x - __uint_as_float(hi));
 }
 
+// A raw stage may go back to the TMA producer only when the shared-memory loads from it have RETURNED.  An mbarrier arrive
+// that merely follows the load instructions in program order does not wait for them (ptxas issues it under the loads'
+// shadow; measured: tiles overwritten under the transform warps), so the arrive is made control-dependent on a warp
+// vote over registers computed from the loaded values.  The vote is never true: a split hi part has 13 zero low bits.
+__device__ __forceinline__ bool loads_returned(const uint32_t (&hi)[32]) {
+    uint32_t f = hi[0];
+#pragma unroll
+    for (int j = 1; j < 32; ++j) f |= hi[j];
+    return __ballot_sync(0xffffffffu, f == 0xffffffffu) == 0u;
+}
+
 __global__ void __launch_bounds__(kThreads, 1)
 gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
                        c64* __restrict__ partial, const GemmGeom g, const int r0) {
@@ -171,8 +182,7 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                     split_tf32(part ? v.y : v.x, hi[16 * b + 2 * ch], lo[16 * b + 2 * ch]);
                     split_tf32(part ? v.w : v.z, hi[16 * b + 2 * ch + 1], lo[16 * b + 2 * ch + 1]);
                 }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_rfree(rs));
+            if (loads_returned(hi) && lane == 0) mbar_arrive(bar_rfree(rs));
             mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
             tc_fence_after();
             const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColA + st * 64;
@@ -258,6 +268,206 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
     if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// adjoint   Xout_w [N_m x k] = Fhat_w^H [N_m x N_d] * Dhat_w [N_d x k],  k = 32, per tile of 128 parameters
+//
+//     P [128 x 64] = A [128 x K] * B [K x 64],   K = 2 N_d,
+//     A[p, (s, 0)] = Re Fhat_w[s, p],  A[p, (s, 1)] = Im Fhat_w[s, p]      (thread p copies its (Re, Im) pairs: no shuffle)
+//     B[(s, 0), .] = Dhat_w[s, .] as it lies in memory (Re, Im interleaved), B[(s, 1), .] = -i Dhat_w[s, .]
+//     P[p, .]      = Xout_w[p, .] as it lies in memory
+//
+// B (hi and lo, the whole K) is built once per CTA and stays in shared memory: a CTA works through a range of parameter
+// tiles of ONE frequency.  Per tile the Fhat_w tile streams through a TMA ring in K-blocks of 16 sensors (rows of 1 KB),
+// the transform warps split it into tensor memory, and the MMA adds the hi*hi products into one accumulator and the two
+// cross products into another (their sum is formed in the epilogue): the tensor core's truncating accumulation then acts
+// once per k-step on the large terms instead of three times.  Tiles alternate between two accumulator pairs.
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int kAdjKB = 16;                         // sensors per K-block (32 K-columns)
+constexpr int kAdjRawBytes = kAdjKB * 128 * 8;     // 16 KB: [16 sensors][128 parameters x 8 B]
+constexpr int kAdjOps = 4;                         // tensor-memory ring of A operands
+constexpr int kAdjColD = 0;                        // two accumulator pairs (hi*hi, cross) of 64 columns each
+constexpr int kAdjColA = 256;
+
+struct AdjArgs {
+    int n_raw;           // stages of the raw ring
+    int n_kb;            // K-blocks per tile = ceil(N_d / 16)
+    int tiles_per_cta;   // parameter tiles per CTA (grid.x CTAs per frequency)
+    int n_tiles;         // ceil(N_m / 128)
+};
+
+__global__ void __launch_bounds__(kThreads, 1)
+gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __restrict__ Dhat, c64* __restrict__ Xout,
+                       const GemmGeom g, const AdjArgs a, const int r0) {
+    extern __shared__ unsigned char smem_dyn[];
+    const int krows = 2 * kAdjKB * a.n_kb;                              // K rows of B (padded sensors x 2)
+    const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
+    const uint32_t b_hi = smem0, b_lo = smem0 + krows * 256;            // each: [2 column halves][krows][128 B]
+    const uint32_t raw0 = smem0 + krows * 512;
+    const uint32_t bars = raw0 + a.n_raw * kAdjRawBytes;
+    constexpr int kMaxRaw = 12;
+    auto bar_full = [&](int s) { return bars + 8u * s; };
+    auto bar_rfree = [&](int s) { return bars + 8u * (kMaxRaw + s); };
+    auto bar_ready = [&](int s) { return bars + 8u * (2 * kMaxRaw + s); };
+    auto bar_free = [&](int s) { return bars + 8u * (2 * kMaxRaw + kAdjOps + s); };
+    auto bar_tfull = [&](int b) { return bars + 8u * (2 * kMaxRaw + 2 * kAdjOps + b); };
+    auto bar_tempty = [&](int b) { return bars + 8u * (2 * kMaxRaw + 2 * kAdjOps + 2 + b); };
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int w = blockIdx.y;
+    const int tile0 = blockIdx.x * a.tiles_per_cta;
+    const int n_my = tile0 >= a.n_tiles ? 0 : (a.n_tiles - tile0 < a.tiles_per_cta ? a.n_tiles - tile0 : a.tiles_per_cta);
+    const int n_it = n_my * a.n_kb;                                     // K-blocks this CTA streams
+
+    if (tid == 0) {
+        for (int s = 0; s < a.n_raw; ++s) {
+            mbar_init(bar_full(s), 1);
+            mbar_init(bar_rfree(s), 4);      // the 4 transform warps (one per lane quadrant) of the stage's set
+        }
+        for (int s = 0; s < kAdjOps; ++s) {
+            mbar_init(bar_ready(s), 4);
+            mbar_init(bar_free(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_tfull(b), 1);
+            mbar_init(bar_tempty(b), 4);
+        }
+        mbar_fence_init();
+        tma_prefetch_desc(&mapF);
+    }
+    if (warp == 1) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
+
+    // B: 16-byte piece (s, c16) of Dhat_w = two complex columns -> rows 2 s and 2 s + 1, column half c16 / 8, piece c16 % 8
+    {
+        const c64* Dw = Dhat + (long long)w * g.N_d * g.k + r0;
+        const int n_pieces = kAdjKB * a.n_kb * 16;
+        for (int idx = tid; idx < n_pieces; idx += kThreads) {
+            const int s = idx >> 4, c16 = idx & 15;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (s < g.N_d) v = *reinterpret_cast<const float4*>(Dw + (long long)s * g.k + 2 * c16);
+            const float4 u = make_float4(v.y, -v.x, v.w, -v.z);         // -i Dhat
+            const uint32_t half = (uint32_t)(c16 >> 3) * (uint32_t)(krows * 128), sub = (uint32_t)(c16 & 1) << 4;
+            const uint32_t p32 = (uint32_t)(c16 & 7) >> 1;
+            const uint32_t k0 = 2 * s, k1 = 2 * s + 1;
+            const uint32_t d0 = half + k0 * 128 + ((p32 ^ (k0 & 3)) << 5) + sub;
+            const uint32_t d1 = half + k1 * 128 + ((p32 ^ (k1 & 3)) << 5) + sub;
+            uint4 h, l;
+            split_tf32(v.x, h.x, l.x); split_tf32(v.y, h.y, l.y); split_tf32(v.z, h.z, l.z); split_tf32(v.w, h.w, l.w);
+            sts128(b_hi + d0, h);
+            sts128(b_lo + d0, l);
+            split_tf32(u.x, h.x, l.x); split_tf32(u.y, h.y, l.y); split_tf32(u.z, h.z, l.z); split_tf32(u.w, h.w, l.w);
+            sts128(b_hi + d1, h);
+            sts128(b_lo + d1, l);
+        }
+        fence_proxy_async_smem();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = tmem_base_s;
+
+    if (warp == 0) {
+        if (elect_one()) {
+            int st = 0, ph = 0;
+            for (int it = 0; it < n_it; ++it) {
+                const int tile = tile0 + it / a.n_kb, kb = it % a.n_kb;
+                mbar_wait(bar_rfree(st), ph ^ 1);
+                mbar_arrive_expect_tx(bar_full(st), kAdjRawBytes);
+                tma_load_3d(raw0 + st * kAdjRawBytes, &mapF, bar_full(st), tile * 256, kb * kAdjKB, w);
+                if (++st == a.n_raw) { st = 0; ph ^= 1; }
+            }
+        }
+    } else if (warp == 1) {
+        if (elect_one()) {
+            constexpr uint32_t idesc = idesc_tf32(128, kN, /*b_mn_major=*/1);
+            const uint32_t lbo = (uint32_t)krows * 128;
+            int it = 0;
+            for (int t = 0; t < n_my; ++t) {
+                const int buf = t & 1;
+                mbar_wait(bar_tempty(buf), ((t >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_h = tmem_base + kAdjColD + buf * 128, d_x = d_h + 64;
+                for (int kb = 0; kb < a.n_kb; ++kb, ++it) {
+                    const int st = it % kAdjOps;
+                    mbar_wait(bar_ready(st), (it / kAdjOps) & 1);
+                    tc_fence_after();
+                    const uint32_t a_hi = tmem_base + kAdjColA + st * 64, a_lo = a_hi + 32;
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks) {
+                        const uint32_t off = (uint32_t)(kb * 32 + ks * 8) * 128;
+                        const uint64_t dh = smem_desc_mnmajor_tf32(b_hi + off, lbo, 512);
+                        const uint64_t dl = smem_desc_mnmajor_tf32(b_lo + off, lbo, 512);
+                        const uint32_t acc = (kb > 0 || ks > 0) ? 1u : 0u;
+                        mma_tf32_ts(d_x, a_lo + ks * 8, dh, idesc, acc);
+                        mma_tf32_ts(d_x, a_hi + ks * 8, dl, idesc, 1u);
+                        mma_tf32_ts(d_h, a_hi + ks * 8, dh, idesc, acc);
+                    }
+                    tc_commit(bar_free(st));
+                }
+                tc_commit(bar_tfull(buf));
+            }
+        }
+    } else if (warp >= 4 && warp < 12) {
+        // A transform: lane l of quadrant q is tensor-memory lane 32 q + l = parameter 32 q + l of the tile; column 2 j of the
+        // stage = Re, 2 j + 1 = Im of sensor j of the K-block.  Two warps per quadrant take the K-blocks in turn.
+        const int q = warp & 3;
+        const uint32_t lane_off = (uint32_t)(32 * q + lane) * 8;
+        for (int it = (warp - 4) >> 2; it < n_it; it += 2) {
+            const int rs = it % a.n_raw, st = it % kAdjOps;
+            mbar_wait(bar_full(rs), (it / a.n_raw) & 1);
+            const uint32_t base = raw0 + rs * kAdjRawBytes + lane_off;
+            uint32_t hi[32], lo[32];
+#pragma unroll
+            for (int j = 0; j < kAdjKB; ++j) {
+                float2 v;
+                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(base + j * 1024));
+                split_tf32(v.x, hi[2 * j], lo[2 * j]);
+                split_tf32(v.y, hi[2 * j + 1], lo[2 * j + 1]);
+            }
+            if (loads_returned(hi) && lane == 0) mbar_arrive(bar_rfree(rs));
+            mbar_wait(bar_free(st), ((it / kAdjOps) & 1) ^ 1);
+            tc_fence_after();
+            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kAdjColA + st * 64;
+            tmem_st_32x32(ta, hi);
+            tmem_st_32x32(ta + 32, lo);
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_ready(st));
+        }
+    } else if (warp >= 12) {
+        const int q = warp & 3;
+        for (int t = 0; t < n_my; ++t) {
+            const int buf = t & 1;
+            mbar_wait(bar_tfull(buf), (t >> 1) & 1);
+            tc_fence_after();
+            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kAdjColD + buf * 128;
+            const long long p = (long long)(tile0 + t) * 128 + 32 * q + lane;
+            float4* dst = reinterpret_cast<float4*>(Xout + (long long)w * g.ldx + p * g.k + r0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint32_t vh[16], vx[16];
+                tmem_ld_32x16(ta + 16 * j, vh);
+                tmem_ld_32x16(ta + 64 + 16 * j, vx);
+                if (p < g.N_m) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        dst[4 * j + i] = make_float4(__uint_as_float(vh[4 * i]) + __uint_as_float(vx[4 * i]),
+                                                     __uint_as_float(vh[4 * i + 1]) + __uint_as_float(vx[4 * i + 1]),
+                                                     __uint_as_float(vh[4 * i + 2]) + __uint_as_float(vx[4 * i + 2]),
+                                                     __uint_as_float(vh[4 * i + 3]) + __uint_as_float(vx[4 * i + 3]));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_tempty(buf));
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, kTmemCols);
+}
+
 int g_enable = 1;   // tt_debug_set("gemm32_umma", 0): keep to the FMA kernels
 
 }  // namespace
@@ -286,6 +496,48 @@ cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* par
     const dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + kSens - 1) / kSens));
     for (int r0 = 0; r0 < g.k; r0 += 32) {
         gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+// adjoint: the whole K (2 N_d rows of B, hi and lo) stays in shared memory beside a raw ring of at least 4 stages
+bool gemm32_umma_adj_ok(const GemmGeom& g) {
+    return g_enable && g.k > 0 && g.k % 32 == 0 && g.N_d <= 128 && 2 * g.ldp < (1LL << 31);
+}
+
+cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g, cudaStream_t s) {
+    CUtensorMap mapF;
+    {   // Fhat as floats: [n_f][N_d][2 ldp]; box = 128 parameters (1 KB) x 16 sensors, no swizzle (thread p reads 8 B at 8 p)
+        const unsigned long long dims[3] = {(unsigned long long)(2 * g.ldp), (unsigned long long)g.N_d, (unsigned long long)g.n_f};
+        const unsigned long long strides[2] = {(unsigned long long)g.ldp * 8, (unsigned long long)g.N_d * g.ldp * 8};
+        const unsigned box[3] = {256, kAdjKB, 1};
+        if (!make_tensor_map_f32(&mapF, Fhat, 3, dims, strides, box, /*swizzle128=*/false)) return cudaErrorInvalidValue;
+    }
+    AdjArgs a;
+    a.n_kb = (g.N_d + kAdjKB - 1) / kAdjKB;
+    a.n_tiles = (int)((g.N_m + 127) / 128);
+    const int b_bytes = 2 * kAdjKB * a.n_kb * 512;
+    a.n_raw = (232448 - 2048 - b_bytes) / kAdjRawBytes;
+    if (a.n_raw > 12) a.n_raw = 12;
+    if (a.n_raw < 4) return cudaErrorInvalidValue;
+    const int smem = b_bytes + a.n_raw * kAdjRawBytes + 1024 + 512;
+    // CTAs per frequency: ~6 waves over the SMs, at least 8 tiles each so that building B stays a small part
+    int dev = 0, sms = 148;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    int per_f = (6 * sms + g.n_f - 1) / g.n_f;
+    if (per_f > (a.n_tiles + 7) / 8) per_f = (a.n_tiles + 7) / 8;
+    if (per_f < 1) per_f = 1;
+    a.tiles_per_cta = (a.n_tiles + per_f - 1) / per_f;
+    per_f = (a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta;
+    e = cudaFuncSetAttribute(gemm32_umma_adj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((unsigned)per_f, (unsigned)g.n_f);
+    for (int r0 = 0; r0 < g.k; r0 += 32) {
+        gemm32_umma_adj_kernel<<<grid, kThreads, smem, s>>>(mapF, static_cast<const c64*>(Dhat), static_cast<c64*>(Xhat_out), g, a, r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

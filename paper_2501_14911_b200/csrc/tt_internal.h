@@ -114,6 +114,8 @@ void gemm32_debug_set(int fwd_variant);
 // the same products on tcgen05 (3xTF32, tt_gemm32_umma.cu) for the shapes *_ok() accepts
 bool gemm32_umma_fwd_ok(const GemmGeom& g);
 cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g, cudaStream_t s);
+bool gemm32_umma_adj_ok(const GemmGeom& g);
+cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g, cudaStream_t s);
 void gemm32_umma_debug_set(int enable);
 
 // Triangular solves with the rescaled Cholesky factor (tt_trsv.cu).
