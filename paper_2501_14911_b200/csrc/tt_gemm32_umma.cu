@@ -287,6 +287,9 @@ constexpr int kAdjRawBytes = kAdjKB * 128 * 8;     // 16 KB: [16 sensors][128 pa
 constexpr int kAdjOps = 4;                         // tensor-memory ring of A operands
 constexpr int kAdjColD = 0;                        // two accumulator pairs (hi*hi, cross) of 64 columns each
 constexpr int kAdjColA = 256;
+constexpr int kAdjStgBytes = 128 * 256;             // staging of one output tile
+constexpr int kAdjSets = 2;                        // transform warps per lane quadrant
+constexpr int kAdjThreads = 32 * (4 + 4 * kAdjSets + 4);   // TMA, MMA, 2 spare | transforms | 4 epilogue warps
 
 struct AdjArgs {
     int n_raw;           // stages of the raw ring
@@ -295,14 +298,15 @@ struct AdjArgs {
     int n_tiles;         // ceil(N_m / 128)
 };
 
-__global__ void __launch_bounds__(kThreads, 1)
-gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __restrict__ Dhat, c64* __restrict__ Xout,
-                       const GemmGeom g, const AdjArgs a, const int r0) {
+__global__ void __launch_bounds__(kAdjThreads, 1)
+gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
+                       const c64* __restrict__ Dhat, const GemmGeom g, const AdjArgs a, const int r0) {
     extern __shared__ unsigned char smem_dyn[];
     const int krows = 2 * kAdjKB * a.n_kb;                              // K rows of B (padded sensors x 2)
     const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
     const uint32_t b_hi = smem0, b_lo = smem0 + krows * 256;            // each: [2 column halves][krows][128 B]
-    const uint32_t raw0 = smem0 + krows * 512;
+    const uint32_t stg = smem0 + krows * 512;                           // output tile: [2 column halves][128 rows][128 B]
+    const uint32_t raw0 = stg + kAdjStgBytes;
     const uint32_t bars = raw0 + a.n_raw * kAdjRawBytes;
     constexpr int kMaxRaw = 12;
     auto bar_full = [&](int s) { return bars + 8u * s; };
@@ -334,6 +338,7 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __re
         }
         mbar_fence_init();
         tma_prefetch_desc(&mapF);
+        tma_prefetch_desc(&mapX);
     }
     if (warp == 1) tmem_alloc(smem_u32(&tmem_base_s), kTmemCols);
 
@@ -341,7 +346,7 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __re
     {
         const c64* Dw = Dhat + (long long)w * g.N_d * g.k + r0;
         const int n_pieces = kAdjKB * a.n_kb * 16;
-        for (int idx = tid; idx < n_pieces; idx += kThreads) {
+        for (int idx = tid; idx < n_pieces; idx += kAdjThreads) {
             const int s = idx >> 4, c16 = idx & 15;
             float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
             if (s < g.N_d) v = *reinterpret_cast<const float4*>(Dw + (long long)s * g.k + 2 * c16);
@@ -369,13 +374,13 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __re
     if (warp == 0) {
         if (elect_one()) {
             int st = 0, ph = 0;
-            for (int it = 0; it < n_it; ++it) {
-                const int tile = tile0 + it / a.n_kb, kb = it % a.n_kb;
-                mbar_wait(bar_rfree(st), ph ^ 1);
-                mbar_arrive_expect_tx(bar_full(st), kAdjRawBytes);
-                tma_load_3d(raw0 + st * kAdjRawBytes, &mapF, bar_full(st), tile * 256, kb * kAdjKB, w);
-                if (++st == a.n_raw) { st = 0; ph ^= 1; }
-            }
+            for (int t = 0; t < n_my; ++t)
+                for (int kb = 0; kb < a.n_kb; ++kb) {
+                    mbar_wait(bar_rfree(st), ph ^ 1);
+                    mbar_arrive_expect_tx(bar_full(st), kAdjRawBytes);
+                    tma_load_3d(raw0 + st * kAdjRawBytes, &mapF, bar_full(st), (tile0 + t) * 256, kb * kAdjKB, w);
+                    if (++st == a.n_raw) { st = 0; ph ^= 1; }
+                }
         }
     } else if (warp == 1) {
         if (elect_one()) {
@@ -407,14 +412,15 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __re
                 tc_commit(bar_tfull(buf));
             }
         }
-    } else if (warp >= 4 && warp < 12) {
+    } else if (warp >= 4 && warp < 4 + 4 * kAdjSets) {
         // A transform: lane l of quadrant q is tensor-memory lane 32 q + l = parameter 32 q + l of the tile; column 2 j of the
-        // stage = Re, 2 j + 1 = Im of sensor j of the K-block.  Two warps per quadrant take the K-blocks in turn.
-        const int q = warp & 3;
+        // stage = Re, 2 j + 1 = Im of sensor j of the K-block.  kAdjSets warps per quadrant take the K-blocks in turn.
+        const int q = warp & 3, set = (warp - 4) >> 2;
         const uint32_t lane_off = (uint32_t)(32 * q + lane) * 8;
-        for (int it = (warp - 4) >> 2; it < n_it; it += 2) {
-            const int rs = it % a.n_raw, st = it % kAdjOps;
-            mbar_wait(bar_full(rs), (it / a.n_raw) & 1);
+        int rs = set % a.n_raw, rph = (set / a.n_raw) & 1;              // raw stage and phase of K-block `it`
+        for (int it = set; it < n_it; it += kAdjSets) {
+            const int st = it % kAdjOps;
+            mbar_wait(bar_full(rs), rph);
             const uint32_t base = raw0 + rs * kAdjRawBytes + lane_off;
             uint32_t hi[32], lo[32];
 #pragma unroll
@@ -434,34 +440,50 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const c64* __re
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_ready(st));
+            rs += kAdjSets;
+            while (rs >= a.n_raw) { rs -= a.n_raw; rph ^= 1; }
         }
-    } else if (warp >= 12) {
-        const int q = warp & 3;
+    } else if (warp >= 4 + 4 * kAdjSets) {
+        // epilogue: the tile leaves through shared memory and a TMA store.  (Each lane owns one 256-byte row of Xout_w: direct
+        // stores put 16 bytes into each of 32 lines per instruction, and at 32 KB per tile that made the epilogue, not the
+        // MMA, the pace of the kernel.)  Staging rows are 128 bytes per column half, 128-byte swizzled like the tensor map.
+        const int q = warp & 3, row = 32 * q + lane;
+        const bool leader = warp == 4 + 4 * kAdjSets && elect_one();
+        const uint32_t srow = stg + (uint32_t)row * 128, sw = (uint32_t)row & 7;
         for (int t = 0; t < n_my; ++t) {
             const int buf = t & 1;
             mbar_wait(bar_tfull(buf), (t >> 1) & 1);
             tc_fence_after();
+            if (leader) tma_store_wait_read();                          // the previous tile has left the staging buffer
+            asm volatile("bar.sync 1, 128;" ::: "memory");
             const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kAdjColD + buf * 128;
-            const long long p = (long long)(tile0 + t) * 128 + 32 * q + lane;
-            float4* dst = reinterpret_cast<float4*>(Xout + (long long)w * g.ldx + p * g.k + r0);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 uint32_t vh[16], vx[16];
                 tmem_ld_32x16(ta + 16 * j, vh);
                 tmem_ld_32x16(ta + 64 + 16 * j, vx);
-                if (p < g.N_m) {
 #pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        dst[4 * j + i] = make_float4(__uint_as_float(vh[4 * i]) + __uint_as_float(vx[4 * i]),
-                                                     __uint_as_float(vh[4 * i + 1]) + __uint_as_float(vx[4 * i + 1]),
-                                                     __uint_as_float(vh[4 * i + 2]) + __uint_as_float(vx[4 * i + 2]),
-                                                     __uint_as_float(vh[4 * i + 3]) + __uint_as_float(vx[4 * i + 3]));
+                for (int i = 0; i < 4; ++i) {
+                    uint4 o;
+                    o.x = __float_as_uint(__uint_as_float(vh[4 * i]) + __uint_as_float(vx[4 * i]));
+                    o.y = __float_as_uint(__uint_as_float(vh[4 * i + 1]) + __uint_as_float(vx[4 * i + 1]));
+                    o.z = __float_as_uint(__uint_as_float(vh[4 * i + 2]) + __uint_as_float(vx[4 * i + 2]));
+                    o.w = __float_as_uint(__uint_as_float(vh[4 * i + 3]) + __uint_as_float(vx[4 * i + 3]));
+                    sts128(srow + (j >> 1) * (kAdjStgBytes / 2) + ((((j & 1) * 4 + i) ^ sw) << 4), o);
                 }
             }
             tc_fence_before();
+            fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_tempty(buf));
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            if (leader) {
+                tma_store_3d(&mapX, stg, 2 * r0, (tile0 + t) * 128, w);
+                tma_store_3d(&mapX, stg + kAdjStgBytes / 2, 2 * r0 + 32, (tile0 + t) * 128, w);
+                tma_store_commit();
+            }
         }
+        if (leader) tma_store_wait_all();
     }
     tc_fence_before();
     __syncthreads();
@@ -515,14 +537,25 @@ cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xha
         const unsigned box[3] = {256, kAdjKB, 1};
         if (!make_tensor_map_f32(&mapF, Fhat, 3, dims, strides, box, /*swizzle128=*/false)) return cudaErrorInvalidValue;
     }
+    CUtensorMap mapX;
+    {   // Xout as floats: [n_f][N_m][2 k]; box = 32 floats (one column half) x 128 parameters, 128-byte swizzle
+        const unsigned long long dims[3] = {(unsigned long long)(2 * g.k), (unsigned long long)g.N_m, (unsigned long long)g.n_f};
+        const unsigned long long strides[2] = {(unsigned long long)g.k * 8, (unsigned long long)g.ldx * 8};
+        const unsigned box[3] = {32, 128, 1};
+        if (!make_tensor_map_f32(&mapX, Xhat_out, 3, dims, strides, box)) return cudaErrorInvalidValue;
+    }
     AdjArgs a;
     a.n_kb = (g.N_d + kAdjKB - 1) / kAdjKB;
     a.n_tiles = (int)((g.N_m + 127) / 128);
     const int b_bytes = 2 * kAdjKB * a.n_kb * 512;
-    a.n_raw = (232448 - 2048 - b_bytes) / kAdjRawBytes;
+    a.n_raw = (232448 - 2048 - b_bytes - kAdjStgBytes) / kAdjRawBytes;
     if (a.n_raw > 12) a.n_raw = 12;
+    // Every raw stage must belong to ONE set of transform warps.  A set meets its stages in order, so it cannot reach a
+    // stage a whole phase early; a second set could, and a parity wait cannot tell "the phase before last has completed"
+    // from "the phase I am waiting for has completed" (measured with 5 stages and 2 sets: tiles read before they landed).
+    a.n_raw -= a.n_raw % kAdjSets;
     if (a.n_raw < 4) return cudaErrorInvalidValue;
-    const int smem = b_bytes + a.n_raw * kAdjRawBytes + 1024 + 512;
+    const int smem = b_bytes + kAdjStgBytes + a.n_raw * kAdjRawBytes + 1024 + 512;
     // CTAs per frequency: ~6 waves over the SMs, at least 8 tiles each so that building B stays a small part
     int dev = 0, sms = 148;
     cudaError_t e = cudaGetDevice(&dev);
@@ -537,7 +570,7 @@ cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xha
     if (e != cudaSuccess) return e;
     const dim3 grid((unsigned)per_f, (unsigned)g.n_f);
     for (int r0 = 0; r0 < g.k; r0 += 32) {
-        gemm32_umma_adj_kernel<<<grid, kThreads, smem, s>>>(mapF, static_cast<const c64*>(Dhat), static_cast<c64*>(Xhat_out), g, a, r0);
+        gemm32_umma_adj_kernel<<<grid, kAdjThreads, smem, s>>>(mapF, mapX, static_cast<const c64*>(Dhat), g, a, r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
