@@ -35,12 +35,12 @@ using namespace umma;
 
 constexpr int kSens = 64;                      // sensors per CTA tile (128 tensor-memory lanes)
 constexpr int kKB = 32;                        // parameters per pipeline stage
-constexpr int kN = 64;                         // floats per Xhat row = 2 k
+// (kN = floats per Xhat row handled by one launch = 2 x 32 or 2 x 16 columns is a template parameter of the kernels)
 constexpr int kRaw = 6;                        // ring of raw tiles: filled by TMA, released by the transforms
 constexpr int kOps = 4;                        // ring of operands (B hi / lo in shared, A hi / lo in tensor memory): -> MMA
 constexpr int kChunkKB = 2;                    // stages per accumulation chunk (64 parameters)
 constexpr int kRawA = kSens * kKB * 8;         // 16 KB: two TMA boxes of [64 rows][16 parameters = 128 B]
-constexpr int kRawB = kKB * kN * 4;            //  8 KB: raw [32 parameters][64 floats]; hi / lo [2 column halves][32][32 floats]
+constexpr int kRawB = kKB * 64 * 4;            //  8 KB: raw [32 parameters][kN floats]; hi / lo [kN / 32 column halves][32][32 floats]
 constexpr int kRawBytes = kRawA + kRawB, kOpBytes = 2 * kRawB;
 constexpr int kFwdSmem = kRaw * kRawBytes + kOps * kOpBytes + 1024 /* alignment slack */ + 256 /* barriers */;
 constexpr int kThreads = 512;
@@ -78,6 +78,7 @@ __device__ __forceinline__ bool loads_returned(const uint32_t (&hi)[32]) {
     return __ballot_sync(0xffffffffu, f == 0xffffffffu) == 0u;
 }
 
+template <int kN>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
                        c64* __restrict__ partial, const GemmGeom g, const int r0) {
@@ -130,7 +131,7 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                 const int st = kb % kRaw;
                 mbar_wait(bar_rfree(st), ((kb / kRaw) & 1) ^ 1);
                 const uint32_t base = smem0 + st * kRawBytes;
-                mbar_arrive_expect_tx(bar_full(st), kRawA + kRawB);
+                mbar_arrive_expect_tx(bar_full(st), kRawA + kKB * kN * 4);
                 const long long p = p_lo + (long long)kb * kKB;
                 tma_load_3d(base, &mapF, bar_full(st), (int)(2 * p), s0, w);
                 tma_load_3d(base + kRawA / 2, &mapF, bar_full(st), (int)(2 * p + 32), s0, w);
@@ -149,7 +150,7 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                 }
                 mbar_wait(bar_ready(st), (kb / kOps) & 1);
                 tc_fence_after();
-                const uint32_t d = tmem_base + kColD + buf * kN;
+                const uint32_t d = tmem_base + kColD + buf * 64;
                 const uint32_t a_hi = tmem_base + kColA + st * 64, a_lo = a_hi + 32;
                 const uint32_t b_hi = ops0 + st * kOpBytes, b_lo = b_hi + kRawB;
 #pragma unroll
@@ -198,23 +199,23 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
         for (int kb = 0; kb < n_kb; ++kb) {
             const int rs = kb % kRaw, st = kb % kOps;
             mbar_wait(bar_full(rs), (kb / kRaw) & 1);
-            // raw 16-byte piece ci = 16 row + c16 (row = parameter, 256-byte rows) -> column half c16 / 8, row, piece c16 % 8
-            // of the operand layout, whose 32-byte pieces are XORed with row % 4
+            // raw 16-byte piece t + 64 i = (row, c16) of the kN-float rows -> column half c16 / 8, row, piece c16 % 8 of the
+            // operand layout, whose 32-byte pieces are XORed with row % 4
+            constexpr int kPR = kN / 4, kPieces = kKB * kPR / 64, kRowStep = 64 / kPR;   // pieces per row, per thread; rows per pass
             const uint32_t raw = smem0 + rs * kRawBytes + kRawA + t * 16;
-            const uint32_t c16 = t & 15, row0 = t >> 4;
-            constexpr int kPieces = kRawB / 16 / 64;
+            const uint32_t c16 = t % kPR, row0 = t / kPR;
             float4 v[kPieces];
 #pragma unroll
             for (int i = 0; i < kPieces; ++i) v[i] = lds128(raw + i * 1024);     // all loads in flight before the first use
             mbar_wait(bar_free(st), ((kb / kOps) & 1) ^ 1);
             const uint32_t dst0 = ops0 + st * kOpBytes + (c16 >> 3) * (kKB * 128) + row0 * 128 +
-                                  ((((c16 & 7) >> 1) ^ (row0 & 3)) << 5) + ((c16 & 1) << 4);   // (row0 + 4 i) % 4 == row0 % 4
+                                  ((((c16 & 7) >> 1) ^ (row0 & 3)) << 5) + ((c16 & 1) << 4);   // (row0 + kRowStep i) % 4 == row0 % 4
 #pragma unroll
             for (int i = 0; i < kPieces; ++i) {
                 uint4 h, l;
                 split_tf32(v[i].x, h.x, l.x); split_tf32(v[i].y, h.y, l.y); split_tf32(v[i].z, h.z, l.z); split_tf32(v[i].w, h.w, l.w);
-                sts128(dst0 + i * 512, h);
-                sts128(dst0 + i * 512 + kRawB, l);
+                sts128(dst0 + i * (kRowStep * 128), h);
+                sts128(dst0 + i * (kRowStep * 128) + kRawB, l);
             }
             fence_proxy_async_smem();
             __syncwarp();
@@ -232,7 +233,7 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             const int buf = ch & 1;
             mbar_wait(bar_tfull(buf), (ch >> 1) & 1);
             tc_fence_after();
-            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColD + buf * kN;
+            const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kColD + buf * 64;
 #pragma unroll
             for (int j = 0; j < kN / 16; ++j) {
                 uint32_t v[16];
@@ -244,21 +245,22 @@ gemm32_umma_fwd_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_tempty(buf));
         }
-        // lanes l and l ^ 16 hold the Re-row and the Im-row products of one sensor: the Re lane finishes columns 0..15,
-        // the Im lane columns 16..31
-        float a[32], b[32];
+        // lanes l and l ^ 16 hold the Re-row and the Im-row products of one sensor: the Re lane finishes the first half of the
+        // columns, the Im lane the second half
+        constexpr int kH = kN / 2;                   // floats of half the columns
+        float a[kH], b[kH];
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            const float send = part ? acc[j] : acc[32 + j];
+        for (int j = 0; j < kH; ++j) {
+            const float send = part ? acc[j] : acc[kH + j];
             const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-            a[j] = part ? recv : acc[j];         // Re-row products of my 16 columns
-            b[j] = part ? acc[32 + j] : recv;    // Im-row products
+            a[j] = part ? recv : acc[j];         // Re-row products of my columns
+            b[j] = part ? acc[kH + j] : recv;    // Im-row products
         }
         const int s = s0 + 16 * q + (lane & 15);
         if (s < g.N_d) {
-            float4* dst = reinterpret_cast<float4*>(partial + (((long long)w * g.split + c) * g.N_d + s) * g.k + r0 + 16 * part);
+            float4* dst = reinterpret_cast<float4*>(partial + (((long long)w * g.split + c) * g.N_d + s) * g.k + r0 + (kH / 2) * part);
 #pragma unroll
-            for (int r = 0; r < 16; r += 2)
+            for (int r = 0; r < kH / 2; r += 2)
                 dst[r / 2] = make_float4(a[2 * r] - b[2 * r + 1], a[2 * r + 1] + b[2 * r], a[2 * r + 2] - b[2 * r + 3],
                                          a[2 * r + 3] + b[2 * r + 2]);
         }
@@ -287,7 +289,6 @@ constexpr int kAdjRawBytes = kAdjKB * 128 * 8;     // 16 KB: [16 sensors][128 pa
 constexpr int kAdjOps = 4;                         // tensor-memory ring of A operands
 constexpr int kAdjColD = 0;                        // two accumulator pairs (hi*hi, cross) of 64 columns each
 constexpr int kAdjColA = 256;
-constexpr int kAdjStgBytes = 128 * 256;             // staging of one output tile
 constexpr int kAdjSets = 2;                        // transform warps per lane quadrant
 constexpr int kAdjThreads = 32 * (4 + 4 * kAdjSets + 4);   // TMA, MMA, 2 spare | transforms | 4 epilogue warps
 
@@ -298,15 +299,16 @@ struct AdjArgs {
     int n_tiles;         // ceil(N_m / 128)
 };
 
+template <int kN>
 __global__ void __launch_bounds__(kAdjThreads, 1)
 gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_constant__ CUtensorMap mapX,
                        const c64* __restrict__ Dhat, const GemmGeom g, const AdjArgs a, const int r0) {
     extern __shared__ unsigned char smem_dyn[];
     const int krows = 2 * kAdjKB * a.n_kb;                              // K rows of B (padded sensors x 2)
     const uint32_t smem0 = (smem_u32(smem_dyn) + 1023u) & ~1023u;
-    const uint32_t b_hi = smem0, b_lo = smem0 + krows * 256;            // each: [2 column halves][krows][128 B]
-    const uint32_t stg = smem0 + krows * 512;                           // output tile: [2 column halves][128 rows][128 B]
-    const uint32_t raw0 = stg + kAdjStgBytes;
+    const uint32_t b_hi = smem0, b_lo = smem0 + krows * kN * 4;         // each: [kN / 32 column halves][krows][128 B]
+    const uint32_t stg = smem0 + krows * kN * 8;                        // output tile: [kN / 32 column halves][128 rows][128 B]
+    const uint32_t raw0 = stg + 128 * kN * 4;
     const uint32_t bars = raw0 + a.n_raw * kAdjRawBytes;
     constexpr int kMaxRaw = 12;
     auto bar_full = [&](int s) { return bars + 8u * s; };
@@ -345,9 +347,10 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
     // B: 16-byte piece (s, c16) of Dhat_w = two complex columns -> rows 2 s and 2 s + 1, column half c16 / 8, piece c16 % 8
     {
         const c64* Dw = Dhat + (long long)w * g.N_d * g.k + r0;
-        const int n_pieces = kAdjKB * a.n_kb * 16;
+        constexpr int kPR = kN / 4;                                      // 16-byte pieces per row of Dhat_w
+        const int n_pieces = kAdjKB * a.n_kb * kPR;
         for (int idx = tid; idx < n_pieces; idx += kAdjThreads) {
-            const int s = idx >> 4, c16 = idx & 15;
+            const int s = idx / kPR, c16 = idx % kPR;
             float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
             if (s < g.N_d) v = *reinterpret_cast<const float4*>(Dw + (long long)s * g.k + 2 * c16);
             const float4 u = make_float4(v.y, -v.x, v.w, -v.z);         // -i Dhat
@@ -458,7 +461,7 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             asm volatile("bar.sync 1, 128;" ::: "memory");
             const uint32_t ta = tmem_base + ((uint32_t)(32 * q) << 16) + kAdjColD + buf * 128;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < kN / 16; ++j) {
                 uint32_t vh[16], vx[16];
                 tmem_ld_32x16(ta + 16 * j, vh);
                 tmem_ld_32x16(ta + 64 + 16 * j, vx);
@@ -469,7 +472,7 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
                     o.y = __float_as_uint(__uint_as_float(vh[4 * i + 1]) + __uint_as_float(vx[4 * i + 1]));
                     o.z = __float_as_uint(__uint_as_float(vh[4 * i + 2]) + __uint_as_float(vx[4 * i + 2]));
                     o.w = __float_as_uint(__uint_as_float(vh[4 * i + 3]) + __uint_as_float(vx[4 * i + 3]));
-                    sts128(srow + (j >> 1) * (kAdjStgBytes / 2) + ((((j & 1) * 4 + i) ^ sw) << 4), o);
+                    sts128(srow + (j >> 1) * (128 * 128) + ((((j & 1) * 4 + i) ^ sw) << 4), o);
                 }
             }
             tc_fence_before();
@@ -479,7 +482,7 @@ gemm32_umma_adj_kernel(const __grid_constant__ CUtensorMap mapF, const __grid_co
             asm volatile("bar.sync 1, 128;" ::: "memory");
             if (leader) {
                 tma_store_3d(&mapX, stg, 2 * r0, (tile0 + t) * 128, w);
-                tma_store_3d(&mapX, stg + kAdjStgBytes / 2, 2 * r0 + 32, (tile0 + t) * 128, w);
+                if (kN == 64) tma_store_3d(&mapX, stg + 128 * 128, 2 * r0 + 32, (tile0 + t) * 128, w);
                 tma_store_commit();
             }
         }
@@ -496,10 +499,11 @@ int g_enable = 1;   // tt_debug_set("gemm32_umma", 0): keep to the FMA kernels
 
 void gemm32_umma_debug_set(int v) { g_enable = v; }
 
-// The shapes the tensor-core path takes: 32-column groups (k a multiple of 32), Fhat rows 16-byte aligned (always).
-bool gemm32_umma_fwd_ok(const GemmGeom& g) { return g_enable && g.k > 0 && g.k % 32 == 0 && 2 * g.ldp < (1LL << 31); }
+// The shapes the tensor-core path takes: groups of 32 columns (k a multiple of 32) or of 16 (k a multiple of 16).
+bool gemm32_umma_fwd_ok(const GemmGeom& g) { return g_enable && g.k > 0 && g.k % 16 == 0 && 2 * g.ldp < (1LL << 31); }
 
 cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* partial, const GemmGeom& g, cudaStream_t s) {
+    const int n = g.k % 32 == 0 ? 64 : 32;       // floats per row handled by one launch
     CUtensorMap mapF, mapX;
     {   // Fhat as floats: [n_f][N_d][2 ldp]; box = 16 parameters x 64 sensors
         const unsigned long long dims[3] = {(unsigned long long)(2 * g.ldp), (unsigned long long)g.N_d, (unsigned long long)g.n_f};
@@ -510,14 +514,15 @@ cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* par
     {   // Xhat as floats: [n_f][N_m][2 k]; box = 64 floats x 32 parameters, rows as they lie in memory
         const unsigned long long dims[3] = {(unsigned long long)(2 * g.k), (unsigned long long)g.N_m, (unsigned long long)g.n_f};
         const unsigned long long strides[2] = {(unsigned long long)g.k * 8, (unsigned long long)g.ldx * 8};
-        const unsigned box[3] = {kN, kKB, 1};
+        const unsigned box[3] = {(unsigned)n, kKB, 1};
         if (!make_tensor_map_f32(&mapX, Xhat, 3, dims, strides, box, /*swizzle128=*/false)) return cudaErrorInvalidValue;
     }
-    cudaError_t e = cudaFuncSetAttribute(gemm32_umma_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kFwdSmem);
+    auto kern = n == 64 ? gemm32_umma_fwd_kernel<64> : gemm32_umma_fwd_kernel<32>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kFwdSmem);
     if (e != cudaSuccess) return e;
     const dim3 grid((unsigned)g.split, (unsigned)g.n_f, (unsigned)((g.N_d + kSens - 1) / kSens));
-    for (int r0 = 0; r0 < g.k; r0 += 32) {
-        gemm32_umma_fwd_kernel<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
+    for (int r0 = 0; r0 < g.k; r0 += n / 2) {
+        kern<<<grid, kThreads, kFwdSmem, s>>>(mapF, mapX, static_cast<c64*>(partial), g, r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -526,10 +531,11 @@ cudaError_t gemm32_umma_fwd_launch(const void* Fhat, const void* Xhat, void* par
 
 // adjoint: the whole K (2 N_d rows of B, hi and lo) stays in shared memory beside a raw ring of at least 4 stages
 bool gemm32_umma_adj_ok(const GemmGeom& g) {
-    return g_enable && g.k > 0 && g.k % 32 == 0 && g.N_d <= 128 && 2 * g.ldp < (1LL << 31);
+    return g_enable && g.k > 0 && g.k % 16 == 0 && g.N_d <= 128 && 2 * g.ldp < (1LL << 31);
 }
 
 cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xhat_out, const GemmGeom& g, cudaStream_t s) {
+    const int n = g.k % 32 == 0 ? 64 : 32;       // floats per row handled by one launch
     CUtensorMap mapF;
     {   // Fhat as floats: [n_f][N_d][2 ldp]; box = 128 parameters (1 KB) x 16 sensors, no swizzle (thread p reads 8 B at 8 p)
         const unsigned long long dims[3] = {(unsigned long long)(2 * g.ldp), (unsigned long long)g.N_d, (unsigned long long)g.n_f};
@@ -547,15 +553,15 @@ cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xha
     AdjArgs a;
     a.n_kb = (g.N_d + kAdjKB - 1) / kAdjKB;
     a.n_tiles = (int)((g.N_m + 127) / 128);
-    const int b_bytes = 2 * kAdjKB * a.n_kb * 512;
-    a.n_raw = (232448 - 2048 - b_bytes - kAdjStgBytes) / kAdjRawBytes;
+    const int b_bytes = 2 * kAdjKB * a.n_kb * n * 8, stg_bytes = 128 * n * 4;
+    a.n_raw = (232448 - 2048 - b_bytes - stg_bytes) / kAdjRawBytes;
     if (a.n_raw > 12) a.n_raw = 12;
     // Every raw stage must belong to ONE set of transform warps.  A set meets its stages in order, so it cannot reach a
     // stage a whole phase early; a second set could, and a parity wait cannot tell "the phase before last has completed"
     // from "the phase I am waiting for has completed" (measured with 5 stages and 2 sets: tiles read before they landed).
     a.n_raw -= a.n_raw % kAdjSets;
     if (a.n_raw < 4) return cudaErrorInvalidValue;
-    const int smem = b_bytes + kAdjStgBytes + a.n_raw * kAdjRawBytes + 1024 + 512;
+    const int smem = b_bytes + stg_bytes + a.n_raw * kAdjRawBytes + 1024 + 512;
     // CTAs per frequency: ~6 waves over the SMs, at least 8 tiles each so that building B stays a small part
     int dev = 0, sms = 148;
     cudaError_t e = cudaGetDevice(&dev);
@@ -566,11 +572,12 @@ cudaError_t gemm32_umma_adj_launch(const void* Fhat, const void* Dhat, void* Xha
     if (per_f < 1) per_f = 1;
     a.tiles_per_cta = (a.n_tiles + per_f - 1) / per_f;
     per_f = (a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta;
-    e = cudaFuncSetAttribute(gemm32_umma_adj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    auto kern = n == 64 ? gemm32_umma_adj_kernel<64> : gemm32_umma_adj_kernel<32>;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     const dim3 grid((unsigned)per_f, (unsigned)g.n_f);
-    for (int r0 = 0; r0 < g.k; r0 += 32) {
-        gemm32_umma_adj_kernel<<<grid, kAdjThreads, smem, s>>>(mapF, mapX, static_cast<const c64*>(Dhat), g, a, r0);
+    for (int r0 = 0; r0 < g.k; r0 += n / 2) {
+        kern<<<grid, kAdjThreads, smem, s>>>(mapF, mapX, static_cast<const c64*>(Dhat), g, a, r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

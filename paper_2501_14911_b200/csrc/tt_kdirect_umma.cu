@@ -153,7 +153,7 @@ kd_umma_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
 
     if (warp < kCtrlWarps) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 32;");           // hand the registers to the epilogue warpgroups
-        if (warp == 0 && lane == 0) {
+        if (warp == 0 && elect_one()) {
             // ===== TMA producer =====
             int stage = 0;
             uint32_t phase = 0;
@@ -171,7 +171,7 @@ kd_umma_kernel(const __grid_constant__ CUtensorMap tmA_hi, const __grid_constant
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
             }
-        } else if (warp == 1 && lane == 0) {
+        } else if (warp == 1 && elect_one()) {
             // ===== MMA issuer: one chunk of kChunkBlocks K-blocks per tensor-memory accumulator, the two accumulators in turn =====
             constexpr uint32_t idesc = idesc_tf32(kBM, kBN);
             int stage = 0;
