@@ -3,8 +3,9 @@
 //     adjoint   Xhat_w [N_m x k] = Fhat_w^H [N_m x N_d] * Dhat_w [N_d x k]
 // (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423 - K assembly pushes
 // N_d N_t unit vectors through G* and F).  With k = 32 columns every Fhat byte feeds 32 flop, far above the
-// ~10 flop/B at which the FP32 FMA pipe saturates, so these are compute-bound register-tiled FMA GEMMs:
-// a TF32 tensor-core product (10-bit mantissa) would miss the 1e-5 bar, and the 3xTF32 split is future work.
+// ~10 flop/B at which the FP32 FMA pipe saturates, so these are compute-bound register-tiled FMA GEMMs.  They are the
+// path for the shapes the tcgen05 3xTF32 kernels (tt_gemm32_umma.cu) do not take: k not a multiple of 16, and the
+// adjoint with N_d > 128.
 // Operands are staged in shared memory with a 2-stage cp.async pipeline; all sums have a fixed order.
 #include "tt_common.cuh"
 #include "tt_internal.h"

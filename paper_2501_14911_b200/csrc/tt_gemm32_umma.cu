@@ -1,5 +1,5 @@
-// tt_gemm32_umma.cu - the per-frequency complex64 GEMMs of TT_F32 plans with 32 right-hand sides on the 5th-generation
-// tensor cores (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423).
+// tt_gemm32_umma.cu - the per-frequency complex64 GEMMs of TT_F32 plans with k right-hand sides (k a multiple of 16; 32 or
+// 16 columns per launch, written for 32 below) on the 5th-generation tensor cores (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423).
 //
 // forward   Dhat_w [N_d x k] = Fhat_w [N_d x N_m] * Xhat_w [N_m x k],  k = 32, as ONE real product per CTA tile
 //
@@ -22,7 +22,7 @@
 //               (two accumulators alternate) into fp32 register sums (round-to-nearest), as in tt_kdirect_umma.cu
 //
 // grid (p-splits, n_f, sensor tiles); the partial sums go through reduce_partials_kernel like those of the FMA kernel
-// (tt_gemm32.cu), which stays the path for k != 32.
+// (tt_gemm32.cu), which stays the path for every other k and, for the adjoint, for N_d > 128.
 #include "tt_common.cuh"
 #include "tt_internal.h"
 #include "tt_umma.cuh"
