@@ -919,8 +919,39 @@ def measure(ctx, args, w, cfg_name, *, steps, warmup, headline):
                                "ms_per_launch": adj[1], "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
             "kernels": describe,
         }
+    elif w.dtype == torch.float32 and K % 16 == 0:
+        # fp32 k-RHS, k a multiple of 16: per-frequency complex64 GEMMs on tcgen05 kind::tf32 with three MMAs per product
+        # (3xTF32, tt_gemm32_umma.cu): a dense contraction, bound "tensor".  Tensor work = 3 x the algorithmic flops; the
+        # tf32 peak is the measured bf16 figure of MEASURED_PEAKS.json x the guide's nominal tf32/bf16 ratio.  These GEMMs
+        # are short and fat (N_d x 2k outputs per frequency): each also streams Fhat and the k spectra once, and that HBM
+        # time is reported beside the tensor fraction - it is the nearer bound at the paper's shapes.
+        peaks, _ = measured_peaks()
+        bf16 = peaks.get("bf16_tflops_sustained") or peaks.get("bf16_tflops")
+        peak_t = bf16 * (1.1 / 2.25) if bf16 else None
+        flops = 8.0 * n_f * w.N_d * w.N_m * K
+        hbm_bytes = fhat_bytes + n_f * w.N_m * K * 8
+        ach_fwd = 3.0 * flops / (fwd[1] * 1e-3) / 1e12 if fwd[1] > 0 else 0.0
+        ach_adj = 3.0 * flops / (adj[1] * 1e-3) / 1e12 if adj[1] > 0 else 0.0
+        adj_umma = w.N_d <= 128
+        roofline = {
+            "bound": "tensor", "kernel": "gemm32_umma_fwd_kernel (k-RHS A2: per-frequency complex64 GEMM, tcgen05.mma kind::tf32, "
+                                         "A from tensor memory, 3 MMAs per fp32 product)",
+            "achieved": ach_fwd, "peak": peak_t, "unit": "TFLOP/s", "frac": ach_fwd / peak_t if peak_t else None, "traffic": None,
+            "peak_kind": "MEASURED_PEAKS.json bf16_tflops(_sustained) x nominal tf32/bf16 ratio 1.1/2.25" if bf16 else "no measured peak",
+            "effective_fp32_TFLOPs": flops / (fwd[1] * 1e-3) / 1e12 if fwd[1] > 0 else 0.0,
+            "algorithmic_flops_per_launch": flops, "tensor_flops_per_launch": 3.0 * flops, "ms_per_launch": fwd[1],
+            "launches_timed": fwd[3], "hbm_bytes_per_launch": hbm_bytes,
+            "hbm_GBs": hbm_bytes / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0,
+            "hbm_frac_of_copy_peak": hbm_bytes / (fwd[1] * 1e-3) / 1e9 / peak if fwd[1] > 0 else None,
+            "adjoint_kernel": {"kernel": "gemm32_umma_adj_kernel (k-RHS B2, tcgen05, TMA-stored tiles)" if adj_umma
+                                         else "gemm32_adj_kernel (k-RHS B2, FP32 FMA: N_d > 128)",
+                               "achieved": ach_adj if adj_umma else ach_adj / 3.0,
+                               "frac": (ach_adj / peak_t if peak_t else None) if adj_umma else None,
+                               "effective_fp32_TFLOPs": flops / (adj[1] * 1e-3) / 1e12 if adj[1] > 0 else 0.0,
+                               "ms_per_launch": adj[1], "hbm_GBs": hbm_bytes / (adj[1] * 1e-3) / 1e9 if adj[1] > 0 else 0.0},
+        }
     elif w.dtype == torch.float32:
-        # fp32 k-RHS: register-tiled complex64 FMA GEMMs (tt_gemm32.cu), bound by the FP32 FMA pipe.  Peak derived from the
+        # fp32 k-RHS, k not a multiple of 16: register-tiled complex64 FMA GEMMs (tt_gemm32.cu), bound by the FP32 FMA pipe.  Peak derived from the
         # unit counts of the guide: 148 SMs x 128 FP32 FMA lanes x 2 flop x the SM clock sampled during this run.
         clk = clocks.summary().get("sm_mhz") or 1965.0
         peak32 = 148 * 128 * 2 * clk * 1e6 / 1e12
@@ -1099,7 +1130,7 @@ def main() -> int:
     ap.add_argument("--k-batch", type=int, default=1, help="--online: right-hand sides per batched call in tt_assemble_K")
     ap.add_argument("--k-rhs", type=int, default=0,
                     help="run the k-RHS batched calls with k right-hand sides on any config (default: the config's own, "
-                         "32 for C4, else 1); fp32 configs then take the complex64 FMA GEMM path")
+                         "32 for C4, else 1); fp32 configs then take the complex64 GEMM path (tcgen05 for k a multiple of 16)")
     ap.add_argument("--out-every", type=int, default=0,
                     help="data side on every r-th time step (tt_plan_create_coarse); default 10 for Q5 (the p2q map), else 1")
     ap.add_argument("--no-cpu-baseline", action="store_true")
