@@ -76,7 +76,8 @@ typedef enum tt_status {
     TT_ERR_CUDA = -9,           /* any other CUDA runtime error (see tt_plan_last_cuda_error) */
     TT_ERR_NO_DEVICE = -10,     /* no CUDA device / wrong architecture: there is no CPU path */
     TT_ERR_NOT_SPD = -11,       /* tt_chol_create: a diagonal entry of the factor is not positive and finite */
-    TT_ERR_MISMATCH = -12       /* plans / factor / vectors of one call disagree in shape, dtype or layout */
+    TT_ERR_MISMATCH = -12,      /* plans / factor / vectors of one call disagree in shape, dtype or layout */
+    TT_ERR_STATIC_LIMIT = -13   /* tt_assemble_K_direct_static: the problem does not fit the library's static scratch */
 } tt_status;
 
 /* Library version, major*10000 + minor*100 + patch. */
@@ -254,6 +255,23 @@ int tt_assemble_K(const tt_plan* F, const tt_plan* G, const void* noise_var, int
  * no synchronisation, TT_ERR_OOM if the device cannot provide it. */
 int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m, int64_t N_t,
                          int dtype, void* K, int64_t ldk, void* stream);
+
+/* tt_assemble_K_direct for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same kernels, same result, TT_F32 only (TT_ERR_DTYPE otherwise - the TT_F64 path of
+ * tt_assemble_K_direct has no scratch), and NO cudaMalloc / cudaMallocAsync / cudaFree or allocating library call on any path.
+ * The scratch (hi / lo tf32 parts of one slab of both block columns, 16 n bytes per parameter of the slab, plus the tile list)
+ * lives in a static device array of 64 MiB inside libtt.so, which every GPU that loads the library holds until the process
+ * exits.  The slab is min(8192, what fits) parameters, a multiple of 32; the call returns TT_ERR_STATIC_LIMIT, having launched
+ * nothing, when fewer than min(128, N_m rounded up to 32) parameters fit:
+ *     16 n * 128 + 8 * ceil(n/128) * ceil(n/256) (rounded up to 256)  <=  64 MiB,   i.e. n = N_t*N_d <= ~32 700
+ * (n = 24 500, the paper's shape, runs with slabs of 160 parameters: more fp64 passes over K than the 8192 of the allocating
+ * call, same accuracy bound).  Smaller slabs change the fp32/fp64 summation split, so results agree with
+ * tt_assemble_K_direct to rounding (~1e-6 relative), not bit for bit, unless both use the same slab.
+ * All calls on a device share the one array and it keeps the previous call's contents; nothing in it needs to start at zero
+ * (each slab pass rewrites what it reads).  Calls that overlap on the GPU - different streams, or graphs replayed
+ * concurrently - RACE on it: serialise them.  Asynchronous on `stream`. */
+int tt_assemble_K_direct_static(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m, int64_t N_t,
+                                int dtype, void* K, int64_t ldk, void* stream);
 
 /* The N_m-sharded assembly: F G* is a SUM over parameter slices, so every rank calls
  * tt_assemble_K_direct on its own slices Fcol[:, :, P_g], Gcol[:, :, P_g] with noise_var == NULL (F G* alone), the partial

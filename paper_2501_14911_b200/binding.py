@@ -86,6 +86,7 @@ def lib() -> ctypes.CDLL:
         "tt_chol_trsv": (ci, [vp, ci, vp, vp, vp]),
         "tt_assemble_K": (ci, [vp, vp, vp, i64, i64, vp, i64, vp]),
         "tt_assemble_K_direct": (ci, [vp, vp, vp, i64, i64, i64, ci, vp, i64, vp]),
+        "tt_assemble_K_direct_static": (ci, [vp, vp, vp, i64, i64, i64, ci, vp, i64, vp]),
         "tt_K_add_noise": (ci, [vp, i64, ci, vp, i64, vp]),
         "tt_qoi_direct": (ci, [vp, vp, vp, i64, i64, i64, i64, i64, ci, vp, vp, i64, vp, i64, vp]),
         "tt_map_create": (ci, [pp, vp, vp, vp, vp, vp]),
@@ -111,7 +112,7 @@ EXPORTS = ["tt_version", "tt_status_string", "tt_plan_create", "tt_plan_create_c
            "tt_matvec_batched", "tt_rmatvec_batched", "tt_normal_batched", "tt_matvec_host", "tt_rmatvec_host", "tt_normal_host",
            "tt_plan_set_profiling", "tt_plan_stage_ms",
            "tt_chol_create", "tt_chol_destroy", "tt_chol_device_bytes", "tt_chol_last_cuda_error", "tt_chol_solve",
-           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_K_add_noise", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
+           "tt_chol_trsv", "tt_assemble_K", "tt_assemble_K_direct", "tt_assemble_K_direct_static", "tt_K_add_noise", "tt_qoi_direct", "tt_map_create", "tt_map_destroy", "tt_map_infer", "tt_map_infer_host",
            "tt_map_infer_partial", "tt_map_infer_finish", "tt_smw_apply",
            "tt_postcov_q_apply", "tt_d2q_apply"]
 
@@ -552,6 +553,14 @@ def assemble_K(F: Plan, G: Plan, noise_var: torch.Tensor, cols: tuple[int, int] 
     col0, ncols = cols if cols is not None else (0, n)
     tt_assemble_K(F.handle, G.handle, noise_var, col0, ncols, K, K.stride(0), stream)
     return K
+
+
+def tt_assemble_K_direct_static(Fcol, Gcol, noise_var, N_d: int, N_m: int, N_t: int, dtype: int, K, ldk: int, stream=None) -> None:
+    """tt_assemble_K_direct without any allocation (TT_F32; scratch in a 64 MiB static device array; TT_ERR_STATIC_LIMIT = -13
+    when the problem does not fit)."""
+    nv = None if noise_var is None else _ptr(noise_var)
+    _check("tt_assemble_K_direct_static", lib().tt_assemble_K_direct_static(_ptr(Fcol), _ptr(Gcol), nv, N_d, N_m, N_t, dtype,
+                                                                              _ptr(K), ldk, _stream(stream)))
 
 
 def assemble_K_direct(Fcol: torch.Tensor, Gcol: torch.Tensor, noise_var: torch.Tensor | None, out: torch.Tensor | None = None,

@@ -504,6 +504,7 @@ const char* tt_status_string(int status) {
         case TT_ERR_NO_DEVICE: return "TT_ERR_NO_DEVICE";
         case TT_ERR_NOT_SPD: return "TT_ERR_NOT_SPD";
         case TT_ERR_MISMATCH: return "TT_ERR_MISMATCH";
+        case TT_ERR_STATIC_LIMIT: return "TT_ERR_STATIC_LIMIT";
         default: return "TT_ERR_UNKNOWN";
     }
 }

@@ -144,6 +144,9 @@ cudaError_t trsv_copy_launch(const double* src, double* dst, long long n, cudaSt
 // fp32 C (fp64) = A B^T on tcgen05 (3 x tf32 split, TMA-fed, accumulators in tensor memory): tt_kdirect_umma.cu
 cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA, long long nB, long long Kdim, long long ldc,
                          int lower_only, cudaStream_t s);
+// the same with the scratch in a static device array (no allocation); *fits = 0 and no launch if the problem is too large for it
+cudaError_t kd_umma_gemm_static(const float* A, const float* B, double* C, long long nA, long long nB, long long Kdim, long long ldc,
+                                int lower_only, cudaStream_t s, int* fits);
 void kd_umma_debug_set_slab(int ks);  // parameters accumulated in tensor memory between fp64 flushes (0 = default)
 
 

@@ -319,6 +319,41 @@ extern "C" int tt_assemble_K_direct(const void* Fcol, const void* Gcol, const vo
     return TT_OK;
 }
 
+// tt_assemble_K_direct for TT_F32 without any allocation: the same kernels, the GEMM's scratch in a static device array
+// (kd_umma_gemm_static, tt_kdirect_umma.cu).
+extern "C" int tt_assemble_K_direct_static(const void* Fcol, const void* Gcol, const void* noise_var, int64_t N_d, int64_t N_m,
+                                           int64_t N_t, int dtype, void* K, int64_t ldk, void* stream) {
+    using namespace tt;
+    if (!Fcol || !Gcol || !K) return TT_ERR_NULL;
+    if (dtype != TT_F32) return TT_ERR_DTYPE;        // the TT_F64 path of tt_assemble_K_direct has no scratch to begin with
+    if (N_d < 1 || N_m < 1 || N_t < 1 || N_d > 65535) return TT_ERR_SHAPE;
+    const long long n = N_d * N_t;
+    if (ldk < n || n > (1LL << 24)) return TT_ERR_SHAPE;
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return TT_ERR_NO_DEVICE;
+    }
+    if (major != 10) return TT_ERR_NO_DEVICE;   // built for sm_100a only
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    double* Kd = static_cast<double*>(K);
+    int fits = 0;
+    cudaError_t e = kd_umma_gemm_static(static_cast<const float*>(Fcol), static_cast<const float*>(Gcol), Kd, n, n, N_m, ldk, 1, s, &fits);
+    if (e == cudaSuccess && !fits) return TT_ERR_STATIC_LIMIT;
+    if (e == cudaSuccess) {
+        const long long chains = n * N_d;
+        kd_diag_kernel<float><<<(unsigned)((chains + 255) / 256), 256, 0, s>>>(Kd, static_cast<const float*>(noise_var), n, (int)N_d, ldk);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        const unsigned nt = (unsigned)((n + 31) / 32);
+        kd_mirror_kernel<<<dim3(nt, nt), 256, 0, s>>>(Kd, n, ldk);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return TT_ERR_CUDA; }
+    return TT_OK;
+}
+
 // K[a][a] += noise_var[a]
 template <typename R>
 __global__ void __launch_bounds__(256)

@@ -27,12 +27,19 @@
 //                     Slab sums meet in fp64 in C in a fixed order (slab after slab on one stream): bit-reproducible.
 #include <cuda.h>
 
+#include <mutex>
 #include <new>
 
 #include "../../include/tt.h"
 #include "tt_common.cuh"
 #include "tt_internal.h"
 #include "tt_umma.cuh"
+
+// Scratch of kd_umma_gemm_static (the entry point tt_assemble_K_direct_static, which may not allocate): a fixed 64 MiB of
+// device memory that every GPU loading this library holds until the process exits.  In HOST code this name is only a
+// stand-in for the symbol - the device address comes from cudaGetSymbolAddress, once per device (static_scratch() below).
+constexpr size_t kStaticScratchBytes = (size_t)64 << 20;
+static __device__ __align__(256) unsigned char g_kd_static_scratch[kStaticScratchBytes];
 
 namespace tt {
 namespace {
@@ -342,6 +349,86 @@ cudaError_t kd_umma_gemm(const float* A, const float* B, double* C, long long nA
     }
     cudaFreeAsync(d_tiles, s);
     cudaFreeAsync(scratch, s);
+    return e;
+}
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+
+// Device address of g_kd_static_scratch on the CURRENT device; looked up once per device, with that device current.
+cudaError_t static_scratch(unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* ptrs[kMaxDevices] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_kd_static_scratch);
+        if (e != cudaSuccess) return e;
+        ptrs[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = ptrs[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+// kd_umma_gemm with its scratch (hi / lo planes of one slab of A and B, the tile list) in g_kd_static_scratch instead of the
+// stream-ordered allocator: no cudaMalloc* / cudaFree* of any kind.  The slab shrinks until the planes fit (at least 128
+// parameters, or all of them); *fits = 0 and nothing is launched when even that does not fit.  Nothing in the scratch has to
+// start at zero: every slab pass rewrites the part of the planes it reads (the split kernel zero-fills up to the K-block) and
+// the tile list is rebuilt per call.  All calls on a device share the array: calls that overlap on the GPU race.
+cudaError_t kd_umma_gemm_static(const float* A, const float* B, double* C, long long nA, long long nB, long long Kdim,
+                                long long ldc, int lower_only, cudaStream_t s, int* fits) {
+    *fits = 0;
+    constexpr int bk = 32;
+    const int tm_n = (int)((nA + kBM - 1) / kBM), tn_n = (int)((nB + kBN - 1) / kBN);
+    const long long n_tiles_ll = kd_tile_order(nullptr, tm_n, tn_n, lower_only);
+    if (n_tiles_ll > 0x7fffffffLL) return cudaSuccess;
+    const int n_tiles = (int)n_tiles_ll;
+    const long long kfull = (Kdim + kMaxBK - 1) / kMaxBK * kMaxBK;
+    const long long tiles_bytes = ((long long)n_tiles * (long long)sizeof(int2) + 255) / 256 * 256;
+    const long long row_bytes = 4 * (2 * nA + 2 * nB);                     // bytes of the four planes per parameter
+    long long ks_max = ((long long)kStaticScratchBytes - tiles_bytes) / row_bytes / kMaxBK * kMaxBK;
+    if (ks_max > 8192) ks_max = 8192;
+    if (ks_max > kfull) ks_max = kfull;
+    if (ks_max < (kfull < 128 ? kfull : 128)) return cudaSuccess;          // does not fit
+    *fits = 1;
+
+    unsigned char* base = nullptr;
+    cudaError_t e = static_scratch(&base);
+    if (e != cudaSuccess) return e;
+    const long long pitch = ks_max;
+    const size_t plane_a = (size_t)nA * pitch, plane_b = (size_t)nB * pitch;
+    float* a_hi = reinterpret_cast<float*>(base);
+    float *a_lo = a_hi + plane_a, *b_hi = a_hi + 2 * plane_a, *b_lo = b_hi + plane_b;
+    int2* d_tiles = reinterpret_cast<int2*>(base + kStaticScratchBytes - tiles_bytes);
+    kd_tiles_kernel<<<1, 32, 0, s>>>(d_tiles, tm_n, tn_n, lower_only);
+
+    CUtensorMap mA_hi, mA_lo, mB_hi, mB_lo;
+    if (!(make_map(&mA_hi, a_hi, nA, (int)ks_max, pitch, kBM, bk) && make_map(&mA_lo, a_lo, nA, (int)ks_max, pitch, kBM, bk) &&
+          make_map(&mB_hi, b_hi, nB, (int)ks_max, pitch, kBN, bk) && make_map(&mB_lo, b_lo, nB, (int)ks_max, pitch, kBN, bk)))
+        return cudaErrorInvalidValue;
+    constexpr int smem = Geo<bk>::kSmemBytes;
+    e = cudaFuncSetAttribute(kd_umma_kernel<bk>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    int dev = 0, sms = 148;
+    if (e == cudaSuccess) e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int grid = n_tiles < sms ? n_tiles : sms;
+    for (long long k0 = 0; e == cudaSuccess && k0 < Kdim; k0 += ks_max) {
+        const int ks = (int)(Kdim - k0 < ks_max ? Kdim - k0 : ks_max);
+        const int kpad = (ks + kMaxBK - 1) / kMaxBK * kMaxBK;
+        const dim3 ga((unsigned)((nA + 7) / 8), (unsigned)((kpad + 1023) / 1024)), gb((unsigned)((nB + 7) / 8), ga.y);
+        kd_split_kernel<<<ga, 256, 0, s>>>(A, nA, Kdim, k0, ks, kpad, a_hi, a_lo, pitch);
+        kd_split_kernel<<<gb, 256, 0, s>>>(B, nB, Kdim, k0, ks, kpad, b_hi, b_lo, pitch);
+        UmmaArgs g{d_tiles, n_tiles, kpad / bk, C, nA, nB, ldc, k0 == 0 ? 1 : 0};
+        kd_umma_kernel<bk><<<grid, kThreads, smem, s>>>(mA_hi, mA_lo, mB_hi, mB_lo, g);
+        e = cudaGetLastError();
+    }
     return e;
 }
 
