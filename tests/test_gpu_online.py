@@ -129,7 +129,7 @@ ONLINE_SHAPES = [(3, 40, 12), (6, 400, 50), (5, 1000, 35), (1, 64, 20), (4, 2100
 
 @pytest.mark.parametrize("N_d,N_m,N_t", ONLINE_SHAPES)
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
-@pytest.mark.parametrize("k_max", [1, 8])
+@pytest.mark.parametrize("k_max", [1, 8, 16, 32])      # 16, 32: the fp32 groups take the tcgen05 GEMMs, the ragged last group the FMA ones
 def test_assemble_K(tt, N_d, N_m, N_t, dtype, k_max):
     w, F, G, nv, _ = online_inputs(N_d, N_m, N_t, dtype)
     K_ref = oo.assemble_K(F.numpy(), G.numpy(), nv.numpy())
