@@ -155,7 +155,10 @@ int tt_normal(const tt_plan* plan, const void* m, void* out, void* stream);
 
 /* k-RHS variants, 1 <= k <= k_max: column r of the result equals the single-vector result
  * on column r.  The per-frequency products are complex GEMMs (N_d x N_m)(N_m x k) and
- * (N_m x N_d)(N_d x k).
+ * (N_m x N_d)(N_d x k): TT_F64 on the FP64 tensor instruction (DMMA); TT_F32 with k a multiple of 16 on the 5th-generation
+ * tensor cores (tcgen05.mma kind::tf32, every fp32 product from the hi/lo tf32 parts of its factors; the adjoint for N_d <= 128),
+ * any other k as register-tiled FP32 FMA GEMMs - several times slower, so callers that can choose k should take 16 or 32.
+ * All three forms meet the same 1e-5 (fp32) / 1e-12 (fp64) bar against the single-vector result.
  *   M  DEVICE, N_t*N_m*k reals;   D  DEVICE, N_t*N_d*k reals (layouts above). */
 int tt_matvec_batched(const tt_plan* plan, int k, const void* M, void* D, void* stream);
 int tt_rmatvec_batched(const tt_plan* plan, int k, const void* D, void* M, void* stream);
