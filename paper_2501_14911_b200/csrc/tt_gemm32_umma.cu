@@ -1,5 +1,6 @@
-// tt_gemm32_umma.cu - the per-frequency complex64 GEMMs of TT_F32 plans with k right-hand sides (k a multiple of 16; 32 or
-// 16 columns per launch, written for 32 below) on the 5th-generation tensor cores (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423).
+// tt_gemm32_umma.cu - the per-frequency complex64 GEMMs of TT_F32 plans with k right-hand sides on the 5th-generation tensor
+// cores (step D of DESIGN.md for fp32; the many-matvec workloads of PAPER.md:296, 407, 421-423).  k a multiple of 16: 32 or 16
+// columns per launch (template parameter kN = floats per row of the column group); the comments below are written for 32.
 //
 // forward   Dhat_w [N_d x k] = Fhat_w [N_d x N_m] * Xhat_w [N_m x k],  k = 32, as ONE real product per CTA tile
 //
