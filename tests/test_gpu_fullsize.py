@@ -194,6 +194,50 @@ def test_c4_krhs_whole_columns(tt):
             assert rel(got_d[r][:, s], ref_d[r][:, s]) <= 1e-12, f"F M, sensor {s}, column {r}"
 
 
+def test_p5_quarter_krhs_fp32_whole_columns(tt):
+    """The fp32 k-RHS path (3xTF32 GEMMs on tcgen05, tt_gemm32_umma.cu) at the paper's sensor and time counts (49 sensors, 500
+    steps, 501 frequencies) and a quarter of its parameters (65 792: 13 GB spectrum, 2056 K-blocks per frequency, 514 parameter
+    tiles): columns 0 and 31 of F M and of F^T D over every sensor and every parameter against the oracle, all 32 columns through
+    the adjoint identity.  (P5 with k = 32 is not a BASELINE.json config: this is the size the oracle does in half a minute.)"""
+    import time
+    w = synth.CONFIGS["P5"].scaled(N_m=65792, k_rhs=32)
+    need_memory(60)
+    k = w.k_rhs
+    F = synth.block_column(w, device="cuda")
+    M, D = synth.vector_m(w, device="cuda"), synth.vector_d(w, device="cuda")   # [N_t, N_m, k], [N_t, N_d, k]
+    cols = [0, k - 1]
+    plan = tt.Plan(F, k_max=k)
+    try:
+        FM = plan.matvec_batched(M)
+        FtD = plan.rmatvec_batched(D)
+        torch.cuda.synchronize()
+    finally:
+        plan.close()
+    lhs, rhs = float((FM.double() * D.double()).sum()), float((M.double() * FtD.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * float(FM.double().norm() * D.double().norm())   # <F M, D> = <M, F^T D>, all columns
+    got_d = {r: FM[..., r].contiguous().cpu().numpy() for r in cols}
+    got_m = {r: FtD[..., r].contiguous().cpu().numpy() for r in cols}
+    m_r = {r: M[..., r].contiguous().cpu().numpy() for r in cols}
+    d_r = {r: D[..., r].contiguous().cpu().numpy() for r in cols}
+    del FM, FtD, M, D
+    torch.cuda.empty_cache()
+    Fh = F.cpu().numpy()
+    del F
+    t0 = time.perf_counter()
+    errs = []
+    for r in cols:
+        ref_d, ref_m = ob.matvec(Fh, m_r[r]), ob.rmatvec(Fh, d_r[r])
+        errs.append((rel(got_d[r], ref_d), rel(got_m[r], ref_m)))
+        for s in range(w.N_d):
+            assert rel(got_d[r][:, s], ref_d[:, s]) <= 1e-5, f"F M, sensor {s}, column {r}"
+        for p0 in range(0, w.N_m, 4096):
+            assert rel(got_m[r][:, p0:p0 + 4096], ref_m[:, p0:p0 + 4096]) <= 1e-5, f"F^T D, parameters {p0}.., column {r}"
+    print(f"P5/4 fp32 k-RHS whole columns {cols} rel-L2 vs the oracle (oracle {time.perf_counter() - t0:.0f} s): "
+          + "  ".join(f"[F M {a:.2e}, F^T D {b:.2e}]" for a, b in errs))
+    for r, (a, b) in zip(cols, errs):
+        assert a <= 1e-5 and b <= 1e-5, f"column {r}: {a}, {b}"
+
+
 # ------------------------------------------------------------------------------------------------
 # Online phase (SURVEY.md 8(f) rows 1-2) at sizes beyond tests/test_gpu_online.py
 # ------------------------------------------------------------------------------------------------
