@@ -166,9 +166,11 @@ int tt_rmatvec_batched(const tt_plan* plan, int k, const void* D, void* M, void*
 int tt_normal_batched(const tt_plan* plan, int k, const void* M, void* Out, void* stream);
 
 /* The same calls with HOST vectors (pinned memory recommended; what bench.py's `e2e` times).  The parameter-sized
- * vector crosses PCIe in 16 ranges of the parameter axis on a copy stream owned by the plan, overlapped with the kernels
+ * vector crosses PCIe in ranges of the parameter axis on a copy stream owned by the plan, overlapped with the kernels
  * of the neighbouring range on `stream` (H2D of range c+1 under the FFT + matvec of range c; D2H of range c under the
- * matvec + inverse FFT of range c+1); `stream` waits for the last copy, so synchronising it is enough.  Results are
+ * matvec + inverse FFT of range c+1); `stream` waits for the last copy, so synchronising it is enough.  The planner picks
+ * the ranges from the shape: where the kernels of a range take longer than its copy (N_d above ~65) 8 ranges in a geometric
+ * sequence with the small one at the exposed end (first for F m, last for F^T d), otherwise 16 equal ones.  Results are
  * bit-identical to the device-pointer calls.  The staging buffers, the copy stream and its events are created on first
  * use (the only apply-time allocation in the library) and freed with the plan. */
 int tt_matvec_host(const tt_plan* plan, const void* m_host, void* d_host, void* stream);

@@ -44,7 +44,8 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
  * "gemm32_fwd" = tile variant of the fp32 k-RHS forward GEMM (1, 2; 0 = planner's choice),
  * "gemm_adj_mt" = m-tiles per warp of the fp64 k-RHS adjoint GEMM (1, 2; 0 = default),
  * "kd_slab" = parameters per slab of the fp32 direct K assembly (multiple of 32; 0 = 8192),
- * "host_chunks" = parameter ranges of the pipelined *_host calls (1..32; default 16).
+ * "host_chunks" = parameter ranges of the pipelined *_host calls (1..32; 0 = planner's choice: 8 graded or 16 equal ones),
+ * "host_growth" = size of each of those ranges in percent of the one before (1..400; 0 = planner's choice).
  * Returns TT_ERR_SHAPE for an unknown key. */
 int tt_debug_set(const char* key, int value);
 

@@ -21,7 +21,8 @@ constexpr int kVersion = 100;  // 0.1.0
 constexpr int kRing = 64;       // profiled apply calls remembered
 constexpr int kSlotEvents = 8;  // two kernel triples (tt_normal) x 4 marks
 constexpr int kMaxHostChunks = 32;  // most parameter ranges the pipelined *_host calls can use
-int g_host_chunks = 16;             // ranges in use (tt_debug_set("host_chunks"))
+int g_host_chunks = 0;              // ranges in use (tt_debug_set("host_chunks")); 0 = planner's choice
+int g_host_growth = 0;              // tt_debug_set("host_growth"): each range this many percent of the one before; 0 = planner's choice
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
 int g_gemv_chunk = 0;  // tt_debug_set("gemv_chunk"): 0 = planner's choice
@@ -375,17 +376,53 @@ int ensure_staging(const tt_plan* cp) {
     return TT_OK;
 }
 
-// Parameter range c of the pipelined host calls: boundaries on multiples of lcm(GEMV chunk, 512) - the forward kernel
+// Parameter ranges of the pipelined host calls: boundaries on multiples of lcm(GEMV chunk, 512) - the forward kernel
 // derives its chunk index from p_begin / chunk, the adjoint kernel works on 512-parameter tiles, and both are multiples of
 // the 16-element row pitch (4096 for the planner's chunks of 2048 / 4096); the last range ends at ldp.
-void host_chunk(const tt_plan* p, int c, long long* p0, long long* p1) {
+// Per parameter the copy moves N_t reals over PCIe (~54 GB/s measured for the strided 2-D copies, with or without a
+// saturating kernel beside them) and the kernels stream (N_t + 1) N_d complex numbers (~7 TB/s): the ratio
+// q = (kernel time) / (copy time) ~ 65 / N_d in either precision decides the shape of the pipeline.
+//   q > 1 (C3, C5: the kernels are the longer leg): 8 ranges in a geometric sequence of ratio min(q, 1.6).  F m starts with
+//     the SMALL range (little copy time exposed before the first kernel) and goes on with few large ones (every A2 launch
+//     ends in a partial wave: 16 equal ranges cost A2 0.8 ms at C3); F^T d runs the sequence backwards (small LAST range:
+//     little copy time exposed after the last kernel).  F m + F^T d from host vectors 25.86 -> 25.13 ms at C3,
+//     20.22 -> 19.54 ms at C5.
+//   q <= 1 (the paper's shape, N_d = 49: the copies are the longer leg, back to back at link speed): 16 equal ranges -
+//     what is exposed is one range of kernels, and graded sequences were measured slower there (20.5 against 22.1 ms).
+// start[c] .. start[c+1] is range c; returns the number of ranges.
+constexpr double kHostLinkGBs = 54.0, kStreamGBs = 7000.0;
+int host_ranges(const tt_plan* p, bool ascending, long long* start) {
     long long a = p->chunk, b = 512;
     while (b) { const long long t = a % b; a = b; b = t; }
     const long long unit = (long long)p->chunk / a * 512;
-    long long per = (p->ldp + g_host_chunks - 1) / g_host_chunks;
-    per = (per + unit - 1) / unit * unit;
-    *p0 = per * c < p->ldp ? per * c : p->ldp;
-    *p1 = per * (c + 1) < p->ldp ? per * (c + 1) : p->ldp;
+    const long long U = (p->ldp + unit - 1) / unit;          // units to distribute
+    const double q_model = ((double)p->n_f * (double)p->N_d * 2.0 / kStreamGBs) / ((double)p->N_t / kHostLinkGBs);
+    long long want = g_host_chunks > 0 ? g_host_chunks : q_model > 1.0 ? 8 : 16;
+    int n = want < U ? (int)want : (int)U;
+    if (n < 1) n = 1;
+    double q = g_host_growth > 0 ? g_host_growth / 100.0 : q_model;
+    if (g_host_growth <= 0) q = q > 1.6 ? 1.6 : q < 1.0 ? 1.0 : q;
+    double wsum = 0.0, w = 1.0;
+    for (int c = 0; c < n; ++c) { wsum += w; w *= q; }
+    long long cnt[kMaxHostChunks];
+    long long used = 0;
+    w = 1.0;
+    for (int c = 0; c < n; ++c) {
+        long long u = (long long)std::floor((double)U * w / wsum);
+        if (u < 1) u = 1;
+        cnt[c] = u; used += u; w *= q;
+    }
+    for (int c = n - 1; used != U; c = c > 0 ? c - 1 : n - 1) {   // rounding remainder: to the large end first
+        if (used < U) { ++cnt[c]; ++used; }
+        else if (cnt[c] > 1) { --cnt[c]; --used; }
+    }
+    long long at = 0;
+    for (int c = 0; c < n; ++c) {
+        start[c] = at * unit < p->ldp ? at * unit : p->ldp;
+        at += ascending ? cnt[c] : cnt[n - 1 - c];
+    }
+    start[n] = p->ldp;
+    return n;
 }
 
 // Copy of the parameters [p0, p1) of a parameter-sized vector between host and device staging (either direction).
@@ -411,9 +448,10 @@ int run_matvec_from_host(const tt_plan* p, const void* m_host, void* d_dev, cuda
     const VecView vm = view(p, p->N_m, p->N_t, 1, 0), vd = view(p, p->N_d, p->N_td, 1, 0);
     TT_CUDA(p, cudaEventRecord(p->cev[kMaxHostChunks], s));                 // the staging buffer is free once s gets here
     TT_CUDA(p, cudaStreamWaitEvent(p->copy_stream, p->cev[kMaxHostChunks], 0));
-    for (int c = 0; c < g_host_chunks; ++c) {
-        long long p0, p1;
-        host_chunk(p, c, &p0, &p1);
+    long long start[kMaxHostChunks + 1];
+    const int n_ranges = host_ranges(p, true, start);
+    for (int c = 0; c < n_ranges; ++c) {
+        const long long p0 = start[c], p1 = start[c + 1];
         if (p1 <= p0) continue;
         TT_CUDA(p, copy_m_range(p, p->m_stage, m_host, p0, p1, cudaMemcpyHostToDevice, p->copy_stream));
         TT_CUDA(p, cudaEventRecord(p->cev[c], p->copy_stream));
@@ -452,9 +490,10 @@ int run_rmatvec_to_host(const tt_plan* p, const void* d_dev, void* m_host, cudaS
     P.r_ys = 0; P.r_bs = vd.bs; P.r_ts = vd.ts; P.dec = (int)p->dec;
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->N_d;
     TT_CUDA(p, fft_r2c_launch(t, t, t, d_dev, p->dhat, P, 1, s));
-    for (int c = 0; c < g_host_chunks; ++c) {
-        long long p0, p1;
-        host_chunk(p, c, &p0, &p1);
+    long long start[kMaxHostChunks + 1];
+    const int n_ranges = host_ranges(p, false, start);
+    for (int c = 0; c < n_ranges; ++c) {
+        const long long p0 = start[c], p1 = start[c + 1];
         if (p1 <= p0) continue;
         GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
         g.p_begin = p0; g.p_end = p1;
@@ -888,8 +927,13 @@ int tt_debug_set(const char* key, int value) {
     if (!std::strcmp(key, "fft_no_static")) { fft_debug_no_static(value); return TT_OK; }
     if (!std::strcmp(key, "gemv_chunk")) { g_gemv_chunk = value; return TT_OK; }
     if (!std::strcmp(key, "host_chunks")) {
-        if (value < 1 || value > kMaxHostChunks) return TT_ERR_SHAPE;
+        if (value < 0 || value > kMaxHostChunks) return TT_ERR_SHAPE;
         g_host_chunks = value;
+        return TT_OK;
+    }
+    if (!std::strcmp(key, "host_growth")) {
+        if (value < 0 || value > 400) return TT_ERR_SHAPE;
+        g_host_growth = value;
         return TT_OK;
     }
     if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }

@@ -75,7 +75,7 @@ def _whole_vector(tt, cfg):
     The block column stays on the device and is streamed to the host in sensor slabs F[:, s0:s1, :]: each slab gives
     complete rows d[:, s0:s1] of oracle.matvec and one term of oracle.rmatvec, accumulated in fp64 (the sum over sensors
     of the definition, split at slab boundaries).  The normal operator's reference has the oracle on both halves:
-    rmatvec(F, matvec(F, m)), the intermediate kept in fp64.  The *_host calls (pipelined over 16 parameter ranges, whose
+    rmatvec(F, matvec(F, m)), the intermediate kept in fp64.  The *_host calls (pipelined over 8 graded or 16 equal parameter ranges, whose
     boundaries only exist at this size) must reproduce the device-pointer calls bit for bit."""
     import time
     w = synth.CONFIGS[cfg]

@@ -335,6 +335,33 @@ def test_host_vector_calls(tt, dtype):
         plan.close()
 
 
+@pytest.mark.parametrize("n_ranges,growth", [(0, 0), (3, 0), (8, 160), (8, 60), (5, 100), (32, 400), (1, 0)])
+def test_host_vector_calls_graded_ranges(tt, n_ranges, growth):
+    """The pipelined *_host calls cut the parameter axis into a geometric sequence of ranges (tt_api.cu host_ranges): whatever
+    the number of ranges and their ratio, and in either direction of the sequence, the result is the device call's bit for bit
+    (N_d = 20 and N_d = 90: the planner's own choice is 8 graded ranges for the first, 16 equal ones for the second; 9 units of
+    2048 parameters to distribute)."""
+    for N_d in (20, 90):
+        w = workload("C3", N_d, 16384 + 7, 40, torch.float32)
+        F, m, d = inputs(w)
+        plan = tt.Plan(F.cuda())
+        try:
+            ref_d, ref_m, ref_n = plan.matvec(m.cuda()).cpu(), plan.rmatvec(d.cuda()).cpu(), plan.normal(m.cuda()).cpu()
+            tt.tt_debug_set("host_chunks", n_ranges)
+            tt.tt_debug_set("host_growth", growth)
+            mh, dh = m.pin_memory(), d.pin_memory()
+            d_out, m_out, n_out = torch.empty_like(d).pin_memory(), torch.empty_like(m).pin_memory(), torch.empty_like(m).pin_memory()
+            tt.tt_matvec_host(plan.handle, mh, d_out)
+            tt.tt_rmatvec_host(plan.handle, dh, m_out)
+            tt.tt_normal_host(plan.handle, mh, n_out)
+            torch.cuda.synchronize()
+            assert torch.equal(d_out, ref_d) and torch.equal(m_out, ref_m) and torch.equal(n_out, ref_n)
+        finally:
+            tt.tt_debug_set("host_chunks", 0)
+            tt.tt_debug_set("host_growth", 0)
+            plan.close()
+
+
 def test_error_codes(tt):
     import ctypes
     L = tt.lib()
