@@ -914,7 +914,8 @@ def measure(ctx, args, w, cfg_name, *, steps, warmup, headline):
             "achieved_kernel_bytes": bytes_fwd_kernel / (fwd[1] * 1e-3) / 1e9 if fwd[1] > 0 else 0.0,
             "whole_op": {"matvec_frac": bytes_op / (ms_fwd * 1e-3) / 1e9 / peak, "rmatvec_frac": bytes_op / (ms_adj * 1e-3) / 1e9 / peak,
                          "what": "the same bytes / the whole F.m and F^T.d (FFTs and un-fused intermediates included)"},
-            "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)", "achieved": ach_adj, "frac": ach_adj / peak,
+            "adjoint_kernel": {"kernel": "gemv_adj_kernel (B2)" + (", with the persistent B3 consumer CTAs running beside it" if "B3 consumer" in describe else ""),
+                               "achieved": ach_adj, "frac": ach_adj / peak,
                                "algorithmic_bytes_per_launch": bytes_op, "kernel_bytes_per_launch": bytes_adj_kernel,
                                "ms_per_launch": adj[1], "frac_of_nominal_8TBs": ach_adj / NOMINAL_HBM_GBS},
             "kernels": describe,
@@ -1056,6 +1057,8 @@ def measure(ctx, args, w, cfg_name, *, steps, warmup, headline):
             torch.cuda.empty_cache()
 
     launches_per_step = 7                      # A1, A2 (matvec or GEMM), partial reduce, A3, B1, B2, B3
+    if K == 1 and "B3 consumer" in describe:   # F^T d in producer / consumer mode: B3 consumer beside B2, clean-up B3 behind it
+        launches_per_step = 8
     out = {
         "metric": METRIC, "value": ms_step if shard else ms_step / args.gpus, "unit": "ms", "n_gpus": args.gpus,
         "steps": steps,
@@ -1153,6 +1156,10 @@ def main() -> int:
                     help="multiply the config's N_m by this factor: for profiler captures of long kernels only (ncu replays a "
                          "kernel ~40 times and saves / restores device memory around each pass); the line it prints names the "
                          "scaled workload and is not a bench line of the config")
+    ap.add_argument("--two-launch-rmatvec", action="store_true",
+                    help="for profiler captures: F^T d as B2 then B3 (tt_debug_set l2r_mb = 0).  The default form runs B3 as "
+                         "persistent consumer CTAs BESIDE B2; a profiler that serialises kernels makes those CTAs give up "
+                         "after 50 ms and shows the clean-up B3 doing all the work - correct, but not the timeline of a real run")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = synth.CONFIGS[args.config]
@@ -1180,6 +1187,8 @@ def main() -> int:
 
     from paper_2501_14911_b200 import binding as tt
     tt.lib()
+    if args.two_launch_rmatvec:
+        tt.tt_debug_set("l2r_mb", 0)
     ctx = Ctx(tt=tt, dev=torch.device("cuda", local_rank), dist=dist, rank=rank, world=world, local_rank=local_rank)
 
     out = measure(ctx, args, w, args.config, steps=args.steps, warmup=args.warmup, headline=True)

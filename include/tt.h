@@ -143,7 +143,11 @@ int tt_plan_get_spectrum(const tt_plan* plan, void* dst_device, void* stream);
 int tt_matvec(const tt_plan* plan, const void* m, void* d, void* stream);
 
 /* m = F^T d  (transpose of eq 2.5; "conjugate-transposed diagonal blocks").
- *   d  DEVICE, N_t*N_d reals, read-only;   m  DEVICE, N_t*N_m reals, overwritten. */
+ *   d  DEVICE, N_t*N_d reals, read-only;   m  DEVICE, N_t*N_m reals, overwritten.
+ * From ~14 GB of spectrum (and N_d >= 32) the inverse FFT of the result runs WHILE the per-frequency matvec runs, on a
+ * stream owned by the plan (forked from and joined back into `stream` with events: capturable, nothing for the caller to
+ * synchronise), and takes the spectrum over in the L2; the result is the two-launch sequence's bit for bit
+ * (tt_plan_describe says which form a plan takes). */
 int tt_rmatvec(const tt_plan* plan, const void* d, void* m, void* stream);
 
 /* out = F^T (F m)  (eq 2.12 with Gamma_noise = I).  The intermediate

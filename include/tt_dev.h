@@ -45,6 +45,9 @@ int tt_debug_trig(int64_t k, int64_t n, double* c, double* s);
  * "gemm_adj_mt" = m-tiles per warp of the fp64 k-RHS adjoint GEMM (1, 2; 0 = default),
  * "kd_slab" = parameters per slab of the fp32 direct K assembly (multiple of 32; 0 = 8192),
  * "host_chunks" = parameter ranges of the pipelined *_host calls (1..32; 0 = planner's choice: 8 graded or 16 equal ones),
+ * "l2r_mb" = F^T d with B3 as a concurrent consumer of B2: megabytes of spectrum per group of B2's grid (0 = the plain two-launch
+ * sequence, -1 = planner's choice), "l2r_ctas" = its persistent consumer CTAs (0 = planner's choice), "l2r_discard" = 0 keeps the
+ * write-back of the spectrum,
  * "host_growth" = size of each of those ranges in percent of the one before (1..400; 0 = planner's choice).
  * Returns TT_ERR_SHAPE for an unknown key. */
 int tt_debug_set(const char* key, int value);

@@ -26,6 +26,10 @@ int g_host_growth = 0;              // tt_debug_set("host_growth"): each range t
 
 inline size_t esize(int dtype) { return dtype == TT_F32 ? 4 : 8; }
 int g_gemv_chunk = 0;  // tt_debug_set("gemv_chunk"): 0 = planner's choice
+// F^T d with B3 as a concurrent consumer of B2 (run_rmatvec): tt_debug_set("l2r_mb") = megabytes of spectrum per group of B2's
+// grid (0 = the plain two-launch sequence, -1 = planner's choice), "l2r_ctas" = persistent consumer CTAs (0 = planner's choice),
+// "l2r_discard" = 0 keeps the write-back of the spectrum.
+int g_l2r_mb = -1, g_l2r_ctas = 0, g_l2r_discard = 1;
 int g_fft_max_radix = 0;  // tt_debug_set("fft_max_radix"): 0 = no limit
 
 }  // namespace
@@ -49,6 +53,10 @@ struct tt_plan {
     void* dwork = nullptr;    // [N_t][N_d] reals (tt_normal)
     void* m_stage = nullptr;  // lazily: N_t*N_m reals (x2: in and out) for the *_host calls
     void* d_stage = nullptr;
+    cudaStream_t fft_stream = nullptr;    // F^T d: the persistent consumer (B3) runs here beside B2 on the caller's stream
+    cudaEvent_t fev[2] = {};              // fork / join of that stream
+    unsigned* l2r_sync = nullptr;         // [ticket, error, one counter per B2 tile]
+    size_t l2r_sync_bytes = 0, l2r_done_off = 0;  // the done flags (one byte per tile of 8+ series) follow the counters
     cudaStream_t copy_stream = nullptr;   // *_host calls: the PCIe copies of the parameter-sized vector run here, chunk by
     cudaEvent_t cev[kMaxHostChunks + 2] = {};  // chunk over ranges of the parameter axis, overlapped with the kernels (lazily created)
     int chunk = 0, n_chunks = 0, fwd_warps = 0;
@@ -226,7 +234,40 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
     return TT_OK;
 }
 
-// m = F^T d on device buffers (steps B1, B2, B3).
+// Producer / consumer plan of F^T d for this shape: CTA tiles per group of B2's grid and consumer CTAs; tpg = 0: the plain
+// two-launch sequence.  The consumers must keep up with B2 or the spectrum leaves the L2 before it is read (and a consumer
+// that falls behind is far worse than none: Q5 with 48 CTAs 6.2 ms against 3.25): B3 alone costs ~5 ps per series and time
+// step on ~518 resident CTAs (C3 0.43 ms, P5 0.75 ms, C5 0.16 ms), B2 streams |Fhat| at ~7 TB/s, so B3 needs
+// ~2270 / N_d CTAs for the duration of B2 in either precision (measured: C3 fails with 24 and works from 37, P5 fails with
+// 37 and works from 48); 1.8 times that are launched, at least 32.  Shapes that would need more than 128 (N_d < 32: B3 is
+// a large part of the call and its CTAs would crowd B2 out) and shapes whose B2 takes under 2 ms (no gain measured at C2)
+// keep the two launches.  Groups of 16 MB (4 - 32 MB measured within 0.3 %).
+struct L2rPlan { int tpg, ctas; };
+L2rPlan l2r_plan(const tt_plan* p) {
+    L2rPlan none{0, 0};
+    if (g_l2r_mb == 0 || !p->fft_stream || !p->l2r_sync) return none;
+    const int t = p->dtype == TT_F32 ? 0 : 1;
+    const int ptile = gemv_adj_tile_params(t);
+    if (!fft_c2r_consumer_ok(t, (int)p->N_t, ptile)) return none;
+    const double fhat_bytes = (double)p->n_f * (double)p->N_d * (double)p->ldp * 2.0 * (double)esize(p->dtype);
+    int ctas = g_l2r_ctas;
+    if (ctas <= 0) {
+        const double need = 2270.0 / (double)p->N_d;
+        if (g_l2r_mb < 0 && (1.8 * need > 128.0 || fhat_bytes < 14.0e9)) return none;
+        ctas = (int)std::ceil(1.8 * need);
+        if (ctas < 32) ctas = 32;
+    }
+    const double tile_bytes = (double)p->n_f * ptile * 2.0 * (double)esize(p->dtype);
+    long long tpg = (long long)((double)(g_l2r_mb < 0 ? 16 : g_l2r_mb) * 1048576.0 / tile_bytes);
+    return L2rPlan{tpg < 1 ? 1 : tpg > (1 << 20) ? (1 << 20) : (int)tpg, ctas};
+}
+
+// m = F^T d on device buffers (steps B1, B2, B3).  Producer / consumer mode (l2r_plan): B3 runs WHILE B2 runs,
+// as a few persistent CTAs on the plan's own high-priority stream that take the tiles of 16 series in order and wait for the
+// per-tile counters B2 advances; B2 walks the parameter axis group by group so that a group's spectrum is complete - and
+// consumed - while it still sits in the L2 (evict-last stores, evict-first Fhat stream, discard after the read).  Same
+// arithmetic, same order: bit-identical to the two-launch sequence.
+// Stage marks: 0-1 B1, 1-2 B2, 2-3 B3 (producer / consumer mode: what is left of B3 when B2 has finished).
 int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev_base, int k = 1, int r = 0) {
     const bool f32 = p->dtype == TT_F32;
     const int t = f32 ? 0 : 1;
@@ -242,13 +283,34 @@ int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev
     TT_CUDA(p, fft_r2c_launch(t, t, t, at(d, vd.off, es), p->dhat, P, 1, s));
     pr.mark(1);
     GemvGeom g{p->n_f, (int)p->N_d, p->ldp, p->chunk, p->n_chunks, p->fwd_warps};
-    TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
-    pr.mark(2);
     fill_fft_common(p, P, f32);
     P.B = p->N_m; P.B_store = p->N_m;
     P.c_ys = 0; P.c_bs = 1; P.c_fs = p->ldp;
     P.r_ys = 0; P.r_bs = vm.bs; P.r_ts = vm.ts;
-    TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
+    const L2rPlan lp = l2r_plan(p);
+    if (lp.tpg == 0) {
+        TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
+        pr.mark(2);
+        TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
+        pr.mark(3);
+        return TT_OK;
+    }
+    const int ptile = gemv_adj_tile_params(t);
+    unsigned char* done = reinterpret_cast<unsigned char*>(p->l2r_sync) + p->l2r_done_off;
+    TT_CUDA(p, cudaMemsetAsync(p->l2r_sync, 0, p->l2r_sync_bytes, s));
+    TT_CUDA(p, cudaEventRecord(p->fev[0], s));                    // fork: dhat, the counters and the output vector are ready
+    TT_CUDA(p, cudaStreamWaitEvent(p->fft_stream, p->fev[0], 0));
+    FftParams Pc = P;
+    Pc.discard_in = g_l2r_discard;
+    TT_CUDA(p, fft_c2r_consumer_launch(t, p->xhat, at(m, vm.off, es), Pc, p->l2r_sync, done, ptile, lp.ctas, p->fft_stream));
+    g.l2r_sync = p->l2r_sync;
+    g.l2r_tpg = lp.tpg;
+    TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
+    pr.mark(2);
+    TT_CUDA(p, cudaEventRecord(p->fev[1], p->fft_stream));        // join
+    TT_CUDA(p, cudaStreamWaitEvent(s, p->fev[1], 0));
+    P.skip = done;                                                // whatever the consumers did not get to (normally nothing)
+    if (g_l2r_discard != 3) TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
     pr.mark(3);
     return TT_OK;
 }
@@ -555,6 +617,10 @@ void tt_plan_destroy(tt_plan* p) {
     for (void* b : bufs)
         if (b) cudaFree(b);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    if (p->fft_stream) cudaStreamDestroy(p->fft_stream);
+    for (cudaEvent_t e : p->fev)
+        if (e) cudaEventDestroy(e);
+    if (p->l2r_sync) cudaFree(p->l2r_sync);
     for (cudaEvent_t e : p->cev)
         if (e) cudaEventDestroy(e);
     if (p->ev) {
@@ -667,6 +733,18 @@ int tt_plan_create_coarse(tt_plan** out, int64_t N_d, int64_t N_m, int64_t N_t, 
         TT_TRYC(cudaStreamSynchronize(s));  // the host vectors die at the end of this scope
     }
 
+    // the plan's own stream for the consumer side of F^T d (highest priority: its few persistent CTAs are placed ahead of the
+    // thousands B2 has queued), the fork / join events and the per-tile counters
+    {
+        int lo = 0, hi = 0;
+        TT_TRYC(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        TT_TRYC(cudaStreamCreateWithPriority(&p->fft_stream, cudaStreamNonBlocking, hi));
+        for (cudaEvent_t& e : p->fev) TT_TRYC(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        p->l2r_done_off = (size_t)(p->ldp / 256 + 8) * sizeof(unsigned);
+        p->l2r_sync_bytes = p->l2r_done_off + (size_t)(p->ldp / 8 + 64);
+        TT_TRY(dev_alloc(p, reinterpret_cast<void**>(&p->l2r_sync), p->l2r_sync_bytes));
+    }
+
     // spectrum and scratch
     const size_t fhat_elems = (size_t)p->n_f * (size_t)N_d * (size_t)p->ldp;
     TT_TRY(dev_alloc(p, &p->Fhat, fhat_elems * cs));
@@ -737,6 +815,12 @@ int tt_plan_describe(const tt_plan* p, char* buf, size_t n) {
         const int k = snprintf(buf + at, n - at, i ? "x%d" : "%d", p->radix[t][i]);
         if (k < 0 || at + (size_t)k >= n) return TT_ERR_SHAPE;
         at += (size_t)k;
+    }
+    const L2rPlan lp = l2r_plan(p);
+    if (lp.tpg > 0) {   // how tt_rmatvec runs B2 and B3 for this shape (8 kernels per F m + F^T d instead of 7)
+        const int k = snprintf(buf + at, n - at, " | F^T d: B2 producer (1-D grid, groups of %d tiles) + %d persistent B3 consumer CTAs + clean-up B3",
+                               lp.tpg, lp.ctas);
+        if (k < 0 || at + (size_t)k >= n) return TT_ERR_SHAPE;
     }
     return TT_OK;
 }
@@ -936,6 +1020,9 @@ int tt_debug_set(const char* key, int value) {
         g_host_growth = value;
         return TT_OK;
     }
+    if (!std::strcmp(key, "l2r_mb")) { if (value < -1) return TT_ERR_SHAPE; g_l2r_mb = value; return TT_OK; }
+    if (!std::strcmp(key, "l2r_ctas")) { if (value < 0 || value > 4096) return TT_ERR_SHAPE; g_l2r_ctas = value; return TT_OK; }
+    if (!std::strcmp(key, "l2r_discard")) { g_l2r_discard = value; return TT_OK; }
     if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }

@@ -104,17 +104,19 @@ fft_r2c_kernel(const Tin* __restrict__ in, Cx<Tout>* __restrict__ out, const __g
 // ---------------------------------------------------------------------------------------
 // inverse: complex-to-real inverse FFT + truncate + scale                               (A3, B3)
 // ---------------------------------------------------------------------------------------
-template <typename Tc, int T, int NT, int NS = 0>
-__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320 || (NS == 0 && NT == 256 && sizeof(Tc) == 4)) ? 3 : 0)
-fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
+// One tile of T series (tile index `tile`, grid row `by`): shared by the one-CTA-per-tile kernel and the persistent consumer.
+// STREAMED: the input was parked in the L2 by the kernel that produced it (tt_gemv.cu, L2R) and is read exactly once here:
+// it is loaded past L1 and its lines are dropped from the L2 afterwards without a write-back (whole 128-byte lines per tile).
+template <typename Tc, int T, int NT, int NS, bool STREAMED = false>
+__device__ __forceinline__ void c2r_tile(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const FftParams& P, long long tile, int by) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<Tc>* sm = reinterpret_cast<Cx<Tc>*>(smem_raw);
     constexpr int G = NT / T;
     const int lane_s = threadIdx.x % T, g = threadIdx.x / T;
-    const long long b = (long long)blockIdx.x * T + lane_s;
+    const long long b = tile * T + lane_s;
     const bool live = b < P.B;
     const int N = NS ? NS : P.N;
-    const Cx<Tc>* src = in + (long long)blockIdx.y * P.c_ys + b * P.c_bs;
+    const Cx<Tc>* src = in + (long long)by * P.c_ys + b * P.c_bs;
 
     // Z_k = (X_k + conj X_{N-k}) + i conj(w^k) (X_k - conj X_{N-k});  store conj(Z_k) so that the
     // forward FFT below yields conj of the inverse transform.  Pairs (k, N-k) are disjoint; both members are read
@@ -129,8 +131,13 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
             const int k = k0 + u * G;
             va[u] = mk<Tc>(Tc(0), Tc(0)); vb[u] = va[u];
             if (live && k <= nh) {
-                va[u] = src[(long long)k * P.c_fs];
-                vb[u] = src[(long long)(N - k) * P.c_fs];
+                if constexpr (STREAMED) {
+                    va[u] = ld_cg(src + (long long)k * P.c_fs);
+                    vb[u] = ld_cg(src + (long long)(N - k) * P.c_fs);
+                } else {
+                    va[u] = src[(long long)k * P.c_fs];
+                    vb[u] = src[(long long)(N - k) * P.c_fs];
+                }
             }
         }
 #pragma unroll
@@ -152,15 +159,71 @@ fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid
             }
         }
     }
+    if constexpr (STREAMED) {
+        constexpr int LINES = (int)(T * sizeof(Cx<Tc>) / 128);   // whole lines per frequency row of the tile (the host checks)
+        if (P.discard_in) {
+            __syncthreads();   // every load of the tile has returned (its value went to shared memory)
+            const char* base = reinterpret_cast<const char*>(in + (long long)by * P.c_ys + tile * T * P.c_bs);
+            for (int i = threadIdx.x; i < (N + 1) * LINES; i += NT)
+                l2_discard_line(base + (long long)(i / LINES) * P.c_fs * (long long)sizeof(Cx<Tc>) + (i % LINES) * 128);
+        }
+    }
     // built where it is used (after the passes over shared memory), so that its fields are not live across them
     auto stz = [&]() {
-        return RealStorer<Tc>{out + (long long)blockIdx.y * P.r_ys + b * P.r_bs, P.r_ts, P.pos + N, N, P.dec, Tc(P.scale), live};
+        return RealStorer<Tc>{out + (long long)by * P.r_ys + b * P.r_bs, P.r_ts, P.pos + N, N, P.dec, Tc(P.scale), live};
     };
     if (N == 1) {  // no pass
         __syncthreads();
         if (g == 0) stz()(0, sm[lane_s]);
     }
     fft_inplace_out<Tc, T, NS>(sm, P, lane_s, g, G, stz);
+}
+
+template <typename Tc, int T, int NT, int NS = 0>
+__global__ void __launch_bounds__(NT, NS == 400 ? 4 : (NS == 500 || NT == 320 || (NS == 0 && NT == 256 && sizeof(Tc) == 4)) ? 3 : 0)
+fft_c2r_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P) {
+    if (P.skip && P.skip[blockIdx.x]) return;   // done by the consumer kernel while B2 was running
+    c2r_tile<Tc, T, NT, NS>(in, out, P, (long long)blockIdx.x, (int)blockIdx.y);
+}
+
+// B3 as the CONSUMER of a running B2 (tt_api.cu run_rmatvec, L2R): a few persistent CTAs take the tiles of T series in
+// ascending order from a ticket, wait until all N + 1 frequencies of the tile's parameters have been stored by B2 (one
+// counter per B2 tile of `ptile` parameters, incremented by every B2 CTA after its store), transform the tile, store the
+// truncated real series and flag the tile as done.  The spectrum is read where B2 parked it, in the L2, and dropped there.
+// The consumer is an ACCELERATOR, not a dependency: a CTA that waits 50 ms for a counter (B2 is not running beside it - a
+// profiler or debugger that serialises kernels, a GPU shared with other work) gives up, and the regular B3 launch that
+// follows B2 on the caller's stream transforms every tile that carries no done flag.
+//   sync[0] = ticket, sync[2 + i] = counter of B2 tile i;  done[t] = 1: tile t of T series is finished
+template <typename Tc, int T, int NT, int NS = 0>
+__global__ void __launch_bounds__(NT, 3)   // <= 80 registers: three or four of B2's CTAs share the SM with one of these
+fft_c2r_consumer_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, const __grid_constant__ FftParams P,
+                        unsigned* sync, unsigned char* done, long long n_tiles, int ptile, unsigned n_f) {
+    __shared__ long long s_tile;
+    for (;;) {
+        __syncthreads();   // the previous tile's last pass has read shared memory
+        if (threadIdx.x == 0) {
+            long long t = (long long)atomicAdd(sync, 1u);
+            if (t < n_tiles) {
+                const unsigned* cnt = sync + 2 + (t * T) / ptile;
+                unsigned long long t0, t1;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+                unsigned v;
+                for (;;) {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(cnt) : "memory");
+                    if (v >= n_f) break;
+                    __nanosleep(256);
+                    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+                    if (t1 - t0 > 50000000ULL) { t = n_tiles; break; }   // 50 ms: the producer is not running beside us
+                }
+                if (t < n_tiles) done[t] = 1;   // taken and never abandoned from here on: the clean-up launch (after this kernel) skips it
+            }
+            s_tile = t;
+        }
+        __syncthreads();
+        const long long tile = s_tile;
+        if (tile >= n_tiles) break;
+        c2r_tile<Tc, T, NT, NS, true>(in, out, P, tile, 0);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -303,6 +366,43 @@ static cudaError_t c2r_dispatch(const void* in, void* out, const FftParams& P, i
     else                { if (c.T == 32) TT_C2R(32, 256) else if (c.T == 16) TT_C2R(16, 256) else TT_C2R(8, 256) }
 #undef TT_C2R
     return cudaGetLastError();
+}
+
+// The persistent consumer (see fft_c2r_consumer_kernel): the plan's usual variant for this length, n_ctas CTAs.
+template <typename Tc>
+static cudaError_t c2r_consumer_dispatch(const void* in, void* out, const FftParams& P, unsigned* sync, unsigned char* done,
+                                         int ptile, int n_ctas, cudaStream_t s) {
+    const FftChoice c = fft_choose(P.N, sizeof(Cx<Tc>));
+    if (c.T == 0 || (c.T * sizeof(Cx<Tc>)) % 128 != 0 || ptile % c.T != 0 || P.c_bs != 1) return cudaErrorInvalidValue;
+    const long long n_tiles = (P.B + c.T - 1) / c.T;
+    const unsigned n_f = (unsigned)P.N + 1u;
+#define TT_C2RC(TT, ...)                                                                                      \
+    {                                                                                                        \
+        auto k = fft_c2r_consumer_kernel<Tc, TT, 256, ##__VA_ARGS__>;                                         \
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);   \
+        if (e != cudaSuccess) return e;                                                                      \
+        k<<<n_ctas, 256, c.smem, s>>>(static_cast<const Cx<Tc>*>(in), static_cast<Tc*>(out), P, sync, done, n_tiles, ptile, n_f); \
+    }
+    const int ns = static_length<Tc>(P, c, 256, true);
+    if (ns) {
+        if constexpr (sizeof(Tc) == 4) { if (ns == 400) TT_C2RC(16, 400) else if (ns == 500) TT_C2RC(16, 500) else TT_C2RC(16, 256) }
+        else                           { if (ns == 512 && c.T == 8) TT_C2RC(8, 512) else if (ns == 512) TT_C2RC(16, 512) else TT_C2RC(16, 256) }
+    }
+    else { if (c.T == 32) TT_C2RC(32) else if (c.T == 16) TT_C2RC(16) else TT_C2RC(8) }
+#undef TT_C2RC
+    return cudaGetLastError();
+}
+
+bool fft_c2r_consumer_ok(int tc, int N, int ptile) {
+    const size_t cs = tc == 0 ? sizeof(c64) : sizeof(c128);
+    const FftChoice c = fft_choose(N, cs);
+    return c.T != 0 && (c.T * cs) % 128 == 0 && ptile % c.T == 0;
+}
+
+cudaError_t fft_c2r_consumer_launch(int tc, const void* in, void* out, const FftParams& P, unsigned* sync, unsigned char* done,
+                                    int ptile, int n_ctas, cudaStream_t s) {
+    return tc == 0 ? c2r_consumer_dispatch<float>(in, out, P, sync, done, ptile, n_ctas, s)
+                   : c2r_consumer_dispatch<double>(in, out, P, sync, done, ptile, n_ctas, s);
 }
 
 cudaError_t fft_c2r_launch(int tc, const void* in, void* out, const FftParams& P, int ny, cudaStream_t s) {

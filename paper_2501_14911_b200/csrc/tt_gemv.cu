@@ -77,8 +77,14 @@ gemv_fwd_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ xhat, 
 // vector of p and walks down the N_d rows with UNROLL independent loads in flight; a warp
 // reads 512 contiguous bytes of every row.  dhat_w (N_d complex numbers) sits in shared
 // memory and is broadcast.  No reduction across threads.
+//
+// PRODUCER mode (L2R, tt_api.cu run_rmatvec): B3 runs at the same time as a few persistent CTAs that consume the spectrum
+// tile by tile (tt_fft.cu fft_c2r_consumer_kernel).  The 1-D grid then runs GROUP by group - l2r_tpg CTA tiles of
+// parameters, all frequencies of a group before the next group - so that the spectrum of a group (tens of MB) is complete
+// soon after its first store and can wait for its consumer in the L2: Fhat is loaded evict-first, the output stored
+// evict-last, and every CTA counts itself into its tile's counter after the store (release by fence + atomic).
 // ---------------------------------------------------------------------------------------
-template <typename R, int UNROLL>
+template <typename R, int UNROLL, bool L2R = false>
 __global__ void __launch_bounds__(512)
 gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, Cx<R>* __restrict__ xout,
                 const GemvGeom g) {
@@ -87,39 +93,70 @@ gemv_adj_kernel(const Cx<R>* __restrict__ Fhat, const Cx<R>* __restrict__ dhat, 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Cx<R>* ds = reinterpret_cast<Cx<R>*>(smem_raw);
 
-    const int w = blockIdx.y;
     const int NT = blockDim.x;
+    const long long rowv = g.ldp / VN;
+    int w;
+    long long tile;
+    if constexpr (L2R) {
+        // x -> (group, frequency, tile in group), tile fastest; the last group may hold fewer tiles
+        const long long n_tiles = (rowv + NT - 1) / NT;
+        const long long per_group = (long long)g.n_f * g.l2r_tpg;
+        const long long grp = (long long)blockIdx.x / per_group;
+        const long long in_grp = (long long)blockIdx.x - grp * per_group;
+        const long long t0 = grp * g.l2r_tpg;
+        const int tpg = (int)(n_tiles - t0 < g.l2r_tpg ? n_tiles - t0 : g.l2r_tpg);
+        w = (int)(in_grp / tpg);
+        tile = t0 + (in_grp - (long long)w * tpg);
+    } else {
+        w = blockIdx.y;
+        tile = blockIdx.x;
+    }
     for (int i = threadIdx.x; i < g.N_d; i += NT) ds[i] = dhat[(long long)w * g.N_d + i];
     __syncthreads();
 
-    const long long rowv = g.ldp / VN;
-    const long long v = (long long)blockIdx.x * NT + threadIdx.x + g.p_begin / VN;
-    if (v >= (g.p_end ? g.p_end / VN : rowv)) return;
-    const V* col = reinterpret_cast<const V*>(Fhat + (long long)w * g.N_d * g.ldp) + v;
-
-    Cx<R> acc[VN];
+    const long long v = tile * NT + threadIdx.x + (L2R ? 0 : g.p_begin / VN);
+    const bool mine = v < (!L2R && g.p_end ? g.p_end / VN : rowv);
+    if (!L2R && !mine) return;
+    uint64_t pol_in = 0, pol_out = 0;
+    if constexpr (L2R) { pol_in = l2_policy_evict_first(); pol_out = l2_policy_evict_last(); }
+    auto ld = [&](const V* q) -> V {
+        if constexpr (L2R) return ldg_stream(q, pol_in);
+        else return ldg_stream(q);
+    };
+    if (mine) {
+        const V* col = reinterpret_cast<const V*>(Fhat + (long long)w * g.N_d * g.ldp) + v;
+        Cx<R> acc[VN];
 #pragma unroll
-    for (int e = 0; e < VN; ++e) acc[e] = mk<R>(R(0), R(0));
-    int s = 0;
-    for (; s + UNROLL <= g.N_d; s += UNROLL) {
-        V f[UNROLL];
+        for (int e = 0; e < VN; ++e) acc[e] = mk<R>(R(0), R(0));
+        int s = 0;
+        for (; s + UNROLL <= g.N_d; s += UNROLL) {
+            V f[UNROLL];
 #pragma unroll
-        for (int u = 0; u < UNROLL; ++u) f[u] = ldg_stream(col + (long long)(s + u) * rowv);
+            for (int u = 0; u < UNROLL; ++u) f[u] = ld(col + (long long)(s + u) * rowv);
 #pragma unroll
-        for (int u = 0; u < UNROLL; ++u) {
-            const Cx<R> dv = ds[s + u];
+            for (int u = 0; u < UNROLL; ++u) {
+                const Cx<R> dv = ds[s + u];
 #pragma unroll
-            for (int e = 0; e < VN; ++e) cmac_conj(acc[e], Vec16<R>::get(f[u], e), dv);
+                for (int e = 0; e < VN; ++e) cmac_conj(acc[e], Vec16<R>::get(f[u], e), dv);
+            }
+        }
+        for (; s < g.N_d; ++s) {
+            const V f = ld(col + (long long)s * rowv);
+            const Cx<R> dv = ds[s];
+#pragma unroll
+            for (int e = 0; e < VN; ++e) cmac_conj(acc[e], Vec16<R>::get(f, e), dv);
+        }
+        V* dst = reinterpret_cast<V*>(xout + (long long)w * g.ldp) + v;
+        if constexpr (L2R) stg_hint(dst, Vec16<R>::pack(acc[0], acc[VN - 1]), pol_out);
+        else *dst = Vec16<R>::pack(acc[0], acc[VN - 1]);
+    }
+    if constexpr (L2R) {
+        __syncthreads();                       // every store of the CTA has been issued ...
+        if (threadIdx.x == 0) {
+            __threadfence();                   // ... and is visible GPU-wide before the tile's counter moves
+            atomicAdd(g.l2r_sync + 2 + tile, 1u);
         }
     }
-    for (; s < g.N_d; ++s) {
-        const V f = ldg_stream(col + (long long)s * rowv);
-        const Cx<R> dv = ds[s];
-#pragma unroll
-        for (int e = 0; e < VN; ++e) cmac_conj(acc[e], Vec16<R>::get(f, e), dv);
-    }
-    V* dst = reinterpret_cast<V*>(xout + (long long)w * g.ldp) + v;
-    *dst = Vec16<R>::pack(acc[0], acc[VN - 1]);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -156,17 +193,25 @@ static cudaError_t adj_dispatch(const void* Fhat, const void* dhat, void* xout, 
                                 cudaStream_t s) {
     constexpr int UN = 10;
     const int NT = g_adj_threads ? g_adj_threads : 256;
-    auto k = gemv_adj_kernel<R, UN>;
+    auto k = g.l2r_sync ? gemv_adj_kernel<R, UN, true> : gemv_adj_kernel<R, UN, false>;
     const size_t smem = (size_t)g.N_d * sizeof(Cx<R>);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long rowv = g.ldp / Vec16<R>::n;
     const long long nv = (g.p_end ? g.p_end : g.ldp) / Vec16<R>::n - g.p_begin / Vec16<R>::n;
     dim3 grid((unsigned)((nv + NT - 1) / NT), (unsigned)g.n_f);
+    if (g.l2r_sync) {   // producer mode: the whole parameter axis, group-major 1-D grid
+        if (g.p_begin || g.p_end || g.l2r_tpg < 1) return cudaErrorInvalidValue;
+        const long long n_cta = ((rowv + NT - 1) / NT) * (long long)g.n_f;
+        if (n_cta > 0x7fffffffLL) return cudaErrorInvalidValue;
+        grid = dim3((unsigned)n_cta, 1u);
+    }
     k<<<grid, NT, smem, s>>>(static_cast<const Cx<R>*>(Fhat), static_cast<const Cx<R>*>(dhat),
                              static_cast<Cx<R>*>(xout), g);
     return cudaGetLastError();
 }
+
+int gemv_adj_tile_params(int dt) { return (g_adj_threads ? g_adj_threads : 256) * (dt == 0 ? 2 : 1); }
 
 // What the two launches above look like for geometry g (tt_plan_describe: bench.py ties its ncu figures to this string)
 int gemv_describe(int dt, const GemvGeom& g, char* buf, size_t n) {

@@ -45,6 +45,8 @@ struct FftParams {
     long long r_ys, r_bs, r_ts;
     long long c_ys, c_bs, c_fs;
     double scale;           // inverse only: factor applied to the real output (1/L)
+    int discard_in;         // consumer kernel only: drop the input lines from the L2 once read (no write-back)
+    const unsigned char* skip;  // inverse only: tiles (CTAs) whose flag is set have been done by the consumer kernel: exit at once
     int dec;                // real side on a coarser time grid: only the time steps j with (j+1) % dec == 0 exist, stored
                             // at index (j+1)/dec - 1 (forward: the others are zeros; inverse: the others are dropped); 1 = all
 };
@@ -62,6 +64,10 @@ cudaError_t fft_r2c_launch(int tin, int tc, int tout, const void* real_in, void*
                            const FftParams& P, int ny, cudaStream_t s);
 cudaError_t fft_c2r_launch(int tc, const void* cplx_in, void* real_out, const FftParams& P, int ny,
                            cudaStream_t s);
+// B3 as persistent consumer of a running B2 (tt_fft.cu fft_c2r_consumer_kernel): sync = [ticket, error, counters per ptile parameters]
+bool fft_c2r_consumer_ok(int tc, int N, int ptile);
+cudaError_t fft_c2r_consumer_launch(int tc, const void* cplx_in, void* real_out, const FftParams& P, unsigned* sync,
+                                    unsigned char* done, int ptile, int n_ctas, cudaStream_t s);
 // dhat[w*N_d + s] = sum_c partial[(w*n_chunks + c)*N_d + s] (fixed order, fp64 accumulator)
 cudaError_t reduce_partials_launch(int dt, const void* partial, void* dhat, int n_f, int n_chunks, int N_d,
                                    cudaStream_t s);
@@ -80,6 +86,8 @@ struct GemvGeom {
     int chunk;      // forward: elements of p per CTA (multiple of 64)
     int n_chunks;
     int warps;      // forward: warps per CTA (0 = kernel default)
+    unsigned* l2r_sync = nullptr;  // adjoint, producer mode (with B3 as consumer): [ticket, error, one counter per CTA tile of parameters]
+    int l2r_tpg = 0;               // producer mode: CTA tiles per group - the grid runs group by group, all frequencies of a group before the next
     long long p_begin = 0, p_end = 0;  // restrict the launch to parameters [p_begin, p_end) (p_end == 0: all); p_begin must be
                                        // a multiple of `chunk` (forward) and of 512 (adjoint) - the pipelined *_host calls
 };
@@ -88,6 +96,7 @@ cudaError_t gemv_fwd_launch(int dt, const void* Fhat, const void* xhat, void* pa
                             cudaStream_t s);
 cudaError_t gemv_adj_launch(int dt, const void* Fhat, const void* dhat, void* xhat_out, const GemvGeom& g,
                             cudaStream_t s);
+int gemv_adj_tile_params(int dt);  // parameters per CTA of the adjoint kernel (the granularity of the producer-mode counters)
 int gemv_describe(int dt, const GemvGeom& g, char* buf, size_t n);  // snprintf semantics
 
 // k-RHS per-frequency complex GEMMs on the FP64 tensor pipe (DMMA) / fp32 FMA.

@@ -388,6 +388,8 @@ def test_apply_calls_are_cuda_graph_capturable(tt):
                 tt.tt_map_infer(mp.handle, tt.TT_MAP_PAPER, d_in, out_map, s)
         s.synchronize()
         ref_map = out_map.clone()
+        tt.tt_debug_set("l2r_mb", 1)                              # F^T d in producer / consumer mode (forked plan stream) too
+        tt.tt_debug_set("l2r_ctas", 8)
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph, stream=s):
             tt.tt_matvec(pF.handle, m_in, out_d, s)
@@ -403,6 +405,8 @@ def test_apply_calls_are_cuda_graph_capturable(tt):
         assert rel(out_map.cpu().numpy(), 2.0 * ref_map.cpu().numpy()) <= 1e-13
         assert rel(out_m.cpu().numpy(), op.rmatvec(F.numpy(), op.matvec(F.numpy(), m_in.cpu().numpy()))) <= 1e-12
     finally:
+        tt.tt_debug_set("l2r_mb", -1)
+        tt.tt_debug_set("l2r_ctas", 0)
         mp.close(); chol.close(); pF.close(); pG.close()
 
 

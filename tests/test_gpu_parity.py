@@ -362,6 +362,62 @@ def test_host_vector_calls_graded_ranges(tt, n_ranges, growth):
             plan.close()
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("base,N_d,N_m,N_t", SHAPES)
+def test_rmatvec_producer_consumer_mode_is_bit_identical(tt, base, N_d, N_m, N_t, dtype):
+    """F^T d with B3 as a concurrent consumer of B2 (tt_api.cu run_rmatvec: group-major B2 grid with per-tile counters,
+    persistent consumer CTAs on the plan's stream, spectrum handed over in the L2 and dropped there, clean-up launch for
+    tiles the consumers did not reach) against the plain two-launch sequence, forced on at every test shape - the planner
+    itself only takes it from ~14 GB of spectrum: tt_rmatvec and tt_normal bit for bit, for small and large groups, few
+    and many consumers, with and without the discard.  (Shapes whose FFT tile is not a whole number of 128-byte lines
+    fall back to the two launches inside the library: equal by construction.)"""
+    w = workload(base, N_d, N_m, N_t, dtype)
+    F, m, d = inputs(w)
+    plan = tt.Plan(F.cuda())
+    try:
+        tt.tt_debug_set("l2r_mb", 0)
+        ref_m, ref_n = plan.rmatvec(d.cuda()), plan.normal(m.cuda())
+        for mb, ctas, discard in ((1, 3, 1), (1, 40, 1), (64, 7, 1), (2, 148, 0)):
+            tt.tt_debug_set("l2r_mb", mb)
+            tt.tt_debug_set("l2r_ctas", ctas)
+            tt.tt_debug_set("l2r_discard", discard)
+            for _ in range(2):
+                assert torch.equal(plan.rmatvec(d.cuda()), ref_m), (mb, ctas, discard)
+                assert torch.equal(plan.normal(m.cuda()), ref_n), (mb, ctas, discard)
+    finally:
+        tt.tt_debug_set("l2r_mb", -1)
+        tt.tt_debug_set("l2r_ctas", 0)
+        tt.tt_debug_set("l2r_discard", 1)
+        plan.close()
+
+
+def test_rmatvec_producer_consumer_mode_survives_serialised_kernels(tt):
+    """The consumer kernel is an accelerator, not a dependency: when kernels cannot run side by side (here
+    CUDA_LAUNCH_BLOCKING=1 in a child process; a profiler that serialises launches does the same) the consumers give up
+    after 50 ms without a producer, and the regular B3 launch behind B2 transforms every tile - same bits, only slower."""
+    import os
+    import subprocess
+    import sys
+    code = (
+        "import torch, synth\n"
+        "from paper_2501_14911_b200 import binding as tt\n"
+        "w = synth.CONFIGS['C3'].scaled(N_d=7, N_m=3000, N_t=400)\n"
+        "F, d = synth.block_column(w).cuda(), synth.vector_d(w, k_rhs=1).cuda()\n"
+        "plan = tt.Plan(F)\n"
+        "tt.tt_debug_set('l2r_mb', 0)\n"
+        "ref = plan.rmatvec(d)\n"
+        "tt.tt_debug_set('l2r_mb', 1); tt.tt_debug_set('l2r_ctas', 16)\n"
+        "out = plan.rmatvec(d)\n"
+        "torch.cuda.synchronize()\n"
+        "assert torch.equal(out, ref)\n"
+        "print('serialised ok')\n"
+    )
+    env = dict(os.environ, CUDA_LAUNCH_BLOCKING="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and "serialised ok" in res.stdout, res.stdout + res.stderr
+
+
 def test_error_codes(tt):
     import ctypes
     L = tt.lib()
