@@ -202,7 +202,11 @@ fft_c2r_consumer_kernel(const Cx<Tc>* __restrict__ in, Tc* __restrict__ out, con
     for (;;) {
         __syncthreads();   // the previous tile's last pass has read shared memory
         if (threadIdx.x == 0) {
-            long long t = (long long)atomicAdd(sync, 1u);
+            // Once B2's LAST tile is complete B2 is (all but) over and the whole GPU is free: the few tiles that are left are
+            // quicker in the clean-up launch (one CTA per tile on every SM) than in these few CTAs - take no more.
+            unsigned last;
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(last) : "l"(sync + 2 + ((n_tiles - 1) * T) / ptile) : "memory");
+            long long t = last >= n_f ? n_tiles : (long long)atomicAdd(sync, 1u);
             if (t < n_tiles) {
                 const unsigned* cnt = sync + 2 + (t * T) / ptile;
                 unsigned long long t0, t1;
