@@ -235,13 +235,14 @@ int run_matvec(const tt_plan* p, const void* m, void* d, cudaStream_t s, int ev_
 }
 
 // Producer / consumer plan of F^T d for this shape: CTA tiles per group of B2's grid and consumer CTAs; tpg = 0: the plain
-// two-launch sequence.  The consumers must keep up with B2 or the spectrum leaves the L2 before it is read (and a consumer
-// that falls behind is far worse than none: Q5 with 48 CTAs 6.2 ms against 3.25): B3 alone costs ~5 ps per series and time
-// step on ~518 resident CTAs (C3 0.43 ms, P5 0.75 ms, C5 0.16 ms), B2 streams |Fhat| at ~7 TB/s, so B3 needs
-// ~2270 / N_d CTAs for the duration of B2 in either precision (measured: C3 fails with 24 and works from 37, P5 fails with
-// 37 and works from 48); 1.8 times that are launched, at least 32.  Shapes that would need more than 128 (N_d < 32: B3 is
-// a large part of the call and its CTAs would crowd B2 out) and shapes whose B2 takes under 2 ms (no gain measured at C2)
-// keep the two launches.  Groups of 16 MB (4 - 32 MB measured within 0.3 %).
+// two-launch sequence.  The consumers should keep up with B2 (what they do not get to goes to HBM and through the clean-up
+// launch): B3 alone costs ~5 ps per series and time step on ~518 resident CTAs (C3 0.43 ms, P5 0.75 ms, C5 0.16 ms), B2
+// streams |Fhat| at ~7 TB/s, so B3 needs ~2270 / N_d CTAs for the duration of B2 in either precision (measured: C3 falls
+// behind with 24 CTAs and keeps up from 32, P5 falls behind with 37 and keeps up from 48).  More than needed costs B2 SM
+// share: 1.4 x the need are launched, at least 32 and at most 72 (measured best at N_d = 32, 40, 49: 64 CTAs; at 64: 50 - 64;
+// at 100 and 150: 32 - 48).  Shapes with N_d < 23 (the need exceeds 100 CTAs: B3 is a large part of the call and cannot
+// hide, Q5 measured without gain at any count) and shapes whose B2 takes under 2 ms (no gain measured at C2) keep the two
+// launches.  Groups of 16 MB (4 - 32 MB measured within 0.3 %).
 struct L2rPlan { int tpg, ctas; };
 L2rPlan l2r_plan(const tt_plan* p) {
     L2rPlan none{0, 0};
@@ -253,9 +254,9 @@ L2rPlan l2r_plan(const tt_plan* p) {
     int ctas = g_l2r_ctas;
     if (ctas <= 0) {
         const double need = 2270.0 / (double)p->N_d;
-        if (g_l2r_mb < 0 && (1.8 * need > 128.0 || fhat_bytes < 14.0e9)) return none;
-        ctas = (int)std::ceil(1.8 * need);
-        if (ctas < 32) ctas = 32;
+        if (g_l2r_mb < 0 && (need > 100.0 || fhat_bytes < 14.0e9)) return none;
+        ctas = (int)std::ceil(1.4 * need);
+        ctas = ctas < 32 ? 32 : ctas > 72 ? 72 : ctas;
     }
     const double tile_bytes = (double)p->n_f * ptile * 2.0 * (double)esize(p->dtype);
     long long tpg = (long long)((double)(g_l2r_mb < 0 ? 16 : g_l2r_mb) * 1048576.0 / tile_bytes);
