@@ -306,12 +306,13 @@ int run_rmatvec(const tt_plan* p, const void* d, void* m, cudaStream_t s, int ev
     TT_CUDA(p, fft_c2r_consumer_launch(t, p->xhat, at(m, vm.off, es), Pc, p->l2r_sync, done, ptile, lp.ctas, p->fft_stream));
     g.l2r_sync = p->l2r_sync;
     g.l2r_tpg = lp.tpg;
-    TT_CUDA(p, gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s));
+    const cudaError_t eb2 = gemv_adj_launch(t, p->Fhat, p->dhat, p->xhat, g, s);
     pr.mark(2);
-    TT_CUDA(p, cudaEventRecord(p->fev[1], p->fft_stream));        // join
+    TT_CUDA(p, cudaEventRecord(p->fev[1], p->fft_stream));        // join (also when B2 could not be launched: the consumers give up by themselves)
     TT_CUDA(p, cudaStreamWaitEvent(s, p->fev[1], 0));
+    if (eb2 != cudaSuccess) return fail_cuda(p, eb2);
     P.skip = done;                                                // whatever the consumers did not get to (normally nothing)
-    if (g_l2r_discard != 3) TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
+    TT_CUDA(p, fft_c2r_launch(t, p->xhat, at(m, vm.off, es), P, 1, s));
     pr.mark(3);
     return TT_OK;
 }
@@ -1023,7 +1024,7 @@ int tt_debug_set(const char* key, int value) {
     }
     if (!std::strcmp(key, "l2r_mb")) { if (value < -1) return TT_ERR_SHAPE; g_l2r_mb = value; return TT_OK; }
     if (!std::strcmp(key, "l2r_ctas")) { if (value < 0 || value > 4096) return TT_ERR_SHAPE; g_l2r_ctas = value; return TT_OK; }
-    if (!std::strcmp(key, "l2r_discard")) { g_l2r_discard = value; return TT_OK; }
+    if (!std::strcmp(key, "l2r_discard")) { g_l2r_discard = value != 0; return TT_OK; }
     if (!std::strcmp(key, "kd_slab")) { kd_umma_debug_set_slab(value); return TT_OK; }
     if (!std::strcmp(key, "trsv_U")) { trsv_debug_set_U(value); return TT_OK; }
     if (!std::strcmp(key, "gemm32_fwd")) { gemm32_debug_set(value); return TT_OK; }
